@@ -1,0 +1,173 @@
+/*
+ * gamma_b200.h -- C-ABI of libgamma_b200.so: the gamma-index hot path of arxiv/paper_1012_1900
+ * (Gu, Jia, Jiang, "GPU-based fast gamma index calculation") for NVIDIA B200 (sm_100a).
+ *
+ * Citations are PAPER.md:<line> (+ section / equation / algorithm); "reading n" refers to the table of
+ * readings in DESIGN.md.  Every entry point is plain C: raw pointers, sizes, a cudaStream_t passed as
+ * void*.  Unless a parameter says HOST, pointers are DEVICE pointers owned by the caller (PyTorch in
+ * the binding); the library never frees or modifies inputs.  The library owns one grow-only device
+ * workspace per process (work lists, sort buffers, offset table), released by gamma_release().
+ *
+ * Conventions
+ *   grids      dense fp32, x fastest: lin = ix + nx*(iy + ny*iz); reference and evaluation dose share
+ *              one grid; an axis of size 1 is dropped (2D input; reading 12).
+ *              N = nx*ny*nz must be < 2^31.
+ *   result     gamma[N] fp32; voxels excluded by the low-dose cutoff (or with dD_v <= 0) hold NaN.
+ *   async      all work is enqueued on `stream`; calls return without synchronising unless stated.
+ *   errors     every int function returns GAMMA_OK (0) or a GAMMA_ERR_* code; on an argument error
+ *              nothing is launched or written.  gamma_last_error_string() describes the last failure
+ *              of the calling thread.  No exceptions, no abort.
+ *   threads    calls are serialised by an internal mutex; consecutive calls on different streams are
+ *              ordered by an event (they share the workspace).
+ *   no fallback: there is no CPU path; without a CUDA device every compute call returns GAMMA_ERR_CUDA.
+ */
+#ifndef GAMMA_B200_H
+#define GAMMA_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GAMMA_OK 0
+#define GAMMA_ERR_INVALID_ARGUMENT 1
+#define GAMMA_ERR_OUT_OF_MEMORY 2
+#define GAMMA_ERR_CUDA 3
+
+#define GAMMA_MODE_GLOBAL 0 /* dD = DD * D_norm                       (reading 8) */
+#define GAMMA_MODE_LOCAL 1  /* dD_v = DD * D_r[v]                     (reading 9) */
+
+/*
+ * gamma_eval -- the per-reference-voxel gamma search (Eq. 1; Algorithm A1 steps 1-4,
+ * PAPER.md:164-190; Algorithm A2 steps 2-7).
+ *
+ *   gamma[v] = min over the continuous evaluation surface of
+ *              | (r_v/DTA, D_r[v]/dD) - (r_e/DTA, D_e(r_e)/dD) |
+ * where the surface is the piecewise-linear interpolant of `eval` on the Kuhn split of every grid cell
+ * (readings 5, 6) and the point-to-simplex distance is exact.  Cells are visited
+ * in ascending order of their minimum spatial distance L and the search of a voxel stops when
+ * L >= current gamma (readings 3, 4); there is no radius cap (reading 18).
+ *
+ *   ref, eval        DEVICE, N fp32 each
+ *   dims             HOST, (nx, ny, nz), each >= 1, at least one > 1
+ *   spacing_mm       HOST, (dx, dy, dz), each > 0
+ *   DD               dose-difference criterion as a fraction (0.03 = 3 %), > 0
+ *   DTA_mm           distance-to-agreement criterion in mm, > 0
+ *   mode             GAMMA_MODE_GLOBAL | GAMMA_MODE_LOCAL
+ *   low_dose_cutoff  in [0, 1): voxels with D_r < cutoff * D_norm are excluded (NaN); D_norm = max(ref)
+ *                    (reading 10; the comparison is done in double so that it is decided identically
+ *                    everywhere).  Excluded voxels still serve as evaluation points of their neighbours.
+ *   out_gamma        DEVICE, N fp32, written entirely
+ *   stream           cudaStream_t
+ */
+int gamma_eval(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
+               float DTA_mm, int mode, float low_dose_cutoff, float* out_gamma, void* stream);
+
+/* Options of gamma_eval_ex / gamma_eval_host.  Zero-initialise, then set what differs. */
+typedef struct gamma_opts {
+    float norm_dose;      /* D_norm; <= 0: max(ref), found on the device                                  */
+    int presort;          /* 0: default (= 1); 1: radix-sort the search work list by its key before the
+                             search (A2 step 3); 2: no sort (Table 2's "without sorting")   */
+    int star_phase;       /* 0: default (= 1); 1: interior voxels first try the 75 faces touching the voxel
+                             and finish there when gamma_star <= distance to the rest of the surface;
+                             2: off -- every voxel goes through the table search with key |DD|/dD, as in
+                             Algorithm A2                                               */
+    int lanes_per_voxel;  /* 0: default (= 8); 1, 8 or 32 lanes cooperate on one reference voxel in the
+                             table search (1 = the paper's thread-per-voxel mapping)        */
+    int sort_key_bits;    /* 0: default (= 16); number of most significant key bits the presort orders by
+                             (8, 16, 24 or 32)                                                             */
+    long long table_cap;  /* 0: default (1<<20); max entries of the sorted offset table; past it the search
+                             continues by exhaustive enumeration, so results never depend on it            */
+} gamma_opts;
+
+/* gamma_eval with options (opts may be NULL = defaults).  Same contract as gamma_eval. */
+int gamma_eval_ex(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
+                  float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts, float* out_gamma,
+                  void* stream);
+
+/*
+ * gamma_eval_host -- the same computation for HOST buffers (A2 steps 1 and 8):
+ * copies ref and eval to the device, runs gamma_eval_ex, copies gamma back and SYNCHRONISES `stream`
+ * before returning.  ref_host, eval_host, out_gamma_host: HOST, N fp32 each (pinned memory makes the
+ * copies asynchronous with respect to other streams).
+ */
+int gamma_eval_host(const float* ref_host, const float* eval_host, const int dims[3], const float spacing_mm[3],
+                    float DD, float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts,
+                    float* out_gamma_host, void* stream);
+
+/* Summary written by gamma_stats (layout fixed, 48 bytes). */
+typedef struct gamma_summary {
+    unsigned long long n_eval; /* voxels with a finite gamma                                  */
+    unsigned long long n_pass; /* of those, gamma <= 1                                        */
+    double sum_gamma;          /* sum of gamma over evaluated voxels                          */
+    double sum_gamma3;         /* sum of gamma^3: the paper's work predictor */
+    float max_gamma;           /* 0 when n_eval == 0                                          */
+    unsigned int n_nan;        /* excluded voxels (low 32 bits)                               */
+    unsigned long long pad_;
+} gamma_summary;
+
+/*
+ * gamma_stats -- pass rate / gamma histogram reduction (BASELINE.json north_star (5); not in the paper).
+ *   gamma     DEVICE, n fp32 (NaN = excluded)
+ *   nbins     1..4096; bin b counts finite gamma with floor(gamma / hist_max * nbins) == b, the last bin
+ *             also takes everything >= hist_max
+ *   hist_dev  DEVICE, nbins u64, overwritten;  out_dev: DEVICE, one gamma_summary, overwritten
+ */
+int gamma_stats(const float* gamma, long long n, int nbins, float hist_max, unsigned long long* hist_dev,
+                gamma_summary* out_dev, void* stream);
+
+/*
+ * gamma_sort_pairs -- the hand-written LSD radix sort of the voxel work list (subsystem (3); PAPER.md:221,
+ * 245 used Thrust): stable ascending sort of (key, value) pairs on key bits [begin_bit, end_bit).
+ *   keys, vals  DEVICE, n u32 each, sorted in place;  n < 2^31; begin_bit, end_bit multiples of 8,
+ *   0 <= begin_bit < end_bit <= 32.  Non-negative fp32 keys sort correctly as their bit patterns.
+ */
+int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int begin_bit, int end_bit,
+                     void* stream);
+
+/*
+ * gamma_offset_table -- the sorted offset table {n, L_n} (Algorithm A1 steps 2-3; A2
+ * steps 4-5) with the cell bound of reading 4.  By the symmetry L(o) = L(-o-1) the
+ * table lists the octant m >= 0 only: entry (m, L^2), L^2 = sum_a (m_a h_a)^2, h = spacing/DTA, for every
+ * m with m_a <= dims_a - 1 and L < radius, sorted ascending by (L^2 as fp32, then m_x + bx*(m_y + by*m_z));
+ * the search expands each entry into its 8 (4 in 2D) offsets o_a in {m_a, -m_a-1}.
+ *   out_entries  DEVICE, max_entries * 4 int32: (bits of L^2 as fp32, m_x, m_y, m_z) per entry
+ *   out_count    DEVICE, 3 int32: number of entries written; 1 if the table was truncated to max_entries'
+ *                worth of box (radius reduced), else 0; bits of the fp32 radius^2 actually covered
+ */
+int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_mm, float radius,
+                       long long max_entries, int* out_entries, int* out_count, void* stream);
+
+/* Counters of the last gamma_eval* call (SYNCHRONISES the stream of that call).  HOST outputs. */
+typedef struct gamma_counters {
+    long long n_voxels;      /* N                                                              */
+    long long n_evaluated;   /* M: voxels that passed the cutoff                               */
+    long long n_table_search;/* voxels that went through the sorted-table search               */
+    long long table_entries; /* octant entries of the offset table                             */
+    long long vertex_visits; /* owner vertices whose 26 faces were evaluated in the table search */
+    float max_key;           /* radius of the table = largest key of the search list           */
+    float norm_dose;         /* D_norm used                                                    */
+    int table_truncated;
+    int pad_;
+} gamma_counters;
+int gamma_get_counters(gamma_counters* out_host);
+
+/*
+ * gamma_fp32_probe -- measures the plain-ALU FP32 rate of the device with independent FFMA chains
+ * (the "alu" roofline denominator of bench.py; DESIGN.md section "Roofline").  SYNCHRONISES.
+ *   out_tflops HOST: 2 * FFMA thread-instructions / second / 1e12, best of `repeats` launches.
+ */
+int gamma_fp32_probe(int repeats, double* out_tflops, void* stream);
+
+/* Frees the workspace.  Safe to call at any time; the next call re-allocates. */
+void gamma_release(void);
+
+/* Description of the last error seen by the calling thread ("" if none). */
+const char* gamma_last_error_string(void);
+
+/* Library version string, e.g. "gamma_b200 0.1 sm_100a". */
+const char* gamma_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GAMMA_B200_H */

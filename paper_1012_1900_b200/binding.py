@@ -1,0 +1,242 @@
+"""Thin ctypes binding of libgamma_b200.so: same names as include/gamma_b200.h, argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device memory and
+streams (``tensor.data_ptr()``, ``torch.cuda.current_stream().cuda_stream``).  There is no CPU fallback:
+if the library cannot be loaded, or a call fails, a ``GammaError`` is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import torch
+
+from . import build as _build
+
+__all__ = [
+    "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
+    "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
+    "gamma_fp32_probe", "gamma_release", "gamma_version", "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
+]
+
+GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
+
+# every symbol include/gamma_b200.h declares
+exported_symbols = (
+    "gamma_eval", "gamma_eval_ex", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table",
+    "gamma_get_counters", "gamma_fp32_probe", "gamma_release", "gamma_last_error_string", "gamma_version",
+)
+
+
+class GammaError(RuntimeError):
+    pass
+
+
+class _COpts(ctypes.Structure):
+    _fields_ = [("norm_dose", ctypes.c_float), ("presort", ctypes.c_int), ("star_phase", ctypes.c_int),
+                ("lanes_per_voxel", ctypes.c_int), ("sort_key_bits", ctypes.c_int), ("table_cap", ctypes.c_longlong)]
+
+
+class _CSummary(ctypes.Structure):
+    _fields_ = [("n_eval", ctypes.c_ulonglong), ("n_pass", ctypes.c_ulonglong), ("sum_gamma", ctypes.c_double),
+                ("sum_gamma3", ctypes.c_double), ("max_gamma", ctypes.c_float), ("n_nan", ctypes.c_uint),
+                ("pad_", ctypes.c_ulonglong)]
+
+
+class _CCounters(ctypes.Structure):
+    _fields_ = [("n_voxels", ctypes.c_longlong), ("n_evaluated", ctypes.c_longlong),
+                ("n_table_search", ctypes.c_longlong), ("table_entries", ctypes.c_longlong),
+                ("vertex_visits", ctypes.c_longlong), ("max_key", ctypes.c_float), ("norm_dose", ctypes.c_float),
+                ("table_truncated", ctypes.c_int), ("pad_", ctypes.c_int)]
+
+
+@dataclass
+class GammaOpts:
+    """Mirror of ``gamma_opts`` (include/gamma_b200.h); 0 means "library default"."""
+    norm_dose: float = 0.0
+    presort: int = 0          # 1 sort, 2 no sort
+    star_phase: int = 0       # 1 on, 2 off
+    lanes_per_voxel: int = 0  # 1, 8, 32
+    sort_key_bits: int = 0    # 8, 16, 24, 32
+    table_cap: int = 0
+
+    def _c(self):
+        return _COpts(float(self.norm_dose), int(self.presort), int(self.star_phase), int(self.lanes_per_voxel),
+                      int(self.sort_key_bits), int(self.table_cap))
+
+
+_lib = None
+
+
+def load_library(build_if_needed: bool = True):
+    """dlopen libgamma_b200.so (building it with nvcc first if missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if build_if_needed:
+        path = _build.build()
+    if not os.path.exists(path):
+        raise GammaError(f"{path} is missing and there is no CPU fallback; run python -m paper_1012_1900_b200.build")
+    lib = ctypes.CDLL(path)
+    vp, ci, cf, cll = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_longlong
+    i3, f3 = ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_float)
+    lib.gamma_eval.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, vp, vp]
+    lib.gamma_eval_ex.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
+    lib.gamma_eval_host.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
+    lib.gamma_stats.argtypes = [vp, cll, ci, cf, vp, vp, vp]
+    lib.gamma_sort_pairs.argtypes = [vp, vp, cll, ci, ci, vp]
+    lib.gamma_offset_table.argtypes = [i3, f3, cf, cf, cll, vp, vp, vp]
+    lib.gamma_get_counters.argtypes = [ctypes.POINTER(_CCounters)]
+    lib.gamma_fp32_probe.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
+    for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
+                 "gamma_offset_table", "gamma_get_counters", "gamma_fp32_probe"):
+        getattr(lib, name).restype = ci
+    lib.gamma_release.restype = None
+    lib.gamma_last_error_string.restype = ctypes.c_char_p
+    lib.gamma_version.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        msg = load_library().gamma_last_error_string().decode()
+        raise GammaError(f"libgamma_b200 error {rc}: {msg}")
+
+
+def _stream(stream):
+    if stream is None:
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _dev_f32(t: torch.Tensor, name: str) -> torch.Tensor:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise GammaError(f"{name} must be a contiguous float32 CUDA tensor")
+    return t
+
+
+def _geom(dims, spacing_mm):
+    return (ctypes.c_int * 3)(*[int(d) for d in dims]), (ctypes.c_float * 3)(*[float(s) for s in spacing_mm])
+
+
+def _numel(dims) -> int:
+    return int(dims[0]) * int(dims[1]) * int(dims[2])
+
+
+def gamma_eval(ref, eval, dims, spacing_mm, DD, DTA_mm, mode=GAMMA_MODE_GLOBAL, low_dose_cutoff=0.1,
+               out_gamma=None, stream=None):
+    """``gamma_eval`` of include/gamma_b200.h.  Returns ``out_gamma`` (float32 CUDA tensor, N elements)."""
+    return gamma_eval_ex(ref, eval, dims, spacing_mm, DD, DTA_mm, mode, low_dose_cutoff, None, out_gamma, stream,
+                         _plain=True)
+
+
+def gamma_eval_ex(ref, eval, dims, spacing_mm, DD, DTA_mm, mode=GAMMA_MODE_GLOBAL, low_dose_cutoff=0.1, opts=None,
+                  out_gamma=None, stream=None, _plain=False):
+    lib = load_library()
+    ref, eval = _dev_f32(ref, "ref"), _dev_f32(eval, "eval")
+    n = _numel(dims)
+    if ref.numel() != n or eval.numel() != n:
+        raise GammaError("ref / eval size does not match dims")
+    if out_gamma is None:
+        out_gamma = torch.empty(n, dtype=torch.float32, device=ref.device)
+    _dev_f32(out_gamma, "out_gamma")
+    if out_gamma.numel() != n:
+        raise GammaError("out_gamma size does not match dims")
+    cd, cs = _geom(dims, spacing_mm)
+    if _plain:
+        rc = lib.gamma_eval(ref.data_ptr(), eval.data_ptr(), cd, cs, float(DD), float(DTA_mm), int(mode),
+                            float(low_dose_cutoff), out_gamma.data_ptr(), _stream(stream))
+    else:
+        co = opts._c() if opts is not None else None
+        rc = lib.gamma_eval_ex(ref.data_ptr(), eval.data_ptr(), cd, cs, float(DD), float(DTA_mm), int(mode),
+                               float(low_dose_cutoff), ctypes.byref(co) if co is not None else None,
+                               out_gamma.data_ptr(), _stream(stream))
+    _check(rc)
+    return out_gamma
+
+
+def gamma_eval_host(ref_host, eval_host, dims, spacing_mm, DD, DTA_mm, mode=GAMMA_MODE_GLOBAL, low_dose_cutoff=0.1,
+                    opts=None, out_gamma_host=None, stream=None):
+    """``gamma_eval_host``: CPU float32 tensors in (pinned for speed), CPU float32 tensor out; synchronises."""
+    lib = load_library()
+    n = _numel(dims)
+    for t, name in ((ref_host, "ref_host"), (eval_host, "eval_host")):
+        if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+                and t.numel() == n):
+            raise GammaError(f"{name} must be a contiguous float32 CPU tensor with nx*ny*nz elements")
+    if out_gamma_host is None:
+        out_gamma_host = torch.empty(n, dtype=torch.float32).pin_memory()
+    if out_gamma_host.is_cuda or out_gamma_host.dtype != torch.float32 or out_gamma_host.numel() != n:
+        raise GammaError("out_gamma_host must be a float32 CPU tensor with nx*ny*nz elements")
+    cd, cs = _geom(dims, spacing_mm)
+    co = opts._c() if opts is not None else None
+    rc = lib.gamma_eval_host(ref_host.data_ptr(), eval_host.data_ptr(), cd, cs, float(DD), float(DTA_mm), int(mode),
+                             float(low_dose_cutoff), ctypes.byref(co) if co is not None else None,
+                             out_gamma_host.data_ptr(), _stream(stream))
+    _check(rc)
+    return out_gamma_host
+
+
+def gamma_stats(gamma, nbins=64, hist_max=4.0, stream=None):
+    """``gamma_stats``: returns (hist int64 CUDA tensor [nbins], summary dict) -- reading the dict synchronises."""
+    lib = load_library()
+    _dev_f32(gamma, "gamma")
+    hist = torch.empty(int(nbins), dtype=torch.int64, device=gamma.device)
+    summ = torch.empty(ctypes.sizeof(_CSummary), dtype=torch.uint8, device=gamma.device)
+    _check(lib.gamma_stats(gamma.data_ptr(), gamma.numel(), int(nbins), float(hist_max), hist.data_ptr(),
+                           summ.data_ptr(), _stream(stream)))
+    raw = bytes(summ.cpu().numpy().tobytes())
+    s = _CSummary.from_buffer_copy(raw)
+    return hist, {"n_eval": s.n_eval, "n_pass": s.n_pass, "sum_gamma": s.sum_gamma, "sum_gamma3": s.sum_gamma3,
+                  "max_gamma": s.max_gamma, "n_nan": s.n_nan}
+
+
+def gamma_sort_pairs(keys, vals, begin_bit=0, end_bit=32, stream=None):
+    """``gamma_sort_pairs``: in-place stable sort of int32/uint32-typed CUDA tensors (bit patterns)."""
+    lib = load_library()
+    for t in (keys, vals):
+        if not (t.is_cuda and t.is_contiguous() and t.element_size() == 4):
+            raise GammaError("keys / vals must be contiguous 4-byte CUDA tensors")
+    if keys.numel() != vals.numel():
+        raise GammaError("keys and vals differ in length")
+    _check(lib.gamma_sort_pairs(keys.data_ptr(), vals.data_ptr(), keys.numel(), int(begin_bit), int(end_bit),
+                                _stream(stream)))
+    return keys, vals
+
+
+def gamma_offset_table(dims, spacing_mm, DTA_mm, radius, max_entries=1 << 20, device="cuda", stream=None):
+    """``gamma_offset_table``: returns (entries int32 [count, 4], truncated flag, covered radius^2)."""
+    lib = load_library()
+    ent = torch.empty((int(max_entries), 4), dtype=torch.int32, device=device)
+    cnt = torch.zeros(3, dtype=torch.int32, device=device)
+    cd, cs = _geom(dims, spacing_mm)
+    _check(lib.gamma_offset_table(cd, cs, float(DTA_mm), float(radius), int(max_entries), ent.data_ptr(),
+                                  cnt.data_ptr(), _stream(stream)))
+    c = cnt.cpu()
+    r2 = c[2:3].view(torch.float32).item()
+    return ent[: int(c[0])], bool(c[1]), r2
+
+
+def gamma_get_counters() -> dict:
+    lib = load_library()
+    c = _CCounters()
+    _check(lib.gamma_get_counters(ctypes.byref(c)))
+    return {k: getattr(c, k) for k, _ in _CCounters._fields_ if k != "pad_"}
+
+
+def gamma_fp32_probe(repeats=5, stream=None) -> float:
+    lib = load_library()
+    v = ctypes.c_double(0.0)
+    _check(lib.gamma_fp32_probe(int(repeats), ctypes.byref(v), _stream(stream)))
+    return v.value
+
+
+def gamma_release():
+    load_library().gamma_release()
+
+
+def gamma_version() -> str:
+    return load_library().gamma_version().decode()

@@ -1,0 +1,83 @@
+// common.cuh -- shared device-side definitions of libgamma_b200 (sm_100a).
+// Notation follows the paper: D_r reference dose, D_e evaluation dose, dD dose criterion, DTA distance
+// criterion, L the normalised spatial distance of the offset table (Algorithm A1).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gamma_b200 {
+
+// Geometry of the dose grid in units of the DTA criterion.  Passed to kernels by value.
+struct GridP {
+    int n[3];        // nx, ny, nz
+    int stride[3];   // 1, nx, nx*ny
+    int N;           // nx*ny*nz
+    float h[3];      // spacing / DTA; 0 for a dropped axis (size 1)
+    float hh[3];     // h^2
+    float invA[8];   // invA[T] = 1 / sum_{a in T} h_a^2 over axis subsets T (bit0 x, bit1 y, bit2 z); 0 if T has a dropped axis
+    float K3, K5, K6;          // h_a^2 h_b^2 / (h_a^2 + h_b^2) for the pairs xy, xz, yz
+    float Kxy7, Kyz7, Kzx7;    // h_a^2 h_b^2 / (h_x^2 + h_y^2 + h_z^2)
+    float rho_link2; // squared distance from a voxel to the boundary of its star (3D only), slightly shrunk
+    int all_active;  // 1 when all three axes have size > 1
+};
+
+// Criteria (Eq. 1) and exclusion policy (readings 8-10).
+struct EvalP {
+    float DD;        // dose-difference criterion, fraction
+    float cutoff;    // low-dose cutoff, fraction of D_norm
+    float norm_dose; // D_norm if > 0, else taken from Ctl::normOrd
+    int mode;        // 0 global, 1 local
+};
+
+// Device control block: everything the pipeline decides on the device (no host sync on the path).
+struct Ctl {
+    unsigned normOrd;      // max(ref) as an order-preserving uint
+    unsigned maxKeyBits;   // largest key of the search list (bits of a non-negative float)
+    unsigned nEval;        // M: evaluated voxels
+    unsigned nSearch;      // voxels in the table-search work list
+    unsigned workCounter;  // dynamic work fetch of the table search
+    unsigned tableCount;   // octant entries in the offset table
+    unsigned tableTrunc;   // 1 if the table was cut at table_cap
+    float Rtab2;           // squared radius the table covers
+    int box[3];            // table box: m_a in [0, box_a)
+    unsigned pad0;
+    unsigned long long visits;  // owner vertices evaluated by the table search
+    unsigned sortN;        // element count for gamma_sort_pairs
+    unsigned pad1;
+};
+
+__host__ __device__ inline unsigned float_to_ordered(float f)
+{
+#if defined(__CUDA_ARCH__)
+    unsigned b = __float_as_uint(f);
+#else
+    union { float f; unsigned u; } cv; cv.f = f; unsigned b = cv.u;
+#endif
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__host__ __device__ inline float ordered_to_float(unsigned u)
+{
+    unsigned b = (u & 0x80000000u) ? (u & 0x7fffffffu) : ~u;
+#if defined(__CUDA_ARCH__)
+    return __uint_as_float(b);
+#else
+    union { float f; unsigned u; } cv; cv.u = b; return cv.f;
+#endif
+}
+
+// squared normalised minimum spatial distance of the cell [o, o+1] with m_a = max(o_a, -o_a-1)
+// (reading 4).  One definition for the table builder and the beyond-table enumeration.
+__device__ __forceinline__ float cell_L2(int mx, int my, int mz, const GridP& g)
+{
+    const float ax = (float)mx * g.h[0], ay = (float)my * g.h[1], az = (float)mz * g.h[2];
+    return fmaf(ax, ax, fmaf(ay, ay, az * az));
+}
+
+__device__ __forceinline__ float warp_max(float v)
+{
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, s));
+    return v;
+}
+
+}  // namespace gamma_b200

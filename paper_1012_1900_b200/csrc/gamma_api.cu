@@ -1,0 +1,551 @@
+// gamma_api.cu -- host side of libgamma_b200.so: argument checks, workspace, kernel launches.
+// The C-ABI is documented in include/gamma_b200.h.  There is no CPU path here: every step of the hot path
+// runs in the kernels of gamma_search.cuh / radix_sort.cuh / offset_table.cuh / stats.cuh.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+
+#include "../../include/gamma_b200.h"
+#include "common.cuh"
+#include "gamma_search.cuh"
+#include "offset_table.cuh"
+#include "radix_sort.cuh"
+#include "stats.cuh"
+
+using namespace gamma_b200;
+
+namespace {
+
+thread_local std::string g_err;
+std::mutex g_mu;
+
+int fail(int code, const std::string& msg)
+{
+    g_err = msg;
+    return code;
+}
+#define CU_TRY(call)                                                                          \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(e_ == cudaErrorMemoryAllocation ? GAMMA_ERR_OUT_OF_MEMORY : GAMMA_ERR_CUDA, \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                 \
+    } while (0)
+
+// grow-only device buffer
+struct Buf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t need(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaFree(p); p = nullptr; cap = 0; }
+        size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) { p = nullptr; return e; }
+        cap = want;
+        return cudaSuccess;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+    }
+};
+
+struct Workspace {
+    Buf ctl;                       // Ctl
+    Buf key0, idx0, key1, idx1;    // search work list, ping-pong for the sort
+    Buf tileHist;                  // radix sort
+    Buf table, tmpL, tmpIdx;       // offset table
+    Buf hRef, hEval, hOut;         // device staging of gamma_eval_host
+    cudaEvent_t done = nullptr;    // orders consecutive calls that share this workspace
+    bool havePending = false;
+    int numSM = 0;
+    // last call, for gamma_get_counters
+    cudaStream_t lastStream = nullptr;
+    long long lastN = 0;
+    bool haveLast = false;
+    void releaseAll()
+    {
+        Buf* all[] = {&ctl, &key0, &idx0, &key1, &idx1, &tileHist, &table, &tmpL, &tmpIdx, &hRef, &hEval, &hOut};
+        for (Buf* b : all) b->release();
+        if (done) { cudaEventDestroy(done); done = nullptr; }
+        havePending = false; haveLast = false;
+    }
+} g_ws;
+
+int ensure_device()
+{
+    if (g_ws.numSM > 0) return GAMMA_OK;
+    int dev = 0;
+    CU_TRY(cudaGetDevice(&dev));
+    int sm = 0;
+    CU_TRY(cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev));
+    g_ws.numSM = sm > 0 ? sm : 148;
+    return GAMMA_OK;
+}
+
+int order_after_previous(cudaStream_t st)
+{
+    if (!g_ws.done) CU_TRY(cudaEventCreateWithFlags(&g_ws.done, cudaEventDisableTiming));
+    if (g_ws.havePending) CU_TRY(cudaStreamWaitEvent(st, g_ws.done, 0));
+    return GAMMA_OK;
+}
+int mark_done(cudaStream_t st)
+{
+    CU_TRY(cudaEventRecord(g_ws.done, st));
+    g_ws.havePending = true;
+    return GAMMA_OK;
+}
+
+// distance from the origin to the triangle (a, b, c) in R^3 (Ericson, Real-Time Collision Detection 5.1.5)
+double origin_triangle_distance(const double a[3], const double b[3], const double c[3])
+{
+    auto dot = [](const double* u, const double* v) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; };
+    double ab[3], ac[3], ap[3], bp[3], cp[3], q[3];
+    for (int i = 0; i < 3; ++i) { ab[i] = b[i] - a[i]; ac[i] = c[i] - a[i]; ap[i] = -a[i]; bp[i] = -b[i]; cp[i] = -c[i]; }
+    const double d1 = dot(ab, ap), d2 = dot(ac, ap);
+    auto norm = [&](const double* v) { return std::sqrt(dot(v, v)); };
+    if (d1 <= 0 && d2 <= 0) return norm(a);
+    const double d3 = dot(ab, bp), d4 = dot(ac, bp);
+    if (d3 >= 0 && d4 <= d3) return norm(b);
+    const double vc = d1 * d4 - d3 * d2;
+    if (vc <= 0 && d1 >= 0 && d3 <= 0) {
+        const double t = d1 / (d1 - d3);
+        for (int i = 0; i < 3; ++i) q[i] = a[i] + t * ab[i];
+        return norm(q);
+    }
+    const double d5 = dot(ab, cp), d6 = dot(ac, cp);
+    if (d6 >= 0 && d5 <= d6) return norm(c);
+    const double vb = d5 * d2 - d1 * d6;
+    if (vb <= 0 && d2 >= 0 && d6 <= 0) {
+        const double t = d2 / (d2 - d6);
+        for (int i = 0; i < 3; ++i) q[i] = a[i] + t * ac[i];
+        return norm(q);
+    }
+    const double va = d3 * d6 - d5 * d4;
+    if (va <= 0 && (d4 - d3) >= 0 && (d5 - d6) >= 0) {
+        const double t = (d4 - d3) / ((d4 - d3) + (d5 - d6));
+        for (int i = 0; i < 3; ++i) q[i] = b[i] + t * (c[i] - b[i]);
+        return norm(q);
+    }
+    const double den = 1.0 / (va + vb + vc), v = vb * den, w = vc * den;
+    for (int i = 0; i < 3; ++i) q[i] = a[i] + ab[i] * v + ac[i] * w;
+    return norm(q);
+}
+
+// Distance (in DTA units) from a voxel to the boundary of its star in the Kuhn mesh: the 24 triangles
+// opposite the voxel in the 24 tetrahedra that contain it.  Everything outside the star is at least this far.
+double star_link_distance(const double h[3])
+{
+    static const int perms[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+    double best = 1e300;
+    for (int oc = 0; oc < 8; ++oc) {
+        const int o[3] = {(oc & 1) ? -1 : 0, (oc & 2) ? -1 : 0, (oc & 4) ? -1 : 0};
+        for (int p = 0; p < 6; ++p) {
+            int vtx[4][3];
+            for (int a = 0; a < 3; ++a) vtx[0][a] = o[a];
+            for (int m = 1; m <= 3; ++m) {
+                for (int a = 0; a < 3; ++a) vtx[m][a] = vtx[m - 1][a];
+                vtx[m][perms[p][m - 1]] += 1;
+            }
+            int self = -1;
+            for (int m = 0; m <= 3; ++m)
+                if (vtx[m][0] == 0 && vtx[m][1] == 0 && vtx[m][2] == 0) self = m;
+            if (self < 0) continue;
+            double tri[3][3];
+            int k = 0;
+            for (int m = 0; m <= 3; ++m) {
+                if (m == self) continue;
+                for (int a = 0; a < 3; ++a) tri[k][a] = vtx[m][a] * h[a];
+                ++k;
+            }
+            const double dist = origin_triangle_distance(tri[0], tri[1], tri[2]);
+            if (dist < best) best = dist;
+        }
+    }
+    return best;
+}
+
+int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP& g)
+{
+    if (!dims || !spacing_mm) return fail(GAMMA_ERR_INVALID_ARGUMENT, "dims / spacing_mm is NULL");
+    if (!(DTA_mm > 0.0f) || !std::isfinite(DTA_mm)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "DTA_mm must be > 0");
+    long long N = 1;
+    int active = 0;
+    for (int a = 0; a < 3; ++a) {
+        if (dims[a] < 1) return fail(GAMMA_ERR_INVALID_ARGUMENT, "dims must be >= 1");
+        if (!(spacing_mm[a] > 0.0f) || !std::isfinite(spacing_mm[a]))
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "spacing_mm must be > 0");
+        N *= dims[a];
+        if (N >= (1ll << 31)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "nx*ny*nz must be < 2^31");
+        active += dims[a] > 1;
+    }
+    if (active == 0) return fail(GAMMA_ERR_INVALID_ARGUMENT, "at least one axis must have size > 1");
+    std::memset(&g, 0, sizeof g);
+    double h[3], hh[3];
+    for (int a = 0; a < 3; ++a) {
+        g.n[a] = dims[a];
+        h[a] = dims[a] > 1 ? (double)spacing_mm[a] / (double)DTA_mm : 0.0;
+        hh[a] = h[a] * h[a];
+        g.h[a] = (float)h[a];
+        g.hh[a] = (float)hh[a];
+    }
+    g.stride[0] = 1; g.stride[1] = dims[0]; g.stride[2] = dims[0] * dims[1];
+    g.N = (int)N;
+    for (int T = 1; T < 8; ++T) {
+        double A = 0.0;
+        bool ok = true;
+        for (int a = 0; a < 3; ++a)
+            if (T & (1 << a)) { ok = ok && h[a] > 0.0; A += hh[a]; }
+        g.invA[T] = ok ? (float)(1.0 / A) : 0.0f;
+    }
+    auto K = [&](int a, int b) { return (hh[a] + hh[b]) > 0.0 ? hh[a] * hh[b] / (hh[a] + hh[b]) : 0.0; };
+    g.K3 = (float)K(0, 1); g.K5 = (float)K(0, 2); g.K6 = (float)K(1, 2);
+    const double A7 = hh[0] + hh[1] + hh[2];
+    g.Kxy7 = (float)(hh[0] * hh[1] / A7); g.Kyz7 = (float)(hh[1] * hh[2] / A7); g.Kzx7 = (float)(hh[2] * hh[0] / A7);
+    g.all_active = active == 3;
+    if (g.all_active) {
+        const double rho = star_link_distance(h) * (1.0 - 1e-5);
+        g.rho_link2 = (float)(rho * rho);
+    }
+    return GAMMA_OK;
+}
+
+struct Resolved {
+    int presort, star, lanes, keyBits;
+    long long tableCap;
+    float normDose;
+};
+
+int resolve_opts(const gamma_opts* o, Resolved& r)
+{
+    r.presort = 1; r.star = 1; r.lanes = 8; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
+    if (!o) return GAMMA_OK;
+    if (o->presort < 0 || o->presort > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.presort must be 0, 1 or 2");
+    if (o->star_phase < 0 || o->star_phase > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.star_phase must be 0, 1 or 2");
+    if (o->presort == 2) r.presort = 0;
+    if (o->star_phase == 2) r.star = 0;
+    if (o->lanes_per_voxel != 0) {
+        if (o->lanes_per_voxel != 1 && o->lanes_per_voxel != 8 && o->lanes_per_voxel != 32)
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.lanes_per_voxel must be 0, 1, 8 or 32");
+        r.lanes = o->lanes_per_voxel;
+    }
+    if (o->sort_key_bits != 0) {
+        if (o->sort_key_bits != 8 && o->sort_key_bits != 16 && o->sort_key_bits != 24 && o->sort_key_bits != 32)
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.sort_key_bits must be 0, 8, 16, 24 or 32");
+        r.keyBits = o->sort_key_bits;
+    }
+    if (o->table_cap != 0) {
+        if (o->table_cap < 1 || o->table_cap > (1ll << 26))
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.table_cap must be in [1, 2^26]");
+        r.tableCap = o->table_cap;
+    }
+    if (o->norm_dose > 0.0f) r.normDose = o->norm_dose;
+    if (std::isnan(o->norm_dose) || std::isinf(o->norm_dose))
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.norm_dose must be finite");
+    return GAMMA_OK;
+}
+
+int check_criteria(float DD, int mode, float cutoff)
+{
+    if (!(DD > 0.0f) || !std::isfinite(DD)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "DD must be > 0");
+    if (mode != GAMMA_MODE_GLOBAL && mode != GAMMA_MODE_LOCAL) return fail(GAMMA_ERR_INVALID_ARGUMENT, "unknown mode");
+    if (!(cutoff >= 0.0f && cutoff < 1.0f)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "low_dose_cutoff must be in [0, 1)");
+    return GAMMA_OK;
+}
+
+// Enqueue the whole hot path on `st` (device pointers).  Caller holds g_mu.
+int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
+                     const Resolved& r, float* out, cudaStream_t st)
+{
+    int rc = ensure_device();
+    if (rc) return rc;
+    const long long N = g.N;
+    const long long maxTiles = (N + SORT_TILE - 1) / SORT_TILE;
+    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    CU_TRY(g_ws.key0.need(N * 4)); CU_TRY(g_ws.idx0.need(N * 4));
+    if (r.presort) {
+        CU_TRY(g_ws.key1.need(N * 4)); CU_TRY(g_ws.idx1.need(N * 4));
+        CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
+    }
+    CU_TRY(g_ws.table.need((size_t)r.tableCap * 16));
+    CU_TRY(g_ws.tmpL.need((size_t)r.tableCap * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)r.tableCap * 4));
+    rc = order_after_previous(st);
+    if (rc) return rc;
+
+    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p);
+    unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p), *i0 = static_cast<unsigned*>(g_ws.idx0.p);
+    unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *i1 = static_cast<unsigned*>(g_ws.idx1.p);
+    EvalP e;
+    e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
+
+    CU_TRY(cudaMemsetAsync(ctl, 0, sizeof(Ctl), st));
+    const int sm = g_ws.numSM;
+    if (!(r.normDose > 0.0f)) {                                          // a0
+        long long blocks = (N + 1023) / 1024;
+        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 8 ? sm * 8 : blocks));
+        k_max_ref<<<grid, 256, 0, st>>>(ref, (int)N, ctl);
+    }
+    {                                                                    // a1 + star
+        long long tiles = (N + PREP_TILE - 1) / PREP_TILE;
+        int grid = (int)(tiles > sm * 16 ? sm * 16 : tiles);
+        if (r.star)
+            k_prep_star<true><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
+        else
+            k_prep_star<false><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
+    }
+    // a3: offset table out to the largest key
+    k_offset_table<<<1, TAB_THREADS, 0, st>>>(g, ctl, -1.0f, r.tableCap, static_cast<int4*>(g_ws.table.p),
+                                              static_cast<unsigned*>(g_ws.tmpL.p), static_cast<unsigned*>(g_ws.tmpIdx.p));
+    const unsigned *lk = k0, *li = i0;
+    if (r.presort) {                                                     // a2
+        int where = radix_sort_enqueue(k0, i0, k1, i1, &ctl->nSearch, N, 32 - r.keyBits, 32,
+                                       static_cast<unsigned*>(g_ws.tileHist.p), st);
+        if (where) { lk = k1; li = i1; }
+    }
+    {                                                                    // a4 + a5
+        const int grid = sm * 8;
+        const int4* tab = static_cast<const int4*>(g_ws.table.p);
+        if (r.lanes == 1)
+            k_table_search<1><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
+        else if (r.lanes == 8)
+            k_table_search<8><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
+        else
+            k_table_search<32><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
+    }
+    CU_TRY(cudaGetLastError());
+    rc = mark_done(st);
+    if (rc) return rc;
+    g_ws.lastStream = st; g_ws.lastN = N; g_ws.haveLast = true;
+    return GAMMA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gamma_eval_ex(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
+                  float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts, float* out_gamma,
+                  void* stream)
+{
+    g_err.clear();
+    if (!ref || !eval || !out_gamma) return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref / eval / out_gamma is NULL");
+    GridP g;
+    int rc = make_grid(dims, spacing_mm, DTA_mm, g);
+    if (rc) return rc;
+    rc = check_criteria(DD, mode, low_dose_cutoff);
+    if (rc) return rc;
+    Resolved r;
+    rc = resolve_opts(opts, r);
+    if (rc) return rc;
+    std::lock_guard<std::mutex> lock(g_mu);
+    return enqueue_pipeline(ref, eval, g, DD, mode, low_dose_cutoff, r, out_gamma, static_cast<cudaStream_t>(stream));
+}
+
+int gamma_eval(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
+               float DTA_mm, int mode, float low_dose_cutoff, float* out_gamma, void* stream)
+{
+    return gamma_eval_ex(ref, eval, dims, spacing_mm, DD, DTA_mm, mode, low_dose_cutoff, nullptr, out_gamma, stream);
+}
+
+int gamma_eval_host(const float* ref_host, const float* eval_host, const int dims[3], const float spacing_mm[3],
+                    float DD, float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts,
+                    float* out_gamma_host, void* stream)
+{
+    g_err.clear();
+    if (!ref_host || !eval_host || !out_gamma_host)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref_host / eval_host / out_gamma_host is NULL");
+    GridP g;
+    int rc = make_grid(dims, spacing_mm, DTA_mm, g);
+    if (rc) return rc;
+    rc = check_criteria(DD, mode, low_dose_cutoff);
+    if (rc) return rc;
+    Resolved r;
+    rc = resolve_opts(opts, r);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::lock_guard<std::mutex> lock(g_mu);
+    const size_t bytes = (size_t)g.N * 4;
+    CU_TRY(g_ws.hRef.need(bytes)); CU_TRY(g_ws.hEval.need(bytes)); CU_TRY(g_ws.hOut.need(bytes));
+    rc = order_after_previous(st);
+    if (rc) return rc;
+    CU_TRY(cudaMemcpyAsync(g_ws.hRef.p, ref_host, bytes, cudaMemcpyHostToDevice, st));     // A2 step 1
+    CU_TRY(cudaMemcpyAsync(g_ws.hEval.p, eval_host, bytes, cudaMemcpyHostToDevice, st));
+    rc = enqueue_pipeline(static_cast<const float*>(g_ws.hRef.p), static_cast<const float*>(g_ws.hEval.p), g, DD, mode,
+                          low_dose_cutoff, r, static_cast<float*>(g_ws.hOut.p), st);
+    if (rc) return rc;
+    CU_TRY(cudaMemcpyAsync(out_gamma_host, g_ws.hOut.p, bytes, cudaMemcpyDeviceToHost, st)); // A2 step 8
+    rc = mark_done(st);
+    if (rc) return rc;
+    CU_TRY(cudaStreamSynchronize(st));
+    return GAMMA_OK;
+}
+
+int gamma_stats(const float* gamma, long long n, int nbins, float hist_max, unsigned long long* hist_dev,
+                gamma_summary* out_dev, void* stream)
+{
+    g_err.clear();
+    if (!gamma || !hist_dev || !out_dev) return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma / hist_dev / out_dev is NULL");
+    if (n < 0 || n >= (1ll << 40)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "n out of range");
+    if (nbins < 1 || nbins > STATS_MAX_BINS) return fail(GAMMA_ERR_INVALID_ARGUMENT, "nbins must be in [1, 4096]");
+    if (!(hist_max > 0.0f) || !std::isfinite(hist_max)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "hist_max must be > 0");
+    std::lock_guard<std::mutex> lock(g_mu);
+    int rc = ensure_device();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    k_stats_clear<<<(nbins + 255) / 256, 256, 0, st>>>(hist_dev, nbins, out_dev);
+    if (n > 0) {
+        long long blocks = (n + STATS_THREADS * 8 - 1) / (STATS_THREADS * 8);
+        int grid = (int)(blocks > g_ws.numSM * 8 ? g_ws.numSM * 8 : blocks);
+        k_stats<<<grid, STATS_THREADS, nbins * sizeof(unsigned), st>>>(gamma, n, nbins, (float)nbins / hist_max, hist_dev, out_dev);
+    }
+    CU_TRY(cudaGetLastError());
+    return GAMMA_OK;
+}
+
+__global__ void k_set_u32(unsigned* p, unsigned v) { *p = v; }
+
+int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int begin_bit, int end_bit, void* stream)
+{
+    g_err.clear();
+    if (n < 0 || n >= (1ll << 31)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "n must be in [0, 2^31)");
+    if (n > 0 && (!keys || !vals)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "keys / vals is NULL");
+    if (begin_bit < 0 || end_bit > 32 || begin_bit >= end_bit || (begin_bit & 7) || (end_bit & 7))
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "need 0 <= begin_bit < end_bit <= 32, multiples of 8");
+    if (n == 0) return GAMMA_OK;
+    std::lock_guard<std::mutex> lock(g_mu);
+    int rc = ensure_device();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const long long maxTiles = (n + SORT_TILE - 1) / SORT_TILE;
+    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    CU_TRY(g_ws.key1.need(n * 4)); CU_TRY(g_ws.idx1.need(n * 4));
+    CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
+    rc = order_after_previous(st);
+    if (rc) return rc;
+    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p);
+    k_set_u32<<<1, 1, 0, st>>>(&ctl->sortN, (unsigned)n);
+    unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *v1 = static_cast<unsigned*>(g_ws.idx1.p);
+    int where = radix_sort_enqueue(keys, vals, k1, v1, &ctl->sortN, n, begin_bit, end_bit,
+                                   static_cast<unsigned*>(g_ws.tileHist.p), st);
+    if (where) {
+        CU_TRY(cudaMemcpyAsync(keys, k1, n * 4, cudaMemcpyDeviceToDevice, st));
+        CU_TRY(cudaMemcpyAsync(vals, v1, n * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    CU_TRY(cudaGetLastError());
+    return mark_done(st);
+}
+
+__global__ void k_table_export(const Ctl* __restrict__ ctl, const int4* __restrict__ table, long long maxEntries,
+                               int* __restrict__ outEntries, int* __restrict__ outCount)
+{
+    const unsigned T = ctl->tableCount;
+    const unsigned lim = (unsigned)(T < maxEntries ? T : maxEntries);
+    for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < lim; i += gridDim.x * blockDim.x) {
+        const int4 t = table[i];
+        outEntries[4 * i + 0] = t.x; outEntries[4 * i + 1] = t.y; outEntries[4 * i + 2] = t.z; outEntries[4 * i + 3] = t.w;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        outCount[0] = (int)lim;
+        outCount[1] = (int)ctl->tableTrunc;
+        outCount[2] = __float_as_int(ctl->Rtab2);
+    }
+}
+
+int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_mm, float radius, long long max_entries,
+                       int* out_entries, int* out_count, void* stream)
+{
+    g_err.clear();
+    if (!out_entries || !out_count) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_entries / out_count is NULL");
+    if (!(radius >= 0.0f) || !std::isfinite(radius)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "radius must be >= 0");
+    if (max_entries < 1 || max_entries > (1ll << 26)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "max_entries must be in [1, 2^26]");
+    GridP g;
+    int rc = make_grid(dims, spacing_mm, DTA_mm, g);
+    if (rc) return rc;
+    std::lock_guard<std::mutex> lock(g_mu);
+    rc = ensure_device();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    CU_TRY(g_ws.table.need((size_t)max_entries * 16));
+    CU_TRY(g_ws.tmpL.need((size_t)max_entries * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)max_entries * 4));
+    rc = order_after_previous(st);
+    if (rc) return rc;
+    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p);
+    k_offset_table<<<1, TAB_THREADS, 0, st>>>(g, ctl, radius, max_entries, static_cast<int4*>(g_ws.table.p),
+                                              static_cast<unsigned*>(g_ws.tmpL.p), static_cast<unsigned*>(g_ws.tmpIdx.p));
+    k_table_export<<<64, 256, 0, st>>>(ctl, static_cast<const int4*>(g_ws.table.p), max_entries, out_entries, out_count);
+    CU_TRY(cudaGetLastError());
+    g_ws.haveLast = false;
+    return mark_done(st);
+}
+
+int gamma_get_counters(gamma_counters* out_host)
+{
+    g_err.clear();
+    if (!out_host) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_host is NULL");
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (!g_ws.haveLast || !g_ws.ctl.p) return fail(GAMMA_ERR_INVALID_ARGUMENT, "no gamma_eval call to report on");
+    CU_TRY(cudaStreamSynchronize(g_ws.lastStream));
+    Ctl c;
+    CU_TRY(cudaMemcpy(&c, g_ws.ctl.p, sizeof c, cudaMemcpyDeviceToHost));
+    std::memset(out_host, 0, sizeof *out_host);
+    out_host->n_voxels = g_ws.lastN;
+    out_host->n_evaluated = c.nEval;
+    out_host->n_table_search = c.nSearch;
+    out_host->table_entries = c.tableCount;
+    out_host->vertex_visits = (long long)c.visits;
+    union { unsigned u; float f; } cv;
+    cv.u = c.maxKeyBits;
+    out_host->max_key = cv.f;
+    out_host->norm_dose = ordered_to_float(c.normOrd);
+    out_host->table_truncated = (int)c.tableTrunc;
+    return GAMMA_OK;
+}
+
+int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
+{
+    g_err.clear();
+    if (!out_tflops || repeats < 1 || repeats > 1000) return fail(GAMMA_ERR_INVALID_ARGUMENT, "bad probe arguments");
+    std::lock_guard<std::mutex> lock(g_mu);
+    int rc = ensure_device();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    cudaEvent_t a, b;
+    CU_TRY(cudaEventCreate(&a)); CU_TRY(cudaEventCreate(&b));
+    const int grid = g_ws.numSM * 8 * 4, threads = 256;
+    double best = 0.0;
+    for (int r = 0; r < repeats + 1; ++r) {
+        CU_TRY(cudaEventRecord(a, st));
+        k_fp32_probe<<<grid, threads, 0, st>>>(reinterpret_cast<float*>(g_ws.ctl.p) + 15, 0.999f, 1e-3f);
+        CU_TRY(cudaEventRecord(b, st));
+        CU_TRY(cudaEventSynchronize(b));
+        float ms = 0.0f;
+        CU_TRY(cudaEventElapsedTime(&ms, a, b));
+        const double flops = 2.0 * (double)grid * threads * PROBE_ITERS * PROBE_CHAINS;
+        if (r > 0 && ms > 0.0f) best = std::max(best, flops / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    CU_TRY(cudaGetLastError());
+    *out_tflops = best;
+    return GAMMA_OK;
+}
+
+void gamma_release(void)
+{
+    std::lock_guard<std::mutex> lock(g_mu);
+    g_ws.releaseAll();
+}
+
+const char* gamma_last_error_string(void) { return g_err.c_str(); }
+
+const char* gamma_version(void) { return "gamma_b200 0.1 sm_100a"; }
+
+}  // extern "C"
