@@ -1,0 +1,356 @@
+#!/usr/bin/env python3
+"""bench.py -- times the gamma-index hot path (one `gamma_eval` = one step) on the headline workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--case cfg3] [--no-cpu-baseline]
+
+Workload (config.workload): BASELINE.json configs[2], the "3D 2%/2 mm case" that north_star and SURVEY.md
+section 8(d) name as the headline roofline case: 128x128x64 beam phantom at 2.5 mm, (2.0, 1.5, -1.0) mm shift,
+scale 0.97, noise 2 %, criteria 2 %/2 mm global, 10 % cutoff.  Synthetic, seeded (paper_1012_1900_b200/phantoms.py).
+
+value     evaluated reference voxels per second (gamma evaluations/s) over all ranks, inputs resident in HBM
+e2e       the same through gamma_eval_host: pinned HOST buffers in, HOST gamma out, copies inside the timed region
+roofline  dominant kernel, bound "alu": algorithmic FLOPs / its CUDA-event duration,
+          against the plain FP32 FMA peak 148 SM x 128 lanes x 2 x 1.965 GHz; the FFMA-chain rate measured on
+          the box is reported beside it
+cpu_baseline / --impl reference: the CPU oracle (oracle/) as it stands, on the host cores
+
+N > 1: replicas only: every rank runs the same case on its own GPU, no data-path
+collective; timing = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SM_COUNT, FP32_LANES, SM_MAX_MHZ_NOMINAL = 148, 128, 1965.0
+F_CELL_3D, F_CELL_2D = 1911.0, 190.0       # canonical flops per visited cell, frozen in BASELINE.md
+L2_BYTES = 126e6
+
+
+def f32(x):
+    return float(np.float32(x))
+
+
+def work_model(case_name):
+    p = os.path.join(ROOT, "tests", "golden", "work_model.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(case_name)
+    return None
+
+
+# ------------------------------------------------------------------------------------------------------
+# clocks: sampled DURING the timed regions through NVML
+# ------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index):
+        self.samples, self.mask, self.ok, self.max_mhz = [], 0, False, None
+        self._stop, self._active = threading.Event(), threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and all(t.strip().isdigit() for t in vis.split(",")) else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+        self.t = threading.Thread(target=self._run, daemon=True)
+        if self.ok:
+            self.t.start()
+
+    def _run(self):
+        while not self._stop.is_set():
+            if self._active.is_set():
+                try:
+                    self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                    self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:  # noqa: BLE001
+                    try:
+                        self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                    except Exception:  # noqa: BLE001
+                        pass
+                time.sleep(0.002)
+            else:
+                time.sleep(0.0005)
+
+    def __enter__(self):
+        self._active.set()
+        return self
+
+    def __exit__(self, *a):
+        self._active.clear()
+
+    def report(self):
+        self._stop.set()
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + getattr(self, "err", "")]}
+        reasons = [n for b, n in self.REASONS.items() if self.mask & b and n != "gpu_idle"]
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------------
+# the CPU oracle legs (the only places this file touches oracle/)
+# ------------------------------------------------------------------------------------------------------
+def oracle_time(case, voxels, reps):
+    import oracle
+    oracle.build()
+    best = float("inf")
+    sp = [f32(s) for s in case.spacing_mm]
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle.gamma(case.ref, case.eval, case.dims, sp, f32(case.dd), f32(case.dta_mm), case.mode, f32(case.cutoff),
+                     voxels=voxels)
+        best = min(best, time.perf_counter() - t0)
+    return best, oracle.num_threads()
+
+
+def evaluated_voxels(case):
+    ref = case.ref.ravel().astype(np.float64)
+    return np.flatnonzero(ref >= f32(case.cutoff) * ref.max())
+
+
+def cpu_baseline(case):
+    """The oracle on the whole workload (all evaluated voxels), best of 3: a few seconds of all host cores."""
+    keep = evaluated_voxels(case)
+    t, cores = oracle_time(case, keep, 3)
+    return {"value": keep.size / t, "unit": "evaluated reference voxels/s", "cores": cores, "kind": "oracle",
+            "sample": f"all {keep.size} evaluated voxels of {case.name}, shell-form double-precision search, "
+                      f"best of 3 runs ({t:.2f} s each)", "seconds_per_case": t}
+
+
+def run_reference(args, case, rank):
+    if rank != 0:
+        return
+    keep = evaluated_voxels(case)
+    rng = np.random.default_rng([0, 99])
+    # bounded sample per step: calibrate on 4 % of the voxels, then size a step to ~0.25 s
+    probe = np.sort(rng.choice(keep, size=max(1, keep.size // 25), replace=False))
+    t_probe, cores = oracle_time(case, probe, 1)
+    per_voxel = t_probe / probe.size
+    n_step = int(min(keep.size, max(256, 0.25 / per_voxel)))
+    sample = np.sort(rng.choice(keep, size=n_step, replace=False))
+    for _ in range(args.warmup):
+        oracle_time(case, sample, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_time(case, sample, 1)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = n_step / dt
+    unit = "evaluated reference voxels/s"
+    print(json.dumps({
+        "impl": "reference", "metric": "gamma evaluations per second", "value": val, "unit": unit,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": case_desc(case), "sample_voxels_per_step": n_step},
+        "cpu_baseline": {"value": val, "unit": unit, "cores": cores, "kind": "oracle",
+                         "sample": f"{n_step} seeded random evaluated voxels of {case.name} per step "
+                                   f"(of {keep.size}); rate is per voxel, so it extrapolates to the case"},
+        "e2e": {"value": val, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def case_desc(case):
+    nx, ny, nz = case.dims
+    return (f"{case.name}: {nx}x{ny}x{nz} fp32 beam phantom, {case.spacing_mm[0]} mm voxels, "
+            f"{case.dd * 100:g}%/{case.dta_mm:g} mm {'global' if case.mode == 0 else 'local'}, "
+            f"{case.cutoff * 100:g}% cutoff (BASELINE.json configs[2])" if case.name == "cfg3" else
+            f"{case.name}: {nx}x{ny}x{nz}, {case.dd * 100:g}%/{case.dta_mm:g} mm")
+
+
+# ------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--case", default="cfg3")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--presort", type=int, default=0)
+    ap.add_argument("--star-phase", type=int, default=0)
+    ap.add_argument("--lanes", type=int, default=0)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from paper_1012_1900_b200 import phantoms
+    case = phantoms.make_case(args.case)
+
+    if args.impl == "reference":
+        run_reference(args, case, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1012_1900_b200 import binding
+    from paper_1012_1900_b200.binding import GammaOpts
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libgamma_b200 has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    N = case.ref.size
+    opts = GammaOpts(presort=args.presort, star_phase=args.star_phase, lanes_per_voxel=args.lanes)
+    popts = GammaOpts(presort=args.presort, star_phase=args.star_phase, lanes_per_voxel=args.lanes, profile_stages=1)
+    # Rotating input sets larger than L2 (126 MB): every timed step reads buffers that the previous steps have
+    # pushed out of L2.  Each set = ref + eval + out = 12 B/voxel.
+    nsets = int(np.ceil(2.0 * L2_BYTES / (12.0 * N))) + 1
+    ref_h = torch.from_numpy(case.ref.ravel().copy()).pin_memory()
+    ev_h = torch.from_numpy(case.eval.ravel().copy()).pin_memory()
+    out_h = torch.empty(N, dtype=torch.float32).pin_memory()
+    refs = [ref_h.to(dev, non_blocking=True) for _ in range(nsets)]
+    evs = [ev_h.to(dev, non_blocking=True) for _ in range(nsets)]
+    outs = [torch.empty(N, dtype=torch.float32, device=dev) for _ in range(nsets)]
+    stream = torch.cuda.current_stream()
+    args_c = (case.dims, case.spacing_mm, case.dd, case.dta_mm, case.mode, case.cutoff)
+
+    def step(i, o=opts):
+        k = i % nsets
+        binding.gamma_eval_ex(refs[k], evs[k], *args_c, o, outs[k], stream)
+
+    clocks = ClockSampler(local_rank)
+
+    # ---- device-resident timing --------------------------------------------------------------------
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    l0 = binding.gamma_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with clocks:
+        e0.record(stream)
+        for i in range(args.steps):
+            step(args.warmup + i)
+        e1.record(stream)
+        barrier()
+    launches = binding.gamma_launch_count() - l0
+    ms_step = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    cnt = binding.gamma_get_counters()
+    M = cnt["n_evaluated"]
+
+    # ---- per-stage CUDA events (library records them on the launching stream), same launch configuration
+    stage_acc = {}
+    nprof = min(args.steps, 50)
+    barrier()
+    with clocks:
+        for i in range(nprof):
+            step(i, popts)
+            for k, v in binding.gamma_get_stage_times().items():
+                stage_acc.setdefault(k, []).append(v)
+    stages = {k: float(np.mean(v)) for k, v in stage_acc.items()}
+
+    # ---- end to end through the host-buffer entry point ---------------------------------------------
+    for _ in range(3):
+        binding.gamma_eval_host(ref_h, ev_h, *args_c, opts, out_h, stream)
+    barrier()
+    ne2e = max(5, min(args.steps, 50))
+    with clocks:
+        t0 = time.perf_counter()
+        for _ in range(ne2e):
+            binding.gamma_eval_host(ref_h, ev_h, *args_c, opts, out_h, stream)   # synchronises before returning
+        torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / ne2e
+    e2e_s = max_over_ranks(e2e_s)
+
+    # ---- stats on the result (not timed: a6 is reported separately) ---------------------------------
+    hist, summ = binding.gamma_stats(outs[0], 64, 4.0)
+    tstat0, tstat1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tstat0.record(stream)
+    for i in range(20):
+        binding.gamma_stats(outs[i % nsets], 64, 4.0)
+    tstat1.record(stream)
+    torch.cuda.synchronize()
+    stats_ms = tstat0.elapsed_time(tstat1) / 20
+
+    probe_tflops = binding.gamma_fp32_probe(5)
+    clk = clocks.report()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel ------------------------------------------------------------
+    wm = work_model(case.name) or {}
+    ndim = sum(d > 1 for d in case.dims)
+    fcell = F_CELL_3D if ndim == 3 else F_CELL_2D
+    kernel_ms = {"k_prep_star": stages["prep_ms"], "k_table_search": stages["search_ms"]}
+    dom = max(kernel_ms, key=kernel_ms.get)
+    peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ_NOMINAL * 1e6 / 1e12
+    roof = {"bound": "alu", "kernel": dom, "peak": peak, "unit": "TFLOP/s", "traffic": None,
+            "peak_source": "148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and clocks.max.sm)",
+            "ffma_chain_measured_tflops": probe_tflops, "stage_ms": stages}
+    if wm:
+        star_flops = wm["sum_touch"] * fcell
+        search_flops = (wm["sum_Ns"] - wm["sum_touch"]) * fcell
+        alg = {"k_prep_star": star_flops, "k_table_search": search_flops}[dom]
+        roof["algorithmic_flops_per_launch"] = alg
+        roof["achieved"] = alg / (kernel_ms[dom] * 1e-3) / 1e12
+        roof["frac"] = roof["achieved"] / peak
+        total_flops = wm["sum_Ns"] * fcell
+        roof["whole_path"] = {"algorithmic_flops": total_flops, "achieved": total_flops / (ms_step * 1e-3) / 1e12,
+                              "frac": total_flops / (ms_step * 1e-3) / 1e12 / peak}
+    else:
+        roof["achieved"], roof["frac"] = None, None
+
+    line = {
+        "metric": "gamma evaluations per second", "value": world * M / (ms_step * 1e-3),
+        "unit": "evaluated reference voxels/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": case_desc(case), "grid_voxels": N, "evaluated_voxels": M,
+                   "l2_policy": f"{nsets} rotating input/output sets ({nsets * 12 * N / 1e6:.0f} MB) > 126 MB L2",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "options": {"presort": args.presort, "star_phase": args.star_phase, "lanes": args.lanes}},
+        "grid_voxels_per_s": world * N / (ms_step * 1e-3), "ms_per_case": ms_step,
+        "e2e": {"value": world * M / e2e_s, "unit": "evaluated reference voxels/s", "ms_per_case": e2e_s * 1e3,
+                "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N},
+        "gpu_launches": int(launches),
+        "clocks": clk, "roofline": roof,
+        "counters": cnt, "stats": summ, "stats_ms": stats_ms,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(case)
+    elif world > 1:
+        line["cpu_baseline"] = None
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -77,6 +77,9 @@ typedef struct gamma_opts {
                              (8, 16, 24 or 32)                                                             */
     long long table_cap;  /* 0: default (1<<20); max entries of the sorted offset table; past it the search
                              continues by exhaustive enumeration, so results never depend on it            */
+    int profile_stages;   /* 1: record CUDA events between the stages of this call on `stream`, to be read
+                             with gamma_get_stage_times (adds a few event records, no synchronisation)     */
+    int pad_;
 } gamma_opts;
 
 /* gamma_eval with options (opts may be NULL = defaults).  Same contract as gamma_eval. */
@@ -107,7 +110,7 @@ typedef struct gamma_summary {
 
 /*
  * gamma_stats -- pass rate / gamma histogram reduction (BASELINE.json north_star (5); not in the paper).
- *   gamma     DEVICE, n fp32 (NaN = excluded)
+ *   gamma     DEVICE, n fp32 (NaN = excluded); may be NULL when n == 0
  *   nbins     1..4096; bin b counts finite gamma with floor(gamma / hist_max * nbins) == b, the last bin
  *             also takes everything >= hist_max
  *   hist_dev  DEVICE, nbins u64, overwritten;  out_dev: DEVICE, one gamma_summary, overwritten
@@ -151,6 +154,22 @@ typedef struct gamma_counters {
 } gamma_counters;
 int gamma_get_counters(gamma_counters* out_host);
 
+/* Device time of each stage of the last gamma_eval* call made with opts.profile_stages = 1 (CUDA events on
+ * the call's stream).  SYNCHRONISES that stream.  HOST output; milliseconds. */
+typedef struct gamma_stage_times {
+    float norm_ms;   /* a0: clear of the control block + max(ref)                  */
+    float prep_ms;   /* a1 + star phase (k_prep_star)                              */
+    float table_ms;  /* a3: offset table                                           */
+    float sort_ms;   /* a2: radix sort of the search work list                     */
+    float search_ms; /* a4 + a5: table search and write-back                       */
+    float total_ms;  /* first event to last event                                  */
+} gamma_stage_times;
+int gamma_get_stage_times(gamma_stage_times* out_host);
+
+/* Number of CUDA kernels this library has launched in this process so far (host counter; memsets and
+ * copies are not counted). */
+long long gamma_launch_count(void);
+
 /*
  * gamma_fp32_probe -- measures the plain-ALU FP32 rate of the device with independent FFMA chains
  * (the "alu" roofline denominator of bench.py; DESIGN.md section "Roofline").  SYNCHRONISES.
@@ -160,6 +179,10 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream);
 
 /* Frees the workspace.  Safe to call at any time; the next call re-allocates. */
 void gamma_release(void);
+
+/* sizeof(gamma_opts), sizeof(gamma_summary), sizeof(gamma_counters), sizeof(gamma_stage_times) as compiled
+ * into the library, for bindings to check their struct layouts against.  out_host: HOST, 4 ints. */
+void gamma_abi_sizes(int out_host[4]);
 
 /* Description of the last error seen by the calling thread ("" if none). */
 const char* gamma_last_error_string(void);

@@ -17,7 +17,8 @@ from . import build as _build
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
     "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
-    "gamma_fp32_probe", "gamma_release", "gamma_version", "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
+    "gamma_get_stage_times", "gamma_launch_count", "gamma_fp32_probe", "gamma_release", "gamma_version",
+    "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
 
 GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
@@ -25,7 +26,8 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 # every symbol include/gamma_b200.h declares
 exported_symbols = (
     "gamma_eval", "gamma_eval_ex", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table",
-    "gamma_get_counters", "gamma_fp32_probe", "gamma_release", "gamma_last_error_string", "gamma_version",
+    "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_fp32_probe", "gamma_release",
+    "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
 
 
@@ -35,7 +37,13 @@ class GammaError(RuntimeError):
 
 class _COpts(ctypes.Structure):
     _fields_ = [("norm_dose", ctypes.c_float), ("presort", ctypes.c_int), ("star_phase", ctypes.c_int),
-                ("lanes_per_voxel", ctypes.c_int), ("sort_key_bits", ctypes.c_int), ("table_cap", ctypes.c_longlong)]
+                ("lanes_per_voxel", ctypes.c_int), ("sort_key_bits", ctypes.c_int), ("table_cap", ctypes.c_longlong),
+                ("profile_stages", ctypes.c_int), ("pad_", ctypes.c_int)]
+
+
+class _CStageTimes(ctypes.Structure):
+    _fields_ = [("norm_ms", ctypes.c_float), ("prep_ms", ctypes.c_float), ("table_ms", ctypes.c_float),
+                ("sort_ms", ctypes.c_float), ("search_ms", ctypes.c_float), ("total_ms", ctypes.c_float)]
 
 
 class _CSummary(ctypes.Structure):
@@ -60,10 +68,11 @@ class GammaOpts:
     lanes_per_voxel: int = 0  # 1, 8, 32
     sort_key_bits: int = 0    # 8, 16, 24, 32
     table_cap: int = 0
+    profile_stages: int = 0   # 1: record per-stage CUDA events (gamma_get_stage_times)
 
     def _c(self):
         return _COpts(float(self.norm_dose), int(self.presort), int(self.star_phase), int(self.lanes_per_voxel),
-                      int(self.sort_key_bits), int(self.table_cap))
+                      int(self.sort_key_bits), int(self.table_cap), int(self.profile_stages), 0)
 
 
 _lib = None
@@ -90,10 +99,20 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_offset_table.argtypes = [i3, f3, cf, cf, cll, vp, vp, vp]
     lib.gamma_get_counters.argtypes = [ctypes.POINTER(_CCounters)]
     lib.gamma_fp32_probe.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
+    lib.gamma_get_stage_times.argtypes = [ctypes.POINTER(_CStageTimes)]
+    lib.gamma_launch_count.argtypes = []
+    lib.gamma_launch_count.restype = cll
     for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
-                 "gamma_offset_table", "gamma_get_counters", "gamma_fp32_probe"):
+                 "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_fp32_probe"):
         getattr(lib, name).restype = ci
     lib.gamma_release.restype = None
+    lib.gamma_abi_sizes.restype = None
+    lib.gamma_abi_sizes.argtypes = [ctypes.POINTER(ctypes.c_int)]
+    sizes = (ctypes.c_int * 4)()
+    lib.gamma_abi_sizes(sizes)
+    mine = [ctypes.sizeof(c) for c in (_COpts, _CSummary, _CCounters, _CStageTimes)]
+    if list(sizes) != mine:
+        raise GammaError(f"struct layout mismatch between binding.py {mine} and libgamma_b200.so {list(sizes)}")
     lib.gamma_last_error_string.restype = ctypes.c_char_p
     lib.gamma_version.restype = ctypes.c_char_p
     _lib = lib
@@ -225,6 +244,17 @@ def gamma_get_counters() -> dict:
     c = _CCounters()
     _check(lib.gamma_get_counters(ctypes.byref(c)))
     return {k: getattr(c, k) for k, _ in _CCounters._fields_ if k != "pad_"}
+
+
+def gamma_get_stage_times() -> dict:
+    lib = load_library()
+    t = _CStageTimes()
+    _check(lib.gamma_get_stage_times(ctypes.byref(t)))
+    return {k: getattr(t, k) for k, _ in _CStageTimes._fields_}
+
+
+def gamma_launch_count() -> int:
+    return int(load_library().gamma_launch_count())
 
 
 def gamma_fp32_probe(repeats=5, stream=None) -> float:

@@ -65,6 +65,9 @@ struct Workspace {
     Buf hRef, hEval, hOut;         // device staging of gamma_eval_host
     cudaEvent_t done = nullptr;    // orders consecutive calls that share this workspace
     bool havePending = false;
+    cudaEvent_t stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // opts.profile_stages
+    bool haveStages = false;
+    long long launches = 0;        // kernels launched so far (gamma_launch_count)
     int numSM = 0;
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
@@ -75,7 +78,9 @@ struct Workspace {
         Buf* all[] = {&ctl, &key0, &idx0, &key1, &idx1, &tileHist, &table, &tmpL, &tmpIdx, &hRef, &hEval, &hOut};
         for (Buf* b : all) b->release();
         if (done) { cudaEventDestroy(done); done = nullptr; }
-        havePending = false; haveLast = false;
+        for (cudaEvent_t& ev : stage)
+            if (ev) { cudaEventDestroy(ev); ev = nullptr; }
+        havePending = false; haveLast = false; haveStages = false;
     }
 } g_ws;
 
@@ -218,7 +223,7 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
 }
 
 struct Resolved {
-    int presort, star, lanes, keyBits;
+    int presort, star, lanes, keyBits, profile;
     long long tableCap;
     float normDose;
 };
@@ -226,7 +231,9 @@ struct Resolved {
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
     r.presort = 1; r.star = 1; r.lanes = 8; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
+    r.profile = 0;
     if (!o) return GAMMA_OK;
+    r.profile = o->profile_stages == 1;
     if (o->presort < 0 || o->presort > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.presort must be 0, 1 or 2");
     if (o->star_phase < 0 || o->star_phase > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.star_phase must be 0, 1 or 2");
     if (o->presort == 2) r.presort = 0;
@@ -285,13 +292,21 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     EvalP e;
     e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
 
+    g_ws.haveStages = false;
+    if (r.profile)
+        for (cudaEvent_t& ev : g_ws.stage)
+            if (!ev) CU_TRY(cudaEventCreate(&ev));
+#define STAGE_MARK(i) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], st)); } while (0)
+    STAGE_MARK(0);
     CU_TRY(cudaMemsetAsync(ctl, 0, sizeof(Ctl), st));
     const int sm = g_ws.numSM;
     if (!(r.normDose > 0.0f)) {                                          // a0
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 8 ? sm * 8 : blocks));
         k_max_ref<<<grid, 256, 0, st>>>(ref, (int)N, ctl);
+        ++g_ws.launches;
     }
+    STAGE_MARK(1);
     {                                                                    // a1 + star
         long long tiles = (N + PREP_TILE - 1) / PREP_TILE;
         int grid = (int)(tiles > sm * 16 ? sm * 16 : tiles);
@@ -299,16 +314,22 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             k_prep_star<true><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
         else
             k_prep_star<false><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
+        ++g_ws.launches;
     }
+    STAGE_MARK(2);
     // a3: offset table out to the largest key
     k_offset_table<<<1, TAB_THREADS, 0, st>>>(g, ctl, -1.0f, r.tableCap, static_cast<int4*>(g_ws.table.p),
                                               static_cast<unsigned*>(g_ws.tmpL.p), static_cast<unsigned*>(g_ws.tmpIdx.p));
+    ++g_ws.launches;
+    STAGE_MARK(3);
     const unsigned *lk = k0, *li = i0;
     if (r.presort) {                                                     // a2
         int where = radix_sort_enqueue(k0, i0, k1, i1, &ctl->nSearch, N, 32 - r.keyBits, 32,
                                        static_cast<unsigned*>(g_ws.tileHist.p), st);
+        g_ws.launches += 3 * (r.keyBits / 8);
         if (where) { lk = k1; li = i1; }
     }
+    STAGE_MARK(4);
     {                                                                    // a4 + a5
         const int grid = sm * 8;
         const int4* tab = static_cast<const int4*>(g_ws.table.p);
@@ -318,7 +339,11 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             k_table_search<8><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
         else
             k_table_search<32><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
+        ++g_ws.launches;
     }
+    STAGE_MARK(5);
+#undef STAGE_MARK
+    g_ws.haveStages = r.profile != 0;
     CU_TRY(cudaGetLastError());
     rc = mark_done(st);
     if (rc) return rc;
@@ -391,8 +416,9 @@ int gamma_stats(const float* gamma, long long n, int nbins, float hist_max, unsi
                 gamma_summary* out_dev, void* stream)
 {
     g_err.clear();
-    if (!gamma || !hist_dev || !out_dev) return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma / hist_dev / out_dev is NULL");
     if (n < 0 || n >= (1ll << 40)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "n out of range");
+    if ((!gamma && n > 0) || !hist_dev || !out_dev)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma / hist_dev / out_dev is NULL");
     if (nbins < 1 || nbins > STATS_MAX_BINS) return fail(GAMMA_ERR_INVALID_ARGUMENT, "nbins must be in [1, 4096]");
     if (!(hist_max > 0.0f) || !std::isfinite(hist_max)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "hist_max must be > 0");
     std::lock_guard<std::mutex> lock(g_mu);
@@ -404,7 +430,9 @@ int gamma_stats(const float* gamma, long long n, int nbins, float hist_max, unsi
         long long blocks = (n + STATS_THREADS * 8 - 1) / (STATS_THREADS * 8);
         int grid = (int)(blocks > g_ws.numSM * 8 ? g_ws.numSM * 8 : blocks);
         k_stats<<<grid, STATS_THREADS, nbins * sizeof(unsigned), st>>>(gamma, n, nbins, (float)nbins / hist_max, hist_dev, out_dev);
+        ++g_ws.launches;
     }
+    ++g_ws.launches;
     CU_TRY(cudaGetLastError());
     return GAMMA_OK;
 }
@@ -434,6 +462,7 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
     unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *v1 = static_cast<unsigned*>(g_ws.idx1.p);
     int where = radix_sort_enqueue(keys, vals, k1, v1, &ctl->sortN, n, begin_bit, end_bit,
                                    static_cast<unsigned*>(g_ws.tileHist.p), st);
+    g_ws.launches += 1 + 3 * ((end_bit - begin_bit) / 8);
     if (where) {
         CU_TRY(cudaMemcpyAsync(keys, k1, n * 4, cudaMemcpyDeviceToDevice, st));
         CU_TRY(cudaMemcpyAsync(vals, v1, n * 4, cudaMemcpyDeviceToDevice, st));
@@ -481,6 +510,7 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     k_offset_table<<<1, TAB_THREADS, 0, st>>>(g, ctl, radius, max_entries, static_cast<int4*>(g_ws.table.p),
                                               static_cast<unsigned*>(g_ws.tmpL.p), static_cast<unsigned*>(g_ws.tmpIdx.p));
     k_table_export<<<64, 256, 0, st>>>(ctl, static_cast<const int4*>(g_ws.table.p), max_entries, out_entries, out_count);
+    g_ws.launches += 2;
     CU_TRY(cudaGetLastError());
     g_ws.haveLast = false;
     return mark_done(st);
@@ -509,6 +539,27 @@ int gamma_get_counters(gamma_counters* out_host)
     return GAMMA_OK;
 }
 
+int gamma_get_stage_times(gamma_stage_times* out_host)
+{
+    g_err.clear();
+    if (!out_host) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_host is NULL");
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (!g_ws.haveStages) return fail(GAMMA_ERR_INVALID_ARGUMENT, "last gamma_eval call did not set opts.profile_stages");
+    CU_TRY(cudaEventSynchronize(g_ws.stage[5]));
+    float ms[5];
+    for (int i = 0; i < 5; ++i) CU_TRY(cudaEventElapsedTime(&ms[i], g_ws.stage[i], g_ws.stage[i + 1]));
+    out_host->norm_ms = ms[0]; out_host->prep_ms = ms[1]; out_host->table_ms = ms[2];
+    out_host->sort_ms = ms[3]; out_host->search_ms = ms[4];
+    CU_TRY(cudaEventElapsedTime(&out_host->total_ms, g_ws.stage[0], g_ws.stage[5]));
+    return GAMMA_OK;
+}
+
+long long gamma_launch_count(void)
+{
+    std::lock_guard<std::mutex> lock(g_mu);
+    return g_ws.launches;
+}
+
 int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
 {
     g_err.clear();
@@ -525,6 +576,7 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
     for (int r = 0; r < repeats + 1; ++r) {
         CU_TRY(cudaEventRecord(a, st));
         k_fp32_probe<<<grid, threads, 0, st>>>(reinterpret_cast<float*>(g_ws.ctl.p) + 15, 0.999f, 1e-3f);
+        ++g_ws.launches;
         CU_TRY(cudaEventRecord(b, st));
         CU_TRY(cudaEventSynchronize(b));
         float ms = 0.0f;
@@ -542,6 +594,13 @@ void gamma_release(void)
 {
     std::lock_guard<std::mutex> lock(g_mu);
     g_ws.releaseAll();
+}
+
+void gamma_abi_sizes(int out_host[4])
+{
+    if (!out_host) return;
+    out_host[0] = (int)sizeof(gamma_opts); out_host[1] = (int)sizeof(gamma_summary);
+    out_host[2] = (int)sizeof(gamma_counters); out_host[3] = (int)sizeof(gamma_stage_times);
 }
 
 const char* gamma_last_error_string(void) { return g_err.c_str(); }

@@ -1,0 +1,334 @@
+"""Parity of the CUDA path (through the C-ABI of libgamma_b200.so) with the CPU oracle, element by element on
+the same seeded inputs.  Needs a B200: every test is marked `gpu`.
+
+Bar (BASELINE.json north_star): |gamma_gpu - gamma_oracle| <= 1e-4 absolute per voxel, identical NaN
+(excluded) masks, and the gamma <= 1 pass count exact except for voxels within 1e-4 of 1.  Integer results
+(sort, histogram, counts, table entries) are bit-exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1012_1900_b200 import binding, phantoms
+from paper_1012_1900_b200.binding import GammaOpts
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+def f32(x):
+    return float(np.float32(x))
+
+
+def gpu_gamma(ref, ev, dims, sp, dd, dta, mode=0, cutoff=0.1, opts=None, plain=False):
+    r = torch.from_numpy(np.ascontiguousarray(ref, dtype=np.float32).ravel()).cuda()
+    e = torch.from_numpy(np.ascontiguousarray(ev, dtype=np.float32).ravel()).cuda()
+    if plain:
+        out = binding.gamma_eval(r, e, dims, sp, dd, dta, mode, cutoff)
+    else:
+        out = binding.gamma_eval_ex(r, e, dims, sp, dd, dta, mode, cutoff, opts)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+def cpu_gamma(oracle_mod, ref, ev, dims, sp, dd, dta, mode=0, cutoff=0.1, norm_dose=0.0, voxels=None):
+    # the oracle gets the float32-rounded criteria the boundary receives (same problem statement)
+    return oracle_mod.gamma(np.asarray(ref, dtype=np.float32), np.asarray(ev, dtype=np.float32), dims,
+                            [f32(s) for s in sp], f32(dd), f32(dta), mode, f32(cutoff), f32(norm_dose),
+                            voxels=voxels)
+
+
+def assert_parity(g_gpu, g_cpu, what=""):
+    nan_g, nan_c = np.isnan(g_gpu), np.isnan(g_cpu)
+    assert np.array_equal(nan_g, nan_c), f"{what}: excluded masks differ at {np.flatnonzero(nan_g != nan_c)[:8]}"
+    m = ~nan_c
+    if m.any():
+        err = np.abs(g_gpu[m] - g_cpu[m])
+        worst = int(np.argmax(err))
+        assert err[worst] <= TOL, (f"{what}: max |dgamma| = {err[worst]:.3e} at evaluated voxel #{worst} "
+                                   f"(gpu {g_gpu[m][worst]:.7f}, oracle {g_cpu[m][worst]:.7f})")
+        sure = np.abs(g_cpu[m] - 1.0) > TOL
+        assert np.array_equal(g_gpu[m][sure] <= 1.0, g_cpu[m][sure] <= 1.0), f"{what}: pass/fail differs"
+    return float(np.abs(g_gpu[m] - g_cpu[m]).max()) if m.any() else 0.0
+
+
+# ----------------------------------------------------------------------------------------------------
+# the BASELINE.json configs, full grids, default options = the configuration bench.py times
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_small", "cfg2", "cfg3", "cfg4_coarse"])
+def test_full_grid_parity_default_options(oracle_mod, name):
+    c = phantoms.make_case(name)
+    g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, plain=True)
+    o = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    err = assert_parity(g, o, name)
+    cnt = binding.gamma_get_counters()
+    assert cnt["n_voxels"] == c.ref.size and cnt["n_evaluated"] == int((~np.isnan(o)).sum())
+    print(f"{name}: max|dgamma| {err:.2e}, M {cnt['n_evaluated']}, table search {cnt['n_table_search']}")
+
+
+def _sample_voxels(c, n_random, n_top, seed):
+    """Seeded sample of evaluated voxels + the voxels with the largest |DD| (deepest searches): chosen from the
+    inputs alone."""
+    ref = c.ref.ravel().astype(np.float64)
+    keep = np.flatnonzero(ref >= f32(c.cutoff) * ref.max())
+    rng = np.random.default_rng([seed, 77])
+    pick = rng.choice(keep, size=min(n_random, keep.size), replace=False)
+    dd = np.abs(c.eval.ravel().astype(np.float64) - ref)[keep]
+    top = keep[np.argsort(dd)[-n_top:]]
+    return np.unique(np.concatenate([pick, top]))
+
+
+@pytest.mark.parametrize("name,n_random,n_top", [("cfg4_fine", 60000, 2000), ("cfg5", 40000, 3000)])
+def test_large_grids_sampled_parity(oracle_mod, name, n_random, n_top):
+    """Full-size configs 4 (1.25 mm) and 5 (load-imbalance stress): the oracle computes a seeded sample of voxels
+    one by one; the NaN mask is checked on the whole grid from its definition."""
+    c = phantoms.make_case(name)
+    g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, plain=True)
+    vox = _sample_voxels(c, n_random, n_top, 0)
+    o = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, voxels=vox)
+    err = assert_parity(g[vox], o, name)
+    ref = c.ref.ravel().astype(np.float64)
+    assert np.array_equal(np.isnan(g), ref < f32(c.cutoff) * ref.max())
+    fin = g[~np.isnan(g)]
+    g0 = np.abs(c.eval.ravel().astype(np.float64) - ref)[~np.isnan(g)] / (f32(c.dd) * ref.max())
+    assert np.all(fin <= g0 + TOL) and np.all(fin >= 0.0)                  # gamma <= gamma_0 at any size
+    print(f"{name}: max|dgamma| {err:.2e} over {vox.size} sampled voxels, max gamma {fin.max():.3f}")
+
+
+def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
+    """Config 5 is run with and without the voxel pre-sort (Table 2) and with the paper's
+    thread-per-voxel mapping: the candidate set is the same, so gamma is bit-identical."""
+    c = phantoms.make_case("cfg5")
+    base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    for o in (GammaOpts(presort=2), GammaOpts(lanes_per_voxel=1), GammaOpts(lanes_per_voxel=1, presort=2),
+              GammaOpts(lanes_per_voxel=32)):
+        g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
+        assert np.array_equal(np.isnan(g), np.isnan(base))
+        assert np.array_equal(g[~np.isnan(g)], base[~np.isnan(base)]), o
+
+
+# ----------------------------------------------------------------------------------------------------
+# every option / kernel variant on grids that span several tiles with ragged tails
+# ----------------------------------------------------------------------------------------------------
+VARIANTS = [
+    GammaOpts(), GammaOpts(star_phase=2), GammaOpts(presort=2), GammaOpts(lanes_per_voxel=1),
+    GammaOpts(lanes_per_voxel=32), GammaOpts(star_phase=2, lanes_per_voxel=1, presort=2),
+    GammaOpts(sort_key_bits=8), GammaOpts(sort_key_bits=32), GammaOpts(table_cap=1),
+    GammaOpts(table_cap=7, star_phase=2), GammaOpts(table_cap=40, lanes_per_voxel=32),
+    GammaOpts(table_cap=3, lanes_per_voxel=1),
+]
+
+
+@pytest.mark.parametrize("vi", range(len(VARIANTS)))
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_small"])
+def test_option_variants_small_cases(oracle_mod, name, vi):
+    c = phantoms.make_case(name)
+    g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, VARIANTS[vi])
+    o = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    assert_parity(g, o, f"{name} {VARIANTS[vi]}")
+
+
+@pytest.mark.parametrize("vi", [1, 3, 4, 5, 8, 10])
+def test_option_variants_cfg3(oracle_mod, vi):
+    c = phantoms.make_case("cfg3")
+    g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, VARIANTS[vi])
+    o = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    assert_parity(g, o, f"cfg3 {VARIANTS[vi]}")
+
+
+def _random_case(shape_xyz, sp, seed, smooth=True, amp=0.15):
+    """Random reference in [0.2, 2.0], evaluation = reference + perturbation: deep searches, border voxels."""
+    nx, ny, nz = shape_xyz
+    rng = np.random.default_rng([seed, 5])
+    ref = rng.uniform(0.2, 2.0, size=(nz, ny, nx))
+    if smooth:
+        from scipy.ndimage import gaussian_filter
+        ref = gaussian_filter(ref, 1.0, mode="nearest")
+        ref *= 2.0 / ref.max()
+    ev = ref * rng.uniform(0.9, 1.1) + rng.normal(0.0, amp, size=ref.shape)
+    return ref.astype(np.float32), ev.astype(np.float32)
+
+
+@pytest.mark.parametrize("dims,sp,dd,dta,mode,cutoff,seed", [
+    ((37, 29, 11), (2.0, 3.0, 2.5), 0.03, 3.0, 0, 0.1, 1),        # ragged, anisotropic
+    ((37, 29, 11), (2.0, 3.0, 2.5), 0.02, 5.0, 1, 0.0, 2),        # local mode, no cutoff, wide DTA
+    ((5, 4, 3), (1.0, 1.0, 1.0), 0.01, 6.0, 0, 0.0, 3),           # search reaches every cell of the grid
+    ((2, 2, 2), (2.5, 2.5, 2.5), 0.03, 3.0, 0, 0.0, 4),           # one cell
+    ((64, 1, 33), (2.5, 2.5, 1.0), 0.03, 3.0, 0, 0.2, 5),         # 2D with the y axis dropped
+    ((1, 50, 41), (1.0, 2.0, 3.0), 0.02, 2.0, 1, 0.1, 6),         # 2D with the x axis dropped
+    ((300, 1, 1), (1.5, 1.0, 1.0), 0.03, 3.0, 0, 0.0, 7),         # 1D polyline
+    ((1, 1, 17), (1.0, 1.0, 0.7), 0.05, 1.0, 0, 0.0, 8),          # 1D along z
+    ((130, 3, 2), (0.5, 4.0, 4.0), 0.03, 3.0, 0, 0.05, 9),        # thin slab, strongly anisotropic
+])
+@pytest.mark.parametrize("opts", [GammaOpts(), GammaOpts(star_phase=2, lanes_per_voxel=1), GammaOpts(table_cap=5)])
+def test_random_grids_edge_shapes(oracle_mod, dims, sp, dd, dta, mode, cutoff, seed, opts):
+    ref, ev = _random_case(dims, sp, seed)
+    g = gpu_gamma(ref, ev, dims, sp, dd, dta, mode, cutoff, opts)
+    o = cpu_gamma(oracle_mod, ref, ev, dims, sp, dd, dta, mode, cutoff)
+    assert_parity(g, o, f"{dims} {opts}")
+
+
+def test_rough_random_field_deep_search(oracle_mod):
+    """White-noise doses: gamma_0 up to ~30, so the table grows to thousands of entries and border handling,
+    the early exit and the table order all matter."""
+    dims, sp = (40, 36, 20), (2.5, 2.5, 2.5)
+    ref, ev = _random_case(dims, sp, 11, smooth=False, amp=0.6)
+    for opts in (GammaOpts(), GammaOpts(lanes_per_voxel=32, star_phase=2), GammaOpts(table_cap=64)):
+        g = gpu_gamma(ref, ev, dims, sp, 0.02, 2.0, 0, 0.0, opts)
+        o = cpu_gamma(oracle_mod, ref, ev, dims, sp, 0.02, 2.0, 0, 0.0)
+        assert_parity(g, o, f"rough {opts}")
+
+
+# ----------------------------------------------------------------------------------------------------
+# closed forms on the device (the same pins the oracle has, Eq. 1)
+# ----------------------------------------------------------------------------------------------------
+def test_identical_grids_flat_offset_and_ramp_closed_form():
+    c = phantoms.make_case("cfg2_small")
+    g = gpu_gamma(c.ref, c.ref, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1)
+    assert np.all(g[~np.isnan(g)] == 0.0)
+    flat = np.full((6, 7, 8), 1.5, dtype=np.float32)
+    g = gpu_gamma(flat, flat + np.float32(0.06), (8, 7, 6), (2, 2, 2), 0.03, 3.0, 0, 0.0)
+    assert np.allclose(g, (f32(1.5 + 0.06) - 1.5) / (f32(0.03) * 1.5), atol=1e-5)
+    # linear ramp shifted by s: gamma = |g.s| / sqrt(dD^2 + dta^2 |g|^2) away from the border
+    n, h, dta = 24, 2.5, 3.0
+    grad, s = np.array([0.05, -0.02, 0.03]), np.array([1.0, -0.7, 0.5])
+    ax = np.arange(n) * h
+    Z, Y, X = np.meshgrid(ax, ax, ax, indexing="ij")
+    ramp = 10.0 + grad[0] * X + grad[1] * Y + grad[2] * Z
+    ev = ramp - grad @ s
+    dnorm = float(np.float32(ramp).max())
+    dD = 0.06
+    g = gpu_gamma(ramp, ev, (n, n, n), (h, h, h), dD / dnorm, dta, 0, 0.0).reshape(n, n, n)
+    expect = abs(grad @ s) / np.sqrt(dD ** 2 + dta ** 2 * (grad @ grad))
+    assert np.allclose(g[3:-3, 3:-3, 3:-3], expect, atol=5e-5)     # fp32 doses near 10 Gy: ulp 1e-6 / dD
+
+
+def test_all_excluded_empty_work_list_and_nonfinite_inputs():
+    c = phantoms.make_case("cfg2_small")
+    g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.5, GammaOpts(norm_dose=100.0))
+    assert np.all(np.isnan(g))                                    # every voxel below the cutoff: M = 0
+    assert binding.gamma_get_counters()["n_evaluated"] == 0
+    ev = c.eval.copy()
+    ev[5, 7, 9] = np.nan
+    ev[8, 3, 2] = np.inf
+    g = gpu_gamma(c.ref, ev, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1)      # must not hang or fault
+    assert g.shape == (c.ref.size,)
+
+
+def test_norm_dose_option_and_cutoff_decision(oracle_mod):
+    c = phantoms.make_case("cfg2_small")
+    for nd in (1.7, 2.5):
+        g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1, GammaOpts(norm_dose=nd))
+        o = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1, norm_dose=nd)
+        assert_parity(g, o, f"norm_dose {nd}")
+
+
+# ----------------------------------------------------------------------------------------------------
+# host-buffer entry point, streams, determinism
+# ----------------------------------------------------------------------------------------------------
+def test_gamma_eval_host_streams_and_determinism():
+    c = phantoms.make_case("cfg2_small")
+    base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    rh = torch.from_numpy(c.ref.ravel().copy()).pin_memory()
+    eh = torch.from_numpy(c.eval.ravel().copy()).pin_memory()
+    out = binding.gamma_eval_host(rh, eh, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    assert np.array_equal(out.numpy().astype(np.float64), base, equal_nan=True)
+    s = torch.cuda.Stream()
+    r, e = rh.cuda(), eh.cuda()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        o1 = binding.gamma_eval(r, e, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+        o2 = binding.gamma_eval(r, e, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, stream=s)
+    o3 = binding.gamma_eval(r, e, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)   # other stream, ordered
+    torch.cuda.synchronize()
+    for o in (o1, o2, o3):
+        assert np.array_equal(o.cpu().numpy().astype(np.float64), base, equal_nan=True)
+    n0 = binding.gamma_launch_count()
+    binding.gamma_eval(r, e, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    assert binding.gamma_launch_count() > n0
+    binding.gamma_release()                                                                # re-allocates on demand
+    o4 = binding.gamma_eval(r, e, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    torch.cuda.synchronize()
+    assert np.array_equal(o4.cpu().numpy().astype(np.float64), base, equal_nan=True)
+
+
+def test_stage_times_are_reported():
+    c = phantoms.make_case("cfg2_small")
+    gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, GammaOpts(profile_stages=1))
+    t = binding.gamma_get_stage_times()
+    assert t["total_ms"] > 0 and t["prep_ms"] > 0 and t["search_ms"] >= 0
+    assert abs(sum(t[k] for k in ("norm_ms", "prep_ms", "table_ms", "sort_ms", "search_ms")) - t["total_ms"]) < 0.05
+
+
+# ----------------------------------------------------------------------------------------------------
+# the other entry points: stats (5), radix sort (3), offset table (1)
+# ----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,nbins,hmax", [(0, 16, 4.0), (1, 1, 1.0), (1000, 64, 4.0), (2_500_003, 4096, 3.0),
+                                          (300_001, 100, 0.5)])
+def test_gamma_stats_against_definition(n, nbins, hmax):
+    from oracle import aux_oracle
+    rng = np.random.default_rng([n, nbins])
+    g = rng.gamma(2.0, 0.4, size=n).astype(np.float32)
+    g[rng.random(n) < 0.3] = np.nan
+    if n > 10:
+        g[:4] = [0.0, 1.0, hmax, np.float32(hmax) * 2]
+    t = torch.from_numpy(g).cuda() if n else torch.empty(0, dtype=torch.float32, device="cuda")
+    hist, s = binding.gamma_stats(t, nbins, hmax)
+    eh, es = aux_oracle.stats(g, nbins, hmax)
+    assert np.array_equal(hist.cpu().numpy(), eh)                                 # integer work: exact
+    for k in ("n_eval", "n_pass", "n_nan"):
+        assert s[k] == es[k], k
+    assert s["max_gamma"] == es["max_gamma"]
+    assert s["sum_gamma"] == pytest.approx(es["sum_gamma"], rel=1e-12, abs=1e-12)
+    assert s["sum_gamma3"] == pytest.approx(es["sum_gamma3"], rel=1e-12, abs=1e-12)
+
+
+@pytest.mark.parametrize("n", [1, 31, 2048, 2049, 100_003, 3_000_001])
+@pytest.mark.parametrize("bits", [(0, 32), (16, 32), (8, 16), (24, 32)])
+def test_radix_sort_pairs_bit_exact(n, bits):
+    from oracle import aux_oracle
+    rng = np.random.default_rng([n, bits[0]])
+    if n % 2:
+        keys = np.abs(rng.normal(0, 3, size=n)).astype(np.float32).view(np.uint32)     # float bit patterns
+    else:
+        keys = rng.integers(0, 2 ** 32, size=n, dtype=np.uint64).astype(np.uint32)
+        keys[: n // 3] &= 0x00FF00FF                                                    # many ties
+    vals = np.arange(n, dtype=np.uint32)
+    k = torch.from_numpy(keys.view(np.int32).copy()).cuda()
+    v = torch.from_numpy(vals.view(np.int32).copy()).cuda()
+    binding.gamma_sort_pairs(k, v, bits[0], bits[1])
+    ek, evv = aux_oracle.sort_pairs(keys, vals, bits[0], bits[1])
+    assert np.array_equal(k.cpu().numpy().view(np.uint32), ek)
+    assert np.array_equal(v.cpu().numpy().view(np.uint32), evv)                          # stable: unique answer
+
+
+@pytest.mark.parametrize("dims,sp,dta,R", [
+    ((128, 128, 64), (2.5, 2.5, 2.5), 2.0, 3.0), ((128, 128, 64), (2.5, 2.5, 2.5), 3.0, 10.0),
+    ((64, 64, 1), (2.5, 2.5, 2.5), 3.0, 10.0), ((9, 7, 5), (2.0, 3.0, 2.5), 3.0, 50.0),
+    ((192, 192, 96), (2.0, 2.0, 2.0), 1.0, 0.0), ((40, 1, 1), (1.0, 1.0, 1.0), 1.0, 7.5),
+])
+def test_offset_table_against_definition(dims, sp, dta, R):
+    from oracle import aux_oracle
+    ent, trunc, r2 = binding.gamma_offset_table(dims, sp, dta, R)
+    ent = ent.cpu().numpy()
+    exp = aux_oracle.offset_table(dims, [f32(s) for s in sp], f32(dta), f32(R))
+    assert not trunc and r2 == pytest.approx(f32(R) ** 2, rel=1e-6)
+    L2 = ent[:, 0].copy().view(np.float32).astype(np.float64)
+    assert np.all(np.diff(L2) >= 0)                                  # ascending: what the early exit relies on
+    # entries whose L is not within rounding of R are decided identically; compare as sets, and L^2 by value
+    got = {tuple(int(x) for x in row[1:]): l2 for row, l2 in zip(ent, L2)}
+    want = {t[1:]: t[0] for t in exp}
+    edge = {m for m, l2 in {**want, **got}.items() if abs(np.sqrt(l2) - f32(R)) <= 1e-5 * max(1.0, R)}
+    assert set(got) - edge == set(want) - edge
+    for m in set(got) & set(want):
+        assert got[m] == pytest.approx(want[m], rel=1e-6, abs=1e-12)
+
+
+def test_offset_table_truncation_is_flagged():
+    ent, trunc, r2 = binding.gamma_offset_table((128, 128, 64), (2.5, 2.5, 2.5), 2.0, 20.0, max_entries=500)
+    assert trunc and ent.shape[0] <= 500 and r2 < 400.0
+
+
+def test_fp32_probe_runs():
+    assert binding.gamma_fp32_probe(2) > 1.0          # TFLOP/s; a B200 is far above 1
