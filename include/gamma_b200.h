@@ -57,7 +57,8 @@ extern "C" {
  *                    (reading 10; the comparison is done in double so that it is decided identically
  *                    everywhere).  Excluded voxels still serve as evaluation points of their neighbours.
  *   out_gamma        DEVICE, N fp32, written entirely
- *   stream           cudaStream_t
+ *   stream           cudaStream_t.  The offset table is built on a library-owned side stream that forks from and
+ *                    joins `stream` through events (legal under stream capture).
  */
 int gamma_eval(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
                float DTA_mm, int mode, float low_dose_cutoff, float* out_gamma, void* stream);
@@ -65,16 +66,17 @@ int gamma_eval(const float* ref, const float* eval, const int dims[3], const flo
 /* Options of gamma_eval_ex / gamma_eval_host.  Zero-initialise, then set what differs. */
 typedef struct gamma_opts {
     float norm_dose;      /* D_norm; <= 0: max(ref), found on the device                                  */
-    int presort;          /* 0: default (= 1); 1: radix-sort the search work list by its key before the
-                             search (A2 step 3); 2: no sort (Table 2's "without sorting")   */
+    int presort;          /* pre-sort of the search work list (A2 step 3).  0: default (= 1);
+                             1: one-pass MSD radix sort on the 8-bit key digit (32 steps per octave of the key);
+                             2: no sort (Table 2's "without sorting"); 3: full LSD radix sort of the
+                             `sort_key_bits` most significant key bits                                     */
     int star_phase;       /* 0: default (= 1); 1: interior voxels first try the 75 faces touching the voxel
                              and finish there when gamma_star <= distance to the rest of the surface;
                              2: off -- every voxel goes through the table search with key |DD|/dD, as in
                              Algorithm A2                                               */
     int lanes_per_voxel;  /* 0: default (= 8); 1, 8 or 32 lanes cooperate on one reference voxel in the
                              table search (1 = the paper's thread-per-voxel mapping)        */
-    int sort_key_bits;    /* 0: default (= 16); number of most significant key bits the presort orders by
-                             (8, 16, 24 or 32)                                                             */
+    int sort_key_bits;    /* presort = 3 only.  0: default (= 16); 8, 16, 24 or 32 most significant key bits   */
     long long table_cap;  /* 0: default (1<<20); max entries of the sorted offset table; past it the search
                              continues by exhaustive enumeration, so results never depend on it            */
     int profile_stages;   /* 1: record CUDA events between the stages of this call on `stream`, to be read
@@ -129,7 +131,8 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
 
 /*
  * gamma_offset_table -- the sorted offset table {n, L_n} (Algorithm A1 steps 2-3; A2
- * steps 4-5) with the cell bound of reading 4.  By the symmetry L(o) = L(-o-1) the
+ * steps 4-5) with the cell bound of reading 4.  (Inside gamma_eval the radius is the
+ * paper's max|DD|/dD over the grid, A1 step 1.)  By the symmetry L(o) = L(-o-1) the
  * table lists the octant m >= 0 only: entry (m, L^2), L^2 = sum_a (m_a h_a)^2, h = spacing/DTA, for every
  * m with m_a <= dims_a - 1 and L < radius, sorted ascending by (L^2 as fp32, then m_x + bx*(m_y + by*m_z));
  * the search expands each entry into its 8 (4 in 2D) offsets o_a in {m_a, -m_a-1}.
@@ -157,12 +160,12 @@ int gamma_get_counters(gamma_counters* out_host);
 /* Device time of each stage of the last gamma_eval* call made with opts.profile_stages = 1 (CUDA events on
  * the call's stream).  SYNCHRONISES that stream.  HOST output; milliseconds. */
 typedef struct gamma_stage_times {
-    float norm_ms;   /* a0: clear of the control block + max(ref)                  */
-    float prep_ms;   /* a1 + star phase (k_prep_star)                              */
-    float table_ms;  /* a3: offset table                                           */
-    float sort_ms;   /* a2: radix sort of the search work list                     */
-    float search_ms; /* a4 + a5: table search and write-back                       */
-    float total_ms;  /* first event to last event                                  */
+    float norm_ms;   /* a0 + A1 step 1: max(ref), max|DD| (k_norm)                               */
+    float prep_ms;   /* a1 + star phase (k_prep_star)                                            */
+    float table_ms;  /* a3: offset table, on the side stream, CONCURRENT with prep_ms/sort_ms    */
+    float sort_ms;   /* a2: presort of the search work list                                      */
+    float search_ms; /* a4 + a5: join with the side stream, table search and write-back          */
+    float total_ms;  /* first event to last event on `stream` = norm + prep + sort + search      */
 } gamma_stage_times;
 int gamma_get_stage_times(gamma_stage_times* out_host);
 

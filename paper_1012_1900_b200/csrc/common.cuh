@@ -30,21 +30,36 @@ struct EvalP {
 };
 
 // Device control block: everything the pipeline decides on the device (no host sync on the path).
+// Two slots alternate between consecutive gamma_eval calls: the first kernel of call i clears the slot of
+// call i+1, so no memset node sits on the critical path.
+constexpr int KEY_DIGITS = 256;
 struct Ctl {
     unsigned normOrd;      // max(ref) as an order-preserving uint
-    unsigned maxKeyBits;   // largest key of the search list (bits of a non-negative float)
+    unsigned maxAbsDD;     // bits of max |D_r - D_e| over all voxels (non-negative float): A1 step 1
+    unsigned maxRatio;     // local mode: bits of max |D_r - D_e| / D_r over voxels with D_r > 0
+    unsigned maxKeyBits;   // largest key of the search list (bits of a non-negative float), diagnostic
     unsigned nEval;        // M: evaluated voxels
     unsigned nSearch;      // voxels in the table-search work list
     unsigned workCounter;  // dynamic work fetch of the table search
+    unsigned tileCounter;  // dynamic chunk fetch of the prep/star kernel
     unsigned tableCount;   // octant entries in the offset table
     unsigned tableTrunc;   // 1 if the table was cut at table_cap
     float Rtab2;           // squared radius the table covers
     int box[3];            // table box: m_a in [0, box_a)
-    unsigned pad0;
-    unsigned long long visits;  // owner vertices evaluated by the table search
     unsigned sortN;        // element count for gamma_sort_pairs
-    unsigned pad1;
+    unsigned pad0;
+    unsigned long long visits;       // owner vertices evaluated by the table search
+    unsigned hist[KEY_DIGITS];       // digit histogram of the search list (bucket presort)
+    unsigned cursor[KEY_DIGITS];     // scatter cursors of the bucket presort
 };
+
+// Monotone 8-bit quantisation of a non-negative key: 32 steps per octave over [2^-3, 2^5), clamped.
+// This is the digit of the one-pass MSD radix presort of the search work list.
+__device__ __forceinline__ unsigned key_digit(float key)
+{
+    const int d = (int)(__float_as_uint(key) >> 18) - ((127 - 3) << 5);
+    return (unsigned)min(max(d, 0), KEY_DIGITS - 1);
+}
 
 __host__ __device__ inline unsigned float_to_ordered(float f)
 {

@@ -65,7 +65,13 @@ struct Workspace {
     Buf hRef, hEval, hOut;         // device staging of gamma_eval_host
     cudaEvent_t done = nullptr;    // orders consecutive calls that share this workspace
     bool havePending = false;
-    cudaEvent_t stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // opts.profile_stages
+    cudaEvent_t stage[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // opts.profile_stages
+    cudaStream_t aux = nullptr;    // side stream: the offset table is built while k_prep_star runs
+    cudaEvent_t evFork = nullptr, evJoin = nullptr;
+    void* ctlOwner = nullptr;      // ctl.p the flags below refer to
+    bool ctlClean = false;         // both call slots of the control block are known to be zero / being zeroed
+    int slot = 0;                  // control-block slot of the next call (0/1); slot 2: stand-alone entry points
+    void* lastCtl = nullptr;
     bool haveStages = false;
     long long launches = 0;        // kernels launched so far (gamma_launch_count)
     int numSM = 0;
@@ -80,7 +86,10 @@ struct Workspace {
         if (done) { cudaEventDestroy(done); done = nullptr; }
         for (cudaEvent_t& ev : stage)
             if (ev) { cudaEventDestroy(ev); ev = nullptr; }
-        havePending = false; haveLast = false; haveStages = false;
+        if (aux) { cudaStreamDestroy(aux); aux = nullptr; }
+        if (evFork) { cudaEventDestroy(evFork); evFork = nullptr; }
+        if (evJoin) { cudaEventDestroy(evJoin); evJoin = nullptr; }
+        havePending = false; haveLast = false; haveStages = false; ctlClean = false; ctlOwner = nullptr;
     }
 } g_ws;
 
@@ -234,9 +243,10 @@ int resolve_opts(const gamma_opts* o, Resolved& r)
     r.profile = 0;
     if (!o) return GAMMA_OK;
     r.profile = o->profile_stages == 1;
-    if (o->presort < 0 || o->presort > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.presort must be 0, 1 or 2");
+    if (o->presort < 0 || o->presort > 3) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.presort must be 0, 1, 2 or 3");
     if (o->star_phase < 0 || o->star_phase > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.star_phase must be 0, 1 or 2");
     if (o->presort == 2) r.presort = 0;
+    if (o->presort == 3) r.presort = 3;
     if (o->star_phase == 2) r.star = 0;
     if (o->lanes_per_voxel != 0) {
         if (o->lanes_per_voxel != 1 && o->lanes_per_voxel != 8 && o->lanes_per_voxel != 32)
@@ -268,6 +278,13 @@ int check_criteria(float DD, int mode, float cutoff)
 }
 
 // Enqueue the whole hot path on `st` (device pointers).  Caller holds g_mu.
+//
+//   st :  k_norm -> k_prep_star -> [k_bucket_scatter | LSD radix sort] -> (join) -> k_table_search
+//   aux:        \-> k_offset_table ------------------------------------------/
+//
+// The offset table only needs k_norm's maxima, so it is built on a library-owned side stream while the
+// prep/star kernel runs.  No memset and no host synchronisation on the path: k_norm clears the control
+// block of the next call (two alternating slots; slot 2 belongs to the stand-alone entry points).
 int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
                      const Resolved& r, float* out, cudaStream_t st)
 {
@@ -275,18 +292,30 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     if (rc) return rc;
     const long long N = g.N;
     const long long maxTiles = (N + SORT_TILE - 1) / SORT_TILE;
-    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
     CU_TRY(g_ws.key0.need(N * 4)); CU_TRY(g_ws.idx0.need(N * 4));
-    if (r.presort) {
-        CU_TRY(g_ws.key1.need(N * 4)); CU_TRY(g_ws.idx1.need(N * 4));
-        CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
-    }
+    if (r.presort) { CU_TRY(g_ws.key1.need(N * 4)); CU_TRY(g_ws.idx1.need(N * 4)); }
+    if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
     CU_TRY(g_ws.table.need((size_t)r.tableCap * 16));
     CU_TRY(g_ws.tmpL.need((size_t)r.tableCap * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)r.tableCap * 4));
+    if (!g_ws.aux) {
+        CU_TRY(cudaStreamCreateWithFlags(&g_ws.aux, cudaStreamNonBlocking));
+        CU_TRY(cudaEventCreateWithFlags(&g_ws.evFork, cudaEventDisableTiming));
+        CU_TRY(cudaEventCreateWithFlags(&g_ws.evJoin, cudaEventDisableTiming));
+        CU_TRY(cudaFuncSetAttribute(k_offset_table, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TAB_DYN_SMEM));
+    }
     rc = order_after_previous(st);
     if (rc) return rc;
 
-    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p);
+    if (g_ws.ctl.p != g_ws.ctlOwner) { g_ws.ctlClean = false; g_ws.ctlOwner = g_ws.ctl.p; }
+    if (!g_ws.ctlClean) {                                  // first call, or a previous call failed half-way
+        CU_TRY(cudaMemsetAsync(g_ws.ctl.p, 0, 3 * sizeof(Ctl), st));
+        g_ws.slot = 0;
+    }
+    g_ws.ctlClean = false;                                 // set again when everything below was enqueued
+    Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
+    Ctl* ctl = base + g_ws.slot;
+    Ctl* next = base + (g_ws.slot ^ 1);
     unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p), *i0 = static_cast<unsigned*>(g_ws.idx0.p);
     unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *i1 = static_cast<unsigned*>(g_ws.idx1.p);
     EvalP e;
@@ -294,42 +323,52 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
 
     g_ws.haveStages = false;
     if (r.profile)
-        for (cudaEvent_t& ev : g_ws.stage)
-            if (!ev) CU_TRY(cudaEventCreate(&ev));
-#define STAGE_MARK(i) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], st)); } while (0)
-    STAGE_MARK(0);
-    CU_TRY(cudaMemsetAsync(ctl, 0, sizeof(Ctl), st));
+        for (cudaEvent_t& evn : g_ws.stage)
+            if (!evn) CU_TRY(cudaEventCreate(&evn));
+#define STAGE_MARK(i, s) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], s)); } while (0)
     const int sm = g_ws.numSM;
-    if (!(r.normDose > 0.0f)) {                                          // a0
+    STAGE_MARK(0, st);
+    {                                                                    // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
-        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 8 ? sm * 8 : blocks));
-        k_max_ref<<<grid, 256, 0, st>>>(ref, (int)N, ctl);
+        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
+        k_norm<<<grid, NORM_THREADS, 0, st>>>(ref, ev, (int)N, mode, ctl, next);
         ++g_ws.launches;
     }
-    STAGE_MARK(1);
+    STAGE_MARK(1, st);
+    {                                                                    // a3 on the side stream
+        CU_TRY(cudaEventRecord(g_ws.evFork, st));
+        CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
+        STAGE_MARK(5, g_ws.aux);
+        k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, g_ws.aux>>>(
+            g, e, ctl, -1.0f, r.tableCap, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
+            static_cast<unsigned*>(g_ws.tmpIdx.p));
+        ++g_ws.launches;
+        STAGE_MARK(6, g_ws.aux);
+        CU_TRY(cudaEventRecord(g_ws.evJoin, g_ws.aux));
+    }
     {                                                                    // a1 + star
-        long long tiles = (N + PREP_TILE - 1) / PREP_TILE;
-        int grid = (int)(tiles > sm * 16 ? sm * 16 : tiles);
+        long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
+        int grid = (int)(chunks > sm * 4 ? sm * 4 : chunks);
         if (r.star)
             k_prep_star<true><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
         else
             k_prep_star<false><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
         ++g_ws.launches;
     }
-    STAGE_MARK(2);
-    // a3: offset table out to the largest key
-    k_offset_table<<<1, TAB_THREADS, 0, st>>>(g, ctl, -1.0f, r.tableCap, static_cast<int4*>(g_ws.table.p),
-                                              static_cast<unsigned*>(g_ws.tmpL.p), static_cast<unsigned*>(g_ws.tmpIdx.p));
-    ++g_ws.launches;
-    STAGE_MARK(3);
+    STAGE_MARK(2, st);
     const unsigned *lk = k0, *li = i0;
-    if (r.presort) {                                                     // a2
+    if (r.presort == 1) {                                                // a2: one-pass MSD bucket presort
+        k_bucket_scatter<<<sm * 2, SCATTER_THREADS, 0, st>>>(ctl, k0, i0, k1, i1);
+        ++g_ws.launches;
+        lk = k1; li = i1;
+    } else if (r.presort == 3) {                                         // a2: full LSD radix sort of the keys
         int where = radix_sort_enqueue(k0, i0, k1, i1, &ctl->nSearch, N, 32 - r.keyBits, 32,
                                        static_cast<unsigned*>(g_ws.tileHist.p), st);
         g_ws.launches += 3 * (r.keyBits / 8);
         if (where) { lk = k1; li = i1; }
     }
-    STAGE_MARK(4);
+    STAGE_MARK(3, st);
+    CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));
     {                                                                    // a4 + a5
         const int grid = sm * 8;
         const int4* tab = static_cast<const int4*>(g_ws.table.p);
@@ -341,12 +380,15 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             k_table_search<32><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
         ++g_ws.launches;
     }
-    STAGE_MARK(5);
+    STAGE_MARK(4, st);
 #undef STAGE_MARK
     g_ws.haveStages = r.profile != 0;
     CU_TRY(cudaGetLastError());
     rc = mark_done(st);
     if (rc) return rc;
+    g_ws.lastCtl = ctl;
+    g_ws.slot ^= 1;
+    g_ws.ctlClean = true;
     g_ws.lastStream = st; g_ws.lastN = N; g_ws.haveLast = true;
     return GAMMA_OK;
 }
@@ -452,12 +494,12 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const long long maxTiles = (n + SORT_TILE - 1) / SORT_TILE;
-    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
     CU_TRY(g_ws.key1.need(n * 4)); CU_TRY(g_ws.idx1.need(n * 4));
     CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
     rc = order_after_previous(st);
     if (rc) return rc;
-    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p);
+    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + 2;
     k_set_u32<<<1, 1, 0, st>>>(&ctl->sortN, (unsigned)n);
     unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *v1 = static_cast<unsigned*>(g_ws.idx1.p);
     int where = radix_sort_enqueue(keys, vals, k1, v1, &ctl->sortN, n, begin_bit, end_bit,
@@ -501,14 +543,18 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
     CU_TRY(g_ws.table.need((size_t)max_entries * 16));
     CU_TRY(g_ws.tmpL.need((size_t)max_entries * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)max_entries * 4));
+    CU_TRY(cudaFuncSetAttribute(k_offset_table, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TAB_DYN_SMEM));
     rc = order_after_previous(st);
     if (rc) return rc;
-    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p);
-    k_offset_table<<<1, TAB_THREADS, 0, st>>>(g, ctl, radius, max_entries, static_cast<int4*>(g_ws.table.p),
-                                              static_cast<unsigned*>(g_ws.tmpL.p), static_cast<unsigned*>(g_ws.tmpIdx.p));
+    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + 2;
+    EvalP e;
+    e.DD = 1.0f; e.cutoff = 0.0f; e.norm_dose = 1.0f; e.mode = 0;
+    k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, st>>>(
+        g, e, ctl, radius, max_entries, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
+        static_cast<unsigned*>(g_ws.tmpIdx.p));
     k_table_export<<<64, 256, 0, st>>>(ctl, static_cast<const int4*>(g_ws.table.p), max_entries, out_entries, out_count);
     g_ws.launches += 2;
     CU_TRY(cudaGetLastError());
@@ -524,7 +570,7 @@ int gamma_get_counters(gamma_counters* out_host)
     if (!g_ws.haveLast || !g_ws.ctl.p) return fail(GAMMA_ERR_INVALID_ARGUMENT, "no gamma_eval call to report on");
     CU_TRY(cudaStreamSynchronize(g_ws.lastStream));
     Ctl c;
-    CU_TRY(cudaMemcpy(&c, g_ws.ctl.p, sizeof c, cudaMemcpyDeviceToHost));
+    CU_TRY(cudaMemcpy(&c, g_ws.lastCtl, sizeof c, cudaMemcpyDeviceToHost));
     std::memset(out_host, 0, sizeof *out_host);
     out_host->n_voxels = g_ws.lastN;
     out_host->n_evaluated = c.nEval;
@@ -545,12 +591,13 @@ int gamma_get_stage_times(gamma_stage_times* out_host)
     if (!out_host) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_host is NULL");
     std::lock_guard<std::mutex> lock(g_mu);
     if (!g_ws.haveStages) return fail(GAMMA_ERR_INVALID_ARGUMENT, "last gamma_eval call did not set opts.profile_stages");
-    CU_TRY(cudaEventSynchronize(g_ws.stage[5]));
-    float ms[5];
-    for (int i = 0; i < 5; ++i) CU_TRY(cudaEventElapsedTime(&ms[i], g_ws.stage[i], g_ws.stage[i + 1]));
-    out_host->norm_ms = ms[0]; out_host->prep_ms = ms[1]; out_host->table_ms = ms[2];
-    out_host->sort_ms = ms[3]; out_host->search_ms = ms[4];
-    CU_TRY(cudaEventElapsedTime(&out_host->total_ms, g_ws.stage[0], g_ws.stage[5]));
+    CU_TRY(cudaEventSynchronize(g_ws.stage[4]));
+    CU_TRY(cudaEventSynchronize(g_ws.stage[6]));
+    float ms[4];
+    for (int i = 0; i < 4; ++i) CU_TRY(cudaEventElapsedTime(&ms[i], g_ws.stage[i], g_ws.stage[i + 1]));
+    out_host->norm_ms = ms[0]; out_host->prep_ms = ms[1]; out_host->sort_ms = ms[2]; out_host->search_ms = ms[3];
+    CU_TRY(cudaEventElapsedTime(&out_host->table_ms, g_ws.stage[5], g_ws.stage[6]));
+    CU_TRY(cudaEventElapsedTime(&out_host->total_ms, g_ws.stage[0], g_ws.stage[4]));
     return GAMMA_OK;
 }
 
@@ -568,14 +615,14 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
     int rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    CU_TRY(g_ws.ctl.need(sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
     cudaEvent_t a, b;
     CU_TRY(cudaEventCreate(&a)); CU_TRY(cudaEventCreate(&b));
     const int grid = g_ws.numSM * 8 * 4, threads = 256;
     double best = 0.0;
     for (int r = 0; r < repeats + 1; ++r) {
         CU_TRY(cudaEventRecord(a, st));
-        k_fp32_probe<<<grid, threads, 0, st>>>(reinterpret_cast<float*>(g_ws.ctl.p) + 15, 0.999f, 1e-3f);
+        k_fp32_probe<<<grid, threads, 0, st>>>(reinterpret_cast<float*>(static_cast<Ctl*>(g_ws.ctl.p) + 2) + 15, 0.999f, 1e-3f);
         ++g_ws.launches;
         CU_TRY(cudaEventRecord(b, st));
         CU_TRY(cudaEventSynchronize(b));

@@ -1,16 +1,20 @@
 // gamma_search.cuh -- subsystems (2) and (4): the gamma kernels.
 //
-//   k_max_ref       a0: D_norm = max(ref)                                   (reading 8)
-//   k_prep_star     a1 + first part of a4: per voxel DD, cutoff, key (Algorithm A2 step 2 / CUDA Kernel 1,
-//                   PAPER.md:231-233), block-local compaction of the evaluated voxels, then for interior
-//                   voxels the 75 faces of the evaluation surface that touch the voxel ("star").  A voxel
-//                   whose gamma_star is not larger than the distance to the rest of the surface is final;
-//                   the others are appended to the search work list with key gamma_star (a much tighter
-//                   key than |DD|/dD).
-//   k_table_search  a4 + a5: Algorithm A1 step 4-b over the sorted offset table, G lanes
-//                   cooperating on one reference voxel, running best shared by shuffles, exit when the
-//                   table's L reaches the running gamma (reading 3); writes gamma at the voxel's own
-//                   position (replaces the sort-back of A2 step 7).
+//   k_norm           a0 + A1 step 1: D_norm = max(ref) (reading 8) and max |D_r - D_e|,
+//                    which bounds every key and so fixes the radius of the offset table before the search
+//                    list exists; also clears the control block of the NEXT call.
+//   k_prep_star      a1 + first part of a4: per voxel DD, cutoff, key (Algorithm A2 step 2 / CUDA Kernel 1,
+//                    PAPER.md:231-233); evaluated voxels are compacted into a block-local queue so that the
+//                    arithmetic always runs on full warps, then interior voxels try the 75 faces of the
+//                    evaluation surface that touch the voxel ("star").  A voxel whose gamma_star is not larger
+//                    than the distance to the rest of the surface is final; the others are appended to the
+//                    search work list with key gamma_star (a much tighter key than |DD|/dD)
+//                    and counted into the digit histogram of the presort.
+//   k_bucket_scatter a2: one-pass MSD radix presort of the work list on the 8-bit key digit.
+//   k_table_search   a4 + a5: Algorithm A1 step 4-b over the sorted offset table, G lanes
+//                    cooperating on one reference voxel, running best shared by shuffles, exit when the
+//                    table's L reaches the running gamma (reading 3); writes gamma at the voxel's own
+//                    position (replaces the sort-back of A2 step 7).
 // The point-to-simplex arithmetic is in features_generated.cuh.
 #pragma once
 #include "common.cuh"
@@ -18,32 +22,59 @@
 
 namespace gamma_b200 {
 
-// ------------------------------------------------------------------------------------------------
-// a0: max(ref)
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_max_ref(const float* __restrict__ ref, int N, Ctl* __restrict__ ctl)
+__device__ __forceinline__ float block_max_256(float v, float* sm8)
 {
-    float m = -INFINITY;
+    v = warp_max(v);
+    if ((threadIdx.x & 31) == 0) sm8[threadIdx.x >> 5] = v;
+    __syncthreads();
+    float m = sm8[0];
+#pragma unroll
+    for (int w = 1; w < 8; ++w) m = fmaxf(m, sm8[w]);
+    __syncthreads();
+    return m;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a0 + A1 step 1: max(ref), max |ref - eval| (and max |ref - eval| / ref for the local criterion)
+// ------------------------------------------------------------------------------------------------
+constexpr int NORM_THREADS = 256;
+
+__global__ void __launch_bounds__(NORM_THREADS)
+k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur,
+       Ctl* __restrict__ next)
+{
+    if (blockIdx.x == gridDim.x - 1 && next != nullptr) {      // the next call finds its control block cleared
+        unsigned* w = reinterpret_cast<unsigned*>(next);
+        for (int i = threadIdx.x; i < (int)(sizeof(Ctl) / 4); i += NORM_THREADS) w[i] = 0u;
+    }
+    float m = -INFINITY, a = 0.0f, r = 0.0f;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
-    if ((reinterpret_cast<uintptr_t>(ref) & 15u) == 0) {
+    auto one = [&](float Dr, float De) {
+        m = fmaxf(m, Dr);
+        const float ad = fabsf(Dr - De);
+        a = fmaxf(a, ad);                                       // fmaxf drops NaN
+        if (mode == 1 && Dr > 0.0f) r = fmaxf(r, ad / Dr);
+    };
+    if (((reinterpret_cast<uintptr_t>(ref) | reinterpret_cast<uintptr_t>(ev)) & 15u) == 0) {
         const float4* r4 = reinterpret_cast<const float4*>(ref);
+        const float4* e4 = reinterpret_cast<const float4*>(ev);
         const int n4 = N >> 2;
         for (int i = tid; i < n4; i += nth) {
-            const float4 v = __ldg(r4 + i);
-            m = fmaxf(fmaxf(m, v.x), fmaxf(v.y, fmaxf(v.z, v.w)));
+            const float4 x = __ldg(r4 + i), y = __ldg(e4 + i);
+            one(x.x, y.x); one(x.y, y.y); one(x.z, y.z); one(x.w, y.w);
         }
-        for (int i = (n4 << 2) + tid; i < N; i += nth) m = fmaxf(m, __ldg(ref + i));
+        for (int i = (n4 << 2) + tid; i < N; i += nth) one(__ldg(ref + i), __ldg(ev + i));
     } else {
-        for (int i = tid; i < N; i += nth) m = fmaxf(m, __ldg(ref + i));
+        for (int i = tid; i < N; i += nth) one(__ldg(ref + i), __ldg(ev + i));
     }
-    m = warp_max(m);
-    __shared__ float sm[8];
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m;
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        m = threadIdx.x < 8 ? sm[threadIdx.x] : -INFINITY;
-        m = warp_max(m);
-        if (threadIdx.x == 0) atomicMax(&ctl->normOrd, float_to_ordered(m));
+    __shared__ float sm8[8];
+    m = block_max_256(m, sm8);
+    a = block_max_256(a, sm8);
+    if (mode == 1) r = block_max_256(r, sm8);
+    if (threadIdx.x == 0) {
+        atomicMax(&cur->normOrd, float_to_ordered(m));
+        if (a > 0.0f) atomicMax(&cur->maxAbsDD, __float_as_uint(a));
+        if (r > 0.0f) atomicMax(&cur->maxRatio, __float_as_uint(r));
     }
 }
 
@@ -51,7 +82,8 @@ __global__ void __launch_bounds__(256) k_max_ref(const float* __restrict__ ref, 
 // a1 + star phase
 // ------------------------------------------------------------------------------------------------
 constexpr int PREP_THREADS = 256;
-constexpr int PREP_TILE = 2048;
+constexpr int PREP_CHUNK = 4 * PREP_THREADS;              // voxels fetched per block iteration (float4 per thread)
+constexpr int PREP_QUEUE = PREP_CHUNK + PREP_THREADS;     // block-local queue of evaluated voxels
 
 __device__ __forceinline__ float criterion_inv_dD(const EvalP& e, double dnorm, float Dr)
 {
@@ -64,110 +96,206 @@ __global__ void __launch_bounds__(PREP_THREADS)
 k_prep_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
             EvalP e, Ctl* __restrict__ ctl, unsigned* __restrict__ listKey, unsigned* __restrict__ listIdx)
 {
-    __shared__ int sList[PREP_TILE];
+    __shared__ int sQueue[PREP_QUEUE];
+    __shared__ unsigned sHist[KEY_DIGITS];
     __shared__ unsigned sCnt;
+    __shared__ int sChunk;
     __shared__ float sMax[PREP_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31;
+    const unsigned FULL = 0xffffffffu;
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
     const double dnorm = (double)dnormF;
     const double thr = (double)e.cutoff * dnorm;      // decided in double (include/gamma_b200.h)
     const float invGlobal = criterion_inv_dD(e, dnorm, 0.0f);
+    const float qnan = __int_as_float(0x7fc00000);
+    const int numChunks = (g.N + PREP_CHUNK - 1) / PREP_CHUNK;
+    const bool vec = ((reinterpret_cast<uintptr_t>(ref) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0;
     float maxKey = 0.0f;
     unsigned nEvalLocal = 0;
-    const float qnan = __int_as_float(0x7fc00000);
-    const int numTiles = (g.N + PREP_TILE - 1) / PREP_TILE;
 
-    for (int tile = blockIdx.x; tile < numTiles; tile += gridDim.x) {
-        if (tid == 0) sCnt = 0;
-        __syncthreads();
-        // ---- a1: exclusion + block-local compaction (keeps warps full for the arithmetic below)
+    sHist[tid] = 0;
+    if (tid == 0) { sCnt = 0; sChunk = blockIdx.x; }
+    __syncthreads();
+
+    // One queued voxel: key, star phase, final write or append to the search list.
+    auto star_item = [&](bool valid, int lin) {
+        bool toSearch = false;
+        float key = 0.0f;
+        if (valid) {
+            const float Dr = __ldg(ref + lin);
+            const float invdD = e.mode == 0 ? invGlobal : criterion_inv_dD(e, dnorm, Dr);
+            const float d0 = (__ldg(ev + lin) - Dr) * invdD;
+            key = fabsf(d0);                              // A1 step 4-a: gamma <- |DD| / dD
+            toSearch = true;
+            if (STAR && g.all_active) {
+                const int ix = lin % g.n[0], iy = (lin / g.n[0]) % g.n[1], iz = lin / g.stride[2];
+                const bool interior = ix >= 1 && ix <= g.n[0] - 2 && iy >= 1 && iy <= g.n[1] - 2 &&
+                                      iz >= 1 && iz <= g.n[2] - 2;
+                if (interior) {
+                    float d[27];
+                    const float* p = ev + lin;
 #pragma unroll
-        for (int j = 0; j < PREP_TILE / PREP_THREADS; ++j) {
-            const int lin = tile * PREP_TILE + j * PREP_THREADS + tid;
-            bool keep = false;
-            if (lin < g.N) {
-                const float Dr = __ldg(ref + lin);
-                const bool excluded = ((double)Dr < thr) ||
-                                      (e.mode == 0 ? !(invGlobal > 0.0f) : !((double)e.DD * (double)Dr > 0.0));
-                if (excluded) out[lin] = qnan;
-                keep = !excluded;
-            }
-            const unsigned bal = __ballot_sync(0xffffffffu, keep);
-            unsigned base = 0;
-            if (lane == 0 && bal) base = atomicAdd(&sCnt, (unsigned)__popc(bal));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            if (keep) sList[base + __popc(bal & ((1u << lane) - 1u))] = lin;
-        }
-        __syncthreads();
-        const int cnt = (int)sCnt;
-        if (tid == 0) nEvalLocal += cnt;
-        // ---- star phase over the compacted voxels of this tile
-        for (int j0 = 0; j0 < cnt; j0 += PREP_THREADS) {
-            const int j = j0 + tid;
-            bool toSearch = false;
-            float key = 0.0f;
-            int lin = 0;
-            if (j < cnt) {
-                lin = sList[j];
-                const float Dr = __ldg(ref + lin);
-                const float invdD = e.mode == 0 ? invGlobal : criterion_inv_dD(e, dnorm, Dr);
-                const float d0 = (__ldg(ev + lin) - Dr) * invdD;
-                key = fabsf(d0);                              // A1 step 4-a: gamma <- |DD| / dD
-                toSearch = true;
-                if (STAR && g.all_active) {
-                    const int ix = lin % g.n[0], iy = (lin / g.n[0]) % g.n[1], iz = lin / g.stride[2];
-                    const bool interior = ix >= 1 && ix <= g.n[0] - 2 && iy >= 1 && iy <= g.n[1] - 2 &&
-                                          iz >= 1 && iz <= g.n[2] - 2;
-                    if (interior) {
-                        float d[27];
-                        const float* p = ev + lin;
+                    for (int oz = -1; oz <= 1; ++oz)
 #pragma unroll
-                        for (int oz = -1; oz <= 1; ++oz)
+                        for (int oy = -1; oy <= 1; ++oy)
 #pragma unroll
-                            for (int oy = -1; oy <= 1; ++oy)
-#pragma unroll
-                                for (int ox = -1; ox <= 1; ++ox)
-                                    d[(ox + 1) + 3 * (oy + 1) + 9 * (oz + 1)] =
-                                        (__ldg(p + ox + oy * g.stride[1] + oz * g.stride[2]) - Dr) * invdD;
-                        d[13] = d0;
-                        const float gmax = gamma_star_gmax(d, g.invA);
-                        key = key / sqrtf(gmax);              // gamma_star
-                        if (key * key <= g.rho_link2) {       // nothing outside the star can be closer
-                            out[lin] = key;
-                            toSearch = false;
-                        }
+                            for (int ox = -1; ox <= 1; ++ox)
+                                d[(ox + 1) + 3 * (oy + 1) + 9 * (oz + 1)] =
+                                    (__ldg(p + ox + oy * g.stride[1] + oz * g.stride[2]) - Dr) * invdD;
+                    d[13] = d0;
+                    const float gmax = gamma_star_gmax(d, g.invA);
+                    key = key / sqrtf(gmax);              // gamma_star
+                    if (key * key <= g.rho_link2) {       // nothing outside the star can be closer
+                        out[lin] = key;
+                        toSearch = false;
                     }
                 }
-                if (!(key == key)) {                          // non-finite doses: no search, NaN out
-                    out[lin] = qnan;
-                    toSearch = false;
-                }
             }
-            // append to the global work list (warp-aggregated)
-            const unsigned bal = __ballot_sync(0xffffffffu, toSearch);
-            if (bal) {
-                unsigned base = 0;
-                if (lane == __ffs(bal) - 1) base = atomicAdd(&ctl->nSearch, (unsigned)__popc(bal));
-                base = __shfl_sync(0xffffffffu, base, __ffs(bal) - 1);
-                if (toSearch) {
-                    const unsigned pos = base + __popc(bal & ((1u << lane) - 1u));
-                    listKey[pos] = __float_as_uint(key);
-                    listIdx[pos] = (unsigned)lin;
-                    maxKey = fmaxf(maxKey, key);
-                }
+            if (!(key == key)) {                          // non-finite doses: no search, NaN out
+                out[lin] = qnan;
+                toSearch = false;
             }
         }
+        const unsigned bal = __ballot_sync(FULL, toSearch);   // append to the global work list, warp-aggregated
+        if (bal) {
+            const int leader = __ffs(bal) - 1;
+            unsigned base = 0;
+            if (lane == leader) base = atomicAdd(&ctl->nSearch, (unsigned)__popc(bal));
+            base = __shfl_sync(FULL, base, leader);
+            if (toSearch) {
+                const unsigned pos = base + __popc(bal & ((1u << lane) - 1u));
+                listKey[pos] = __float_as_uint(key);
+                listIdx[pos] = (unsigned)lin;
+                atomicAdd(&sHist[key_digit(key)], 1u);
+                maxKey = fmaxf(maxKey, key);
+            }
+        }
+    };
+
+    for (;;) {
+        const int chunk = sChunk;
+        if (chunk >= numChunks) break;
+        // ---- a1: exclusion (4 consecutive voxels per thread) + compaction into the block queue
+        const int lin0 = chunk * PREP_CHUNK + tid * 4;
+        float Dr[4];
+        int nval = 0;
+        if (vec && lin0 + 3 < g.N) {
+            const float4 v = __ldg(reinterpret_cast<const float4*>(ref + lin0));
+            Dr[0] = v.x; Dr[1] = v.y; Dr[2] = v.z; Dr[3] = v.w;
+            nval = 4;
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (lin0 + j < g.N) { Dr[j] = __ldg(ref + lin0 + j); nval = j + 1; } else Dr[j] = 0.0f;
+        }
+        unsigned keepMask = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool excluded = ((double)Dr[j] < thr) ||
+                                  (e.mode == 0 ? !(invGlobal > 0.0f) : !((double)e.DD * (double)Dr[j] > 0.0));
+            if (j < nval && !excluded) keepMask |= 1u << j;
+        }
+        if (keepMask == 0 && nval == 4 && vec) {
+            *reinterpret_cast<float4*>(out + lin0) = make_float4(qnan, qnan, qnan, qnan);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (j < nval && !(keepMask & (1u << j))) out[lin0 + j] = qnan;
+        }
+        const int c = __popc(keepMask);
+        nEvalLocal += (unsigned)c;
+        int incl = c;
+#pragma unroll
+        for (int s = 1; s < 32; s <<= 1) {
+            const int t = __shfl_up_sync(FULL, incl, s);
+            if (lane >= s) incl += t;
+        }
+        const int wtot = __shfl_sync(FULL, incl, 31);
+        unsigned wbase = 0;
+        if (lane == 31 && wtot) wbase = atomicAdd(&sCnt, (unsigned)wtot);
+        wbase = __shfl_sync(FULL, wbase, 31);
+        int pos = (int)wbase + incl - c;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (keepMask & (1u << j)) sQueue[pos++] = lin0 + j;
+        __syncthreads();
+        int cnt = (int)sCnt;
+        if (tid == 0) sChunk = (int)atomicAdd(&ctl->tileCounter, 1u) + (int)gridDim.x;   // next chunk, fetched early
+        // ---- star phase on full batches popped from the end of the queue
+        while (cnt >= PREP_THREADS) {
+            star_item(true, sQueue[cnt - PREP_THREADS + tid]);
+            cnt -= PREP_THREADS;
+        }
+        __syncthreads();
+        if (tid == 0) sCnt = (unsigned)cnt;
         __syncthreads();
     }
+    {   // leftovers (< one batch)
+        const int cnt = (int)sCnt;
+        star_item(tid < cnt, tid < cnt ? sQueue[tid] : 0);
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) nEvalLocal += __shfl_xor_sync(FULL, nEvalLocal, s);
+    if (lane == 0 && nEvalLocal) atomicAdd(&ctl->nEval, nEvalLocal);
     maxKey = warp_max(maxKey);
     if (lane == 0) sMax[tid >> 5] = maxKey;
     __syncthreads();
+    if (sHist[tid]) atomicAdd(&ctl->hist[tid], sHist[tid]);
     if (tid == 0) {
         float m = 0.0f;
 #pragma unroll
         for (int w = 0; w < PREP_THREADS / 32; ++w) m = fmaxf(m, sMax[w]);
         if (m > 0.0f) atomicMax(&ctl->maxKeyBits, __float_as_uint(m));
-        if (nEvalLocal) atomicAdd(&ctl->nEval, nEvalLocal);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2: one-pass MSD radix presort of the search work list on the 8-bit key digit.  The digit histogram
+// was accumulated by k_prep_star; every block scans it (256 values) and scatters its share of the list.
+// Order inside a digit is arbitrary (the search result does not depend on the order of the list).
+// ------------------------------------------------------------------------------------------------
+constexpr int SCATTER_THREADS = 256;
+
+__global__ void __launch_bounds__(SCATTER_THREADS)
+k_bucket_scatter(Ctl* __restrict__ ctl, const unsigned* __restrict__ keyIn, const unsigned* __restrict__ idxIn,
+                 unsigned* __restrict__ keyOut, unsigned* __restrict__ idxOut)
+{
+    __shared__ unsigned sBase[KEY_DIGITS];
+    __shared__ unsigned sWarp[SCATTER_THREADS / 32];
+    const unsigned FULL = 0xffffffffu;
+    const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const unsigned n = ctl->nSearch;
+    if (blockIdx.x * SCATTER_THREADS >= n) return;
+    {   // exclusive scan of the 256-bin histogram
+        const unsigned h = ctl->hist[tid];
+        unsigned incl = h;
+#pragma unroll
+        for (int s = 1; s < 32; s <<= 1) {
+            const unsigned t = __shfl_up_sync(FULL, incl, s);
+            if (lane >= (unsigned)s) incl += t;
+        }
+        if (lane == 31) sWarp[warp] = incl;
+        __syncthreads();
+        unsigned off = 0;
+        for (unsigned w = 0; w < warp; ++w) off += sWarp[w];
+        sBase[tid] = off + incl - h;
+        __syncthreads();
+    }
+    for (unsigned i0 = blockIdx.x * SCATTER_THREADS; i0 < n; i0 += gridDim.x * SCATTER_THREADS) {
+        const unsigned i = i0 + tid;
+        const bool valid = i < n;
+        unsigned key = 0, idx = 0, d = KEY_DIGITS;            // invalid lanes form their own match group
+        if (valid) { key = keyIn[i]; idx = idxIn[i]; d = key_digit(__uint_as_float(key)); }
+        const unsigned peers = __match_any_sync(FULL, d);
+        const int leader = __ffs(peers) - 1;
+        unsigned base = 0;
+        if (valid && (int)lane == leader) base = atomicAdd(&ctl->cursor[d], (unsigned)__popc(peers));
+        base = __shfl_sync(FULL, base, leader);
+        if (valid) {
+            const unsigned pos = sBase[d] + base + __popc(peers & ((1u << lane) - 1u));
+            keyOut[pos] = key;
+            idxOut[pos] = idx;
+        }
     }
 }
 
@@ -237,7 +365,13 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int gid = lane / G, gl = lane % G;
-    const unsigned nS = ctl->nSearch, T = ctl->tableCount;
+    const unsigned nS = ctl->nSearch;
+    const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
+    // first round: static assignment (no atomic storm at kernel start); later rounds: dynamic fetch
+    unsigned base = (blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5)) * (unsigned)VPW;
+    if (base >= nS) return;
+    const bool dynamic = nS > warpsTotal * (unsigned)VPW;     // otherwise the first round covers the whole list
+    const unsigned T = ctl->tableCount;
     const bool trunc = ctl->tableTrunc != 0;
     const float Rtab2 = ctl->Rtab2;
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
@@ -246,10 +380,6 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     unsigned visits = 0;
 
     for (;;) {
-        unsigned base = 0;
-        if (lane == 0) base = atomicAdd(&ctl->workCounter, (unsigned)VPW);
-        base = __shfl_sync(FULL, base, 0);
-        if (base >= nS) break;
         const unsigned item = base + gid;
         const bool have = item < nS;
         VoxelCtx vc;
@@ -267,6 +397,9 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
         } else {
             vc.lin = 0; vc.Dr = 0.0f; vc.invdD = 0.0f; vc.v[0] = vc.v[1] = vc.v[2] = 0;
         }
+        // next work item, fetched early so that its latency hides behind this search
+        unsigned nextBase = nS;
+        if (dynamic && lane == 0) nextBase = atomicAdd(&ctl->workCounter, (unsigned)VPW) + warpsTotal * (unsigned)VPW;
         // ---- Algorithm A1 step 4-b over the sorted table
         for (unsigned e0 = 0;; e0 += EPP) {
             bool more = have && e0 < T;
@@ -346,6 +479,8 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
             }
         }
         if (have && gl == 0) out[vc.lin] = fminf(key, sqrtf(best2));   // a5: write at the voxel's own place
+        base = __shfl_sync(FULL, nextBase, 0);
+        if (base >= nS) break;
     }
     // diagnostic counter: one atomic per warp
     for (int s = 16; s > 0; s >>= 1) visits += __shfl_xor_sync(FULL, visits, s);

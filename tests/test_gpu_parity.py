@@ -101,8 +101,8 @@ def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
     thread-per-voxel mapping: the candidate set is the same, so gamma is bit-identical."""
     c = phantoms.make_case("cfg5")
     base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
-    for o in (GammaOpts(presort=2), GammaOpts(lanes_per_voxel=1), GammaOpts(lanes_per_voxel=1, presort=2),
-              GammaOpts(lanes_per_voxel=32)):
+    for o in (GammaOpts(presort=2), GammaOpts(presort=3), GammaOpts(lanes_per_voxel=1),
+              GammaOpts(lanes_per_voxel=1, presort=2), GammaOpts(lanes_per_voxel=32)):
         g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
         assert np.array_equal(np.isnan(g), np.isnan(base))
         assert np.array_equal(g[~np.isnan(g)], base[~np.isnan(base)]), o
@@ -114,7 +114,7 @@ def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
 VARIANTS = [
     GammaOpts(), GammaOpts(star_phase=2), GammaOpts(presort=2), GammaOpts(lanes_per_voxel=1),
     GammaOpts(lanes_per_voxel=32), GammaOpts(star_phase=2, lanes_per_voxel=1, presort=2),
-    GammaOpts(sort_key_bits=8), GammaOpts(sort_key_bits=32), GammaOpts(table_cap=1),
+    GammaOpts(presort=3, sort_key_bits=8), GammaOpts(presort=3, sort_key_bits=32), GammaOpts(table_cap=1),
     GammaOpts(table_cap=7, star_phase=2), GammaOpts(table_cap=40, lanes_per_voxel=32),
     GammaOpts(table_cap=3, lanes_per_voxel=1),
 ]
@@ -258,7 +258,8 @@ def test_stage_times_are_reported():
     gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, GammaOpts(profile_stages=1))
     t = binding.gamma_get_stage_times()
     assert t["total_ms"] > 0 and t["prep_ms"] > 0 and t["search_ms"] >= 0
-    assert abs(sum(t[k] for k in ("norm_ms", "prep_ms", "table_ms", "sort_ms", "search_ms")) - t["total_ms"]) < 0.05
+    assert abs(sum(t[k] for k in ("norm_ms", "prep_ms", "sort_ms", "search_ms")) - t["total_ms"]) < 0.05
+    assert t["table_ms"] > 0                         # built on the side stream, concurrent with prep
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -328,6 +329,20 @@ def test_offset_table_against_definition(dims, sp, dta, R):
 def test_offset_table_truncation_is_flagged():
     ent, trunc, r2 = binding.gamma_offset_table((128, 128, 64), (2.5, 2.5, 2.5), 2.0, 20.0, max_entries=500)
     assert trunc and ent.shape[0] <= 500 and r2 < 400.0
+
+
+def test_offset_table_large_slices_use_global_scratch():
+    """More entries per block slice than fit in shared memory (8192): the global-scratch path."""
+    from oracle import aux_oracle
+    dims, sp, dta, R = (200, 200, 200), (1.0, 1.0, 1.0), 1.0, 90.0
+    ent, trunc, r2 = binding.gamma_offset_table(dims, sp, dta, R, max_entries=1 << 20)
+    ent = ent.cpu().numpy()
+    exp = aux_oracle.offset_table(dims, sp, dta, R)
+    assert not trunc and ent.shape[0] == len(exp) and ent.shape[0] > 32 * 8192
+    L2 = ent[:, 0].copy().view(np.float32)
+    assert np.all(np.diff(L2) >= 0)
+    assert np.array_equal(np.sort(L2), np.array([t[0] for t in exp], dtype=np.float32))
+    assert {tuple(r) for r in ent[:, 1:].tolist()} == {t[1:] for t in exp}
 
 
 def test_fp32_probe_runs():
