@@ -253,8 +253,10 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with clocks:
         e0.record(stream)
+        t_sub = time.perf_counter()
         for i in range(args.steps):
             step(args.warmup + i)
+        t_sub = (time.perf_counter() - t_sub) / args.steps
         e1.record(stream)
         barrier()
     launches = binding.gamma_launch_count() - l0
@@ -339,7 +341,7 @@ def main():
         "grid_voxels_per_s": world * N / (ms_step * 1e-3), "ms_per_case": ms_step,
         "e2e": {"value": world * M / e2e_s, "unit": "evaluated reference voxels/s", "ms_per_case": e2e_s * 1e3,
                 "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N},
-        "gpu_launches": int(launches),
+        "gpu_launches": int(launches), "host_submit_us_per_step": t_sub * 1e6,
         "clocks": clk, "roofline": roof,
         "counters": cnt, "stats": summ, "stats_ms": stats_ms,
     }

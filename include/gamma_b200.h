@@ -74,8 +74,10 @@ typedef struct gamma_opts {
                              and finish there when gamma_star <= distance to the rest of the surface;
                              2: off -- every voxel goes through the table search with key |DD|/dD, as in
                              Algorithm A2                                               */
-    int lanes_per_voxel;  /* 0: default (= 8); 1, 8 or 32 lanes cooperate on one reference voxel in the
-                             table search (1 = the paper's thread-per-voxel mapping)        */
+    int lanes_per_voxel;  /* lanes that cooperate on one reference voxel in the table search.  0: default =
+                             adaptive (a whole warp for the deep items at the head of the pre-sorted list,
+                             8 lanes for the others; needs presort 1 or 3, else 8); 1 = the paper's
+                             thread-per-voxel mapping; 8; 32                               */
     int sort_key_bits;    /* presort = 3 only.  0: default (= 16); 8, 16, 24 or 32 most significant key bits   */
     long long table_cap;  /* 0: default (1<<20); max entries of the sorted offset table; past it the search
                              continues by exhaustive enumeration, so results never depend on it            */

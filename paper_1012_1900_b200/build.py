@@ -45,7 +45,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile if needed; returns the path of the shared library."""
     if not force and not is_stale():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    extra = os.environ.get("GAMMA_NVCC_EXTRA", "").split()     # e.g. -DGAMMA_STAR_MIN_BLOCKS=4 for tuning runs
+    cmd = [_nvcc()] + NVCC_FLAGS + extra + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     log = res.stdout + res.stderr
     with open(os.path.join(HERE, "build.log"), "w") as f:

@@ -18,8 +18,24 @@ struct GridP {
     float K3, K5, K6;          // h_a^2 h_b^2 / (h_a^2 + h_b^2) for the pairs xy, xz, yz
     float Kxy7, Kyz7, Kzx7;    // h_a^2 h_b^2 / (h_x^2 + h_y^2 + h_z^2)
     float rho_link2; // squared distance from a voxel to the boundary of its star (3D only), slightly shrunk
+    float hmin2;     // squared smallest h over the active axes, slightly shrunk: nothing outside the 2^n cells
+                     // that touch a voxel is closer than this
     int all_active;  // 1 when all three axes have size > 1
+    unsigned divMul[2], divSh[2];  // exact division of lin < 2^31 by nx (0) and by nx*ny (1): see fast_div
 };
+
+// q = n / d for n < 2^31 with M = floor(2^(31+l) / d) + 1, l = ceil(log2 d) (set up on the host).
+__device__ __forceinline__ unsigned fast_div(unsigned n, unsigned mul, unsigned sh)
+{
+    return (unsigned)(((unsigned long long)n * mul) >> sh);
+}
+__device__ __forceinline__ void voxel_coords(const GridP& g, int lin, int& ix, int& iy, int& iz)
+{
+    iz = (int)fast_div((unsigned)lin, g.divMul[1], g.divSh[1]);
+    const int rem = lin - iz * g.stride[2];
+    iy = (int)fast_div((unsigned)rem, g.divMul[0], g.divSh[0]);
+    ix = rem - iy * g.n[0];
+}
 
 // Criteria (Eq. 1) and exclusion policy (readings 8-10).
 struct EvalP {
@@ -47,7 +63,7 @@ struct Ctl {
     float Rtab2;           // squared radius the table covers
     int box[3];            // table box: m_a in [0, box_a)
     unsigned sortN;        // element count for gamma_sort_pairs
-    unsigned pad0;
+    float invGlobal;       // 1 / (DD * D_norm) rounded to fp32 (global criterion), written by k_classify
     unsigned long long visits;       // owner vertices evaluated by the table search
     unsigned hist[KEY_DIGITS];       // digit histogram of the search list (bucket presort)
     unsigned cursor[KEY_DIGITS];     // scatter cursors of the bucket presort

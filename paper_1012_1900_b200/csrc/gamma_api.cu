@@ -59,6 +59,7 @@ struct Buf {
 
 struct Workspace {
     Buf ctl;                       // Ctl
+    Buf evalIdx;                   // compacted indices of the evaluated voxels
     Buf key0, idx0, key1, idx1;    // search work list, ping-pong for the sort
     Buf tileHist;                  // radix sort
     Buf table, tmpL, tmpIdx;       // offset table
@@ -75,13 +76,14 @@ struct Workspace {
     bool haveStages = false;
     long long launches = 0;        // kernels launched so far (gamma_launch_count)
     int numSM = 0;
+    int occStar[2] = {0, 0};       // resident blocks per SM of k_star<false/true>
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
     long long lastN = 0;
     bool haveLast = false;
     void releaseAll()
     {
-        Buf* all[] = {&ctl, &key0, &idx0, &key1, &idx1, &tileHist, &table, &tmpL, &tmpIdx, &hRef, &hEval, &hOut};
+        Buf* all[] = {&ctl, &evalIdx, &key0, &idx0, &key1, &idx1, &tileHist, &table, &tmpL, &tmpIdx, &hRef, &hEval, &hOut};
         for (Buf* b : all) b->release();
         if (done) { cudaEventDestroy(done); done = nullptr; }
         for (cudaEvent_t& ev : stage)
@@ -102,6 +104,15 @@ int ensure_device()
     CU_TRY(cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev));
     g_ws.numSM = sm > 0 ? sm : 148;
     return GAMMA_OK;
+}
+
+// host copy of key_digit (common.cuh): the digit of the one-pass presort
+int host_key_digit(float key)
+{
+    unsigned b;
+    std::memcpy(&b, &key, 4);
+    const int d = (int)(b >> 18) - ((127 - 3) << 5);
+    return d < 0 ? 0 : (d > KEY_DIGITS - 1 ? KEY_DIGITS - 1 : d);
 }
 
 int order_after_previous(cudaStream_t st)
@@ -224,6 +235,20 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
     const double A7 = hh[0] + hh[1] + hh[2];
     g.Kxy7 = (float)(hh[0] * hh[1] / A7); g.Kyz7 = (float)(hh[1] * hh[2] / A7); g.Kzx7 = (float)(hh[2] * hh[0] / A7);
     g.all_active = active == 3;
+    {
+        double hm = 0.0;
+        for (int a = 0; a < 3; ++a)
+            if (h[a] > 0.0 && (hm == 0.0 || h[a] < hm)) hm = h[a];
+        hm *= (1.0 - 1e-5);
+        g.hmin2 = (float)(hm * hm);
+        const unsigned dv[2] = {(unsigned)dims[0], (unsigned)dims[0] * (unsigned)dims[1]};
+        for (int k = 0; k < 2; ++k) {
+            unsigned l = 0;
+            while ((1ull << l) < dv[k]) ++l;
+            g.divMul[k] = (unsigned)((1ull << (31 + l)) / dv[k] + 1ull);
+            g.divSh[k] = 31 + l;
+        }
+    }
     if (g.all_active) {
         const double rho = star_link_distance(h) * (1.0 - 1e-5);
         g.rho_link2 = (float)(rho * rho);
@@ -239,7 +264,7 @@ struct Resolved {
 
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
-    r.presort = 1; r.star = 1; r.lanes = 8; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
+    r.presort = 1; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
     r.profile = 0;
     if (!o) return GAMMA_OK;
     r.profile = o->profile_stages == 1;
@@ -293,7 +318,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     const long long N = g.N;
     const long long maxTiles = (N + SORT_TILE - 1) / SORT_TILE;
     CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
-    CU_TRY(g_ws.key0.need(N * 4)); CU_TRY(g_ws.idx0.need(N * 4));
+    CU_TRY(g_ws.key0.need(N * 4)); CU_TRY(g_ws.idx0.need(N * 4)); CU_TRY(g_ws.evalIdx.need(N * 4));
     if (r.presort) { CU_TRY(g_ws.key1.need(N * 4)); CU_TRY(g_ws.idx1.need(N * 4)); }
     if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
     CU_TRY(g_ws.table.need((size_t)r.tableCap * 16));
@@ -318,6 +343,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     Ctl* next = base + (g_ws.slot ^ 1);
     unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p), *i0 = static_cast<unsigned*>(g_ws.idx0.p);
     unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *i1 = static_cast<unsigned*>(g_ws.idx1.p);
+    unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p);
     EvalP e;
     e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
 
@@ -346,13 +372,26 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         STAGE_MARK(6, g_ws.aux);
         CU_TRY(cudaEventRecord(g_ws.evJoin, g_ws.aux));
     }
-    {                                                                    // a1 + star
+    {                                                                    // a1: exclusion + compaction
         long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
-        int grid = (int)(chunks > sm * 4 ? sm * 4 : chunks);
+        int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
+        k_classify<<<grid, PREP_THREADS, 0, st>>>(ref, out, g, e, ctl, e0);
+        ++g_ws.launches;
+    }
+    {                                                                    // star phase over the compacted voxels
+        long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
+        if (g_ws.occStar[r.star] == 0) {
+            int occ = 0;
+            if (r.star) CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_star<true>, STAR_THREADS, 0));
+            else CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_star<false>, STAR_THREADS, 0));
+            g_ws.occStar[r.star] = occ > 0 ? occ : 1;
+        }
+        const long long resident = (long long)sm * g_ws.occStar[r.star];
+        int grid = (int)(blocks > resident ? resident : blocks);
         if (r.star)
-            k_prep_star<true><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
+            k_star<true><<<grid, STAR_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, e0, k0, i0);
         else
-            k_prep_star<false><<<grid, PREP_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, k0, i0);
+            k_star<false><<<grid, STAR_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, e0, k0, i0);
         ++g_ws.launches;
     }
     STAGE_MARK(2, st);
@@ -370,14 +409,21 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     STAGE_MARK(3, st);
     CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));
     {                                                                    // a4 + a5
-        const int grid = sm * 8;
+        const int grid = sm * 4;                                         // resident blocks at 64 registers
         const int4* tab = static_cast<const int4*>(g_ws.table.p);
+        // adaptive lanes: an item is "deep" when its key exceeds the smallest non-zero table distance
+        float hmin = 0.0f;
+        for (int a = 0; a < 3; ++a)
+            if (g.h[a] > 0.0f && (hmin == 0.0f || g.h[a] < hmin)) hmin = g.h[a];
+        const int deepDigit = r.presort ? host_key_digit(hmin) + 1 : KEY_DIGITS;
         if (r.lanes == 1)
-            k_table_search<1><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
+            k_table_search<1><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
         else if (r.lanes == 8)
-            k_table_search<8><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
+            k_table_search<8><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
+        else if (r.lanes == 32)
+            k_table_search<32><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
         else
-            k_table_search<32><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab);
+            k_table_search<0><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
         ++g_ws.launches;
     }
     STAGE_MARK(4, st);

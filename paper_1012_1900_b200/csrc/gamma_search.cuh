@@ -79,11 +79,12 @@ k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int m
 }
 
 // ------------------------------------------------------------------------------------------------
-// a1 + star phase
+// a1: exclusion + compaction of the evaluated voxels (Algorithm A2 step 2 / CUDA Kernel 1)
+// A pure stream over ref: float4 in, NaN out for excluded voxels, indices of evaluated voxels appended to
+// evalIdx in chunk order (so neighbours stay neighbours).  One global atomic per 1024-voxel chunk.
 // ------------------------------------------------------------------------------------------------
 constexpr int PREP_THREADS = 256;
-constexpr int PREP_CHUNK = 4 * PREP_THREADS;              // voxels fetched per block iteration (float4 per thread)
-constexpr int PREP_QUEUE = PREP_CHUNK + PREP_THREADS;     // block-local queue of evaluated voxels
+constexpr int PREP_CHUNK = 4 * PREP_THREADS;
 
 __device__ __forceinline__ float criterion_inv_dD(const EvalP& e, double dnorm, float Dr)
 {
@@ -91,63 +92,163 @@ __device__ __forceinline__ float criterion_inv_dD(const EvalP& e, double dnorm, 
     return dD > 0.0 ? (float)(1.0 / dD) : 0.0f;   // 0 marks "excluded: dD_v <= 0"
 }
 
-template <bool STAR>
 __global__ void __launch_bounds__(PREP_THREADS)
-k_prep_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
-            EvalP e, Ctl* __restrict__ ctl, unsigned* __restrict__ listKey, unsigned* __restrict__ listIdx)
+k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, EvalP e, Ctl* __restrict__ ctl,
+           unsigned* __restrict__ evalIdx)
 {
-    __shared__ int sQueue[PREP_QUEUE];
-    __shared__ unsigned sHist[KEY_DIGITS];
-    __shared__ unsigned sCnt;
-    __shared__ int sChunk;
-    __shared__ float sMax[PREP_THREADS / 32];
-    const int tid = threadIdx.x, lane = tid & 31;
+    __shared__ unsigned sWarp[PREP_THREADS / 32];
+    __shared__ unsigned sBase;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned FULL = 0xffffffffu;
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
     const double dnorm = (double)dnormF;
     const double thr = (double)e.cutoff * dnorm;      // decided in double (include/gamma_b200.h)
     const float invGlobal = criterion_inv_dD(e, dnorm, 0.0f);
+    const bool globalOk = invGlobal > 0.0f;
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->invGlobal = invGlobal;   // the later kernels read it from here
     const float qnan = __int_as_float(0x7fc00000);
     const int numChunks = (g.N + PREP_CHUNK - 1) / PREP_CHUNK;
     const bool vec = ((reinterpret_cast<uintptr_t>(ref) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0;
+
+    for (int chunk = blockIdx.x; chunk < numChunks; chunk += gridDim.x) {
+        const int lin0 = chunk * PREP_CHUNK + tid * 4;
+        float Dr[4];
+        int nval = 0;
+        if (vec && lin0 + 3 < g.N) {
+            const float4 v = __ldg(reinterpret_cast<const float4*>(ref + lin0));
+            Dr[0] = v.x; Dr[1] = v.y; Dr[2] = v.z; Dr[3] = v.w;
+            nval = 4;
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (lin0 + j < g.N) { Dr[j] = __ldg(ref + lin0 + j); nval = j + 1; } else Dr[j] = 0.0f;
+        }
+        unsigned keepMask = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool excluded = ((double)Dr[j] < thr) ||
+                                  (e.mode == 0 ? !globalOk : !((double)e.DD * (double)Dr[j] > 0.0));
+            if (j < nval && !excluded) keepMask |= 1u << j;
+        }
+        if (keepMask == 0 && nval == 4 && vec) {
+            *reinterpret_cast<float4*>(out + lin0) = make_float4(qnan, qnan, qnan, qnan);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (j < nval && !(keepMask & (1u << j))) out[lin0 + j] = qnan;
+        }
+        const int c = __popc(keepMask);
+        int incl = c;
+#pragma unroll
+        for (int s = 1; s < 32; s <<= 1) {
+            const int t = __shfl_up_sync(FULL, incl, s);
+            if (lane >= s) incl += t;
+        }
+        if (lane == 31) sWarp[warp] = (unsigned)incl;
+        __syncthreads();
+        if (tid == 0) {
+            unsigned tot = 0;
+#pragma unroll
+            for (int w = 0; w < PREP_THREADS / 32; ++w) { const unsigned t = sWarp[w]; sWarp[w] = tot; tot += t; }
+            sBase = tot ? atomicAdd(&ctl->nEval, tot) : 0u;
+        }
+        __syncthreads();
+        unsigned pos = sBase + sWarp[warp] + (unsigned)(incl - c);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (keepMask & (1u << j)) evalIdx[pos++] = (unsigned)(lin0 + j);
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// first part of a4: the star phase over the compacted voxels, one voxel per thread, one warp per 32
+// consecutive list entries (first round static, later rounds fetched dynamically).
+// ------------------------------------------------------------------------------------------------
+constexpr int STAR_THREADS = 256;
+#ifndef GAMMA_STAR_MIN_BLOCKS
+#define GAMMA_STAR_MIN_BLOCKS 3
+#endif
+
+template <bool STAR>
+__global__ void __launch_bounds__(STAR_THREADS, GAMMA_STAR_MIN_BLOCKS)
+k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g, EvalP e,
+       Ctl* __restrict__ ctl, const unsigned* __restrict__ evalIdx, unsigned* __restrict__ listKey,
+       unsigned* __restrict__ listIdx)
+{
+    __shared__ unsigned sHist[KEY_DIGITS];
+    __shared__ float sMax[STAR_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const unsigned FULL = 0xffffffffu;
+    const unsigned M = ctl->nEval;
+    const unsigned warpsTotal = gridDim.x * (STAR_THREADS / 32);
+    const unsigned numItems = (M + 31u) / 32u;
+    const bool dynamic = numItems > warpsTotal;
+    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
+    const double dnorm = (double)dnormF;
+    const float invGlobal = ctl->invGlobal;
+    const float qnan = __int_as_float(0x7fc00000);
+    // squared spatial distance of the 26 neighbours, by the set T of axes they differ in
+    float A[8];
+    A[0] = 0.0f;
+#pragma unroll
+    for (int T = 1; T < 8; ++T) A[T] = ((T & 1) ? g.hh[0] : 0.0f) + ((T & 2) ? g.hh[1] : 0.0f) + ((T & 4) ? g.hh[2] : 0.0f);
     float maxKey = 0.0f;
-    unsigned nEvalLocal = 0;
 
     sHist[tid] = 0;
-    if (tid == 0) { sCnt = 0; sChunk = blockIdx.x; }
     __syncthreads();
 
-    // One queued voxel: key, star phase, final write or append to the search list.
-    auto star_item = [&](bool valid, int lin) {
+    unsigned item = blockIdx.x * (STAR_THREADS / 32) + (tid >> 5);
+    while (item < numItems) {
+        unsigned nextItem = numItems;
+        if (dynamic && lane == 0) nextItem = atomicAdd(&ctl->tileCounter, 1u) + warpsTotal;
+        const unsigned j = item * 32u + lane;
         bool toSearch = false;
         float key = 0.0f;
-        if (valid) {
+        int lin = 0;
+        if (j < M) {
+            lin = (int)evalIdx[j];
             const float Dr = __ldg(ref + lin);
             const float invdD = e.mode == 0 ? invGlobal : criterion_inv_dD(e, dnorm, Dr);
             const float d0 = (__ldg(ev + lin) - Dr) * invdD;
             key = fabsf(d0);                              // A1 step 4-a: gamma <- |DD| / dD
             toSearch = true;
             if (STAR && g.all_active) {
-                const int ix = lin % g.n[0], iy = (lin / g.n[0]) % g.n[1], iz = lin / g.stride[2];
+                int ix, iy, iz;
+                voxel_coords(g, lin, ix, iy, iz);
                 const bool interior = ix >= 1 && ix <= g.n[0] - 2 && iy >= 1 && iy <= g.n[1] - 2 &&
                                       iz >= 1 && iz <= g.n[2] - 2;
                 if (interior) {
                     float d[27];
                     const float* p = ev + lin;
+                    float vb = d0 * d0;                   // squared distance to the nearest of the 27 grid points
+                    float dlo = d0, dhi = d0;             // dose range of the 27 grid points
 #pragma unroll
                     for (int oz = -1; oz <= 1; ++oz)
 #pragma unroll
                         for (int oy = -1; oy <= 1; ++oy)
 #pragma unroll
-                            for (int ox = -1; ox <= 1; ++ox)
-                                d[(ox + 1) + 3 * (oy + 1) + 9 * (oz + 1)] =
-                                    (__ldg(p + ox + oy * g.stride[1] + oz * g.stride[2]) - Dr) * invdD;
-                    d[13] = d0;
+                            for (int ox = -1; ox <= 1; ++ox) {
+                                const int k = (ox + 1) + 3 * (oy + 1) + 9 * (oz + 1);
+                                if (k == 13) { d[13] = d0; continue; }
+                                const float dv = (__ldg(p + ox + oy * g.stride[1] + oz * g.stride[2]) - Dr) * invdD;
+                                d[k] = dv;
+                                vb = fminf(vb, fmaf(dv, dv, A[(ox ? 1 : 0) | (oy ? 2 : 0) | (oz ? 4 : 0)]));
+                                dlo = fminf(dlo, dv);
+                                dhi = fmaxf(dhi, dv);
+                            }
                     const float gmax = gamma_star_gmax(d, g.invA);
                     key = key / sqrtf(gmax);              // gamma_star
-                    if (key * key <= g.rho_link2) {       // nothing outside the star can be closer
+                    // Lower bound of everything OUTSIDE the star: beyond the 8 touching cells the spatial distance
+                    // alone is >= hmin; inside them (but outside the star) it is >= rho_link and the dose is a
+                    // convex combination of the 27 grid doses, so its distance from 0 is >= that of their range.
+                    const float dr = fmaxf(fmaxf(dlo, -dhi), 0.0f);
+                    const float outside2 = fminf(g.hmin2, fmaf(dr, dr, g.rho_link2));
+                    if (key * key <= outside2) {          // nothing outside the star can be closer
                         out[lin] = key;
                         toSearch = false;
+                    } else {
+                        key = fminf(key, sqrtf(vb));      // the 26 neighbour grid points also bound gamma from above
                     }
                 }
             }
@@ -170,73 +271,8 @@ k_prep_star(const float* __restrict__ ref, const float* __restrict__ ev, float* 
                 maxKey = fmaxf(maxKey, key);
             }
         }
-    };
-
-    for (;;) {
-        const int chunk = sChunk;
-        if (chunk >= numChunks) break;
-        // ---- a1: exclusion (4 consecutive voxels per thread) + compaction into the block queue
-        const int lin0 = chunk * PREP_CHUNK + tid * 4;
-        float Dr[4];
-        int nval = 0;
-        if (vec && lin0 + 3 < g.N) {
-            const float4 v = __ldg(reinterpret_cast<const float4*>(ref + lin0));
-            Dr[0] = v.x; Dr[1] = v.y; Dr[2] = v.z; Dr[3] = v.w;
-            nval = 4;
-        } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (lin0 + j < g.N) { Dr[j] = __ldg(ref + lin0 + j); nval = j + 1; } else Dr[j] = 0.0f;
-        }
-        unsigned keepMask = 0;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const bool excluded = ((double)Dr[j] < thr) ||
-                                  (e.mode == 0 ? !(invGlobal > 0.0f) : !((double)e.DD * (double)Dr[j] > 0.0));
-            if (j < nval && !excluded) keepMask |= 1u << j;
-        }
-        if (keepMask == 0 && nval == 4 && vec) {
-            *reinterpret_cast<float4*>(out + lin0) = make_float4(qnan, qnan, qnan, qnan);
-        } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (j < nval && !(keepMask & (1u << j))) out[lin0 + j] = qnan;
-        }
-        const int c = __popc(keepMask);
-        nEvalLocal += (unsigned)c;
-        int incl = c;
-#pragma unroll
-        for (int s = 1; s < 32; s <<= 1) {
-            const int t = __shfl_up_sync(FULL, incl, s);
-            if (lane >= s) incl += t;
-        }
-        const int wtot = __shfl_sync(FULL, incl, 31);
-        unsigned wbase = 0;
-        if (lane == 31 && wtot) wbase = atomicAdd(&sCnt, (unsigned)wtot);
-        wbase = __shfl_sync(FULL, wbase, 31);
-        int pos = (int)wbase + incl - c;
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (keepMask & (1u << j)) sQueue[pos++] = lin0 + j;
-        __syncthreads();
-        int cnt = (int)sCnt;
-        if (tid == 0) sChunk = (int)atomicAdd(&ctl->tileCounter, 1u) + (int)gridDim.x;   // next chunk, fetched early
-        // ---- star phase on full batches popped from the end of the queue
-        while (cnt >= PREP_THREADS) {
-            star_item(true, sQueue[cnt - PREP_THREADS + tid]);
-            cnt -= PREP_THREADS;
-        }
-        __syncthreads();
-        if (tid == 0) sCnt = (unsigned)cnt;
-        __syncthreads();
+        item = __shfl_sync(FULL, nextItem, 0);
     }
-    {   // leftovers (< one batch)
-        const int cnt = (int)sCnt;
-        star_item(tid < cnt, tid < cnt ? sQueue[tid] : 0);
-    }
-#pragma unroll
-    for (int s = 16; s > 0; s >>= 1) nEvalLocal += __shfl_xor_sync(FULL, nEvalLocal, s);
-    if (lane == 0 && nEvalLocal) atomicAdd(&ctl->nEval, nEvalLocal);
     maxKey = warp_max(maxKey);
     if (lane == 0) sMax[tid >> 5] = maxKey;
     __syncthreads();
@@ -244,7 +280,7 @@ k_prep_star(const float* __restrict__ ref, const float* __restrict__ ev, float* 
     if (tid == 0) {
         float m = 0.0f;
 #pragma unroll
-        for (int w = 0; w < PREP_THREADS / 32; ++w) m = fmaxf(m, sMax[w]);
+        for (int w = 0; w < STAR_THREADS / 32; ++w) m = fmaxf(m, sMax[w]);
         if (m > 0.0f) atomicMax(&ctl->maxKeyBits, __float_as_uint(m));
     }
 }
@@ -353,134 +389,170 @@ __device__ __forceinline__ float group_min(float v)
 
 constexpr int SEARCH_THREADS = 256;
 
-// G lanes per reference voxel: 1 (thread per voxel), 8 or 32.
+struct SearchCtx {
+    const float* ref; const float* ev; float* out;
+    const unsigned* listKey; const unsigned* listIdx; const int4* table;
+    unsigned nS, T;
+    bool trunc;
+    float Rtab2, invGlobal;
+    double dnorm;
+};
+
+// One warp searches 32/G consecutive work items (firstItem .. firstItem + 32/G - 1, counted from the END of the
+// sorted list: deepest first), G lanes per reference voxel.  Returns the owner vertices it evaluated.
 template <int G>
-__global__ void __launch_bounds__(SEARCH_THREADS)
-k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
-               EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
-               const unsigned* __restrict__ listIdx, const int4* __restrict__ table)
+__device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP& g, const EvalP& e, unsigned firstItem,
+                                                 int lane)
 {
-    constexpr int VPW = 32 / G;                 // voxels per warp
     constexpr int EPP = G >= 8 ? G / 8 : 1;     // table entries per pass
     const unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
     const int gid = lane / G, gl = lane % G;
-    const unsigned nS = ctl->nSearch;
-    const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
-    // first round: static assignment (no atomic storm at kernel start); later rounds: dynamic fetch
-    unsigned base = (blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5)) * (unsigned)VPW;
-    if (base >= nS) return;
-    const bool dynamic = nS > warpsTotal * (unsigned)VPW;     // otherwise the first round covers the whole list
-    const unsigned T = ctl->tableCount;
-    const bool trunc = ctl->tableTrunc != 0;
-    const float Rtab2 = ctl->Rtab2;
-    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
-    const double dnorm = (double)dnormF;
-    const float invGlobal = criterion_inv_dD(e, dnorm, 0.0f);
+    const unsigned item = firstItem + gid;
+    const bool have = item < c.nS;
+    const unsigned T = c.T;
     unsigned visits = 0;
-
-    for (;;) {
-        const unsigned item = base + gid;
-        const bool have = item < nS;
-        VoxelCtx vc;
-        float key = 0.0f, best2 = 0.0f;
-        if (have) {
-            const unsigned idx = nS - 1u - item;              // deepest searches first
-            vc.lin = (int)listIdx[idx];
-            key = __uint_as_float(listKey[idx]);
-            vc.Dr = __ldg(ref + vc.lin);
-            vc.invdD = e.mode == 0 ? invGlobal : criterion_inv_dD(e, dnorm, vc.Dr);
-            vc.v[0] = vc.lin % g.n[0];
-            vc.v[1] = (vc.lin / g.n[0]) % g.n[1];
-            vc.v[2] = vc.lin / g.stride[2];
-            best2 = key * key;
+    VoxelCtx vc;
+    float key = 0.0f, best2 = 0.0f;
+    if (have) {
+        const unsigned idx = c.nS - 1u - item;
+        vc.lin = (int)c.listIdx[idx];
+        key = __uint_as_float(c.listKey[idx]);
+        vc.Dr = __ldg(c.ref + vc.lin);
+        vc.invdD = e.mode == 0 ? c.invGlobal : criterion_inv_dD(e, c.dnorm, vc.Dr);
+        voxel_coords(g, vc.lin, vc.v[0], vc.v[1], vc.v[2]);
+        best2 = key * key;
+    } else {
+        vc.lin = 0; vc.Dr = 0.0f; vc.invdD = 0.0f; vc.v[0] = vc.v[1] = vc.v[2] = 0;
+    }
+    // ---- Algorithm A1 step 4-b over the sorted table
+    for (unsigned e0 = 0;; e0 += EPP) {
+        bool more = have && e0 < T;
+        if (more) more = __int_as_float(__ldg(&c.table[e0].x)) < best2;    // 4-b-ii: stop at L >= gamma
+        if (!__any_sync(FULL, more)) break;
+        if (G >= 8) {
+            const unsigned en = e0 + (unsigned)(gl >> 3);
+            float cand = best2;
+            if (more && en < T) {
+                const int4 t = __ldg(&c.table[en]);
+                if (__int_as_float(t.x) < best2) {
+                    const int ox = (gl & 1) ? -t.y - 1 : t.y;
+                    const int oy = (gl & 2) ? -t.z - 1 : t.z;
+                    const int oz = (gl & 4) ? -t.w - 1 : t.w;
+                    cand = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                    ++visits;
+                }
+            }
+            best2 = group_min<(G >= 8 ? G : 8)>(cand);
         } else {
-            vc.lin = 0; vc.Dr = 0.0f; vc.invdD = 0.0f; vc.v[0] = vc.v[1] = vc.v[2] = 0;
+            if (more) {
+                const int4 t = __ldg(&c.table[e0]);
+#pragma unroll 1
+                for (int var = 0; var < 8; ++var) {
+                    const int ox = (var & 1) ? -t.y - 1 : t.y;
+                    const int oy = (var & 2) ? -t.z - 1 : t.z;
+                    const int oz = (var & 4) ? -t.w - 1 : t.w;
+                    best2 = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                    ++visits;
+                }
+            }
         }
-        // next work item, fetched early so that its latency hides behind this search
-        unsigned nextBase = nS;
-        if (dynamic && lane == 0) nextBase = atomicAdd(&ctl->workCounter, (unsigned)VPW) + warpsTotal * (unsigned)VPW;
-        // ---- Algorithm A1 step 4-b over the sorted table
-        for (unsigned e0 = 0;; e0 += EPP) {
-            bool more = have && e0 < T;
-            if (more) more = __int_as_float(__ldg(&table[e0].x)) < best2;    // 4-b-ii: stop at L >= gamma
+    }
+    // ---- beyond a truncated table: exhaustive enumeration of the remaining octant box (exact, slow)
+    if (c.trunc) {
+        const float Rtab2 = c.Rtab2;
+        int rx = 0, ry = 0, rz = 0;
+        unsigned V = 0;
+        if (have && best2 > Rtab2) {
+            const float b = sqrtf(best2);
+            rx = g.h[0] > 0.0f ? (int)fminf((float)(g.n[0] - 1), floorf(b / g.h[0])) + 1 : 1;
+            ry = g.h[1] > 0.0f ? (int)fminf((float)(g.n[1] - 1), floorf(b / g.h[1])) + 1 : 1;
+            rz = g.h[2] > 0.0f ? (int)fminf((float)(g.n[2] - 1), floorf(b / g.h[2])) + 1 : 1;
+            V = (unsigned)(rx * ry * rz);
+        }
+        for (unsigned i0 = 0;; i0 += EPP) {
+            const bool more = i0 < V && best2 > Rtab2;
             if (!__any_sync(FULL, more)) break;
             if (G >= 8) {
-                const unsigned en = e0 + (unsigned)(gl >> 3);
+                const unsigned i = i0 + (unsigned)(gl >> 3);
                 float cand = best2;
-                if (more && en < T) {
-                    const int4 t = __ldg(&table[en]);
-                    if (__int_as_float(t.x) < best2) {
-                        const int ox = (gl & 1) ? -t.y - 1 : t.y;
-                        const int oy = (gl & 2) ? -t.z - 1 : t.z;
-                        const int oz = (gl & 4) ? -t.w - 1 : t.w;
-                        cand = eval_owner_vertex(ev, g, vc, ox, oy, oz, best2);
+                if (more && i < V) {
+                    const int mx = i % rx, my = (i / rx) % ry, mz = i / (rx * ry);
+                    const float L2 = cell_L2(mx, my, mz, g);
+                    if (L2 >= Rtab2 && L2 < best2) {
+                        const int ox = (gl & 1) ? -mx - 1 : mx;
+                        const int oy = (gl & 2) ? -my - 1 : my;
+                        const int oz = (gl & 4) ? -mz - 1 : mz;
+                        cand = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
                         ++visits;
                     }
                 }
                 best2 = group_min<(G >= 8 ? G : 8)>(cand);
-            } else {
-                if (more) {
-                    const int4 t = __ldg(&table[e0]);
+            } else if (more) {
+                const int mx = i0 % rx, my = (i0 / rx) % ry, mz = i0 / (rx * ry);
+                const float L2 = cell_L2(mx, my, mz, g);
+                if (L2 >= Rtab2 && L2 < best2) {
 #pragma unroll 1
                     for (int var = 0; var < 8; ++var) {
-                        const int ox = (var & 1) ? -t.y - 1 : t.y;
-                        const int oy = (var & 2) ? -t.z - 1 : t.z;
-                        const int oz = (var & 4) ? -t.w - 1 : t.w;
-                        best2 = eval_owner_vertex(ev, g, vc, ox, oy, oz, best2);
+                        const int ox = (var & 1) ? -mx - 1 : mx;
+                        const int oy = (var & 2) ? -my - 1 : my;
+                        const int oz = (var & 4) ? -mz - 1 : mz;
+                        best2 = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
                         ++visits;
                     }
                 }
             }
         }
-        // ---- beyond a truncated table: exhaustive enumeration of the remaining octant box (exact, slow)
-        if (trunc) {
-            int rx = 0, ry = 0, rz = 0;
-            unsigned V = 0;
-            if (have && best2 > Rtab2) {
-                const float b = sqrtf(best2);
-                rx = g.h[0] > 0.0f ? (int)fminf((float)(g.n[0] - 1), floorf(b / g.h[0])) + 1 : 1;
-                ry = g.h[1] > 0.0f ? (int)fminf((float)(g.n[1] - 1), floorf(b / g.h[1])) + 1 : 1;
-                rz = g.h[2] > 0.0f ? (int)fminf((float)(g.n[2] - 1), floorf(b / g.h[2])) + 1 : 1;
-                V = (unsigned)(rx * ry * rz);
-            }
-            for (unsigned i0 = 0;; i0 += EPP) {
-                const bool more = i0 < V && best2 > Rtab2;
-                if (!__any_sync(FULL, more)) break;
-                if (G >= 8) {
-                    const unsigned i = i0 + (unsigned)(gl >> 3);
-                    float cand = best2;
-                    if (more && i < V) {
-                        const int mx = i % rx, my = (i / rx) % ry, mz = i / (rx * ry);
-                        const float L2 = cell_L2(mx, my, mz, g);
-                        if (L2 >= Rtab2 && L2 < best2) {
-                            const int ox = (gl & 1) ? -mx - 1 : mx;
-                            const int oy = (gl & 2) ? -my - 1 : my;
-                            const int oz = (gl & 4) ? -mz - 1 : mz;
-                            cand = eval_owner_vertex(ev, g, vc, ox, oy, oz, best2);
-                            ++visits;
-                        }
-                    }
-                    best2 = group_min<(G >= 8 ? G : 8)>(cand);
-                } else if (more) {
-                    const int mx = i0 % rx, my = (i0 / rx) % ry, mz = i0 / (rx * ry);
-                    const float L2 = cell_L2(mx, my, mz, g);
-                    if (L2 >= Rtab2 && L2 < best2) {
-#pragma unroll 1
-                        for (int var = 0; var < 8; ++var) {
-                            const int ox = (var & 1) ? -mx - 1 : mx;
-                            const int oy = (var & 2) ? -my - 1 : my;
-                            const int oz = (var & 4) ? -mz - 1 : mz;
-                            best2 = eval_owner_vertex(ev, g, vc, ox, oy, oz, best2);
-                            ++visits;
-                        }
-                    }
-                }
-            }
+    }
+    if (have && gl == 0) c.out[vc.lin] = fminf(key, sqrtf(best2));   // a5: write at the voxel's own place
+    return visits;
+}
+
+// MODE = lanes per reference voxel: 1 (thread per voxel), 8, 32, or 0 = adaptive: the nDeep
+// deepest items of the sorted list (key digit >= deepDigit: the search will pass the first table entry) get a
+// whole warp each, the others 8 lanes each.  Work units are handed out deepest first: first round static,
+// later rounds by an atomic counter whose latency hides behind the current search.
+template <int MODE>
+__global__ void __launch_bounds__(SEARCH_THREADS)
+k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
+               EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
+               const unsigned* __restrict__ listIdx, const int4* __restrict__ table, int deepDigit)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    SearchCtx c;
+    c.nS = ctl->nSearch;
+    if (c.nS == 0) return;
+    unsigned nDeep = 0;
+    if (MODE == 0 && deepDigit < KEY_DIGITS) {                // sum of the histogram tail = number of deep items
+        for (int d = deepDigit + lane; d < KEY_DIGITS; d += 32) nDeep += ctl->hist[d];
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) nDeep += __shfl_xor_sync(FULL, nDeep, s);
+    }
+    constexpr unsigned VPW = MODE == 0 ? 4u : 32u / (unsigned)(MODE == 0 ? 8 : MODE);
+    const unsigned numUnits = MODE == 0 ? nDeep + (c.nS - nDeep + 3u) / 4u : (c.nS + VPW - 1u) / VPW;
+    const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
+    unsigned unit = blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5);
+    if (unit >= numUnits) return;
+    const bool dynamic = numUnits > warpsTotal;
+    c.ref = ref; c.ev = ev; c.out = out; c.listKey = listKey; c.listIdx = listIdx; c.table = table;
+    c.T = ctl->tableCount;
+    c.trunc = ctl->tableTrunc != 0;
+    c.Rtab2 = ctl->Rtab2;
+    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
+    c.dnorm = (double)dnormF;
+    c.invGlobal = ctl->invGlobal;
+    unsigned visits = 0;
+
+    while (unit < numUnits) {
+        unsigned nextUnit = numUnits;
+        if (dynamic && lane == 0) nextUnit = atomicAdd(&ctl->workCounter, 1u) + warpsTotal;
+        if (MODE == 0) {
+            if (unit < nDeep) visits += search_items<32>(c, g, e, unit, lane);
+            else visits += search_items<8>(c, g, e, nDeep + 4u * (unit - nDeep), lane);
+        } else {
+            visits += search_items<(MODE == 0 ? 8 : MODE)>(c, g, e, unit * VPW, lane);
         }
-        if (have && gl == 0) out[vc.lin] = fminf(key, sqrtf(best2));   // a5: write at the voxel's own place
-        base = __shfl_sync(FULL, nextBase, 0);
-        if (base >= nS) break;
+        unit = __shfl_sync(FULL, nextUnit, 0);
     }
     // diagnostic counter: one atomic per warp
     for (int s = 16; s > 0; s >>= 1) visits += __shfl_xor_sync(FULL, visits, s);

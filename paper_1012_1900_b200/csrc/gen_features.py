@@ -185,7 +185,7 @@ def emit_owned(w):
         conds.append("%s >= 0.0f" % ts[-1])
         c = cval(ch)
         dist = "fmaf(%s, r, %s)" % (N, c) if c else "%s * r" % N
-        w("        if (%s) best2 = fminf(best2, %s);\n" % (" && ".join("(%s)" % x for x in conds), dist))
+        w("        best2 = (%s) ? fminf(best2, %s) : best2;\n" % (" & ".join("(%s)" % x for x in conds), dist))
         w("    }\n")
     w("    return best2;\n}\n")
 
@@ -200,7 +200,11 @@ def main():
         w("// closed form for chains of orthogonal steps; see gen_features.py and DESIGN.md.\n")
         w("#pragma once\n#include <math.h>\n")
         w("#if defined(__CUDACC__)\n#define GAMMA_HD __host__ __device__ __forceinline__\n#else\n#define GAMMA_HD inline\n#endif\n")
-        w("#if defined(__CUDA_ARCH__)\n#define GAMMA_FDIV(a, b) __fdividef((a), (b))\n#else\n#define GAMMA_FDIV(a, b) ((a) / (b))\n#endif\n\n")
+        w("// N / G with G >= 1: one MUFU.RCP and one FMUL (relative error ~1e-7; __fdividef adds range fix-ups\n")
+        w("// that G >= 1 never needs).\n")
+        w("#if defined(__CUDA_ARCH__)\n__device__ __forceinline__ float gamma_fdiv(float a, float b)\n{\n"
+          "    float r;\n    asm(\"rcp.approx.ftz.f32 %0, %1;\" : \"=f\"(r) : \"f\"(b));\n    return a * r;\n}\n"
+          "#define GAMMA_FDIV(a, b) gamma_fdiv((a), (b))\n#else\n#define GAMMA_FDIV(a, b) ((a) / (b))\n#endif\n\n")
         emit_star(w)
         emit_owned(w)
     print("wrote", path)
