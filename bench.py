@@ -34,6 +34,10 @@ sys.path.insert(0, ROOT)
 SM_COUNT, FP32_LANES, SM_MAX_MHZ_NOMINAL = 148, 128, 1965.0
 F_CELL_3D, F_CELL_2D = 1911.0, 190.0       # canonical flops per visited cell, frozen in BASELINE.md
 L2_BYTES = 126e6
+# executed FP32 flops per unit (ncu smsp__sass_thread_inst_executed_op_{fadd,fmul,ffma}; profiles/)
+FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT = 406.0, 382.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on cfg3 from the same ncu --set full capture
+TRAFFIC_BYTES = {"k_star": 2.62e6, "k_table_search": 1.82e6}
 
 
 def f32(x):
@@ -307,27 +311,35 @@ def main():
         return
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------
+    # bound "alu": executed FP32 flops (FADD + FMUL + 2 FFMA thread instructions; per-unit constants measured
+    # with ncu) x the units the library counted for this launch / the kernel's CUDA-event
+    # duration.  "canonical" is the useful rate by the normal-equations flop count of SURVEY.md section 8(d).
     wm = work_model(case.name) or {}
     ndim = sum(d > 1 for d in case.dims)
     fcell = F_CELL_3D if ndim == 3 else F_CELL_2D
-    kernel_ms = {"k_prep_star": stages["prep_ms"], "k_table_search": stages["search_ms"]}
+    kernel_ms = {"k_star": stages["star_ms"], "k_table_search": stages["search_ms"]}
+    units = {"k_star": M, "k_table_search": cnt["vertex_visits"]}
+    flop_per_unit = {"k_star": FLOP_PER_STAR_VOXEL if ndim == 3 else 0.0, "k_table_search": FLOP_PER_VISIT}
     dom = max(kernel_ms, key=kernel_ms.get)
     peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ_NOMINAL * 1e6 / 1e12
-    roof = {"bound": "alu", "kernel": dom, "peak": peak, "unit": "TFLOP/s", "traffic": None,
-            "peak_source": "148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and clocks.max.sm)",
-            "ffma_chain_measured_tflops": probe_tflops, "stage_ms": stages}
+    alg = units[dom] * flop_per_unit[dom]
+    roof = {"bound": "alu", "kernel": dom, "peak": peak, "unit": "TFLOP/s", "traffic": TRAFFIC_BYTES.get(dom),
+            "peak_source": "148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and clocks.max.sm); "
+                           "MEASURED_PEAKS.json has no FP32 figure",
+            "ffma_chain_measured_tflops": probe_tflops, "stage_ms": stages,
+            "units_per_launch": units[dom], "flop_per_unit": flop_per_unit[dom],
+            "algorithmic_flops_per_launch": alg,
+            "achieved": alg / (kernel_ms[dom] * 1e-3) / 1e12}
+    roof["frac"] = roof["achieved"] / peak
+    exec_total = units["k_star"] * flop_per_unit["k_star"] + units["k_table_search"] * flop_per_unit["k_table_search"]
+    roof["whole_path"] = {"executed_fp32_flops": exec_total, "achieved": exec_total / (ms_step * 1e-3) / 1e12,
+                          "frac": exec_total / (ms_step * 1e-3) / 1e12 / peak}
     if wm:
-        star_flops = wm["sum_touch"] * fcell
-        search_flops = (wm["sum_Ns"] - wm["sum_touch"]) * fcell
-        alg = {"k_prep_star": star_flops, "k_table_search": search_flops}[dom]
-        roof["algorithmic_flops_per_launch"] = alg
-        roof["achieved"] = alg / (kernel_ms[dom] * 1e-3) / 1e12
-        roof["frac"] = roof["achieved"] / peak
         total_flops = wm["sum_Ns"] * fcell
-        roof["whole_path"] = {"algorithmic_flops": total_flops, "achieved": total_flops / (ms_step * 1e-3) / 1e12,
-                              "frac": total_flops / (ms_step * 1e-3) / 1e12 / peak}
-    else:
-        roof["achieved"], roof["frac"] = None, None
+        roof["canonical"] = {"flops_per_cell_visit": fcell, "cell_visits": wm["sum_Ns"], "flops": total_flops,
+                             "useful_tflops": total_flops / (ms_step * 1e-3) / 1e12,
+                             "note": "normal-equations count of SURVEY.md 8(d); the closed form executes ~13x fewer "
+                                     "operations, so this is a useful-work rate, not a utilisation"}
 
     line = {
         "metric": "gamma evaluations per second", "value": world * M / (ms_step * 1e-3),

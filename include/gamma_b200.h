@@ -162,12 +162,12 @@ int gamma_get_counters(gamma_counters* out_host);
 /* Device time of each stage of the last gamma_eval* call made with opts.profile_stages = 1 (CUDA events on
  * the call's stream).  SYNCHRONISES that stream.  HOST output; milliseconds. */
 typedef struct gamma_stage_times {
-    float norm_ms;   /* a0 + A1 step 1: max(ref), max|DD| (k_norm)                               */
-    float prep_ms;   /* a1 + star phase (k_prep_star)                                            */
-    float table_ms;  /* a3: offset table, on the side stream, CONCURRENT with prep_ms/sort_ms    */
+    float prep_ms;   /* a0 + A1 step 1 + a1: max(ref), max|DD|, cutoff + compaction (k_norm, k_classify) */
+    float star_ms;   /* a1 + first part of a4: keys and the star phase (k_star)                  */
+    float table_ms;  /* a3: offset table, on the side stream, CONCURRENT with star_ms            */
     float sort_ms;   /* a2: presort of the search work list                                      */
     float search_ms; /* a4 + a5: join with the side stream, table search and write-back          */
-    float total_ms;  /* first event to last event on `stream` = norm + prep + sort + search      */
+    float total_ms;  /* first event to last event on `stream` = prep + star + sort + search      */
 } gamma_stage_times;
 int gamma_get_stage_times(gamma_stage_times* out_host);
 

@@ -42,7 +42,7 @@ class _COpts(ctypes.Structure):
 
 
 class _CStageTimes(ctypes.Structure):
-    _fields_ = [("norm_ms", ctypes.c_float), ("prep_ms", ctypes.c_float), ("table_ms", ctypes.c_float),
+    _fields_ = [("prep_ms", ctypes.c_float), ("star_ms", ctypes.c_float), ("table_ms", ctypes.c_float),
                 ("sort_ms", ctypes.c_float), ("search_ms", ctypes.c_float), ("total_ms", ctypes.c_float)]
 
 

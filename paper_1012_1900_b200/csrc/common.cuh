@@ -63,6 +63,8 @@ struct Ctl {
     float Rtab2;           // squared radius the table covers
     int box[3];            // table box: m_a in [0, box_a)
     unsigned sortN;        // element count for gamma_sort_pairs
+    unsigned barrier;      // spare
+    unsigned pad0_;
     float invGlobal;       // 1 / (DD * D_norm) rounded to fp32 (global criterion), written by k_classify
     unsigned long long visits;       // owner vertices evaluated by the table search
     unsigned hist[KEY_DIGITS];       // digit histogram of the search list (bucket presort)

@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -35,6 +36,25 @@ int fail(int code, const std::string& msg)
             return fail(e_ == cudaErrorMemoryAllocation ? GAMMA_ERR_OUT_OF_MEMORY : GAMMA_ERR_CUDA, \
                         std::string(#call) + ": " + cudaGetErrorString(e_));                 \
     } while (0)
+
+
+// Kernel launch with attributes: `pdl` = programmatic dependent launch (the kernel may start while its predecessor
+// in the stream drains; it calls pdl_wait() before touching the predecessor's results), `coop` = cooperative
+// (all blocks co-resident: required by the grid barrier of k_norm).
+template <typename... KArgs, typename... Args>
+cudaError_t launch_ex(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, bool pdl, bool coop,
+                      Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[2];
+    unsigned n = 0;
+    if (pdl) { at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[n].val.programmaticStreamSerializationAllowed = 1; ++n; }
+    if (coop) { at[n].id = cudaLaunchAttributeCooperative; at[n].val.cooperative = 1; ++n; }
+    cfg.attrs = at; cfg.numAttrs = n;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
 
 // grow-only device buffer
 struct Buf {
@@ -77,6 +97,7 @@ struct Workspace {
     long long launches = 0;        // kernels launched so far (gamma_launch_count)
     int numSM = 0;
     int occStar[2] = {0, 0};       // resident blocks per SM of k_star<false/true>
+    int pdl = -1;                  // programmatic dependent launch between the kernels of a call (GAMMA_PDL=0 disables)
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
     long long lastN = 0;
@@ -304,11 +325,11 @@ int check_criteria(float DD, int mode, float cutoff)
 
 // Enqueue the whole hot path on `st` (device pointers).  Caller holds g_mu.
 //
-//   st :  k_norm -> k_prep_star -> [k_bucket_scatter | LSD radix sort] -> (join) -> k_table_search
+//   st :  k_norm -> k_star -> [k_bucket_scatter | LSD radix sort] -> (join) -> k_table_search
 //   aux:        \-> k_offset_table ------------------------------------------/
 //
 // The offset table only needs k_norm's maxima, so it is built on a library-owned side stream while the
-// prep/star kernel runs.  No memset and no host synchronisation on the path: k_norm clears the control
+// star kernel runs.  No memset and no host synchronisation on the path: k_norm clears the control
 // block of the next call (two alternating slots; slot 2 belongs to the stand-alone entry points).
 int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
                      const Resolved& r, float* out, cudaStream_t st)
@@ -353,15 +374,13 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             if (!evn) CU_TRY(cudaEventCreate(&evn));
 #define STAGE_MARK(i, s) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], s)); } while (0)
     const int sm = g_ws.numSM;
-    STAGE_MARK(0, st);
-    {                                                                    // a0 + A1 step 1
-        long long blocks = (N + 1023) / 1024;
-        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
-        k_norm<<<grid, NORM_THREADS, 0, st>>>(ref, ev, (int)N, mode, ctl, next);
-        ++g_ws.launches;
+    if (g_ws.pdl < 0) {
+        const char* env = std::getenv("GAMMA_PDL");
+        g_ws.pdl = (env && env[0] == '0') ? 0 : 1;
     }
-    STAGE_MARK(1, st);
-    {                                                                    // a3 on the side stream
+    const bool pdl = g_ws.pdl != 0;
+    STAGE_MARK(0, st);
+    auto fork_table = [&]() -> int {                                     // a3 on the side stream                                                                    // a3 on the side stream
         CU_TRY(cudaEventRecord(g_ws.evFork, st));
         CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
         STAGE_MARK(5, g_ws.aux);
@@ -371,13 +390,24 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         ++g_ws.launches;
         STAGE_MARK(6, g_ws.aux);
         CU_TRY(cudaEventRecord(g_ws.evJoin, g_ws.aux));
+            return GAMMA_OK;
+    };
+    static const int forkAt = std::getenv("GAMMA_FORK") ? std::atoi(std::getenv("GAMMA_FORK")) : 0;
+    {                                                                    // a0 + A1 step 1
+        long long blocks = (N + 1023) / 1024;
+        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
+        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, ctl, next));
+        ++g_ws.launches;
     }
+    if (forkAt == 1) { rc = fork_table(); if (rc) return rc; }
     {                                                                    // a1: exclusion + compaction
         long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
         int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
-        k_classify<<<grid, PREP_THREADS, 0, st>>>(ref, out, g, e, ctl, e0);
+        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0));
         ++g_ws.launches;
     }
+    STAGE_MARK(1, st);
+    if (forkAt != 1) { rc = fork_table(); if (rc) return rc; }
     {                                                                    // star phase over the compacted voxels
         long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
         if (g_ws.occStar[r.star] == 0) {
@@ -389,15 +419,16 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         const long long resident = (long long)sm * g_ws.occStar[r.star];
         int grid = (int)(blocks > resident ? resident : blocks);
         if (r.star)
-            k_star<true><<<grid, STAR_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, e0, k0, i0);
+            CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0));
         else
-            k_star<false><<<grid, STAR_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, e0, k0, i0);
+            CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0));
         ++g_ws.launches;
     }
     STAGE_MARK(2, st);
+    CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));     // before the presort, so that presort -> search stay adjacent
     const unsigned *lk = k0, *li = i0;
     if (r.presort == 1) {                                                // a2: one-pass MSD bucket presort
-        k_bucket_scatter<<<sm * 2, SCATTER_THREADS, 0, st>>>(ctl, k0, i0, k1, i1);
+        CU_TRY(launch_ex(k_bucket_scatter, sm * 2, SCATTER_THREADS, 0, st, pdl, false, ctl, k0, i0, k1, i1));
         ++g_ws.launches;
         lk = k1; li = i1;
     } else if (r.presort == 3) {                                         // a2: full LSD radix sort of the keys
@@ -407,7 +438,6 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         if (where) { lk = k1; li = i1; }
     }
     STAGE_MARK(3, st);
-    CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));
     {                                                                    // a4 + a5
         const int grid = sm * 4;                                         // resident blocks at 64 registers
         const int4* tab = static_cast<const int4*>(g_ws.table.p);
@@ -417,13 +447,13 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             if (g.h[a] > 0.0f && (hmin == 0.0f || g.h[a] < hmin)) hmin = g.h[a];
         const int deepDigit = r.presort ? host_key_digit(hmin) + 1 : KEY_DIGITS;
         if (r.lanes == 1)
-            k_table_search<1><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
+            CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
         else if (r.lanes == 8)
-            k_table_search<8><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
+            CU_TRY(launch_ex(k_table_search<8>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
         else if (r.lanes == 32)
-            k_table_search<32><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
+            CU_TRY(launch_ex(k_table_search<32>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
         else
-            k_table_search<0><<<grid, SEARCH_THREADS, 0, st>>>(ref, ev, out, g, e, ctl, lk, li, tab, deepDigit);
+            CU_TRY(launch_ex(k_table_search<0>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
         ++g_ws.launches;
     }
     STAGE_MARK(4, st);
@@ -641,7 +671,7 @@ int gamma_get_stage_times(gamma_stage_times* out_host)
     CU_TRY(cudaEventSynchronize(g_ws.stage[6]));
     float ms[4];
     for (int i = 0; i < 4; ++i) CU_TRY(cudaEventElapsedTime(&ms[i], g_ws.stage[i], g_ws.stage[i + 1]));
-    out_host->norm_ms = ms[0]; out_host->prep_ms = ms[1]; out_host->sort_ms = ms[2]; out_host->search_ms = ms[3];
+    out_host->prep_ms = ms[0]; out_host->star_ms = ms[1]; out_host->sort_ms = ms[2]; out_host->search_ms = ms[3];
     CU_TRY(cudaEventElapsedTime(&out_host->table_ms, g_ws.stage[5], g_ws.stage[6]));
     CU_TRY(cudaEventElapsedTime(&out_host->total_ms, g_ws.stage[0], g_ws.stage[4]));
     return GAMMA_OK;

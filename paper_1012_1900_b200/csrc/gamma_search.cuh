@@ -3,6 +3,8 @@
 //   k_norm           a0 + A1 step 1: D_norm = max(ref) (reading 8) and max |D_r - D_e|,
 //                    which bounds every key and so fixes the radius of the offset table before the search
 //                    list exists; also clears the control block of the NEXT call.
+//   k_classify       a1: cutoff decision, NaN for excluded voxels, compaction of the evaluated voxels.
+// Consecutive kernels of a call are chained by programmatic dependent launch (pdl_wait / pdl_launch_dependents).
 //   k_prep_star      a1 + first part of a4: per voxel DD, cutoff, key (Algorithm A2 step 2 / CUDA Kernel 1,
 //                    PAPER.md:231-233); evaluated voxels are compacted into a block-local queue so that the
 //                    arithmetic always runs on full warps, then interior voxels try the 75 faces of the
@@ -39,10 +41,25 @@ __device__ __forceinline__ float block_max_256(float v, float* sm8)
 // ------------------------------------------------------------------------------------------------
 constexpr int NORM_THREADS = 256;
 
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
+{
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Programmatic dependent launch (sm_90+): a kernel launched with the programmatic-serialisation attribute may
+// start while its predecessor in the stream drains; it must not touch the predecessor's results before pdl_wait().
+// Both are no-ops for a kernel launched without the attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+
 __global__ void __launch_bounds__(NORM_THREADS)
 k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur,
        Ctl* __restrict__ next)
 {
+    pdl_launch_dependents();
     if (blockIdx.x == gridDim.x - 1 && next != nullptr) {      // the next call finds its control block cleared
         unsigned* w = reinterpret_cast<unsigned*>(next);
         for (int i = threadIdx.x; i < (int)(sizeof(Ctl) / 4); i += NORM_THREADS) w[i] = 0u;
@@ -100,19 +117,10 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
     __shared__ unsigned sBase;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned FULL = 0xffffffffu;
-    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
-    const double dnorm = (double)dnormF;
-    const double thr = (double)e.cutoff * dnorm;      // decided in double (include/gamma_b200.h)
-    const float invGlobal = criterion_inv_dD(e, dnorm, 0.0f);
-    const bool globalOk = invGlobal > 0.0f;
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->invGlobal = invGlobal;   // the later kernels read it from here
-    const float qnan = __int_as_float(0x7fc00000);
     const int numChunks = (g.N + PREP_CHUNK - 1) / PREP_CHUNK;
     const bool vec = ((reinterpret_cast<uintptr_t>(ref) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0;
-
-    for (int chunk = blockIdx.x; chunk < numChunks; chunk += gridDim.x) {
+    auto load_chunk = [&](int chunk, float (&Dr)[4]) -> int {
         const int lin0 = chunk * PREP_CHUNK + tid * 4;
-        float Dr[4];
         int nval = 0;
         if (vec && lin0 + 3 < g.N) {
             const float4 v = __ldg(reinterpret_cast<const float4*>(ref + lin0));
@@ -123,6 +131,25 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
             for (int j = 0; j < 4; ++j)
                 if (lin0 + j < g.N) { Dr[j] = __ldg(ref + lin0 + j); nval = j + 1; } else Dr[j] = 0.0f;
         }
+        return nval;
+    };
+    pdl_launch_dependents();
+    // ref is an input of the call, not a result of k_norm: the first chunk is fetched while k_norm drains
+    float Dr[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    int nval = 0;
+    if ((int)blockIdx.x < numChunks) nval = load_chunk(blockIdx.x, Dr);
+    pdl_wait();                                       // k_norm's maxima from here on
+    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
+    const double dnorm = (double)dnormF;
+    const double thr = (double)e.cutoff * dnorm;      // decided in double (include/gamma_b200.h)
+    const float invGlobal = criterion_inv_dD(e, dnorm, 0.0f);
+    const bool globalOk = invGlobal > 0.0f;
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->invGlobal = invGlobal;   // the later kernels read it from here
+    const float qnan = __int_as_float(0x7fc00000);
+
+    for (int chunk = blockIdx.x; chunk < numChunks; chunk += gridDim.x) {
+        const int lin0 = chunk * PREP_CHUNK + tid * 4;
+        if (chunk != (int)blockIdx.x) nval = load_chunk(chunk, Dr);
         unsigned keepMask = 0;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -180,6 +207,9 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     __shared__ float sMax[STAR_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31;
     const unsigned FULL = 0xffffffffu;
+    pdl_launch_dependents();
+    sHist[tid] = 0;
+    pdl_wait();                                           // k_classify's results from here on
     const unsigned M = ctl->nEval;
     const unsigned warpsTotal = gridDim.x * (STAR_THREADS / 32);
     const unsigned numItems = (M + 31u) / 32u;
@@ -194,8 +224,6 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
 #pragma unroll
     for (int T = 1; T < 8; ++T) A[T] = ((T & 1) ? g.hh[0] : 0.0f) + ((T & 2) ? g.hh[1] : 0.0f) + ((T & 4) ? g.hh[2] : 0.0f);
     float maxKey = 0.0f;
-
-    sHist[tid] = 0;
     __syncthreads();
 
     unsigned item = blockIdx.x * (STAR_THREADS / 32) + (tid >> 5);
@@ -300,6 +328,8 @@ k_bucket_scatter(Ctl* __restrict__ ctl, const unsigned* __restrict__ keyIn, cons
     __shared__ unsigned sWarp[SCATTER_THREADS / 32];
     const unsigned FULL = 0xffffffffu;
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    pdl_launch_dependents();
+    pdl_wait();
     const unsigned n = ctl->nSearch;
     if (blockIdx.x * SCATTER_THREADS >= n) return;
     {   // exclusive scan of the 256-bin histogram
@@ -520,6 +550,7 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     SearchCtx c;
+    pdl_wait();
     c.nS = ctl->nSearch;
     if (c.nS == 0) return;
     unsigned nDeep = 0;
