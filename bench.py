@@ -205,28 +205,16 @@ def main():
         return
 
     import torch
-    import torch.distributed as dist
     from paper_1012_1900_b200 import binding
     from paper_1012_1900_b200.binding import GammaOpts
+    from paper_1012_1900_b200.replicas import Replicas
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: libgamma_b200 has no CPU path")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    rep = Replicas(device=dev)              # nccl group when WORLD_SIZE > 1; replicas only, no data-path collective
+    barrier, max_over_ranks = rep.barrier, rep.max_over_ranks
 
     N = case.ref.size
     opts = GammaOpts(presort=args.presort, star_phase=args.star_phase, lanes_per_voxel=args.lanes)
@@ -306,8 +294,7 @@ def main():
     clk = clocks.report()
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        rep.close()
         return
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------
@@ -362,8 +349,7 @@ def main():
     elif world > 1:
         line["cpu_baseline"] = None
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 if __name__ == "__main__":
