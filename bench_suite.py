@@ -1,0 +1,239 @@
+#!/usr/bin/env python3
+"""bench_suite.py -- the per-config measurements SURVEY.md section 8(d) lists, beside bench.py's headline line.
+
+    python bench_suite.py [--suite configs|criteria|all] [--reps 30] [--oracle-seconds 8] [--md out.md]
+
+configs   every BASELINE.json config (cfg1, cfg2, cfg3, cfg4 coarse/fine, cfg5): grid voxels N, evaluated voxels M,
+          ms per case (t_total), stage times t_p / t_gamma, M/t_gamma, N/t_total, sum gamma^3, pass rate,
+          the resolution exponent of cfg4 (Fig. 2) and cfg5 with the voxel pre-sort on / off and
+          with the paper's thread-per-voxel mapping (Table 2)
+criteria  the 9 DD x DTA combinations of Table 3 on the cfg3 phantom: time against sum gamma^3
+          (Fig. 1) and the exact law gamma(k DD, k DTA) = gamma(DD, DTA) / k checked on the device maps
+
+Timing: one gamma_eval per repetition on device-resident inputs, rotating input/output sets larger than L2, CUDA
+events per repetition, median.  The CPU oracle is timed on a bounded seeded sample of each workload (--oracle-seconds
+of host time per config; 0 skips it).  One JSON line per measurement on stdout; --md also writes a table.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+L2_BYTES = 126e6
+
+
+def f32(x):
+    return float(np.float32(x))
+
+
+def measure(case, opts_kw, reps, dd=None, dta=None, keep_map=False):
+    import torch
+    from paper_1012_1900_b200 import binding
+    from paper_1012_1900_b200.binding import GammaOpts
+
+    dd = case.dd if dd is None else dd
+    dta = case.dta_mm if dta is None else dta
+    dev = torch.device("cuda", 0)
+    N = case.ref.size
+    nsets = max(2, min(24, int(np.ceil(2.0 * L2_BYTES / (12.0 * N))) + 1))
+    ref_h = torch.from_numpy(case.ref.ravel().copy())
+    ev_h = torch.from_numpy(case.eval.ravel().copy())
+    refs = [ref_h.to(dev) for _ in range(nsets)]
+    evs = [ev_h.to(dev) for _ in range(nsets)]
+    outs = [torch.empty(N, dtype=torch.float32, device=dev) for _ in range(nsets)]
+    stream = torch.cuda.current_stream()
+    a = (case.dims, case.spacing_mm, dd, dta, case.mode, case.cutoff)
+    opts = GammaOpts(**opts_kw)
+    popts = GammaOpts(profile_stages=1, **opts_kw)
+    for i in range(4):
+        binding.gamma_eval_ex(refs[i % nsets], evs[i % nsets], *a, opts, outs[i % nsets], stream)
+    torch.cuda.synchronize()
+    times = []
+    for i in range(reps):
+        k = i % nsets
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        binding.gamma_eval_ex(refs[k], evs[k], *a, opts, outs[k], stream)
+        e1.record(stream)
+        e1.synchronize()
+        times.append(e0.elapsed_time(e1))
+    # back-to-back rate (what bench.py reports): the launches of consecutive calls overlap
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(reps):
+        k = i % nsets
+        binding.gamma_eval_ex(refs[k], evs[k], *a, opts, outs[k], stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_stream = e0.elapsed_time(e1) / reps
+    cnt = binding.gamma_get_counters()
+    acc = {}
+    for i in range(min(reps, 20)):
+        k = i % nsets
+        binding.gamma_eval_ex(refs[k], evs[k], *a, popts, outs[k], stream)
+        for kk, v in binding.gamma_get_stage_times().items():
+            acc.setdefault(kk, []).append(v)
+    stages = {k: float(np.median(v)) for k, v in acc.items()}
+    hist, summ = binding.gamma_stats(outs[0], 64, 4.0)
+    torch.cuda.synchronize()
+    res = {"N": N, "M": int(cnt["n_evaluated"]), "ms_case_median": float(np.median(times)),
+           "ms_case_min": float(np.min(times)), "ms_case_back_to_back": ms_stream, "stages_ms": stages,
+           "n_table_search": int(cnt["n_table_search"]), "vertex_visits": int(cnt["vertex_visits"]),
+           "table_entries": int(cnt["table_entries"]), "max_key": float(cnt["max_key"]),
+           "sum_gamma3": float(summ["sum_gamma3"]), "pass_rate": summ["n_pass"] / max(1, summ["n_eval"]),
+           "max_gamma": float(summ["max_gamma"]), "options": opts_kw, "criteria": f"{dd * 100:g}%/{dta:g}mm"}
+    t_gamma = stages.get("star_ms", 0.0) + stages.get("search_ms", 0.0)
+    res["t_gamma_ms"] = t_gamma
+    res["t_p_ms"] = max(0.0, stages.get("total_ms", 0.0) - t_gamma)
+    res["evaluated_voxels_per_s"] = res["M"] / (ms_stream * 1e-3)
+    res["grid_voxels_per_s"] = N / (ms_stream * 1e-3)
+    if keep_map:
+        res["_map"] = outs[0].clone()
+    del refs, evs, outs
+    torch.cuda.empty_cache()
+    return res
+
+
+def oracle_sample(case, seconds, dd=None, dta=None):
+    """The oracle as it stands on a bounded seeded sample of the evaluated voxels (all host cores)."""
+    if seconds <= 0:
+        return None
+    import oracle
+    oracle.build()
+    dd = case.dd if dd is None else dd
+    dta = case.dta_mm if dta is None else dta
+    ref = case.ref.ravel().astype(np.float64)
+    keep = np.flatnonzero(ref >= f32(case.cutoff) * ref.max())
+    rng = np.random.default_rng([0, 77])
+    sp = [f32(s) for s in case.spacing_mm]
+
+    def run(vox):
+        t0 = time.perf_counter()
+        oracle.gamma(case.ref, case.eval, case.dims, sp, f32(dd), f32(dta), case.mode, f32(case.cutoff), voxels=vox)
+        return time.perf_counter() - t0
+
+    probe = np.sort(rng.choice(keep, size=min(keep.size, 2000), replace=False))
+    tp = run(probe)
+    n = int(min(keep.size, max(probe.size, seconds / (tp / probe.size))))
+    vox = np.sort(rng.choice(keep, size=n, replace=False))
+    t = run(vox)
+    return {"voxels": n, "of": int(keep.size), "seconds": t, "voxels_per_s": n / t, "cores": oracle.num_threads(),
+            "seconds_per_case_extrapolated": t / n * keep.size}
+
+
+def suite_configs(args, emit):
+    from paper_1012_1900_b200 import phantoms
+    rows = []
+    for name in ("cfg1", "cfg2", "cfg3", "cfg4_coarse", "cfg4_fine", "cfg5"):
+        case = phantoms.make_case(name)
+        variants = [("default", {})]
+        if name == "cfg5":
+            variants += [("presort off", {"presort": 2}), ("full radix sort", {"presort": 3}),
+                         ("thread per voxel, presort on", {"lanes_per_voxel": 1, "star_phase": 2, "presort": 3}),
+                         ("thread per voxel, presort off", {"lanes_per_voxel": 1, "star_phase": 2, "presort": 2})]
+        orc = oracle_sample(case, args.oracle_seconds)
+        for label, kw in variants:
+            reps = args.reps if "thread per voxel" not in label else max(3, args.reps // 6)
+            r = measure(case, kw, reps)
+            r.update({"suite": "configs", "case": name, "variant": label, "cpu_oracle": orc if label == "default" else None})
+            emit(r)
+            rows.append(r)
+    fine = next(r for r in rows if r["case"] == "cfg4_fine")
+    mid = next(r for r in rows if r["case"] == "cfg2")
+    coarse = next(r for r in rows if r["case"] == "cfg4_coarse")
+    xs = np.log([coarse["N"], mid["N"], fine["N"]])
+    ys = np.log([coarse["ms_case_median"], mid["ms_case_median"], fine["ms_case_median"]])
+    yg = np.log([coarse["t_gamma_ms"], mid["t_gamma_ms"], fine["t_gamma_ms"]])
+    emit({"suite": "configs", "resolution_exponent_t_total": float(np.polyfit(xs, ys, 1)[0]),
+          "resolution_exponent_t_gamma": float(np.polyfit(xs, yg, 1)[0]),
+          "paper": "T_gamma^C ~ N^1.90, T_gamma^G ~ N^1.68 (PAPER.md:382-388); same phantom at 5 / 2.5 / 1.25 mm"})
+    return rows
+
+
+def suite_criteria(args, emit):
+    import torch
+    from paper_1012_1900_b200 import phantoms
+    case = phantoms.make_case("cfg3")
+    rows, maps = [], {}
+    for dd in (0.01, 0.02, 0.03):
+        for dta in (1.0, 2.0, 3.0):
+            r = measure(case, {}, args.reps, dd=dd, dta=dta, keep_map=True)
+            maps[(dd, dta)] = r.pop("_map")
+            r.update({"suite": "criteria", "case": "cfg3 phantom", "variant": f"{dd * 100:g}%/{dta:g}mm"})
+            emit(r)
+            rows.append(r)
+    # gamma(k DD, k DTA) = gamma(DD, DTA) / k: exact in real arithmetic
+    base = maps[(0.01, 1.0)]
+    m = ~torch.isnan(base)
+    law = {}
+    for k in (2, 3):
+        other = maps[(0.01 * k, 1.0 * k)]
+        assert bool((torch.isnan(other) == ~m).all())
+        law[f"k={k}"] = float((other[m] * k - base[m]).abs().max().item())
+    mono_dd = all(bool((maps[(0.02, t)][m] <= maps[(0.01, t)][m] + 1e-5).all()) for t in (1.0, 2.0, 3.0))
+    mono_dta = all(bool((maps[(d, 2.0)][m] <= maps[(d, 1.0)][m] + 1e-5).all()) for d in (0.01, 0.02, 0.03))
+    t = np.array([r["t_gamma_ms"] for r in rows])
+    s3 = np.array([r["sum_gamma3"] for r in rows])
+    emit({"suite": "criteria", "scaling_law_max_abs_dev": law, "monotone_in_DD": mono_dd, "monotone_in_DTA": mono_dta,
+          "corr_t_gamma_vs_sum_gamma3": float(np.corrcoef(t, s3)[0, 1]),
+          "corr_log_t_gamma_vs_log_sum_gamma3": float(np.corrcoef(np.log(t), np.log(s3))[0, 1])})
+    return rows
+
+
+def write_md(path, rows):
+    with open(path, "w") as f:
+        f.write("| suite | case | variant | criteria | N | M | ms/case (median) | ms/case (back to back) | t_p ms | "
+                "t_gamma ms | M/t_gamma (1/s) | N/t_total (1/s) | table search items | vertex visits | sum gamma^3 | "
+                "pass rate | max gamma | oracle s/case (cores) |\n")
+        f.write("|" + "---|" * 18 + "\n")
+        for r in rows:
+            if "case" not in r:
+                continue
+            o = r.get("cpu_oracle")
+            f.write(f"| {r['suite']} | {r['case']} | {r['variant']} | {r['criteria']} | {r['N']} | {r['M']} | "
+                    f"{r['ms_case_median']:.4f} | {r['ms_case_back_to_back']:.4f} | {r['t_p_ms']:.4f} | "
+                    f"{r['t_gamma_ms']:.4f} | {r['M'] / (r['t_gamma_ms'] * 1e-3):.3e} | {r['grid_voxels_per_s']:.3e} | "
+                    f"{r['n_table_search']} | {r['vertex_visits']} | {r['sum_gamma3']:.4g} | {r['pass_rate']:.4f} | "
+                    f"{r['max_gamma']:.3f} | "
+                    + (f"{o['seconds_per_case_extrapolated']:.2f} ({o['cores']})" if o else "-") + " |\n")
+        for r in rows:
+            if "case" not in r:
+                f.write("\n`" + json.dumps(r) + "`\n")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--suite", default="all", choices=["configs", "criteria", "all"])
+    ap.add_argument("--reps", type=int, default=30)
+    ap.add_argument("--oracle-seconds", type=float, default=8.0)
+    ap.add_argument("--md", default=None)
+    args = ap.parse_args()
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench_suite.py needs a CUDA device: libgamma_b200 has no CPU path")
+    torch.cuda.set_device(0)
+    rows = []
+
+    def emit(r):
+        rows.append(r)
+        print(json.dumps({k: v for k, v in r.items() if not k.startswith("_")}), flush=True)
+
+    if args.suite in ("configs", "all"):
+        suite_configs(args, emit)
+    if args.suite in ("criteria", "all"):
+        suite_criteria(args, emit)
+    if args.md:
+        write_md(args.md, rows)
+
+
+if __name__ == "__main__":
+    main()

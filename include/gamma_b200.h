@@ -66,17 +66,20 @@ int gamma_eval(const float* ref, const float* eval, const int dims[3], const flo
 /* Options of gamma_eval_ex / gamma_eval_host.  Zero-initialise, then set what differs. */
 typedef struct gamma_opts {
     float norm_dose;      /* D_norm; <= 0: max(ref), found on the device                                  */
-    int presort;          /* pre-sort of the search work list (A2 step 3).  0: default (= 1);
+    int presort;          /* pre-sort of the search work list (A2 step 3).  0: default (= 4);
                              1: one-pass MSD radix sort on the 8-bit key digit (32 steps per octave of the key);
                              2: no sort (Table 2's "without sorting"); 3: full LSD radix sort of the
-                             `sort_key_bits` most significant key bits                                     */
+                             `sort_key_bits` most significant key bits; 4: depth classes -- a 1-bit radix
+                             sort done while the list is written: items whose key exceeds the first non-zero
+                             table distance go to a list of their own and are searched first, a warp each
+                             (adaptive lanes only; with lanes_per_voxel != 0 it means 1)                   */
     int star_phase;       /* 0: default (= 1); 1: interior voxels first try the 75 faces touching the voxel
                              and finish there when gamma_star <= distance to the rest of the surface;
                              2: off -- every voxel goes through the table search with key |DD|/dD, as in
                              Algorithm A2                                               */
     int lanes_per_voxel;  /* lanes that cooperate on one reference voxel in the table search.  0: default =
                              adaptive (a whole warp for the deep items at the head of the pre-sorted list,
-                             8 lanes for the others; needs presort 1 or 3, else 8); 1 = the paper's
+                             8 lanes for the others; needs presort 1, 3 or 4, else 8); 1 = the paper's
                              thread-per-voxel mapping; 8; 32                               */
     int sort_key_bits;    /* presort = 3 only.  0: default (= 16); 8, 16, 24 or 32 most significant key bits   */
     long long table_cap;  /* 0: default (1<<20); max entries of the sorted offset table; past it the search

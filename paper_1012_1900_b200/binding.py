@@ -63,7 +63,7 @@ class _CCounters(ctypes.Structure):
 class GammaOpts:
     """Mirror of ``gamma_opts`` (include/gamma_b200.h); 0 means "library default"."""
     norm_dose: float = 0.0
-    presort: int = 0          # 1 bucket presort (default), 2 no sort, 3 full LSD radix sort
+    presort: int = 0          # 1 bucket presort, 2 no sort, 3 full LSD radix sort, 4 depth classes (default)
     star_phase: int = 0       # 1 on, 2 off
     lanes_per_voxel: int = 0  # 1, 8, 32
     sort_key_bits: int = 0    # presort=3: 8, 16, 24, 32

@@ -63,7 +63,7 @@ struct Ctl {
     float Rtab2;           // squared radius the table covers
     int box[3];            // table box: m_a in [0, box_a)
     unsigned sortN;        // element count for gamma_sort_pairs
-    unsigned barrier;      // spare
+    unsigned nDeep;        // depth-class lists (presort 4): items in the deep list
     unsigned pad0_;
     float invGlobal;       // 1 / (DD * D_norm) rounded to fp32 (global criterion), written by k_classify
     unsigned long long visits;       // owner vertices evaluated by the table search

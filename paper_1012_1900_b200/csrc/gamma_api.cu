@@ -285,12 +285,13 @@ struct Resolved {
 
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
-    r.presort = 1; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
+    r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
     r.profile = 0;
     if (!o) return GAMMA_OK;
     r.profile = o->profile_stages == 1;
-    if (o->presort < 0 || o->presort > 3) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.presort must be 0, 1, 2 or 3");
+    if (o->presort < 0 || o->presort > 4) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.presort must be 0, 1, 2, 3 or 4");
     if (o->star_phase < 0 || o->star_phase > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.star_phase must be 0, 1 or 2");
+    if (o->presort == 1) r.presort = 1;
     if (o->presort == 2) r.presort = 0;
     if (o->presort == 3) r.presort = 3;
     if (o->star_phase == 2) r.star = 0;
@@ -309,6 +310,7 @@ int resolve_opts(const gamma_opts* o, Resolved& r)
             return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.table_cap must be in [1, 2^26]");
         r.tableCap = o->table_cap;
     }
+    if (r.presort == 4 && r.lanes != 0) r.presort = 1;   // depth classes only exist for the adaptive search
     if (o->norm_dose > 0.0f) r.normDose = o->norm_dose;
     if (std::isnan(o->norm_dose) || std::isinf(o->norm_dose))
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.norm_dose must be finite");
@@ -368,6 +370,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     EvalP e;
     e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
 
+    const int classes = r.presort == 4 ? 1 : 0;
     g_ws.haveStages = false;
     if (r.profile)
         for (cudaEvent_t& evn : g_ws.stage)
@@ -419,9 +422,9 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         const long long resident = (long long)sm * g_ws.occStar[r.star];
         int grid = (int)(blocks > resident ? resident : blocks);
         if (r.star)
-            CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0));
+            CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes));
         else
-            CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0));
+            CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes));
         ++g_ws.launches;
     }
     STAGE_MARK(2, st);
@@ -445,15 +448,15 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         float hmin = 0.0f;
         for (int a = 0; a < 3; ++a)
             if (g.h[a] > 0.0f && (hmin == 0.0f || g.h[a] < hmin)) hmin = g.h[a];
-        const int deepDigit = r.presort ? host_key_digit(hmin) + 1 : KEY_DIGITS;
+        const int deepDigit = (r.presort == 1 || r.presort == 3) ? host_key_digit(hmin) + 1 : KEY_DIGITS;
         if (r.lanes == 1)
-            CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
+            CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
         else if (r.lanes == 8)
-            CU_TRY(launch_ex(k_table_search<8>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
+            CU_TRY(launch_ex(k_table_search<8>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
         else if (r.lanes == 32)
-            CU_TRY(launch_ex(k_table_search<32>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
+            CU_TRY(launch_ex(k_table_search<32>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
         else
-            CU_TRY(launch_ex(k_table_search<0>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, tab, deepDigit));
+            CU_TRY(launch_ex(k_table_search<0>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
         ++g_ws.launches;
     }
     STAGE_MARK(4, st);
@@ -650,7 +653,7 @@ int gamma_get_counters(gamma_counters* out_host)
     std::memset(out_host, 0, sizeof *out_host);
     out_host->n_voxels = g_ws.lastN;
     out_host->n_evaluated = c.nEval;
-    out_host->n_table_search = c.nSearch;
+    out_host->n_table_search = (long long)c.nSearch + (long long)c.nDeep;
     out_host->table_entries = c.tableCount;
     out_host->vertex_visits = (long long)c.visits;
     union { unsigned u; float f; } cv;

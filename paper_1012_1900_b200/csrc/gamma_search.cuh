@@ -201,8 +201,11 @@ template <bool STAR>
 __global__ void __launch_bounds__(STAR_THREADS, GAMMA_STAR_MIN_BLOCKS)
 k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g, EvalP e,
        Ctl* __restrict__ ctl, const unsigned* __restrict__ evalIdx, unsigned* __restrict__ listKey,
-       unsigned* __restrict__ listIdx)
+       unsigned* __restrict__ listIdx, unsigned* __restrict__ deepKey, unsigned* __restrict__ deepIdx, int classes)
 {
+    // classes != 0: the work list is split by depth class at append time instead of being sorted afterwards --
+    // "deep" items (key beyond the first non-zero table distance: the walk will pass table entry 0) go to
+    // (deepKey, deepIdx), the others to (listKey, listIdx); no digit histogram is kept.
     __shared__ unsigned sHist[KEY_DIGITS];
     __shared__ float sMax[STAR_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31;
@@ -285,17 +288,31 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
                 toSearch = false;
             }
         }
-        const unsigned bal = __ballot_sync(FULL, toSearch);   // append to the global work list, warp-aggregated
+        const bool deep = toSearch && classes && key * key > g.hmin2;
+        const unsigned bal = __ballot_sync(FULL, toSearch && !deep);   // append to the work list, warp-aggregated
         if (bal) {
             const int leader = __ffs(bal) - 1;
             unsigned base = 0;
             if (lane == leader) base = atomicAdd(&ctl->nSearch, (unsigned)__popc(bal));
             base = __shfl_sync(FULL, base, leader);
-            if (toSearch) {
+            if (toSearch && !deep) {
                 const unsigned pos = base + __popc(bal & ((1u << lane) - 1u));
                 listKey[pos] = __float_as_uint(key);
                 listIdx[pos] = (unsigned)lin;
-                atomicAdd(&sHist[key_digit(key)], 1u);
+                if (!classes) atomicAdd(&sHist[key_digit(key)], 1u);
+                maxKey = fmaxf(maxKey, key);
+            }
+        }
+        const unsigned balDeep = __ballot_sync(FULL, deep);
+        if (balDeep) {
+            const int leader = __ffs(balDeep) - 1;
+            unsigned base = 0;
+            if (lane == leader) base = atomicAdd(&ctl->nDeep, (unsigned)__popc(balDeep));
+            base = __shfl_sync(FULL, base, leader);
+            if (deep) {
+                const unsigned pos = base + __popc(balDeep & ((1u << lane) - 1u));
+                deepKey[pos] = __float_as_uint(key);
+                deepIdx[pos] = (unsigned)lin;
                 maxKey = fmaxf(maxKey, key);
             }
         }
@@ -304,7 +321,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     maxKey = warp_max(maxKey);
     if (lane == 0) sMax[tid >> 5] = maxKey;
     __syncthreads();
-    if (sHist[tid]) atomicAdd(&ctl->hist[tid], sHist[tid]);
+    if (!classes && sHist[tid]) atomicAdd(&ctl->hist[tid], sHist[tid]);
     if (tid == 0) {
         float m = 0.0f;
 #pragma unroll
@@ -421,8 +438,8 @@ constexpr int SEARCH_THREADS = 256;
 
 struct SearchCtx {
     const float* ref; const float* ev; float* out;
-    const unsigned* listKey; const unsigned* listIdx; const int4* table;
-    unsigned nS, T;
+    const int4* table;
+    unsigned T;
     bool trunc;
     float Rtab2, invGlobal;
     double dnorm;
@@ -431,22 +448,24 @@ struct SearchCtx {
 // One warp searches 32/G consecutive work items (firstItem .. firstItem + 32/G - 1, counted from the END of the
 // sorted list: deepest first), G lanes per reference voxel.  Returns the owner vertices it evaluated.
 template <int G>
-__device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP& g, const EvalP& e, unsigned firstItem,
-                                                 int lane)
+__device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP& g, const EvalP& e,
+                                                 const unsigned* __restrict__ listKey,
+                                                 const unsigned* __restrict__ listIdx, unsigned nList,
+                                                 unsigned firstItem, int lane)
 {
     constexpr int EPP = G >= 8 ? G / 8 : 1;     // table entries per pass
     const unsigned FULL = 0xffffffffu;
     const int gid = lane / G, gl = lane % G;
     const unsigned item = firstItem + gid;
-    const bool have = item < c.nS;
+    const bool have = item < nList;
     const unsigned T = c.T;
     unsigned visits = 0;
     VoxelCtx vc;
     float key = 0.0f, best2 = 0.0f;
     if (have) {
-        const unsigned idx = c.nS - 1u - item;
-        vc.lin = (int)c.listIdx[idx];
-        key = __uint_as_float(c.listKey[idx]);
+        const unsigned idx = nList - 1u - item;
+        vc.lin = (int)listIdx[idx];
+        key = __uint_as_float(listKey[idx]);
         vc.Dr = __ldg(c.ref + vc.lin);
         vc.invdD = e.mode == 0 ? c.invGlobal : criterion_inv_dD(e, c.dnorm, vc.Dr);
         voxel_coords(g, vc.lin, vc.v[0], vc.v[1], vc.v[2]);
@@ -537,35 +556,43 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
     return visits;
 }
 
-// MODE = lanes per reference voxel: 1 (thread per voxel), 8, 32, or 0 = adaptive: the nDeep
-// deepest items of the sorted list (key digit >= deepDigit: the search will pass the first table entry) get a
-// whole warp each, the others 8 lanes each.  Work units are handed out deepest first: first round static,
-// later rounds by an atomic counter whose latency hides behind the current search.
+// MODE = lanes per reference voxel: 1 (thread per voxel), 8, 32, or 0 = adaptive: deep items (the
+// walk will pass the first table entry) get a whole warp each, the others 8 lanes each.  Deep items are either
+// the tail of the sorted list (key digit >= deepDigit, counted from the digit histogram) or, with depth-class
+// lists (classes != 0), the separate list (deepKey, deepIdx) that k_star filled.  Work units are handed out
+// deepest first: first round static, later rounds by an atomic counter whose latency hides behind the search.
 template <int MODE>
 __global__ void __launch_bounds__(SEARCH_THREADS)
 k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
                EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
-               const unsigned* __restrict__ listIdx, const int4* __restrict__ table, int deepDigit)
+               const unsigned* __restrict__ listIdx, const unsigned* __restrict__ deepKey,
+               const unsigned* __restrict__ deepIdx, const int4* __restrict__ table, int deepDigit, int classes)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     SearchCtx c;
     pdl_wait();
-    c.nS = ctl->nSearch;
-    if (c.nS == 0) return;
+    const unsigned nS = ctl->nSearch;
     unsigned nDeep = 0;
-    if (MODE == 0 && deepDigit < KEY_DIGITS) {                // sum of the histogram tail = number of deep items
+    if (MODE == 0 && classes) {
+        nDeep = ctl->nDeep;
+    } else if (MODE == 0 && deepDigit < KEY_DIGITS) {         // sum of the histogram tail = number of deep items
         for (int d = deepDigit + lane; d < KEY_DIGITS; d += 32) nDeep += ctl->hist[d];
 #pragma unroll
         for (int s = 16; s > 0; s >>= 1) nDeep += __shfl_xor_sync(FULL, nDeep, s);
+        deepKey = listKey; deepIdx = listIdx;
     }
+    // shallow items: all of the list with depth classes, else what is left of the sorted list before its deep tail
+    const unsigned nShallow = (MODE == 0 && classes) ? nS : nS - nDeep;
+    const unsigned nDeepList = (MODE == 0 && classes) ? nDeep : nS;   // deep item i is entry nDeepList - 1 - i
+    if (nS + nDeep == 0) return;
     constexpr unsigned VPW = MODE == 0 ? 4u : 32u / (unsigned)(MODE == 0 ? 8 : MODE);
-    const unsigned numUnits = MODE == 0 ? nDeep + (c.nS - nDeep + 3u) / 4u : (c.nS + VPW - 1u) / VPW;
+    const unsigned numUnits = MODE == 0 ? nDeep + (nShallow + 3u) / 4u : (nS + VPW - 1u) / VPW;
     const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
     unsigned unit = blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5);
     if (unit >= numUnits) return;
     const bool dynamic = numUnits > warpsTotal;
-    c.ref = ref; c.ev = ev; c.out = out; c.listKey = listKey; c.listIdx = listIdx; c.table = table;
+    c.ref = ref; c.ev = ev; c.out = out; c.table = table;
     c.T = ctl->tableCount;
     c.trunc = ctl->tableTrunc != 0;
     c.Rtab2 = ctl->Rtab2;
@@ -578,10 +605,11 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
         unsigned nextUnit = numUnits;
         if (dynamic && lane == 0) nextUnit = atomicAdd(&ctl->workCounter, 1u) + warpsTotal;
         if (MODE == 0) {
-            if (unit < nDeep) visits += search_items<32>(c, g, e, unit, lane);
-            else visits += search_items<8>(c, g, e, nDeep + 4u * (unit - nDeep), lane);
+            if (unit < nDeep) visits += search_items<32>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane);
+            else if (classes) visits += search_items<8>(c, g, e, listKey, listIdx, nS, 4u * (unit - nDeep), lane);
+            else visits += search_items<8>(c, g, e, listKey, listIdx, nS, nDeep + 4u * (unit - nDeep), lane);
         } else {
-            visits += search_items<(MODE == 0 ? 8 : MODE)>(c, g, e, unit * VPW, lane);
+            visits += search_items<(MODE == 0 ? 8 : MODE)>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);
         }
         unit = __shfl_sync(FULL, nextUnit, 0);
     }

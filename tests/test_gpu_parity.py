@@ -101,7 +101,7 @@ def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
     thread-per-voxel mapping: the candidate set is the same, so gamma is bit-identical."""
     c = phantoms.make_case("cfg5")
     base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
-    for o in (GammaOpts(presort=2), GammaOpts(presort=3), GammaOpts(lanes_per_voxel=1),
+    for o in (GammaOpts(presort=1), GammaOpts(presort=2), GammaOpts(presort=3), GammaOpts(lanes_per_voxel=1),
               GammaOpts(lanes_per_voxel=1, presort=2), GammaOpts(lanes_per_voxel=32)):
         g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
         assert np.array_equal(np.isnan(g), np.isnan(base))
@@ -112,7 +112,8 @@ def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
 # every option / kernel variant on grids that span several tiles with ragged tails
 # ----------------------------------------------------------------------------------------------------
 VARIANTS = [
-    GammaOpts(), GammaOpts(star_phase=2), GammaOpts(presort=2), GammaOpts(lanes_per_voxel=1),
+    GammaOpts(), GammaOpts(star_phase=2), GammaOpts(presort=2), GammaOpts(lanes_per_voxel=1), GammaOpts(presort=1),
+    GammaOpts(presort=4, star_phase=2), GammaOpts(presort=4, table_cap=2),
     GammaOpts(lanes_per_voxel=32), GammaOpts(star_phase=2, lanes_per_voxel=1, presort=2),
     GammaOpts(presort=3, sort_key_bits=8), GammaOpts(presort=3, sort_key_bits=32), GammaOpts(table_cap=1),
     GammaOpts(table_cap=7, star_phase=2), GammaOpts(table_cap=40, lanes_per_voxel=32),
