@@ -86,7 +86,12 @@ typedef struct gamma_opts {
                              continues by exhaustive enumeration, so results never depend on it            */
     int profile_stages;   /* 1: record CUDA events between the stages of this call on `stream`, to be read
                              with gamma_get_stage_times (adds a few event records, no synchronisation)     */
-    int pad_;
+    int graph;            /* 0: default (= 2); 1: a call whose arguments (pointers included) were seen before
+                             replays a cached CUDA graph of its kernels (up to 64 argument sets are kept):
+                             less host time per call, but replays do not overlap with the previous call the
+                             way stream launches do; 2: launch the kernels one by one.  Ignored (= 2) while
+                             `stream` is being captured by the caller (the kernels then become nodes of the
+                             caller's graph, with their own control block) and with profile_stages          */
 } gamma_opts;
 
 /* gamma_eval with options (opts may be NULL = defaults).  Same contract as gamma_eval. */

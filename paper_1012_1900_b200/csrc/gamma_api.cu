@@ -56,6 +56,8 @@ cudaError_t launch_ex(void (*kernel)(KArgs...), int grid, int block, size_t smem
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
+unsigned long long g_allocGen = 0;   // bumped whenever a workspace buffer moves: cached graphs hold its old address
+
 // grow-only device buffer
 struct Buf {
     void* p = nullptr;
@@ -63,6 +65,7 @@ struct Buf {
     cudaError_t need(size_t bytes)
     {
         if (bytes <= cap) return cudaSuccess;
+        ++g_allocGen;
         if (p) { cudaFree(p); p = nullptr; cap = 0; }
         size_t want = bytes + bytes / 8 + 256;
         cudaError_t e = cudaMalloc(&p, want);
@@ -72,10 +75,30 @@ struct Buf {
     }
     void release()
     {
-        if (p) cudaFree(p);
+        if (p) { cudaFree(p); ++g_allocGen; }
         p = nullptr; cap = 0;
     }
 };
+
+// One instantiated CUDA graph of the whole pipeline for one exact set of arguments (pointers included).
+struct GraphKey {
+    const void *ref, *ev, *out;
+    void* ctl;
+    GridP g;
+    float DD, cutoff, normDose;
+    int mode, presort, star, lanes, keyBits;
+    long long tableCap;
+    bool operator==(const GraphKey& o) const { return std::memcmp(this, &o, sizeof *this) == 0; }
+};
+struct GraphEntry {
+    GraphKey key;
+    cudaGraphExec_t exec = nullptr;
+    unsigned long long lastUse = 0;
+    int kernels = 0;
+};
+constexpr int GRAPH_CACHE = 64;
+// control-block slots: 0/1 alternate between calls, 2 stand-alone entry points, 3 calls captured by the caller
+constexpr int CTL_SLOTS = 4;
 
 struct Workspace {
     Buf ctl;                       // Ctl
@@ -98,6 +121,17 @@ struct Workspace {
     int numSM = 0;
     int occStar[2] = {0, 0};       // resident blocks per SM of k_star<false/true>
     int pdl = -1;                  // programmatic dependent launch between the kernels of a call (GAMMA_PDL=0 disables)
+    int graphs = -1;               // replay the call as a cached CUDA graph (GAMMA_GRAPH=0 disables)
+    cudaStream_t cap = nullptr;    // capture stream (the caller's may be the legacy default stream, which cannot capture)
+    GraphEntry graph[GRAPH_CACHE];
+    int numGraphs = 0;
+    unsigned long long graphGen = 0, useClock = 0;
+    void dropGraphs()
+    {
+        for (int i = 0; i < numGraphs; ++i)
+            if (graph[i].exec) { cudaGraphExecDestroy(graph[i].exec); graph[i].exec = nullptr; }
+        numGraphs = 0;
+    }
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
     long long lastN = 0;
@@ -109,7 +143,9 @@ struct Workspace {
         if (done) { cudaEventDestroy(done); done = nullptr; }
         for (cudaEvent_t& ev : stage)
             if (ev) { cudaEventDestroy(ev); ev = nullptr; }
+        dropGraphs();
         if (aux) { cudaStreamDestroy(aux); aux = nullptr; }
+        if (cap) { cudaStreamDestroy(cap); cap = nullptr; }
         if (evFork) { cudaEventDestroy(evFork); evFork = nullptr; }
         if (evJoin) { cudaEventDestroy(evJoin); evJoin = nullptr; }
         havePending = false; haveLast = false; haveStages = false; ctlClean = false; ctlOwner = nullptr;
@@ -278,7 +314,7 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
 }
 
 struct Resolved {
-    int presort, star, lanes, keyBits, profile;
+    int presort, star, lanes, keyBits, profile, graph;
     long long tableCap;
     float normDose;
 };
@@ -286,9 +322,11 @@ struct Resolved {
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
     r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
-    r.profile = 0;
+    r.profile = 0; r.graph = 0;
     if (!o) return GAMMA_OK;
     r.profile = o->profile_stages == 1;
+    if (o->graph < 0 || o->graph > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.graph must be 0, 1 or 2");
+    r.graph = o->graph == 1;
     if (o->presort < 0 || o->presort > 4) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.presort must be 0, 1, 2, 3 or 4");
     if (o->star_phase < 0 || o->star_phase > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.star_phase must be 0, 1 or 2");
     if (o->presort == 1) r.presort = 1;
@@ -325,22 +363,14 @@ int check_criteria(float DD, int mode, float cutoff)
     return GAMMA_OK;
 }
 
-// Enqueue the whole hot path on `st` (device pointers).  Caller holds g_mu.
-//
-//   st :  k_norm -> k_star -> [k_bucket_scatter | LSD radix sort] -> (join) -> k_table_search
-//   aux:        \-> k_offset_table ------------------------------------------/
-//
-// The offset table only needs k_norm's maxima, so it is built on a library-owned side stream while the
-// star kernel runs.  No memset and no host synchronisation on the path: k_norm clears the control
-// block of the next call (two alternating slots; slot 2 belongs to the stand-alone entry points).
-int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
-                     const Resolved& r, float* out, cudaStream_t st)
+// Workspace of one call: allocations, side stream, events.  Nothing is allocated once the sizes have been seen.
+int prepare_workspace(const GridP& g, const Resolved& r)
 {
     int rc = ensure_device();
     if (rc) return rc;
     const long long N = g.N;
     const long long maxTiles = (N + SORT_TILE - 1) / SORT_TILE;
-    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
     CU_TRY(g_ws.key0.need(N * 4)); CU_TRY(g_ws.idx0.need(N * 4)); CU_TRY(g_ws.evalIdx.need(N * 4));
     if (r.presort) { CU_TRY(g_ws.key1.need(N * 4)); CU_TRY(g_ws.idx1.need(N * 4)); }
     if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
@@ -348,96 +378,100 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     CU_TRY(g_ws.tmpL.need((size_t)r.tableCap * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)r.tableCap * 4));
     if (!g_ws.aux) {
         CU_TRY(cudaStreamCreateWithFlags(&g_ws.aux, cudaStreamNonBlocking));
+        CU_TRY(cudaStreamCreateWithFlags(&g_ws.cap, cudaStreamNonBlocking));
         CU_TRY(cudaEventCreateWithFlags(&g_ws.evFork, cudaEventDisableTiming));
         CU_TRY(cudaEventCreateWithFlags(&g_ws.evJoin, cudaEventDisableTiming));
         CU_TRY(cudaFuncSetAttribute(k_offset_table, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TAB_DYN_SMEM));
     }
-    rc = order_after_previous(st);
-    if (rc) return rc;
-
-    if (g_ws.ctl.p != g_ws.ctlOwner) { g_ws.ctlClean = false; g_ws.ctlOwner = g_ws.ctl.p; }
-    if (!g_ws.ctlClean) {                                  // first call, or a previous call failed half-way
-        CU_TRY(cudaMemsetAsync(g_ws.ctl.p, 0, 3 * sizeof(Ctl), st));
-        g_ws.slot = 0;
+    for (int star = 0; star < 2; ++star)
+        if (g_ws.occStar[star] == 0) {
+            int occ = 0;
+            if (star) CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_star<true>, STAR_THREADS, 0));
+            else CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_star<false>, STAR_THREADS, 0));
+            g_ws.occStar[star] = occ > 0 ? occ : 1;
+        }
+    if (g_ws.pdl < 0) {
+        const char* env = std::getenv("GAMMA_PDL");
+        g_ws.pdl = (env && env[0] == '0') ? 0 : 1;
     }
-    g_ws.ctlClean = false;                                 // set again when everything below was enqueued
-    Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
-    Ctl* ctl = base + g_ws.slot;
-    Ctl* next = base + (g_ws.slot ^ 1);
+    if (g_ws.graphs < 0) {
+        const char* env = std::getenv("GAMMA_GRAPH");
+        g_ws.graphs = (env && env[0] == '0') ? 0 : 1;
+    }
+    if (r.profile)
+        for (cudaEvent_t& evn : g_ws.stage)
+            if (!evn) CU_TRY(cudaEventCreate(&evn));
+    return GAMMA_OK;
+}
+
+// The kernels of one call on `st` (which may be capturing).  Returns the number of kernels in *launched.
+//
+//   st :  k_norm -> k_classify -> k_star -> [k_bucket_scatter | LSD radix sort] -> (join) -> k_table_search
+//   aux:                    \-> k_offset_table ------------------------------------/
+//
+// The offset table only needs k_norm's maxima, so it is built on a library-owned side stream while the
+// star kernel runs.  No memset and no host synchronisation on the path: k_norm clears the control
+// block of the next call (two alternating slots; slot 2 belongs to the stand-alone entry points).
+int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
+                    const Resolved& r, float* out, cudaStream_t st, Ctl* ctl, Ctl* next, int* launched)
+{
+    const long long N = g.N;
+    int nk = 0;
     unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p), *i0 = static_cast<unsigned*>(g_ws.idx0.p);
     unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *i1 = static_cast<unsigned*>(g_ws.idx1.p);
     unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p);
     EvalP e;
     e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
-
     const int classes = r.presort == 4 ? 1 : 0;
-    g_ws.haveStages = false;
-    if (r.profile)
-        for (cudaEvent_t& evn : g_ws.stage)
-            if (!evn) CU_TRY(cudaEventCreate(&evn));
 #define STAGE_MARK(i, s) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], s)); } while (0)
     const int sm = g_ws.numSM;
-    if (g_ws.pdl < 0) {
-        const char* env = std::getenv("GAMMA_PDL");
-        g_ws.pdl = (env && env[0] == '0') ? 0 : 1;
-    }
     const bool pdl = g_ws.pdl != 0;
     STAGE_MARK(0, st);
-    auto fork_table = [&]() -> int {                                     // a3 on the side stream                                                                    // a3 on the side stream
+    {                                                                    // a0 + A1 step 1
+        long long blocks = (N + 1023) / 1024;
+        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
+        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, ctl, next));
+        ++nk;
+    }
+    {                                                                    // a1: exclusion + compaction
+        long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
+        int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
+        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0));
+        ++nk;
+    }
+    STAGE_MARK(1, st);
+    {                                                                    // a3 on the side stream
         CU_TRY(cudaEventRecord(g_ws.evFork, st));
         CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
         STAGE_MARK(5, g_ws.aux);
         k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, g_ws.aux>>>(
             g, e, ctl, -1.0f, r.tableCap, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
             static_cast<unsigned*>(g_ws.tmpIdx.p));
-        ++g_ws.launches;
+        ++nk;
         STAGE_MARK(6, g_ws.aux);
         CU_TRY(cudaEventRecord(g_ws.evJoin, g_ws.aux));
-            return GAMMA_OK;
-    };
-    static const int forkAt = std::getenv("GAMMA_FORK") ? std::atoi(std::getenv("GAMMA_FORK")) : 0;
-    {                                                                    // a0 + A1 step 1
-        long long blocks = (N + 1023) / 1024;
-        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
-        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, ctl, next));
-        ++g_ws.launches;
     }
-    if (forkAt == 1) { rc = fork_table(); if (rc) return rc; }
-    {                                                                    // a1: exclusion + compaction
-        long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
-        int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
-        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0));
-        ++g_ws.launches;
-    }
-    STAGE_MARK(1, st);
-    if (forkAt != 1) { rc = fork_table(); if (rc) return rc; }
     {                                                                    // star phase over the compacted voxels
         long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
-        if (g_ws.occStar[r.star] == 0) {
-            int occ = 0;
-            if (r.star) CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_star<true>, STAR_THREADS, 0));
-            else CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_star<false>, STAR_THREADS, 0));
-            g_ws.occStar[r.star] = occ > 0 ? occ : 1;
-        }
         const long long resident = (long long)sm * g_ws.occStar[r.star];
         int grid = (int)(blocks > resident ? resident : blocks);
         if (r.star)
             CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes));
         else
             CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes));
-        ++g_ws.launches;
+        ++nk;
     }
     STAGE_MARK(2, st);
     CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));     // before the presort, so that presort -> search stay adjacent
     const unsigned *lk = k0, *li = i0;
     if (r.presort == 1) {                                                // a2: one-pass MSD bucket presort
         CU_TRY(launch_ex(k_bucket_scatter, sm * 2, SCATTER_THREADS, 0, st, pdl, false, ctl, k0, i0, k1, i1));
-        ++g_ws.launches;
+        ++nk;
         lk = k1; li = i1;
     } else if (r.presort == 3) {                                         // a2: full LSD radix sort of the keys
         int where = radix_sort_enqueue(k0, i0, k1, i1, &ctl->nSearch, N, 32 - r.keyBits, 32,
                                        static_cast<unsigned*>(g_ws.tileHist.p), st);
-        g_ws.launches += 3 * (r.keyBits / 8);
+        nk += 3 * (r.keyBits / 8);
         if (where) { lk = k1; li = i1; }
     }
     STAGE_MARK(3, st);
@@ -457,18 +491,109 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             CU_TRY(launch_ex(k_table_search<32>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
         else
             CU_TRY(launch_ex(k_table_search<0>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
-        ++g_ws.launches;
+        ++nk;
     }
     STAGE_MARK(4, st);
 #undef STAGE_MARK
-    g_ws.haveStages = r.profile != 0;
+    *launched = nk;
+    return GAMMA_OK;
+}
+
+// Enqueue the whole hot path on `st` (device pointers).  Caller holds g_mu.
+// A call with arguments seen before (same pointers, geometry, criteria, options, control-block slot) replays a cached
+// CUDA graph of its kernels -- one driver call instead of five launches plus the fork/join of the side stream; the
+// graph is captured on a library-owned stream on first sight.  Not used when the caller's stream is itself being
+// captured, with opts.profile_stages, or GAMMA_GRAPH=0.  Opt-in (opts.graph = 1): measured on B200, a replay costs
+// less host time (24 vs 31 us per call) but back-to-back replays do not overlap their ramp-up with the previous call's
+// tail the way stream launches do (0.055 vs 0.045 ms per cfg3 case), so stream launches stay the default.
+int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
+                     const Resolved& r, float* out, cudaStream_t st)
+{
+    int rc = prepare_workspace(g, r);
+    if (rc) return rc;
+    cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
+    CU_TRY(cudaStreamIsCapturing(st, &capStatus));
+    if (capStatus != cudaStreamCaptureStatusNone) {
+        // The caller is capturing `st`: the kernels become nodes of the caller's graph.  The call must then be
+        // self-contained (its replays do not pass through this function): it owns control-block slot 3 and
+        // clears it with a memset node; ordering against other work is the captured stream's.
+        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + 3;
+        CU_TRY(cudaMemsetAsync(ctl, 0, sizeof(Ctl), st));
+        int launched = 0;
+        Resolved rr = r;
+        rr.profile = 0;
+        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, rr, out, st, ctl, nullptr, &launched);
+        if (rc) return rc;
+        g_ws.launches += launched;
+        g_ws.haveStages = false;
+        g_ws.lastCtl = ctl; g_ws.lastStream = nullptr; g_ws.lastN = g.N; g_ws.haveLast = true;
+        return GAMMA_OK;
+    }
+    rc = order_after_previous(st);
+    if (rc) return rc;
+    if (g_ws.ctl.p != g_ws.ctlOwner) { g_ws.ctlClean = false; g_ws.ctlOwner = g_ws.ctl.p; }
+    if (!g_ws.ctlClean) {                                  // first call, or a previous call failed half-way
+        CU_TRY(cudaMemsetAsync(g_ws.ctl.p, 0, CTL_SLOTS * sizeof(Ctl), st));
+        g_ws.slot = 0;
+    }
+    g_ws.ctlClean = false;                                 // set again when everything below was enqueued
+    Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
+    Ctl* ctl = base + g_ws.slot;
+    Ctl* next = base + (g_ws.slot ^ 1);
+    g_ws.haveStages = false;
+
+    const bool useGraph = g_ws.graphs != 0 && r.graph && !r.profile;
+    int launched = 0;
+    if (!useGraph) {
+        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, ctl, next, &launched);
+        if (rc) return rc;
+    } else {
+        if (g_ws.graphGen != g_allocGen) { g_ws.dropGraphs(); g_ws.graphGen = g_allocGen; }
+        GraphKey key;
+        std::memset(&key, 0, sizeof key);
+        key.ref = ref; key.ev = ev; key.out = out; key.ctl = ctl; key.g = g;
+        key.DD = DD; key.cutoff = cutoff; key.normDose = r.normDose;
+        key.mode = mode; key.presort = r.presort; key.star = r.star; key.lanes = r.lanes; key.keyBits = r.keyBits;
+        key.tableCap = r.tableCap;
+        GraphEntry* hit = nullptr;
+        for (int i = 0; i < g_ws.numGraphs; ++i)
+            if (g_ws.graph[i].key == key) { hit = &g_ws.graph[i]; break; }
+        if (!hit) {
+            cudaGraph_t graph = nullptr;
+            CU_TRY(cudaStreamBeginCapture(g_ws.cap, cudaStreamCaptureModeThreadLocal));
+            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, g_ws.cap, ctl, next, &launched);
+            cudaError_t ce = cudaStreamEndCapture(g_ws.cap, &graph);
+            if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (ce != cudaSuccess) return fail(GAMMA_ERR_CUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(ce));
+            cudaGraphExec_t exec = nullptr;
+            ce = cudaGraphInstantiate(&exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (ce != cudaSuccess) return fail(GAMMA_ERR_CUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ce));
+            int victim = g_ws.numGraphs;
+            if (victim == GRAPH_CACHE) {                   // evict the least recently used
+                victim = 0;
+                for (int i = 1; i < GRAPH_CACHE; ++i)
+                    if (g_ws.graph[i].lastUse < g_ws.graph[victim].lastUse) victim = i;
+                cudaGraphExecDestroy(g_ws.graph[victim].exec);
+            } else {
+                ++g_ws.numGraphs;
+            }
+            hit = &g_ws.graph[victim];
+            hit->key = key; hit->exec = exec; hit->kernels = launched;
+        }
+        hit->lastUse = ++g_ws.useClock;
+        launched = hit->kernels;
+        CU_TRY(cudaGraphLaunch(hit->exec, st));
+    }
+    g_ws.launches += launched;
+    g_ws.haveStages = r.profile != 0 && !useGraph;
     CU_TRY(cudaGetLastError());
     rc = mark_done(st);
     if (rc) return rc;
     g_ws.lastCtl = ctl;
     g_ws.slot ^= 1;
     g_ws.ctlClean = true;
-    g_ws.lastStream = st; g_ws.lastN = N; g_ws.haveLast = true;
+    g_ws.lastStream = st; g_ws.lastN = g.N; g_ws.haveLast = true;
     return GAMMA_OK;
 }
 
@@ -573,7 +698,7 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const long long maxTiles = (n + SORT_TILE - 1) / SORT_TILE;
-    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
     CU_TRY(g_ws.key1.need(n * 4)); CU_TRY(g_ws.idx1.need(n * 4));
     CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
     rc = order_after_previous(st);
@@ -622,7 +747,7 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
     CU_TRY(g_ws.table.need((size_t)max_entries * 16));
     CU_TRY(g_ws.tmpL.need((size_t)max_entries * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)max_entries * 4));
     CU_TRY(cudaFuncSetAttribute(k_offset_table, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TAB_DYN_SMEM));
@@ -647,7 +772,8 @@ int gamma_get_counters(gamma_counters* out_host)
     if (!out_host) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_host is NULL");
     std::lock_guard<std::mutex> lock(g_mu);
     if (!g_ws.haveLast || !g_ws.ctl.p) return fail(GAMMA_ERR_INVALID_ARGUMENT, "no gamma_eval call to report on");
-    CU_TRY(cudaStreamSynchronize(g_ws.lastStream));
+    if (g_ws.lastStream) CU_TRY(cudaStreamSynchronize(g_ws.lastStream));
+    else CU_TRY(cudaDeviceSynchronize());            // last call was captured by the caller: no stream to wait on
     Ctl c;
     CU_TRY(cudaMemcpy(&c, g_ws.lastCtl, sizeof c, cudaMemcpyDeviceToHost));
     std::memset(out_host, 0, sizeof *out_host);
@@ -694,7 +820,7 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
     int rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    CU_TRY(g_ws.ctl.need(3 * sizeof(Ctl)));
+    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
     cudaEvent_t a, b;
     CU_TRY(cudaEventCreate(&a)); CU_TRY(cudaEventCreate(&b));
     const int grid = g_ws.numSM * 8 * 4, threads = 256;

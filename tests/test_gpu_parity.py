@@ -254,6 +254,60 @@ def test_gamma_eval_host_streams_and_determinism():
     assert np.array_equal(o4.cpu().numpy().astype(np.float64), base, equal_nan=True)
 
 
+def test_graph_replay_sees_new_data_and_matches_plain_launches(oracle_mod):
+    """A repeated call (same pointers and arguments) replays a cached CUDA graph: the replay must read the
+    buffers' CURRENT contents, agree bit for bit with kernel-by-kernel launches (opts.graph = 2), survive more
+    argument sets than the cache holds, and step aside when the caller captures the stream itself."""
+    c = phantoms.make_case("cfg2_small")
+    n = c.ref.size
+    r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+    e = torch.from_numpy(c.eval.ravel().copy()).cuda()
+    out = torch.empty(n, dtype=torch.float32, device="cuda")
+    a = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    l0 = binding.gamma_launch_count()
+    gr = GammaOpts(graph=1)
+    for _ in range(3):                                       # capture on the first call(s), then replays
+        binding.gamma_eval_ex(r, e, *a, gr, out)
+    torch.cuda.synchronize()
+    assert binding.gamma_launch_count() - l0 == 15           # 5 kernels per call, counted for replays too
+    first = out.clone()
+    plain = binding.gamma_eval_ex(r, e, *a, GammaOpts(graph=2))
+    torch.cuda.synchronize()
+    assert torch.equal(torch.nan_to_num(first, nan=-1.0), torch.nan_to_num(plain, nan=-1.0))
+    # new data in the same buffers: eval scaled, reference shifted -> the replay must follow
+    e.mul_(1.03)
+    r.add_(0.01)
+    for _ in range(2):
+        binding.gamma_eval_ex(r, e, *a, gr, out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().astype(np.float64)
+    want = cpu_gamma(oracle_mod, r.cpu().numpy(), e.cpu().numpy(), *a)
+    assert_parity(got, want, "graph replay after the inputs changed in place")
+    assert not torch.equal(torch.nan_to_num(first, nan=-1.0), torch.nan_to_num(out, nan=-1.0))
+    # more argument sets than the cache keeps (64): eviction, then the first set again
+    outs = []
+    for k in range(70):
+        outs.append(binding.gamma_eval_ex(r, e, c.dims, c.spacing_mm, c.dd, c.dta_mm + 0.01 * k, c.mode, c.cutoff, gr))
+    again = binding.gamma_eval_ex(r, e, *a, gr, out).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(torch.nan_to_num(again, nan=-1.0), torch.nan_to_num(outs[0], nan=-1.0))
+    assert float(torch.nan_to_num(outs[69], nan=0.0).sum()) < float(torch.nan_to_num(outs[0], nan=0.0).sum())
+    # the caller captures the stream: the library launches its kernels into that capture instead
+    side = torch.cuda.Stream()
+    out2 = torch.empty_like(out)
+    with torch.cuda.stream(side):
+        binding.gamma_eval_ex(r, e, *a, None, out2)          # warm (workspace exists)
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            binding.gamma_eval_ex(r, e, *a, None, out2)
+        out2.zero_()
+        g.replay()
+        g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(torch.nan_to_num(out2, nan=-1.0), torch.nan_to_num(again, nan=-1.0))
+
+
 def test_stage_times_are_reported():
     c = phantoms.make_case("cfg2_small")
     gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, GammaOpts(profile_stages=1))
