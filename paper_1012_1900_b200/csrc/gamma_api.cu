@@ -422,7 +422,8 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p);
     EvalP e;
     e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
-    const int classes = r.presort == 4 ? 1 : 0;
+    const int classes = (r.presort == 4 && r.star && g.all_active) ? 1 : 0;   // needs the 3D star phase
+    const int presort = (r.presort == 4 && !classes) ? 1 : r.presort;
 #define STAGE_MARK(i, s) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], s)); } while (0)
     const int sm = g_ws.numSM;
     const bool pdl = g_ws.pdl != 0;
@@ -464,11 +465,11 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     STAGE_MARK(2, st);
     CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));     // before the presort, so that presort -> search stay adjacent
     const unsigned *lk = k0, *li = i0;
-    if (r.presort == 1) {                                                // a2: one-pass MSD bucket presort
+    if (presort == 1) {                                                // a2: one-pass MSD bucket presort
         CU_TRY(launch_ex(k_bucket_scatter, sm * 2, SCATTER_THREADS, 0, st, pdl, false, ctl, k0, i0, k1, i1));
         ++nk;
         lk = k1; li = i1;
-    } else if (r.presort == 3) {                                         // a2: full LSD radix sort of the keys
+    } else if (presort == 3) {                                         // a2: full LSD radix sort of the keys
         int where = radix_sort_enqueue(k0, i0, k1, i1, &ctl->nSearch, N, 32 - r.keyBits, 32,
                                        static_cast<unsigned*>(g_ws.tileHist.p), st);
         nk += 3 * (r.keyBits / 8);
@@ -476,21 +477,27 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     }
     STAGE_MARK(3, st);
     {                                                                    // a4 + a5
-        const int grid = sm * 4;                                         // resident blocks at 64 registers
+        const int grid = sm * (r.lanes == 0 ? 3 : 4);                    // resident blocks at 80 / 64 registers
         const int4* tab = static_cast<const int4*>(g_ws.table.p);
         // adaptive lanes: an item is "deep" when its key exceeds the smallest non-zero table distance
         float hmin = 0.0f;
         for (int a = 0; a < 3; ++a)
             if (g.h[a] > 0.0f && (hmin == 0.0f || g.h[a] < hmin)) hmin = g.h[a];
-        const int deepDigit = (r.presort == 1 || r.presort == 3) ? host_key_digit(hmin) + 1 : KEY_DIGITS;
+        const int deepDigit = (presort == 1 || presort == 3) ? host_key_digit(hmin) + 1 : KEY_DIGITS;
+        GammaRingP ring;
+        std::memset(&ring, 0, sizeof ring);
+        if (classes) {
+            const double hh[3] = {(double)g.h[0] * g.h[0], (double)g.h[1] * g.h[1], (double)g.h[2] * g.h[2]};
+            gamma_ring_constants(hh, ring);
+        }
         if (r.lanes == 1)
-            CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
+            CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
         else if (r.lanes == 8)
-            CU_TRY(launch_ex(k_table_search<8>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
+            CU_TRY(launch_ex(k_table_search<8>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
         else if (r.lanes == 32)
-            CU_TRY(launch_ex(k_table_search<32>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
+            CU_TRY(launch_ex(k_table_search<32>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
         else
-            CU_TRY(launch_ex(k_table_search<0>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes));
+            CU_TRY(launch_ex(k_table_search<0>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
         ++nk;
     }
     STAGE_MARK(4, st);

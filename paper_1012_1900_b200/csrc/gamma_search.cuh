@@ -234,7 +234,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
         unsigned nextItem = numItems;
         if (dynamic && lane == 0) nextItem = atomicAdd(&ctl->tileCounter, 1u) + warpsTotal;
         const unsigned j = item * 32u + lane;
-        bool toSearch = false;
+        bool toSearch = false, starDone = false;
         float key = 0.0f;
         int lin = 0;
         if (j < M) {
@@ -269,6 +269,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
                                 dhi = fmaxf(dhi, dv);
                             }
                     const float gmax = gamma_star_gmax(d, g.invA);
+                    starDone = true;
                     key = key / sqrtf(gmax);              // gamma_star
                     // Lower bound of everything OUTSIDE the star: beyond the 8 touching cells the spatial distance
                     // alone is >= hmin; inside them (but outside the star) it is >= rho_link and the dose is a
@@ -288,7 +289,9 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
                 toSearch = false;
             }
         }
-        const bool deep = toSearch && classes && key * key > g.hmin2;
+        // "ring" items: the star is done and what is left of the voxel's 2x2x2 block of cells decides (everything
+        // else is at least hmin away); all other items walk the table from its first entry
+        const bool deep = toSearch && classes && !(starDone && key * key < g.hmin2);
         const unsigned bal = __ballot_sync(FULL, toSearch && !deep);   // append to the work list, warp-aggregated
         if (bal) {
             const int leader = __ffs(bal) - 1;
@@ -556,17 +559,47 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
     return visits;
 }
 
+// One thread per "ring" item (depth classes): an interior voxel whose star phase is done and whose running
+// gamma is below the smallest voxel spacing.  Everything that can still be closer lies in the 72 ring faces of its
+// 2x2x2 block of cells (gamma_ring_min); the 27 doses are re-read (L1/L2 hits) and no table is walked.
+__device__ __forceinline__ void ring_items(const SearchCtx& c, const GridP& g, const EvalP& e, const GammaRingP& R,
+                                           const unsigned* __restrict__ listKey,
+                                           const unsigned* __restrict__ listIdx, unsigned nList, unsigned firstItem,
+                                           int lane)
+{
+    const unsigned item = firstItem + (unsigned)lane;
+    if (item >= nList) return;
+    const int lin = (int)listIdx[item];
+    const float key = __uint_as_float(listKey[item]);
+    const float Dr = __ldg(c.ref + lin);
+    const float invdD = e.mode == 0 ? c.invGlobal : criterion_inv_dD(e, c.dnorm, Dr);
+    const float* p = c.ev + lin;
+    float d[27];
+#pragma unroll
+    for (int oz = -1; oz <= 1; ++oz)
+#pragma unroll
+        for (int oy = -1; oy <= 1; ++oy)
+#pragma unroll
+            for (int ox = -1; ox <= 1; ++ox)
+                d[(ox + 1) + 3 * (oy + 1) + 9 * (oz + 1)] =
+                    (__ldg(p + ox + oy * g.stride[1] + oz * g.stride[2]) - Dr) * invdD;
+    const float best2 = gamma_ring_min(d, g.invA, R, key * key);
+    c.out[lin] = fminf(key, sqrtf(best2));                 // a5: write at the voxel's own place
+}
+
 // MODE = lanes per reference voxel: 1 (thread per voxel), 8, 32, or 0 = adaptive: deep items (the
 // walk will pass the first table entry) get a whole warp each, the others 8 lanes each.  Deep items are either
 // the tail of the sorted list (key digit >= deepDigit, counted from the digit histogram) or, with depth-class
-// lists (classes != 0), the separate list (deepKey, deepIdx) that k_star filled.  Work units are handed out
+// lists (classes != 0), the separate list (deepKey, deepIdx) that k_star filled; the other list then holds "ring"
+// items only, searched one per thread (ring_items).  Work units are handed out
 // deepest first: first round static, later rounds by an atomic counter whose latency hides behind the search.
 template <int MODE>
-__global__ void __launch_bounds__(SEARCH_THREADS)
+__global__ void __launch_bounds__(SEARCH_THREADS, MODE == 0 ? 3 : 1)
 k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
                EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
                const unsigned* __restrict__ listIdx, const unsigned* __restrict__ deepKey,
-               const unsigned* __restrict__ deepIdx, const int4* __restrict__ table, int deepDigit, int classes)
+               const unsigned* __restrict__ deepIdx, const int4* __restrict__ table, int deepDigit, int classes,
+               const __grid_constant__ GammaRingP ring)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -587,7 +620,8 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     const unsigned nDeepList = (MODE == 0 && classes) ? nDeep : nS;   // deep item i is entry nDeepList - 1 - i
     if (nS + nDeep == 0) return;
     constexpr unsigned VPW = MODE == 0 ? 4u : 32u / (unsigned)(MODE == 0 ? 8 : MODE);
-    const unsigned numUnits = MODE == 0 ? nDeep + (nShallow + 3u) / 4u : (nS + VPW - 1u) / VPW;
+    const unsigned numUnits = MODE != 0 ? (nS + VPW - 1u) / VPW
+                              : classes ? nDeep + (nShallow + 31u) / 32u : nDeep + (nShallow + 3u) / 4u;
     const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
     unsigned unit = blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5);
     if (unit >= numUnits) return;
@@ -606,7 +640,7 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
         if (dynamic && lane == 0) nextUnit = atomicAdd(&ctl->workCounter, 1u) + warpsTotal;
         if (MODE == 0) {
             if (unit < nDeep) visits += search_items<32>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane);
-            else if (classes) visits += search_items<8>(c, g, e, listKey, listIdx, nS, 4u * (unit - nDeep), lane);
+            else if (classes) ring_items(c, g, e, ring, listKey, listIdx, nS, 32u * (unit - nDeep), lane);
             else visits += search_items<8>(c, g, e, listKey, listIdx, nS, nDeep + 4u * (unit - nDeep), lane);
         } else {
             visits += search_items<(MODE == 0 ? 8 : MODE)>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);

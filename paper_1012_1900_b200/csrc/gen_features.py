@@ -16,11 +16,16 @@ mutually orthogonal spatial parts, so the normal equations (V^T V) w = V^T P of 
     t_i = lam_i - r w_i                 feasible  <=>  1 >= t_1 >= ... >= t_k >= 0
     dist^2 = C + N r                    C = squared distance from the reference point to the spatial
                                             affine hull of the face (depends on the offset only)
-Two routines are emitted:
+Three routines are emitted:
   * gamma_star_gmax   -- the 75 faces that contain the reference voxel itself (C = 0, N = d0,
                          lam in {0,1}):  gamma_star^2 = d0^2 / max feasible G1, no division per face;
   * gamma_owned_min   -- the 26 faces owned by a grid vertex c (= faces whose lowest vertex is c),
-                         any offset, with per-face validity (faces that would leave the grid).
+                         any offset, with per-face validity (faces that would leave the grid);
+  * gamma_ring_min    -- the 72 faces of the 2x2x2 block of cells around an interior reference voxel that neither
+                         contain the voxel (those are the star) nor lie on the block's boundary (those are at least
+                         one voxel spacing away): together with the star, everything closer than min_a h_a.  The
+                         offsets are compile-time, so lam_i and C are per-geometry constants (gamma_ring_constants,
+                         evaluated once on the host in double precision).
 """
 import itertools
 import os
@@ -190,6 +195,103 @@ def emit_owned(w):
     w("    return best2;\n}\n")
 
 
+def ring_faces():
+    """(owner o, neg mask, chain) of the 72 ring faces, in emission order."""
+    out = []
+    for o in itertools.product((-1, 0), repeat=3):
+        neg = sum(AX[a] for a in range(3) if o[a] == -1)
+        for ch in chains():
+            full = (0,) + ch
+            if neg in full:
+                continue                                     # contains the reference voxel: star
+            verts = [add(o, s) for s in full]
+            if any(all(v[a] == -1 for v in verts) or all(v[a] == 1 for v in verts) for a in range(3)):
+                continue                                     # lies in a boundary plane of the block
+            out.append((o, neg, ch))
+    assert len(out) == 72, len(out)
+    return out
+
+
+def emit_ring(w):
+    faces = ring_faces()
+    w("\n// Per-geometry constants of gamma_ring_min: lam[neg][T] = (sum of h_a^2 over a in T with o_a = -1) / A_T for the\n")
+    w("// owner o (neg = mask of its -1 coordinates) and axis subset T;  C[f] = squared distance from the reference\n")
+    w("// voxel to the spatial affine hull of ring face f.\n")
+    w("struct GammaRingP {\n    float lam[8][8];\n    float C[72];\n};\n\n")
+    w("// hh[a] = (spacing_a / DTA)^2 in double; every axis must be active.\n")
+    w("inline void gamma_ring_constants(const double (&hh)[3], GammaRingP& R)\n{\n")
+    w("    double lam[8][8], X[8][8], q[8][3];\n")
+    w("    for (int neg = 0; neg < 8; ++neg) {\n")
+    w("        for (int a = 0; a < 3; ++a) q[neg][a] = (neg >> a) & 1 ? hh[a] : 0.0;\n")
+    w("        for (int T = 0; T < 8; ++T) {\n")
+    w("            double A = 0.0, s = 0.0;\n")
+    w("            for (int a = 0; a < 3; ++a)\n")
+    w("                if ((T >> a) & 1) { A += hh[a]; if ((neg >> a) & 1) s += hh[a]; }\n")
+    w("            lam[neg][T] = T ? s / A : 0.0;\n")
+    w("            X[neg][T] = T ? s * (A - s) / A : 0.0;\n")
+    w("            R.lam[neg][T] = (float)lam[neg][T];\n")
+    w("        }\n    }\n")
+    for f, (o, neg, ch) in enumerate(faces):
+        full = (0,) + ch
+        steps = [full[i] ^ full[i - 1] for i in range(1, len(full))]
+        terms = ["X[%d][%d]" % (neg, t) for t in steps if bin(t).count("1") >= 2]
+        terms += ["q[%d][%d]" % (neg, a) for a in range(3) if not (ch[-1] & AX[a])]
+        w("    R.C[%d] = (float)(%s);\n" % (f, " + ".join(terms) if terms else "0.0"))
+    w("}\n\n")
+    w("// The 72 ring faces (12 edges, 36 triangles, 24 tetrahedra), generated.  d[27] and invA as in gamma_star_gmax.\n")
+    w("// Returns min(best2, squared distance to every feasible ring face).\n")
+    w("GAMMA_HD float gamma_ring_min(const float (&d)[27], const float (&invA)[8], const GammaRingP& R, float best2)\n{\n")
+    done_e, done_n, done_g = set(), set(), set()
+
+    def edge(a_off, tmask):
+        nm = "%d_%d" % (vid(a_off), tmask)
+        if nm not in done_e:
+            w("    const float dl%s = d[%d] - d[%d];\n" % (nm, vid(add(a_off, tmask)), vid(a_off)))
+            w("    const float w%s = dl%s * invA[%d];\n" % (nm, nm, tmask))
+            done_e.add(nm)
+        return nm
+
+    def chain_edges(o, full):
+        return [edge(add(o, full[i - 1]), full[i] ^ full[i - 1]) for i in range(1, len(full))]
+
+    def nsum(o, neg, full):
+        nm = "N%d_" % vid(o) + "_".join(str(s) for s in full)
+        if nm not in done_n:
+            e = chain_edges(o, full)[-1]
+            prev = "d[%d]" % vid(o) if len(full) == 2 else nsum(o, neg, full[:-1])
+            w("    const float %s = fmaf(dl%s, R.lam[%d][%d], %s);\n" % (nm, e, neg, full[-1] ^ full[-2], prev))
+            done_n.add(nm)
+        return nm
+
+    def gsum(o, full):
+        nm = "G%d_" % vid(o) + "_".join(str(s) for s in full)
+        if nm not in done_g:
+            e = chain_edges(o, full)[-1]
+            prev = "1.0f" if len(full) == 2 else gsum(o, full[:-1])
+            w("    const float %s = fmaf(dl%s, w%s, %s);\n" % (nm, e, e, prev))
+            done_g.add(nm)
+        return nm
+
+    for f, (o, neg, ch) in enumerate(faces):
+        full = (0,) + ch
+        k = len(ch)
+        names = chain_edges(o, full)
+        N, G = nsum(o, neg, full), gsum(o, full)
+        w("    {   // face %d: owner (%d,%d,%d) chain %s\n" % (f, o[0], o[1], o[2], "<".join(str(s) for s in full)))
+        w("        const float r = GAMMA_FDIV(%s, %s);\n" % (N, G))
+        ts = []
+        for i in range(k):
+            w("        const float t%d = fmaf(-r, w%s, R.lam[%d][%d]);\n" % (i + 1, names[i], neg, full[i + 1] ^ full[i]))
+            ts.append("t%d" % (i + 1))
+        conds = ["1.0f >= t1"]
+        conds += ["%s >= %s" % (ts[i], ts[i + 1]) for i in range(k - 1)]
+        conds.append("%s >= 0.0f" % ts[-1])
+        w("        best2 = (%s) ? fminf(best2, fmaf(%s, r, R.C[%d])) : best2;\n"
+          % (" & ".join("(%s)" % x for x in conds), N, f))
+        w("    }\n")
+    w("    return best2;\n}\n")
+
+
 def main():
     here = os.path.dirname(os.path.abspath(__file__))
     path = os.path.join(here, "features_generated.cuh")
@@ -207,6 +309,7 @@ def main():
           "#define GAMMA_FDIV(a, b) gamma_fdiv((a), (b))\n#else\n#define GAMMA_FDIV(a, b) ((a) / (b))\n#endif\n\n")
         emit_star(w)
         emit_owned(w)
+        emit_ring(w)
     print("wrote", path)
 
 

@@ -98,14 +98,20 @@ def test_large_grids_sampled_parity(oracle_mod, name, n_random, n_top):
 
 def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
     """Config 5 is run with and without the voxel pre-sort (Table 2) and with the paper's
-    thread-per-voxel mapping: the candidate set is the same, so gamma is bit-identical."""
+    thread-per-voxel mapping: the candidate set and the arithmetic of the table walk are the same, so gamma is
+    bit-identical among these.  The default (depth classes) evaluates the ring faces of shallow voxels with
+    host-rounded constants instead: same faces, other rounding, so it agrees to a few ulp."""
     c = phantoms.make_case("cfg5")
-    base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
-    for o in (GammaOpts(presort=1), GammaOpts(presort=2), GammaOpts(presort=3), GammaOpts(lanes_per_voxel=1),
+    base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, GammaOpts(presort=1))
+    for o in (GammaOpts(presort=2), GammaOpts(presort=3), GammaOpts(lanes_per_voxel=1),
               GammaOpts(lanes_per_voxel=1, presort=2), GammaOpts(lanes_per_voxel=32)):
         g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
         assert np.array_equal(np.isnan(g), np.isnan(base))
         assert np.array_equal(g[~np.isnan(g)], base[~np.isnan(base)]), o
+    g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    assert np.array_equal(np.isnan(g), np.isnan(base))
+    m = ~np.isnan(g)
+    assert np.abs(g[m] - base[m]).max() <= 2e-6
 
 
 # ----------------------------------------------------------------------------------------------------
