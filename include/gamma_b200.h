@@ -82,7 +82,8 @@ typedef struct gamma_opts {
                              8 lanes for the others; needs presort 1, 3 or 4, else 8); 1 = the paper's
                              thread-per-voxel mapping; 8; 32                               */
     int sort_key_bits;    /* presort = 3 only.  0: default (= 16); 8, 16, 24 or 32 most significant key bits   */
-    long long table_cap;  /* 0: default (1<<20); max entries of the sorted offset table; past it the search
+    long long table_cap;  /* 0: default (8192 with table_radius 1, 1<<20 with 2); max cells of the candidate box
+                             of the sorted offset table (>= its entries); past the table the search
                              continues by exhaustive enumeration, so results never depend on it            */
     int profile_stages;   /* 1: record CUDA events between the stages of this call on `stream`, to be read
                              with gamma_get_stage_times (adds a few event records, no synchronisation)     */
@@ -92,6 +93,11 @@ typedef struct gamma_opts {
                              way stream launches do; 2: launch the kernels one by one.  Ignored (= 2) while
                              `stream` is being captured by the caller (the kernels then become nodes of the
                              caller's graph, with their own control block) and with profile_stages          */
+    int table_radius;     /* 0: default (= 1); 1: the table is a data-independent PREFIX of the paper's table,
+                             as far as table_cap allows, built beside a0 (nothing on the critical path);
+                             2: the paper's radius max |DD| / dD (A1 steps 1-2), built once
+                             a0's maxima exist                                                              */
+    int pad_;
 } gamma_opts;
 
 /* gamma_eval with options (opts may be NULL = defaults).  Same contract as gamma_eval. */

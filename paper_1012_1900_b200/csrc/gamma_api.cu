@@ -86,7 +86,7 @@ struct GraphKey {
     void* ctl;
     GridP g;
     float DD, cutoff, normDose;
-    int mode, presort, star, lanes, keyBits;
+    int mode, presort, star, lanes, keyBits, tableMode;
     long long tableCap;
     bool operator==(const GraphKey& o) const { return std::memcmp(this, &o, sizeof *this) == 0; }
 };
@@ -314,16 +314,16 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
 }
 
 struct Resolved {
-    int presort, star, lanes, keyBits, profile, graph;
+    int presort, star, lanes, keyBits, profile, graph, tableMode;
     long long tableCap;
     float normDose;
 };
 
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
-    r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 1ll << 20; r.normDose = 0.0f;
+    r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 0; r.tableMode = 1; r.normDose = 0.0f;
     r.profile = 0; r.graph = 0;
-    if (!o) return GAMMA_OK;
+    if (!o) { r.tableCap = 8192; return GAMMA_OK; }
     r.profile = o->profile_stages == 1;
     if (o->graph < 0 || o->graph > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.graph must be 0, 1 or 2");
     r.graph = o->graph == 1;
@@ -349,6 +349,10 @@ int resolve_opts(const gamma_opts* o, Resolved& r)
         r.tableCap = o->table_cap;
     }
     if (r.presort == 4 && r.lanes != 0) r.presort = 1;   // depth classes only exist for the adaptive search
+    if (o->table_radius < 0 || o->table_radius > 2)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.table_radius must be 0, 1 or 2");
+    if (o->table_radius == 2) r.tableMode = 2;
+    if (r.tableCap == 0) r.tableCap = r.tableMode == 1 ? 8192 : (1ll << 20);
     if (o->norm_dose > 0.0f) r.normDose = o->norm_dose;
     if (std::isnan(o->norm_dose) || std::isinf(o->norm_dose))
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.norm_dose must be finite");
@@ -428,6 +432,35 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     const int sm = g_ws.numSM;
     const bool pdl = g_ws.pdl != 0;
     STAGE_MARK(0, st);
+    // a3 on the side stream.  Default: a data-independent PREFIX of the paper's table, as large as table_cap allows,
+    // forked before k_norm so that it is ready long before the search; beyond it the search enumerates (exact).
+    // table_radius = 2: the paper's radius max |DD| / dD (A1 steps 1-2), forked once k_norm's maxima exist.
+    auto fork_table = [&]() -> int {
+        float radius = -1.0f;
+        if (r.tableMode == 1) {                            // largest radius whose candidate box has <= cap cells
+            float lo = 0.0f, hi = grid_diagonal(g);
+            int bx, by, bz;
+            if (table_box_cells(g, hi, bx, by, bz) <= r.tableCap) lo = hi;
+            else
+                for (int it = 0; it < 48; ++it) {
+                    const float mid = 0.5f * (lo + hi);
+                    if (table_box_cells(g, mid, bx, by, bz) <= r.tableCap) lo = mid; else hi = mid;
+                }
+            radius = lo;
+        }
+        CU_TRY(cudaEventRecord(g_ws.evFork, st));
+        CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
+        STAGE_MARK(5, g_ws.aux);
+        k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, g_ws.aux>>>(
+            g, e, ctl, radius, r.tableCap, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
+            static_cast<unsigned*>(g_ws.tmpIdx.p), r.tableMode == 1 ? 1 : 0);
+        ++nk;
+        STAGE_MARK(6, g_ws.aux);
+        CU_TRY(cudaEventRecord(g_ws.evJoin, g_ws.aux));
+        return GAMMA_OK;
+    };
+    int rc = GAMMA_OK;
+    if (r.tableMode == 1) { rc = fork_table(); if (rc) return rc; }
     {                                                                    // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
@@ -441,17 +474,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         ++nk;
     }
     STAGE_MARK(1, st);
-    {                                                                    // a3 on the side stream
-        CU_TRY(cudaEventRecord(g_ws.evFork, st));
-        CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
-        STAGE_MARK(5, g_ws.aux);
-        k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, g_ws.aux>>>(
-            g, e, ctl, -1.0f, r.tableCap, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
-            static_cast<unsigned*>(g_ws.tmpIdx.p));
-        ++nk;
-        STAGE_MARK(6, g_ws.aux);
-        CU_TRY(cudaEventRecord(g_ws.evJoin, g_ws.aux));
-    }
+    if (r.tableMode != 1) { rc = fork_table(); if (rc) return rc; }      // paper's radius: needs k_norm's max |DD|
     {                                                                    // star phase over the compacted voxels
         long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
         const long long resident = (long long)sm * g_ws.occStar[r.star];
@@ -561,7 +584,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         key.ref = ref; key.ev = ev; key.out = out; key.ctl = ctl; key.g = g;
         key.DD = DD; key.cutoff = cutoff; key.normDose = r.normDose;
         key.mode = mode; key.presort = r.presort; key.star = r.star; key.lanes = r.lanes; key.keyBits = r.keyBits;
-        key.tableCap = r.tableCap;
+        key.tableCap = r.tableCap; key.tableMode = r.tableMode;
         GraphEntry* hit = nullptr;
         for (int i = 0; i < g_ws.numGraphs; ++i)
             if (g_ws.graph[i].key == key) { hit = &g_ws.graph[i]; break; }
@@ -765,7 +788,7 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     e.DD = 1.0f; e.cutoff = 0.0f; e.norm_dose = 1.0f; e.mode = 0;
     k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, st>>>(
         g, e, ctl, radius, max_entries, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
-        static_cast<unsigned*>(g_ws.tmpIdx.p));
+        static_cast<unsigned*>(g_ws.tmpIdx.p), 0);
     k_table_export<<<64, 256, 0, st>>>(ctl, static_cast<const int4*>(g_ws.table.p), max_entries, out_entries, out_count);
     g_ws.launches += 2;
     CU_TRY(cudaGetLastError());

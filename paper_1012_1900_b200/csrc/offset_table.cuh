@@ -24,6 +24,22 @@ constexpr int TAB_SLICE = TAB_BUCKETS / TAB_BLOCKS;      // buckets finished by 
 constexpr int TAB_SMEM_ENTRIES = 8192;                   // slice entries kept in shared memory (else global scratch)
 constexpr size_t TAB_DYN_SMEM = (size_t)TAB_SMEM_ENTRIES * 2 * sizeof(unsigned);
 
+// Diagonal of the grid in DTA units: nothing is farther away than this.
+__host__ __device__ inline float grid_diagonal(const GridP& g)
+{
+    const float ax = (float)(g.n[0] - 1) * g.h[0], ay = (float)(g.n[1] - 1) * g.h[1], az = (float)(g.n[2] - 1) * g.h[2];
+    return sqrtf(ax * ax + ay * ay + az * az) * 1.0001f + 1e-3f;
+}
+
+// Cells of the candidate box of radius R (m_a in [0, box_a)), the quantity `cap` limits.
+__host__ __device__ inline long long table_box_cells(const GridP& g, float R, int& bx, int& by, int& bz)
+{
+    bx = g.h[0] > 0.0f ? (int)fminf((float)(g.n[0] - 1), floorf(R / g.h[0])) + 1 : 1;
+    by = g.h[1] > 0.0f ? (int)fminf((float)(g.n[1] - 1), floorf(R / g.h[1])) + 1 : 1;
+    bz = g.h[2] > 0.0f ? (int)fminf((float)(g.n[2] - 1), floorf(R / g.h[2])) + 1 : 1;
+    return (long long)bx * by * bz;
+}
+
 // Upper bound of every key of the search list (the paper's table radius max(DD)/dD), from k_norm's maxima.
 __device__ inline float table_radius_from_ctl(const GridP& g, const EvalP& e, const Ctl* ctl)
 {
@@ -42,15 +58,16 @@ __device__ inline float table_radius_from_ctl(const GridP& g, const EvalP& e, co
     }
     if (!(R >= 0.0f)) R = 0.0f;                                       // NaN guard
     // nothing in the grid is farther than its diagonal: clamp (also makes an infinite bound finite)
-    const float ax = (float)(g.n[0] - 1) * g.h[0], ay = (float)(g.n[1] - 1) * g.h[1], az = (float)(g.n[2] - 1) * g.h[2];
-    const float Rgrid = sqrtf(ax * ax + ay * ay + az * az) * 1.0001f + 1e-3f;
-    return fminf(R, Rgrid);
+    return fminf(R, grid_diagonal(g));
 }
 
 // radius_in >= 0: use it; < 0: radius from the control block (table_radius_from_ctl).
+// prefix != 0: radius_in is a data-independent radius (as far as `cap` allows): the table is a PREFIX of the
+// paper's table, flagged truncated unless it reaches the grid diagonal, and the search goes on beyond it by
+// enumeration -- so the kernel needs nothing from k_norm and runs beside it.
 __global__ void __launch_bounds__(TAB_THREADS)
 k_offset_table(GridP g, EvalP e, Ctl* __restrict__ ctl, float radius_in, long long cap, int4* __restrict__ table,
-               unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx)
+               unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx, int prefix)
 {
     extern __shared__ unsigned sSlice[];                 // [TAB_SMEM_ENTRIES] L^2 bits, [TAB_SMEM_ENTRIES] box index
     __shared__ unsigned start[TAB_BUCKETS + 1];
@@ -65,13 +82,10 @@ k_offset_table(GridP g, EvalP e, Ctl* __restrict__ ctl, float radius_in, long lo
         float R = radius_in >= 0.0f ? radius_in : table_radius_from_ctl(g, e, ctl);
         if (!(R >= 0.0f)) R = 0.0f;
         R = fminf(R, 3.0e18f);
-        unsigned trunc = 0;
+        unsigned trunc = (prefix && R < grid_diagonal(g)) ? 1u : 0u;
         int bx, by, bz;
         for (;;) {
-            bx = g.h[0] > 0.0f ? (int)fminf((float)(g.n[0] - 1), floorf(R / g.h[0])) + 1 : 1;
-            by = g.h[1] > 0.0f ? (int)fminf((float)(g.n[1] - 1), floorf(R / g.h[1])) + 1 : 1;
-            bz = g.h[2] > 0.0f ? (int)fminf((float)(g.n[2] - 1), floorf(R / g.h[2])) + 1 : 1;
-            if ((long long)bx * by * bz <= cap) break;
+            if (table_box_cells(g, R, bx, by, bz) <= cap) break;
             // 0.8 per step terminates because cap >= 1 and R -> 0 gives a 1x1x1 box
             R *= 0.8f;
             trunc = 1;

@@ -119,7 +119,8 @@ def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
 # ----------------------------------------------------------------------------------------------------
 VARIANTS = [
     GammaOpts(), GammaOpts(star_phase=2), GammaOpts(presort=2), GammaOpts(lanes_per_voxel=1), GammaOpts(presort=1),
-    GammaOpts(presort=4, star_phase=2), GammaOpts(presort=4, table_cap=2),
+    GammaOpts(presort=4, star_phase=2), GammaOpts(presort=4, table_cap=2), GammaOpts(table_radius=2),
+    GammaOpts(table_radius=2, presort=1, table_cap=9),
     GammaOpts(lanes_per_voxel=32), GammaOpts(star_phase=2, lanes_per_voxel=1, presort=2),
     GammaOpts(presort=3, sort_key_bits=8), GammaOpts(presort=3, sort_key_bits=32), GammaOpts(table_cap=1),
     GammaOpts(table_cap=7, star_phase=2), GammaOpts(table_cap=40, lanes_per_voxel=32),
