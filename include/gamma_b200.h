@@ -82,7 +82,7 @@ typedef struct gamma_opts {
                              8 lanes for the others; needs presort 1, 3 or 4, else 8); 1 = the paper's
                              thread-per-voxel mapping; 8; 32                               */
     int sort_key_bits;    /* presort = 3 only.  0: default (= 16); 8, 16, 24 or 32 most significant key bits   */
-    long long table_cap;  /* 0: default (8192 with table_radius 1, 1<<20 with 2); max cells of the candidate box
+    long long table_cap;  /* 0: default (1024 with table_radius 1, 1<<20 with 2); max cells of the candidate box
                              of the sorted offset table (>= its entries); past the table the search
                              continues by exhaustive enumeration, so results never depend on it            */
     int profile_stages;   /* 1: record CUDA events between the stages of this call on `stream`, to be read

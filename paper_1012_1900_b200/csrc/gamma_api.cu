@@ -323,7 +323,7 @@ int resolve_opts(const gamma_opts* o, Resolved& r)
 {
     r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 0; r.tableMode = 1; r.normDose = 0.0f;
     r.profile = 0; r.graph = 0;
-    if (!o) { r.tableCap = 8192; return GAMMA_OK; }
+    if (!o) { r.tableCap = TAB_EMBED_MAX_CELLS; return GAMMA_OK; }
     r.profile = o->profile_stages == 1;
     if (o->graph < 0 || o->graph > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.graph must be 0, 1 or 2");
     r.graph = o->graph == 1;
@@ -352,7 +352,7 @@ int resolve_opts(const gamma_opts* o, Resolved& r)
     if (o->table_radius < 0 || o->table_radius > 2)
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.table_radius must be 0, 1 or 2");
     if (o->table_radius == 2) r.tableMode = 2;
-    if (r.tableCap == 0) r.tableCap = r.tableMode == 1 ? 8192 : (1ll << 20);
+    if (r.tableCap == 0) r.tableCap = r.tableMode == 1 ? TAB_EMBED_MAX_CELLS : (1ll << 20);
     if (o->norm_dose > 0.0f) r.normDose = o->norm_dose;
     if (std::isnan(o->norm_dose) || std::isinf(o->norm_dose))
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.norm_dose must be finite");
@@ -435,19 +435,24 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     // a3 on the side stream.  Default: a data-independent PREFIX of the paper's table, as large as table_cap allows,
     // forked before k_norm so that it is ready long before the search; beyond it the search enumerates (exact).
     // table_radius = 2: the paper's radius max |DD| / dD (A1 steps 1-2), forked once k_norm's maxima exist.
+    float radius = -1.0f;
+    if (r.tableMode == 1) {                                // largest radius whose candidate box has <= cap cells
+        float lo = 0.0f, hi = grid_diagonal(g);
+        int bx, by, bz;
+        if (table_box_cells(g, hi, bx, by, bz) <= r.tableCap) lo = hi;
+        else
+            for (int it = 0; it < 48; ++it) {
+                const float mid = 0.5f * (lo + hi);
+                if (table_box_cells(g, mid, bx, by, bz) <= r.tableCap) lo = mid; else hi = mid;
+            }
+        radius = lo;
+    }
+    // small prefix tables are built inside k_star, by its first blocks, while they wait for k_classify
+    const int embed = (r.tableMode == 1 && r.tableCap <= TAB_EMBED_MAX_CELLS) ? 1 : 0;
+    TablePlan plan;
+    std::memset(&plan, 0, sizeof plan);
+    if (embed) plan = table_plan_make(g, radius, r.tableCap, 1, TAB_EMBED_BUCKETS);
     auto fork_table = [&]() -> int {
-        float radius = -1.0f;
-        if (r.tableMode == 1) {                            // largest radius whose candidate box has <= cap cells
-            float lo = 0.0f, hi = grid_diagonal(g);
-            int bx, by, bz;
-            if (table_box_cells(g, hi, bx, by, bz) <= r.tableCap) lo = hi;
-            else
-                for (int it = 0; it < 48; ++it) {
-                    const float mid = 0.5f * (lo + hi);
-                    if (table_box_cells(g, mid, bx, by, bz) <= r.tableCap) lo = mid; else hi = mid;
-                }
-            radius = lo;
-        }
         CU_TRY(cudaEventRecord(g_ws.evFork, st));
         CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
         STAGE_MARK(5, g_ws.aux);
@@ -460,7 +465,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         return GAMMA_OK;
     };
     int rc = GAMMA_OK;
-    if (r.tableMode == 1) { rc = fork_table(); if (rc) return rc; }
+    if (r.tableMode == 1 && !embed) { rc = fork_table(); if (rc) return rc; }
     {                                                                    // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
@@ -476,17 +481,22 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     STAGE_MARK(1, st);
     if (r.tableMode != 1) { rc = fork_table(); if (rc) return rc; }      // paper's radius: needs k_norm's max |DD|
     {                                                                    // star phase over the compacted voxels
+        int4* tab4 = static_cast<int4*>(g_ws.table.p);
+        unsigned *tabL = static_cast<unsigned*>(g_ws.tmpL.p), *tabI = static_cast<unsigned*>(g_ws.tmpIdx.p);
         long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
         const long long resident = (long long)sm * g_ws.occStar[r.star];
         int grid = (int)(blocks > resident ? resident : blocks);
         if (r.star)
-            CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes));
+            CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes,
+                             embed, plan, tab4, tabL, tabI));
         else
-            CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes));
+            CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes,
+                             embed, plan, tab4, tabL, tabI));
         ++nk;
     }
     STAGE_MARK(2, st);
-    CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));     // before the presort, so that presort -> search stay adjacent
+    if (!embed) CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));   // before the presort: presort -> search stay adjacent
+    else { STAGE_MARK(5, st); STAGE_MARK(6, st); }
     const unsigned *lk = k0, *li = i0;
     if (presort == 1) {                                                // a2: one-pass MSD bucket presort
         CU_TRY(launch_ex(k_bucket_scatter, sm * 2, SCATTER_THREADS, 0, st, pdl, false, ctl, k0, i0, k1, i1));

@@ -21,6 +21,7 @@
 #pragma once
 #include "common.cuh"
 #include "features_generated.cuh"
+#include "offset_table.cuh"
 
 namespace gamma_b200 {
 
@@ -201,7 +202,9 @@ template <bool STAR>
 __global__ void __launch_bounds__(STAR_THREADS, GAMMA_STAR_MIN_BLOCKS)
 k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g, EvalP e,
        Ctl* __restrict__ ctl, const unsigned* __restrict__ evalIdx, unsigned* __restrict__ listKey,
-       unsigned* __restrict__ listIdx, unsigned* __restrict__ deepKey, unsigned* __restrict__ deepIdx, int classes)
+       unsigned* __restrict__ listIdx, unsigned* __restrict__ deepKey, unsigned* __restrict__ deepIdx, int classes,
+       int buildTable, const __grid_constant__ TablePlan tabPlan, int4* __restrict__ table,
+       unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx)
 {
     // classes != 0: the work list is split by depth class at append time instead of being sorted afterwards --
     // "deep" items (key beyond the first non-zero table distance: the walk will pass table entry 0) go to
@@ -212,6 +215,14 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     const unsigned FULL = 0xffffffffu;
     pdl_launch_dependents();
     sHist[tid] = 0;
+    // a3 inside the wait: the prefix table depends on the geometry only, so the first blocks build it (one slice of
+    // buckets each) while k_classify is still running -- no side stream, no join, nothing added to the chain.
+    if (buildTable) {
+        __shared__ TableSmem<TAB_EMBED_ENTRIES, TAB_EMBED_BUCKETS, TAB_EMBED_BLOCKS> sTab;
+        for (int slice = blockIdx.x; slice < TAB_EMBED_BLOCKS; slice += gridDim.x)
+            table_build_slice<STAR_THREADS, TAB_EMBED_ENTRIES, TAB_EMBED_BUCKETS, TAB_EMBED_BLOCKS>(
+                sTab, g, e, ctl, &tabPlan, 0.0f, TAB_EMBED_MAX_CELLS, table, tmpL, tmpIdx, slice);
+    }
     pdl_wait();                                           // k_classify's results from here on
     const unsigned M = ctl->nEval;
     const unsigned warpsTotal = gridDim.x * (STAR_THREADS / 32);

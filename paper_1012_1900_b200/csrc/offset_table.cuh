@@ -19,10 +19,35 @@ namespace gamma_b200 {
 
 constexpr int TAB_THREADS = 1024;
 constexpr int TAB_BUCKETS = 4096;
-constexpr int TAB_BLOCKS = 32;
+constexpr int TAB_BLOCKS = 32;                           // slices: blocks that each finish 4096 / 32 buckets
 constexpr int TAB_SLICE = TAB_BUCKETS / TAB_BLOCKS;      // buckets finished by one block
 constexpr int TAB_SMEM_ENTRIES = 8192;                   // slice entries kept in shared memory (else global scratch)
-constexpr size_t TAB_DYN_SMEM = (size_t)TAB_SMEM_ENTRIES * 2 * sizeof(unsigned);
+// the builder embedded in k_star (small prefix tables): 4 slices of a 1024-bucket counting sort, all entries in smem
+constexpr long long TAB_EMBED_MAX_CELLS = 1024;          // largest candidate box the embedded builder takes
+constexpr int TAB_EMBED_BUCKETS = 1024;
+constexpr int TAB_EMBED_BLOCKS = 4;
+constexpr int TAB_EMBED_ENTRIES = 1024;
+
+// What a table build needs to know before it touches a cell: radius, candidate box, bucket scale, and the magic
+// numbers of the exact division by box_x (0) and box_x * box_y (1) (fast_div).  Made on the host when the radius is
+// data-independent, else by thread 0 of every building block.
+struct TablePlan {
+    float R2, scale;
+    int box[3];
+    unsigned trunc;
+    unsigned divMul[2], divSh[2];
+};
+
+// Shared-memory working set of one table-building block: NB buckets, NS slices, ENT slice entries in smem.
+template <int ENT, int NB, int NS>
+struct TableSmem {
+    unsigned start[NB + 1];
+    unsigned cursor[NB / NS];
+    unsigned warpSums[32];
+    unsigned slice[2 * ENT];                             // [ENT] L^2 bits, [ENT] box index
+    TablePlan plan;
+};
+constexpr size_t TAB_DYN_SMEM = sizeof(TableSmem<TAB_SMEM_ENTRIES, TAB_BUCKETS, TAB_BLOCKS>);
 
 // Diagonal of the grid in DTA units: nothing is farther away than this.
 __host__ __device__ inline float grid_diagonal(const GridP& g)
@@ -38,6 +63,34 @@ __host__ __device__ inline long long table_box_cells(const GridP& g, float R, in
     by = g.h[1] > 0.0f ? (int)fminf((float)(g.n[1] - 1), floorf(R / g.h[1])) + 1 : 1;
     bz = g.h[2] > 0.0f ? (int)fminf((float)(g.n[2] - 1), floorf(R / g.h[2])) + 1 : 1;
     return (long long)bx * by * bz;
+}
+
+// prefix != 0: R is a data-independent radius: the table is flagged truncated unless it reaches the grid diagonal.
+__host__ __device__ inline TablePlan table_plan_make(const GridP& g, float R, long long cap, int prefix, int buckets)
+{
+    TablePlan P;
+    if (!(R >= 0.0f)) R = 0.0f;
+    R = fminf(R, 3.0e18f);
+    unsigned trunc = (prefix && R < grid_diagonal(g)) ? 1u : 0u;
+    int bx, by, bz;
+    for (;;) {
+        if (table_box_cells(g, R, bx, by, bz) <= cap) break;
+        // 0.8 per step terminates because cap >= 1 and R -> 0 gives a 1x1x1 box
+        R *= 0.8f;
+        trunc = 1;
+    }
+    P.box[0] = bx; P.box[1] = by; P.box[2] = bz;
+    const unsigned dv[2] = {(unsigned)bx, (unsigned)(bx * by)};
+    for (int k = 0; k < 2; ++k) {                        // same magic numbers as GridP::divMul (box cells < 2^31)
+        unsigned l = 0;
+        while ((1ull << l) < dv[k]) ++l;
+        P.divMul[k] = (unsigned)((1ull << (31 + l)) / dv[k] + 1ull);
+        P.divSh[k] = 31 + l;
+    }
+    P.R2 = R * R;
+    P.scale = R > 0.0f ? (float)buckets / (R * R) : 0.0f;
+    P.trunc = trunc;
+    return P;
 }
 
 // Upper bound of every key of the search list (the paper's table radius max(DD)/dD), from k_norm's maxima.
@@ -61,59 +114,53 @@ __device__ inline float table_radius_from_ctl(const GridP& g, const EvalP& e, co
     return fminf(R, grid_diagonal(g));
 }
 
-// radius_in >= 0: use it; < 0: radius from the control block (table_radius_from_ctl).
-// prefix != 0: radius_in is a data-independent radius (as far as `cap` allows): the table is a PREFIX of the
-// paper's table, flagged truncated unless it reaches the grid diagonal, and the search goes on beyond it by
-// enumeration -- so the kernel needs nothing from k_norm and runs beside it.
-__global__ void __launch_bounds__(TAB_THREADS)
-k_offset_table(GridP g, EvalP e, Ctl* __restrict__ ctl, float radius_in, long long cap, int4* __restrict__ table,
-               unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx, int prefix)
+// One block's share of the table: slice `slice` of NS.  NT threads (a multiple of 32, <= 1024, dividing NB), all of
+// which must call.  hostPlan: the plan made on the host (data-independent radius: a PREFIX of the paper's table, the
+// search goes on beyond it by enumeration, nothing is needed from k_norm), or nullptr: radius_in >= 0 or, if < 0, the
+// paper's radius from the control block (table_radius_from_ctl).
+template <int NT, int ENT, int NB, int NS>
+__device__ __forceinline__ void table_build_slice(TableSmem<ENT, NB, NS>& S, const GridP& g, const EvalP& e,
+                                                  Ctl* __restrict__ ctl, const TablePlan* hostPlan, float radius_in,
+                                                  long long cap, int4* __restrict__ table,
+                                                  unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx, int slice)
 {
-    extern __shared__ unsigned sSlice[];                 // [TAB_SMEM_ENTRIES] L^2 bits, [TAB_SMEM_ENTRIES] box index
-    __shared__ unsigned start[TAB_BUCKETS + 1];
-    __shared__ unsigned cursor[TAB_SLICE];
-    __shared__ unsigned warpSums[32];
-    __shared__ float sR2, sScale;
-    __shared__ int sBox[3];
-    __shared__ unsigned sTrunc;
+    static_assert(NB % NT == 0 && NT % 32 == 0 && NT <= 1024 && NB % NS == 0, "thread count");
+    constexpr int PER = NB / NT;
+    constexpr int TAB_BUCKETS = NB, TAB_SLICE = NB / NS;
     const unsigned tid = threadIdx.x;
 
-    if (tid == 0) {
-        float R = radius_in >= 0.0f ? radius_in : table_radius_from_ctl(g, e, ctl);
-        if (!(R >= 0.0f)) R = 0.0f;
-        R = fminf(R, 3.0e18f);
-        unsigned trunc = (prefix && R < grid_diagonal(g)) ? 1u : 0u;
-        int bx, by, bz;
-        for (;;) {
-            if (table_box_cells(g, R, bx, by, bz) <= cap) break;
-            // 0.8 per step terminates because cap >= 1 and R -> 0 gives a 1x1x1 box
-            R *= 0.8f;
-            trunc = 1;
-        }
-        sBox[0] = bx; sBox[1] = by; sBox[2] = bz;
-        sR2 = R * R;
-        sScale = R > 0.0f ? (float)TAB_BUCKETS / (R * R) : 0.0f;
-        sTrunc = trunc;
-    }
-    for (unsigned b = tid; b < TAB_BUCKETS; b += TAB_THREADS) start[b] = 0;
+    if (tid == 0)
+        S.plan = hostPlan ? *hostPlan
+                          : table_plan_make(g, radius_in >= 0.0f ? radius_in : table_radius_from_ctl(g, e, ctl), cap, 0, NB);
+    for (unsigned b = tid; b < TAB_BUCKETS; b += NT) S.start[b] = 0;
     __syncthreads();
-    const int bx = sBox[0], by = sBox[1], bz = sBox[2];
+    const TablePlan P = S.plan;
+    const int bx = P.box[0], by = P.box[1], bz = P.box[2];
     const unsigned V = (unsigned)(bx * by * bz);
-    const float R2 = sR2, scale = sScale;
+    const float R2 = P.R2, scale = P.scale;
+    const unsigned mul0 = P.divMul[0], sh0 = P.divSh[0], mul1 = P.divMul[1], sh1 = P.divSh[1];
     auto bucket_of = [&](float L2) { return min(TAB_BUCKETS - 1, (int)(L2 * scale)); };
+    auto cell_of = [&](unsigned i, int& mx, int& my, int& mz) {      // i = mx + bx * (my + by * mz), no division
+        mz = (int)fast_div(i, mul1, sh1);
+        const unsigned rem = i - (unsigned)mz * (unsigned)(bx * by);
+        my = (int)fast_div(rem, mul0, sh0);
+        mx = (int)(rem - (unsigned)my * (unsigned)bx);
+    };
 
     // (1) histogram of the whole box (every block)
-    for (unsigned i = tid; i < V; i += TAB_THREADS) {
-        const int mx = i % bx, my = (i / bx) % by, mz = i / (bx * by);
+#pragma unroll 4
+    for (unsigned i = tid; i < V; i += NT) {
+        int mx, my, mz;
+        cell_of(i, mx, my, mz);
         const float L2 = cell_L2(mx, my, mz, g);
-        if (L2 < R2) atomicAdd(&start[bucket_of(L2)], 1u);
+        if (L2 < R2) atomicAdd(&S.start[bucket_of(L2)], 1u);
     }
     __syncthreads();
-    // (2) exclusive scan of the 4096 bucket counts (4 per thread)
+    // (2) exclusive scan of the 4096 bucket counts (PER per thread)
     {
-        unsigned c[4], s = 0;
+        unsigned c[PER], s = 0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) { c[j] = start[tid * 4 + j]; s += c[j]; }
+        for (int j = 0; j < PER; ++j) { c[j] = S.start[tid * PER + j]; s += c[j]; }
         const unsigned lane = tid & 31u, warp = tid >> 5;
         unsigned incl = s;
 #pragma unroll
@@ -121,41 +168,43 @@ k_offset_table(GridP g, EvalP e, Ctl* __restrict__ ctl, float radius_in, long lo
             const unsigned t = __shfl_up_sync(0xffffffffu, incl, k);
             if (lane >= (unsigned)k) incl += t;
         }
-        if (lane == 31) warpSums[warp] = incl;
+        if (lane == 31) S.warpSums[warp] = incl;
         __syncthreads();
         if (warp == 0) {
-            unsigned w = warpSums[lane], wi = w;
+            unsigned w = lane < NT / 32 ? S.warpSums[lane] : 0u, wi = w;
 #pragma unroll
             for (int k = 1; k < 32; k <<= 1) {
                 const unsigned t = __shfl_up_sync(0xffffffffu, wi, k);
                 if (lane >= (unsigned)k) wi += t;
             }
-            warpSums[lane] = wi - w;
+            S.warpSums[lane] = wi - w;
         }
         __syncthreads();
-        unsigned run = warpSums[warp] + incl - s;
+        unsigned run = S.warpSums[warp] + incl - s;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) { start[tid * 4 + j] = run; run += c[j]; }
-        if (tid == TAB_THREADS - 1) start[TAB_BUCKETS] = run;
+        for (int j = 0; j < PER; ++j) { S.start[tid * PER + j] = run; run += c[j]; }
+        if (tid == NT - 1) S.start[TAB_BUCKETS] = run;
     }
     __syncthreads();
-    const unsigned T = start[TAB_BUCKETS];
+    const unsigned T = S.start[TAB_BUCKETS];
     // (3) this block's slice of buckets: collect its entries (order inside a bucket is arbitrary here)
-    const int b0 = blockIdx.x * TAB_SLICE;
-    const unsigned lo0 = start[b0], cnt = start[b0 + TAB_SLICE] - lo0;
-    const bool inSmem = cnt <= (unsigned)TAB_SMEM_ENTRIES;
-    unsigned* const Ls = inSmem ? sSlice : tmpL + lo0;
-    unsigned* const Is = inSmem ? sSlice + TAB_SMEM_ENTRIES : tmpIdx + lo0;
-    if (tid < TAB_SLICE) cursor[tid] = start[b0 + tid] - lo0;
+    const int b0 = slice * TAB_SLICE;
+    const unsigned lo0 = S.start[b0], cnt = S.start[b0 + TAB_SLICE] - lo0;
+    const bool inSmem = cnt <= (unsigned)ENT;
+    unsigned* const Ls = inSmem ? S.slice : tmpL + lo0;
+    unsigned* const Is = inSmem ? S.slice + ENT : tmpIdx + lo0;
+    if (tid < TAB_SLICE) S.cursor[tid] = S.start[b0 + tid] - lo0;
     __syncthreads();
     if (cnt > 0) {
-        for (unsigned i = tid; i < V; i += TAB_THREADS) {
-            const int mx = i % bx, my = (i / bx) % by, mz = i / (bx * by);
+#pragma unroll 4
+        for (unsigned i = tid; i < V; i += NT) {
+            int mx, my, mz;
+            cell_of(i, mx, my, mz);
             const float L2 = cell_L2(mx, my, mz, g);
             if (L2 < R2) {
                 const int b = bucket_of(L2) - b0;
                 if (b >= 0 && b < TAB_SLICE) {
-                    const unsigned pos = atomicAdd(&cursor[b], 1u);
+                    const unsigned pos = atomicAdd(&S.cursor[b], 1u);
                     Ls[pos] = __float_as_uint(L2);
                     Is[pos] = i;
                 }
@@ -165,24 +214,43 @@ k_offset_table(GridP g, EvalP e, Ctl* __restrict__ ctl, float radius_in, long lo
     __threadfence_block();
     __syncthreads();
     // (4) exact rank inside the bucket, write the final entry
-    for (unsigned i = tid; i < cnt; i += TAB_THREADS) {
+    for (unsigned i = tid; i < cnt; i += NT) {
         const unsigned Lb = Ls[i], id = Is[i];
         const int b = bucket_of(__uint_as_float(Lb));
-        const unsigned lo = start[b] - lo0, hi = start[b + 1] - lo0;
+        const unsigned lo = S.start[b] - lo0, hi = S.start[b + 1] - lo0;
         unsigned rank = 0;
         for (unsigned j = lo; j < hi; ++j) {
             const unsigned Lj = Ls[j];
             rank += (Lj < Lb) || (Lj == Lb && Is[j] < id);
         }
-        const int mx = id % bx, my = (id / bx) % by, mz = id / (bx * by);
+        int mx, my, mz;
+        cell_of(id, mx, my, mz);
         table[lo0 + lo + rank] = make_int4((int)Lb, mx, my, mz);
     }
-    if (blockIdx.x == 0 && tid == 0) {
+    if (slice == 0 && tid == 0) {
         ctl->tableCount = T;
-        ctl->tableTrunc = sTrunc;
+        ctl->tableTrunc = P.trunc;
         ctl->Rtab2 = R2;
         ctl->box[0] = bx; ctl->box[1] = by; ctl->box[2] = bz;
     }
+    __syncthreads();                                     // the caller may reuse the shared memory
+}
+
+// Stand-alone builder: TAB_BLOCKS blocks of TAB_THREADS threads, TAB_DYN_SMEM bytes of dynamic shared memory.
+__global__ void __launch_bounds__(TAB_THREADS)
+k_offset_table(GridP g, EvalP e, Ctl* __restrict__ ctl, float radius_in, long long cap, int4* __restrict__ table,
+               unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx, int prefix)
+{
+    using Smem = TableSmem<TAB_SMEM_ENTRIES, TAB_BUCKETS, TAB_BLOCKS>;
+    extern __shared__ __align__(16) unsigned char tabRaw[];
+    Smem& S = *reinterpret_cast<Smem*>(tabRaw);
+    __shared__ TablePlan prefixPlan;
+    if (prefix) {
+        if (threadIdx.x == 0) prefixPlan = table_plan_make(g, radius_in, cap, 1, TAB_BUCKETS);
+        __syncthreads();
+    }
+    table_build_slice<TAB_THREADS, TAB_SMEM_ENTRIES, TAB_BUCKETS, TAB_BLOCKS>(
+        S, g, e, ctl, prefix ? &prefixPlan : nullptr, radius_in, cap, table, tmpL, tmpIdx, (int)blockIdx.x);
 }
 
 }  // namespace gamma_b200
