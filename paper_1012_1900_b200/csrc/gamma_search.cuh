@@ -195,7 +195,7 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
 // ------------------------------------------------------------------------------------------------
 constexpr int STAR_THREADS = 256;
 #ifndef GAMMA_STAR_MIN_BLOCKS
-#define GAMMA_STAR_MIN_BLOCKS 3
+#define GAMMA_STAR_MIN_BLOCKS 4
 #endif
 
 template <bool STAR>
@@ -224,6 +224,10 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
                 sTab, g, e, ctl, &tabPlan, 0.0f, TAB_EMBED_MAX_CELLS, table, tmpL, tmpIdx, slice);
     }
     pdl_wait();                                           // k_classify's results from here on
+    // The index of the warp's first voxel is fetched together with the control block, not after it: one L2 round
+    // trip less in front of the first round.  Entries at or beyond M are never used (and never dereferenced).
+    unsigned item = blockIdx.x * (STAR_THREADS / 32) + (tid >> 5);
+    unsigned linAhead = item * 32u + lane < (unsigned)g.N ? evalIdx[item * 32u + lane] : 0u;
     const unsigned M = ctl->nEval;
     const unsigned warpsTotal = gridDim.x * (STAR_THREADS / 32);
     const unsigned numItems = (M + 31u) / 32u;
@@ -240,7 +244,6 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     float maxKey = 0.0f;
     __syncthreads();
 
-    unsigned item = blockIdx.x * (STAR_THREADS / 32) + (tid >> 5);
     while (item < numItems) {
         unsigned nextItem = numItems;
         if (dynamic && lane == 0) nextItem = atomicAdd(&ctl->tileCounter, 1u) + warpsTotal;
@@ -249,7 +252,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
         float key = 0.0f;
         int lin = 0;
         if (j < M) {
-            lin = (int)evalIdx[j];
+            lin = (int)linAhead;
             const float Dr = __ldg(ref + lin);
             const float invdD = e.mode == 0 ? invGlobal : criterion_inv_dD(e, dnorm, Dr);
             const float d0 = (__ldg(ev + lin) - Dr) * invdD;
@@ -331,6 +334,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
             }
         }
         item = __shfl_sync(FULL, nextItem, 0);
+        if (item < numItems && item * 32u + lane < M) linAhead = evalIdx[item * 32u + lane];
     }
     maxKey = warp_max(maxKey);
     if (lane == 0) sMax[tid >> 5] = maxKey;
