@@ -202,18 +202,30 @@ def gamma_eval_host(ref_host, eval_host, dims, spacing_mm, DD, DTA_mm, mode=GAMM
     return out_gamma_host
 
 
-def gamma_stats(gamma, nbins=64, hist_max=4.0, stream=None):
-    """``gamma_stats``: returns (hist int64 CUDA tensor [nbins], summary dict) -- reading the dict synchronises."""
+def gamma_stats_async(gamma, nbins=64, hist_max=4.0, hist=None, summary_buf=None, stream=None):
+    """``gamma_stats`` without reading anything back: enqueues a6 and returns (hist int64 CUDA tensor [nbins],
+    summary bytes CUDA tensor) -- decode the latter with ``decode_summary`` (which synchronises)."""
     lib = load_library()
     _dev_f32(gamma, "gamma")
-    hist = torch.empty(int(nbins), dtype=torch.int64, device=gamma.device)
-    summ = torch.empty(ctypes.sizeof(_CSummary), dtype=torch.uint8, device=gamma.device)
+    if hist is None:
+        hist = torch.empty(int(nbins), dtype=torch.int64, device=gamma.device)
+    if summary_buf is None:
+        summary_buf = torch.empty(ctypes.sizeof(_CSummary), dtype=torch.uint8, device=gamma.device)
     _check(lib.gamma_stats(gamma.data_ptr(), gamma.numel(), int(nbins), float(hist_max), hist.data_ptr(),
-                           summ.data_ptr(), _stream(stream)))
-    raw = bytes(summ.cpu().numpy().tobytes())
-    s = _CSummary.from_buffer_copy(raw)
-    return hist, {"n_eval": s.n_eval, "n_pass": s.n_pass, "sum_gamma": s.sum_gamma, "sum_gamma3": s.sum_gamma3,
-                  "max_gamma": s.max_gamma, "n_nan": s.n_nan}
+                           summary_buf.data_ptr(), _stream(stream)))
+    return hist, summary_buf
+
+
+def decode_summary(summary_buf) -> dict:
+    s = _CSummary.from_buffer_copy(bytes(summary_buf.cpu().numpy().tobytes()))
+    return {"n_eval": s.n_eval, "n_pass": s.n_pass, "sum_gamma": s.sum_gamma, "sum_gamma3": s.sum_gamma3,
+            "max_gamma": s.max_gamma, "n_nan": s.n_nan}
+
+
+def gamma_stats(gamma, nbins=64, hist_max=4.0, stream=None):
+    """``gamma_stats``: returns (hist int64 CUDA tensor [nbins], summary dict) -- reading the dict synchronises."""
+    hist, buf = gamma_stats_async(gamma, nbins, hist_max, stream=stream)
+    return hist, decode_summary(buf)
 
 
 def gamma_sort_pairs(keys, vals, begin_bit=0, end_bit=32, stream=None):

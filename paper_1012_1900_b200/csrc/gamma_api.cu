@@ -714,8 +714,10 @@ int gamma_stats(const float* gamma, long long n, int nbins, float hist_max, unsi
     k_stats_clear<<<(nbins + 255) / 256, 256, 0, st>>>(hist_dev, nbins, out_dev);
     if (n > 0) {
         long long blocks = (n + STATS_THREADS * 8 - 1) / (STATS_THREADS * 8);
-        int grid = (int)(blocks > g_ws.numSM * 8 ? g_ws.numSM * 8 : blocks);
-        k_stats<<<grid, STATS_THREADS, nbins * sizeof(unsigned), st>>>(gamma, n, nbins, (float)nbins / hist_max, hist_dev, out_dev);
+        int grid = (int)(blocks > g_ws.numSM * 4 ? g_ws.numSM * 4 : blocks);
+        const size_t smem = (size_t)nbins * (nbins <= STATS_WARP_BINS ? STATS_WARPS : 1) * sizeof(unsigned);
+        CU_TRY(launch_ex(k_stats, grid, STATS_THREADS, smem, st, true, false, gamma, n, nbins, (float)nbins / hist_max,
+                         hist_dev, out_dev));
         ++g_ws.launches;
     }
     ++g_ws.launches;

@@ -20,19 +20,31 @@ __global__ void k_stats_clear(unsigned long long* __restrict__ hist, int nbins, 
     }
 }
 
+// One pass over gamma: float4 loads, per-thread counters, a shared-memory histogram (one private copy per warp when
+// nbins <= STATS_WARP_BINS, so that the few populated bins are not hammered by all 256 threads), block reduction, then
+// ONE set of global atomics per block.  Launched with programmatic dependent launch behind k_stats_clear: everything
+// up to the global atomics runs while the clear drains.
+constexpr int STATS_WARP_BINS = 128;
+constexpr int STATS_WARPS = STATS_THREADS / 32;
+
 __global__ void __launch_bounds__(STATS_THREADS)
 k_stats(const float* __restrict__ gam, long long n, int nbins, float binScale,
         unsigned long long* __restrict__ hist, gamma_summary* __restrict__ out)
 {
-    extern __shared__ unsigned sHist[];
-    for (int b = threadIdx.x; b < nbins; b += blockDim.x) sHist[b] = 0;
+    extern __shared__ unsigned sHist[];                    // nbins * (private ? STATS_WARPS : 1)
+    __shared__ unsigned sCnt[STATS_WARPS][3];
+    __shared__ double sSum[STATS_WARPS][2];
+    __shared__ float sMax[STATS_WARPS];
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const bool priv = nbins <= STATS_WARP_BINS;
+    const int copies = priv ? STATS_WARPS : 1;
+    for (int b = threadIdx.x; b < nbins * copies; b += blockDim.x) sHist[b] = 0;
     __syncthreads();
+    unsigned* myHist = sHist + (priv ? (threadIdx.x >> 5) * nbins : 0);
     unsigned nEval = 0, nPass = 0, nNan = 0;
     double s1 = 0.0, s3 = 0.0;
     float mx = 0.0f;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const float v = __ldg(gam + i);
+    auto one = [&](float v) {
         if (v == v) {
             ++nEval;
             nPass += v <= 1.0f;
@@ -42,12 +54,25 @@ k_stats(const float* __restrict__ gam, long long n, int nbins, float binScale,
             mx = fmaxf(mx, v);
             const float fb = v * binScale;
             const int b = fb >= (float)(nbins - 1) ? nbins - 1 : (fb > 0.0f ? (int)fb : 0);
-            atomicAdd(&sHist[b], 1u);
+            atomicAdd(&myHist[b], 1u);
         } else {
             ++nNan;
         }
+    };
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    if ((reinterpret_cast<uintptr_t>(gam) & 15u) == 0) {
+        const float4* g4 = reinterpret_cast<const float4*>(gam);
+        const long long n4 = n >> 2;
+        for (long long i = tid; i < n4; i += stride) {
+            const float4 v = __ldg(g4 + i);
+            one(v.x); one(v.y); one(v.z); one(v.w);
+        }
+        for (long long i = (n4 << 2) + tid; i < n; i += stride) one(__ldg(gam + i));
+    } else {
+        for (long long i = tid; i < n; i += stride) one(__ldg(gam + i));
     }
-    // block reduction
+    // warp, then block reduction (fixed order inside the block)
 #pragma unroll
     for (int s = 16; s > 0; s >>= 1) {
         nEval += __shfl_xor_sync(0xffffffffu, nEval, s);
@@ -57,19 +82,38 @@ k_stats(const float* __restrict__ gam, long long n, int nbins, float binScale,
         s3 += __shfl_xor_sync(0xffffffffu, s3, s);
         mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, s));
     }
+    const int warp = threadIdx.x >> 5;
     if ((threadIdx.x & 31) == 0) {
-        if (nEval) atomicAdd(&out->n_eval, (unsigned long long)nEval);
-        if (nPass) atomicAdd(&out->n_pass, (unsigned long long)nPass);
-        if (nNan) atomicAdd(&out->n_nan, nNan);
-        if (nEval) {
-            atomicAdd(&out->sum_gamma, s1);
-            atomicAdd(&out->sum_gamma3, s3);
-            atomicMax(reinterpret_cast<unsigned*>(&out->max_gamma), __float_as_uint(mx));  // mx >= 0
-        }
+        sCnt[warp][0] = nEval; sCnt[warp][1] = nPass; sCnt[warp][2] = nNan;
+        sSum[warp][0] = s1; sSum[warp][1] = s3;
+        sMax[warp] = mx;
     }
     __syncthreads();
-    for (int b = threadIdx.x; b < nbins; b += blockDim.x)
-        if (sHist[b]) atomicAdd(&hist[b], (unsigned long long)sHist[b]);
+    asm volatile("griddepcontrol.wait;" ::: "memory");    // hist / out are cleared from here on
+    if (threadIdx.x == 0) {
+        unsigned long long cE = 0, cP = 0;
+        unsigned cN = 0;
+        double a1 = 0.0, a3 = 0.0;
+        float m = 0.0f;
+        for (int w = 0; w < STATS_WARPS; ++w) {
+            cE += sCnt[w][0]; cP += sCnt[w][1]; cN += sCnt[w][2];
+            a1 += sSum[w][0]; a3 += sSum[w][1];
+            m = fmaxf(m, sMax[w]);
+        }
+        if (cE) atomicAdd(&out->n_eval, cE);
+        if (cP) atomicAdd(&out->n_pass, cP);
+        if (cN) atomicAdd(&out->n_nan, cN);
+        if (cE) {
+            atomicAdd(&out->sum_gamma, a1);
+            atomicAdd(&out->sum_gamma3, a3);
+            atomicMax(reinterpret_cast<unsigned*>(&out->max_gamma), __float_as_uint(m));  // m >= 0
+        }
+    }
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) {
+        unsigned c = 0;
+        for (int w = 0; w < copies; ++w) c += sHist[w * nbins + b];
+        if (c) atomicAdd(&hist[b], (unsigned long long)c);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
