@@ -169,7 +169,7 @@ typedef struct gamma_counters {
     float max_key;           /* radius of the table = largest key of the search list           */
     float norm_dose;         /* D_norm used                                                    */
     int table_truncated;
-    int pad_;
+    int n_ring_search;    /* of n_table_search: voxels finished by the ring search (depth classes), no table walk */
 } gamma_counters;
 int gamma_get_counters(gamma_counters* out_host);
 

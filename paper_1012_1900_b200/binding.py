@@ -57,7 +57,7 @@ class _CCounters(ctypes.Structure):
     _fields_ = [("n_voxels", ctypes.c_longlong), ("n_evaluated", ctypes.c_longlong),
                 ("n_table_search", ctypes.c_longlong), ("table_entries", ctypes.c_longlong),
                 ("vertex_visits", ctypes.c_longlong), ("max_key", ctypes.c_float), ("norm_dose", ctypes.c_float),
-                ("table_truncated", ctypes.c_int), ("pad_", ctypes.c_int)]
+                ("table_truncated", ctypes.c_int), ("n_ring_search", ctypes.c_int)]
 
 
 @dataclass

@@ -134,6 +134,7 @@ struct Workspace {
     }
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
+    int lastClasses = 0;           // last call used depth classes: list A holds the ring items
     long long lastN = 0;
     bool haveLast = false;
     void releaseAll()
@@ -536,6 +537,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     STAGE_MARK(4, st);
 #undef STAGE_MARK
     *launched = nk;
+    g_ws.lastClasses = classes;
     return GAMMA_OK;
 }
 
@@ -829,6 +831,7 @@ int gamma_get_counters(gamma_counters* out_host)
     out_host->max_key = cv.f;
     out_host->norm_dose = ordered_to_float(c.normOrd);
     out_host->table_truncated = (int)c.tableTrunc;
+    out_host->n_ring_search = g_ws.lastClasses ? (int)c.nSearch : 0;
     return GAMMA_OK;
 }
 
