@@ -35,9 +35,11 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ_NOMINAL = 148, 128, 1965.0
 F_CELL_3D, F_CELL_2D = 1911.0, 190.0       # canonical flops per visited cell, frozen in BASELINE.md
 L2_BYTES = 126e6
 # executed FP32 flops per unit (ncu smsp__sass_thread_inst_executed_op_{fadd,fmul,ffma}; profiles/)
-FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT = 406.0, 382.0
+# r1e: k_star 65.7 Mflop / 160 256 voxels; k_table_search = 379 per owner-vertex visit + 1210 per ring item (solved from
+# the cfg2 and cfg3 launches, checked on cfg5 and cfg4_fine to 0.1 %)
+FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT, FLOP_PER_RING_ITEM = 410.0, 379.0, 1210.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on cfg3 from the same ncu --set full capture
-TRAFFIC_BYTES = {"k_star": 2.62e6, "k_table_search": 1.82e6}
+TRAFFIC_BYTES = {"k_star": 2.64e6, "k_table_search": 1.83e6}
 
 
 def f32(x):
@@ -307,8 +309,10 @@ def main():
     ndim = sum(d > 1 for d in case.dims)
     fcell = F_CELL_3D if ndim == 3 else F_CELL_2D
     kernel_ms = {"k_star": stages["star_ms"], "k_table_search": stages["search_ms"]}
-    units = {"k_star": M, "k_table_search": cnt["vertex_visits"]}
-    flop_per_unit = {"k_star": FLOP_PER_STAR_VOXEL if ndim == 3 else 0.0, "k_table_search": FLOP_PER_VISIT}
+    search_flops = cnt["vertex_visits"] * FLOP_PER_VISIT + cnt["n_ring_search"] * FLOP_PER_RING_ITEM
+    units = {"k_star": M, "k_table_search": max(1, cnt["n_table_search"])}       # voxels the launch works on
+    flop_per_unit = {"k_star": FLOP_PER_STAR_VOXEL if ndim == 3 else 0.0,
+                     "k_table_search": search_flops / max(1, cnt["n_table_search"])}
     dom = max(kernel_ms, key=kernel_ms.get)
     peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ_NOMINAL * 1e6 / 1e12
     alg = units[dom] * flop_per_unit[dom]

@@ -7,6 +7,7 @@ configs   every BASELINE.json config (cfg1, cfg2, cfg3, cfg4 coarse/fine, cfg5):
           ms per case (t_total), stage times t_p / t_gamma, M/t_gamma, N/t_total, sum gamma^3, pass rate,
           the resolution exponent of cfg4 (Fig. 2) and cfg5 with the voxel pre-sort on / off and
           with the paper's thread-per-voxel mapping (Table 2)
+batch     independent cfg3 cases per call through gamma_eval_batch against the same cases one by one
 criteria  the 9 DD x DTA combinations of Table 3 on the cfg3 phantom: time against sum gamma^3
           (Fig. 1) and the exact law gamma(k DD, k DTA) = gamma(DD, DTA) / k checked on the device maps
 
@@ -159,6 +160,43 @@ def suite_configs(args, emit):
     return rows
 
 
+def suite_batch(args, emit):
+    """independent cases per call (gamma_eval_batch) against the same cases one by one."""
+    import torch
+    from paper_1012_1900_b200 import binding, phantoms
+    case = phantoms.make_case("cfg3")
+    dev = torch.device("cuda", 0)
+    N = case.ref.size
+    for nb in (4, 16, 32):
+        refs = [torch.from_numpy(case.ref.ravel().copy()).to(dev) for _ in range(nb)]
+        evs = [torch.from_numpy(case.eval.ravel().copy()).to(dev) for _ in range(nb)]
+        outs = [torch.empty(N, dtype=torch.float32, device=dev) for _ in range(nb)]
+        dims, sps = [case.dims] * nb, [case.spacing_mm] * nb
+        a = (case.dd, case.dta_mm, case.mode, case.cutoff)
+        stream = torch.cuda.current_stream()
+        res = {}
+        for label, fn in (("batch", lambda: binding.gamma_eval_batch(refs, evs, dims, sps, *a, None, outs, stream)),
+                          ("one by one", lambda: [binding.gamma_eval_ex(refs[i], evs[i], case.dims, case.spacing_mm, *a,
+                                                                        None, outs[i], stream) for i in range(nb)])):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            reps = max(5, args.reps // 2)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            res[label] = e0.elapsed_time(e1) / reps / nb
+        cnt_m = int((~torch.isnan(outs[0])).sum().item())
+        emit({"suite": "batch", "case": "cfg3", "cases_per_call": nb, "working_set_MB": nb * 12 * N / 1e6,
+              "ms_per_case_batch": res["batch"], "ms_per_case_one_by_one": res["one by one"],
+              "evaluated_voxels_per_s_batch": cnt_m / (res["batch"] * 1e-3), "speedup": res["one by one"] / res["batch"]})
+        del refs, evs, outs
+        torch.cuda.empty_cache()
+
+
 def suite_criteria(args, emit):
     import torch
     from paper_1012_1900_b200 import phantoms
@@ -196,7 +234,7 @@ def write_md(path, rows):
                 "pass rate | max gamma | oracle s/case (cores) |\n")
         f.write("|" + "---|" * 18 + "\n")
         for r in rows:
-            if "case" not in r:
+            if "variant" not in r:
                 continue
             o = r.get("cpu_oracle")
             f.write(f"| {r['suite']} | {r['case']} | {r['variant']} | {r['criteria']} | {r['N']} | {r['M']} | "
@@ -206,13 +244,13 @@ def write_md(path, rows):
                     f"{r['max_gamma']:.3f} | "
                     + (f"{o['seconds_per_case_extrapolated']:.2f} ({o['cores']})" if o else "-") + " |\n")
         for r in rows:
-            if "case" not in r:
+            if "variant" not in r:
                 f.write("\n`" + json.dumps(r) + "`\n")
 
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--suite", default="all", choices=["configs", "criteria", "all"])
+    ap.add_argument("--suite", default="all", choices=["configs", "criteria", "batch", "all"])
     ap.add_argument("--reps", type=int, default=30)
     ap.add_argument("--oracle-seconds", type=float, default=8.0)
     ap.add_argument("--md", default=None)
@@ -231,6 +269,8 @@ def main():
         suite_configs(args, emit)
     if args.suite in ("criteria", "all"):
         suite_criteria(args, emit)
+    if args.suite in ("batch", "all"):
+        suite_batch(args, emit)
     if args.md:
         write_md(args.md, rows)
 

@@ -100,6 +100,20 @@ typedef struct gamma_opts {
     int pad_;
 } gamma_opts;
 
+/* Several independent cases in one call (every reference voxel and every case is independent,
+ * PAPER.md:141).  One case is tens of microseconds of dependent kernels that cannot fill 148 SMs; the batch spreads
+ * the cases over 4 library-owned streams, each with its own workspace, so that their kernels overlap on the device.
+ * Results are those of n_cases gamma_eval_ex calls, bit for bit.
+ *   ref, eval, out_gamma   HOST arrays of n_cases DEVICE pointers (fp32, layout as in gamma_eval); the outputs must
+ *                          not alias each other or any input
+ *   dims, spacing_mm       HOST, n_cases x 3 (case-major); the criteria and options are shared by all cases
+ *   stream                 the batch starts after the work already on `stream` and `stream` continues after the last
+ *                          case; asynchronous.  Cannot be captured into a CUDA graph (INVALID_ARGUMENT).
+ * Errors: as gamma_eval; every case is checked before anything is enqueued.  n_cases = 0 is a no-op. */
+int gamma_eval_batch(int n_cases, const float* const* ref, const float* const* eval, const int* dims,
+                     const float* spacing_mm, float DD, float DTA_mm, int mode, float low_dose_cutoff,
+                     const gamma_opts* opts, float* const* out_gamma, void* stream);
+
 /* gamma_eval with options (opts may be NULL = defaults).  Same contract as gamma_eval. */
 int gamma_eval_ex(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
                   float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts, float* out_gamma,

@@ -16,7 +16,7 @@ from . import build as _build
 
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
-    "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
+    "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
     "gamma_get_stage_times", "gamma_launch_count", "gamma_fp32_probe", "gamma_release", "gamma_version",
     "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
@@ -25,7 +25,7 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 
 # every symbol include/gamma_b200.h declares
 exported_symbols = (
-    "gamma_eval", "gamma_eval_ex", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table",
+    "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table",
     "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_fp32_probe", "gamma_release",
     "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
@@ -96,6 +96,7 @@ def load_library(build_if_needed: bool = True):
     i3, f3 = ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_float)
     lib.gamma_eval.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, vp, vp]
     lib.gamma_eval_ex.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
+    lib.gamma_eval_batch.argtypes = [ci, vp, vp, vp, vp, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
     lib.gamma_eval_host.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
     lib.gamma_stats.argtypes = [vp, cll, ci, cf, vp, vp, vp]
     lib.gamma_sort_pairs.argtypes = [vp, vp, cll, ci, ci, vp]
@@ -105,7 +106,7 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_get_stage_times.argtypes = [ctypes.POINTER(_CStageTimes)]
     lib.gamma_launch_count.argtypes = []
     lib.gamma_launch_count.restype = cll
-    for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
+    for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
                  "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_fp32_probe"):
         getattr(lib, name).restype = ci
     lib.gamma_release.restype = None
@@ -178,6 +179,34 @@ def gamma_eval_ex(ref, eval, dims, spacing_mm, DD, DTA_mm, mode=GAMMA_MODE_GLOBA
                                out_gamma.data_ptr(), _stream(stream))
     _check(rc)
     return out_gamma
+
+
+def gamma_eval_batch(refs, evals, dims_list, spacing_list, DD, DTA_mm, mode=GAMMA_MODE_GLOBAL, low_dose_cutoff=0.1,
+                     opts=None, outs=None, stream=None):
+    """``gamma_eval_batch``: independent cases (lists of CUDA float32 tensors with their dims / spacings) in one
+    call; the cases overlap on the device.  Returns the list of gamma tensors; asynchronous."""
+    lib = load_library()
+    n = len(refs)
+    if not (len(evals) == len(dims_list) == len(spacing_list) == n):
+        raise ValueError("refs, evals, dims_list and spacing_list must have the same length")
+    if outs is None:
+        outs = [torch.empty(_numel(d), dtype=torch.float32, device=r.device) for r, d in zip(refs, dims_list)]
+    for i in range(n):
+        _dev_f32(refs[i], "ref")
+        _dev_f32(evals[i], "eval")
+        _dev_f32(outs[i], "out_gamma")
+        if not (refs[i].numel() == evals[i].numel() == outs[i].numel() == _numel(dims_list[i])):
+            raise ValueError(f"case {i}: ref / eval / out_gamma must have nx*ny*nz elements")
+    ptr = ctypes.c_void_p * max(n, 1)
+    pr = ptr(*[t.data_ptr() for t in refs])
+    pe = ptr(*[t.data_ptr() for t in evals])
+    po = ptr(*[t.data_ptr() for t in outs])
+    cd = (ctypes.c_int * (3 * max(n, 1)))(*[int(x) for d in dims_list for x in d])
+    cs = (ctypes.c_float * (3 * max(n, 1)))(*[float(x) for sp in spacing_list for x in sp])
+    o = opts._c() if opts is not None else None
+    _check(lib.gamma_eval_batch(n, pr, pe, cd, cs, float(DD), float(DTA_mm), int(mode), float(low_dose_cutoff),
+                                ctypes.byref(o) if o is not None else None, po, _stream(stream)))
+    return outs
 
 
 def gamma_eval_host(ref_host, eval_host, dims, spacing_mm, DD, DTA_mm, mode=GAMMA_MODE_GLOBAL, low_dose_cutoff=0.1,

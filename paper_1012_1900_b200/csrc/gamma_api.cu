@@ -151,7 +151,19 @@ struct Workspace {
         if (evJoin) { cudaEventDestroy(evJoin); evJoin = nullptr; }
         havePending = false; haveLast = false; haveStages = false; ctlClean = false; ctlOwner = nullptr;
     }
-} g_ws;
+};
+
+// Workspace 0 serves the single-case entry points; 1 .. BATCH_LANES serve gamma_eval_batch, one per lane (own stream,
+// own control block, lists and table), so that the kernels of different cases overlap on the device.
+constexpr int BATCH_LANES = 4;
+Workspace g_pool[1 + BATCH_LANES];
+Workspace* g_cur = &g_pool[0];
+#define g_ws (*g_cur)
+struct BatchLanes {
+    cudaStream_t stream[BATCH_LANES] = {};
+    cudaEvent_t start = nullptr, done[BATCH_LANES] = {};
+    bool ready = false;
+} g_lanes;
 
 int ensure_device()
 {
@@ -667,6 +679,63 @@ int gamma_eval(const float* ref, const float* eval, const int dims[3], const flo
     return gamma_eval_ex(ref, eval, dims, spacing_mm, DD, DTA_mm, mode, low_dose_cutoff, nullptr, out_gamma, stream);
 }
 
+int gamma_eval_batch(int n_cases, const float* const* ref, const float* const* eval, const int* dims,
+                     const float* spacing_mm, float DD, float DTA_mm, int mode, float low_dose_cutoff,
+                     const gamma_opts* opts, float* const* out_gamma, void* stream)
+{
+    g_err.clear();
+    if (n_cases < 0) return fail(GAMMA_ERR_INVALID_ARGUMENT, "n_cases must be >= 0");
+    if (n_cases == 0) return GAMMA_OK;
+    if (!ref || !eval || !out_gamma || !dims || !spacing_mm)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref / eval / out_gamma / dims / spacing_mm is NULL");
+    int rc = check_criteria(DD, mode, low_dose_cutoff);
+    if (rc) return rc;
+    Resolved r;
+    rc = resolve_opts(opts, r);
+    if (rc) return rc;
+    r.profile = 0;
+    // every case is checked before anything is enqueued: nothing is launched on an argument error
+    for (int i = 0; i < n_cases; ++i) {
+        if (!ref[i] || !eval[i] || !out_gamma[i]) return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref[i] / eval[i] / out_gamma[i] is NULL");
+        GridP g;
+        rc = make_grid(dims + 3 * i, spacing_mm + 3 * i, DTA_mm, g);
+        if (rc) return rc;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::lock_guard<std::mutex> lock(g_mu);
+    cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
+    CU_TRY(cudaStreamIsCapturing(st, &capStatus));
+    if (capStatus != cudaStreamCaptureStatusNone)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_batch cannot be captured into a CUDA graph; capture gamma_eval calls");
+    if (!g_lanes.ready) {
+        CU_TRY(cudaEventCreateWithFlags(&g_lanes.start, cudaEventDisableTiming));
+        for (int l = 0; l < BATCH_LANES; ++l) {
+            CU_TRY(cudaStreamCreateWithFlags(&g_lanes.stream[l], cudaStreamNonBlocking));
+            CU_TRY(cudaEventCreateWithFlags(&g_lanes.done[l], cudaEventDisableTiming));
+        }
+        g_lanes.ready = true;
+    }
+    const int lanes = n_cases < BATCH_LANES ? n_cases : BATCH_LANES;
+    CU_TRY(cudaEventRecord(g_lanes.start, st));                       // the lanes start after what is already on `stream`
+    for (int l = 0; l < lanes; ++l) CU_TRY(cudaStreamWaitEvent(g_lanes.stream[l], g_lanes.start, 0));
+    rc = GAMMA_OK;
+    for (int i = 0; i < n_cases && rc == GAMMA_OK; ++i) {
+        const int l = i % lanes;
+        GridP g;
+        make_grid(dims + 3 * i, spacing_mm + 3 * i, DTA_mm, g);
+        g_cur = &g_pool[1 + l];
+        rc = enqueue_pipeline(ref[i], eval[i], g, DD, mode, low_dose_cutoff, r, out_gamma[i], g_lanes.stream[l]);
+        g_cur = &g_pool[0];
+    }
+    for (int l = 0; l < lanes; ++l) {                                 // `stream` continues when every lane is done
+        cudaEventRecord(g_lanes.done[l], g_lanes.stream[l]);
+        cudaStreamWaitEvent(st, g_lanes.done[l], 0);
+    }
+    if (rc) return rc;
+    CU_TRY(cudaGetLastError());
+    return GAMMA_OK;
+}
+
 int gamma_eval_host(const float* ref_host, const float* eval_host, const int dims[3], const float spacing_mm[3],
                     float DD, float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts,
                     float* out_gamma_host, void* stream)
@@ -854,7 +923,9 @@ int gamma_get_stage_times(gamma_stage_times* out_host)
 long long gamma_launch_count(void)
 {
     std::lock_guard<std::mutex> lock(g_mu);
-    return g_ws.launches;
+    long long n = 0;
+    for (const Workspace& w : g_pool) n += w.launches;
+    return n;
 }
 
 int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
@@ -890,7 +961,13 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
 void gamma_release(void)
 {
     std::lock_guard<std::mutex> lock(g_mu);
-    g_ws.releaseAll();
+    for (Workspace& w : g_pool) w.releaseAll();
+    for (int l = 0; l < BATCH_LANES; ++l) {
+        if (g_lanes.stream[l]) { cudaStreamDestroy(g_lanes.stream[l]); g_lanes.stream[l] = nullptr; }
+        if (g_lanes.done[l]) { cudaEventDestroy(g_lanes.done[l]); g_lanes.done[l] = nullptr; }
+    }
+    if (g_lanes.start) { cudaEventDestroy(g_lanes.start); g_lanes.start = nullptr; }
+    g_lanes.ready = false;
 }
 
 void gamma_abi_sizes(int out_host[4])

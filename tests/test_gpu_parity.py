@@ -315,6 +315,44 @@ def test_graph_replay_sees_new_data_and_matches_plain_launches(oracle_mod):
     assert torch.equal(torch.nan_to_num(out2, nan=-1.0), torch.nan_to_num(again, nan=-1.0))
 
 
+def test_batch_equals_single_calls_bit_for_bit():
+    """gamma_eval_batch (cases spread over the library's lanes) returns what gamma_eval_ex returns case by case,
+    for mixed geometries (2D, anisotropic 3D, ragged sizes), more cases than lanes, and in order with the stream."""
+    rng = np.random.default_rng([0, 41])
+    cases = [phantoms.make_case("cfg1"), phantoms.make_case("cfg2_small")]
+    refs, evs, dims, sps = [], [], [], []
+    for c in cases:
+        refs.append(torch.from_numpy(c.ref.ravel().copy()).cuda())
+        evs.append(torch.from_numpy(c.eval.ravel().copy()).cuda())
+        dims.append(c.dims)
+        sps.append(c.spacing_mm)
+    for d, sp in (((37, 5, 19), (2.0, 3.0, 2.5)), ((64, 33, 2), (1.5, 1.5, 4.0)), ((9, 9, 9), (3.0, 3.0, 3.0)),
+                  ((130, 1, 7), (1.0, 1.0, 2.0)), ((31, 29, 23), (2.5, 2.0, 3.0))):
+        n = d[0] * d[1] * d[2]
+        r = (1.0 + rng.random(n)).astype(np.float32)
+        e = (r * 1.03 + rng.normal(0, 0.05, n)).astype(np.float32)
+        refs.append(torch.from_numpy(r).cuda())
+        evs.append(torch.from_numpy(e).cuda())
+        dims.append(d)
+        sps.append(sp)
+    single = [binding.gamma_eval_ex(r, e, d, sp, 0.03, 3.0, 0, 0.1) for r, e, d, sp in zip(refs, evs, dims, sps)]
+    torch.cuda.synchronize()
+    # work queued on the stream before the batch must be seen by it: the inputs of case 0 are written just before
+    r0 = refs[0].clone()
+    refs[0].zero_()
+    refs[0].copy_(r0)
+    outs = binding.gamma_eval_batch(refs, evs, dims, sps, 0.03, 3.0, 0, 0.1)
+    after = [o.clone() for o in outs]                        # queued behind the batch on the same stream
+    torch.cuda.synchronize()
+    assert len(outs) == len(single) == 7
+    for a, b in zip(after, single):
+        assert torch.equal(torch.nan_to_num(a, nan=-1.0), torch.nan_to_num(b, nan=-1.0))
+    assert binding.gamma_eval_batch([], [], [], [], 0.03, 3.0) == []
+    with pytest.raises(binding.GammaError):
+        binding.gamma_eval_batch(refs[:2], evs[:2], [dims[0], (1, 1, 1)], sps[:2], 0.03, 3.0,
+                                 outs=[outs[0], torch.empty(1, device="cuda")])
+
+
 def test_stage_times_are_reported():
     c = phantoms.make_case("cfg2_small")
     gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, GammaOpts(profile_stages=1))
