@@ -175,7 +175,10 @@ def suite_batch(args, emit):
         a = (case.dd, case.dta_mm, case.mode, case.cutoff)
         stream = torch.cuda.current_stream()
         res = {}
+        gopts = binding.GammaOpts(graph=1)
         for label, fn in (("batch", lambda: binding.gamma_eval_batch(refs, evs, dims, sps, *a, None, outs, stream)),
+                          ("batch, graph replay", lambda: binding.gamma_eval_batch(refs, evs, dims, sps, *a, gopts, outs,
+                                                                                   stream)),
                           ("one by one", lambda: [binding.gamma_eval_ex(refs[i], evs[i], case.dims, case.spacing_mm, *a,
                                                                         None, outs[i], stream) for i in range(nb)])):
             for _ in range(3):
@@ -191,7 +194,8 @@ def suite_batch(args, emit):
             res[label] = e0.elapsed_time(e1) / reps / nb
         cnt_m = int((~torch.isnan(outs[0])).sum().item())
         emit({"suite": "batch", "case": "cfg3", "cases_per_call": nb, "working_set_MB": nb * 12 * N / 1e6,
-              "ms_per_case_batch": res["batch"], "ms_per_case_one_by_one": res["one by one"],
+              "ms_per_case_batch": res["batch"], "ms_per_case_batch_graph_replay": res["batch, graph replay"],
+              "ms_per_case_one_by_one": res["one by one"],
               "evaluated_voxels_per_s_batch": cnt_m / (res["batch"] * 1e-3), "speedup": res["one by one"] / res["batch"]})
         del refs, evs, outs
         torch.cuda.empty_cache()

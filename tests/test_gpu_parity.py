@@ -348,9 +348,20 @@ def test_batch_equals_single_calls_bit_for_bit():
     for a, b in zip(after, single):
         assert torch.equal(torch.nan_to_num(a, nan=-1.0), torch.nan_to_num(b, nan=-1.0))
     assert binding.gamma_eval_batch([], [], [], [], 0.03, 3.0) == []
-    with pytest.raises(binding.GammaError):
-        binding.gamma_eval_batch(refs[:2], evs[:2], [dims[0], (1, 1, 1)], sps[:2], 0.03, 3.0,
-                                 outs=[outs[0], torch.empty(1, device="cuda")])
+    one = torch.ones(1, device="cuda")
+    before = outs[0].clone()
+    with pytest.raises(binding.GammaError):                 # second case has no axis of size > 1: nothing is launched
+        binding.gamma_eval_batch([refs[0], one], [evs[0], one], [dims[0], (1, 1, 1)], [sps[0], sps[0]], 0.03, 3.0,
+                                 outs=[outs[0].zero_(), torch.empty(1, device="cuda")])
+    torch.cuda.synchronize()
+    assert float(outs[0].abs().sum()) == 0.0 and before.numel() == outs[0].numel()
+    # replayed as CUDA graphs (opts.graph = 1): same results
+    gouts = None
+    for _ in range(3):
+        gouts = binding.gamma_eval_batch(refs, evs, dims, sps, 0.03, 3.0, 0, 0.1, GammaOpts(graph=1), gouts)
+    torch.cuda.synchronize()
+    for a, b in zip(gouts, single):
+        assert torch.equal(torch.nan_to_num(a, nan=-1.0), torch.nan_to_num(b, nan=-1.0))
 
 
 def test_stage_times_are_reported():
