@@ -212,6 +212,49 @@ def test_identical_grids_flat_offset_and_ramp_closed_form():
     assert np.allclose(g[3:-3, 3:-3, 3:-3], expect, atol=5e-5)     # fp32 doses near 10 Gy: ulp 1e-6 / dD
 
 
+def test_maximum_size_grid_ramp_closed_form():
+    """Largest sizes: 1024 x 1024 x 640 = 6.7e8 voxels (2.7 GB per grid; indices and byte counts beyond 2^31 / 2^29),
+    inputs made on the device.  A linear ramp evaluated against its shifted copy has gamma = |g.s| / sqrt(dD^2 +
+    dta^2 |g|^2) at every voxel away from the border (closed form, no oracle needed at this size); a cutoff keeps the
+    evaluated set to the upper part of the ramp so that the run stays short."""
+    free, _ = torch.cuda.mem_get_info()
+    nx, ny, nz = 1024, 1024, 640
+    n = nx * ny * nz
+    if free < 9 * 4 * n + (2 << 30):
+        pytest.skip("not enough free device memory for the maximum-size case")
+    h, dta, dD = 1.0, 2.0, 0.05
+    grad, s = np.array([0.004, -0.002, 0.003]), np.array([0.6, -0.4, 0.3])
+    x = torch.arange(nx, device="cuda", dtype=torch.float64) * h
+    y = torch.arange(ny, device="cuda", dtype=torch.float64) * h
+    ref = torch.empty(n, dtype=torch.float32, device="cuda")
+    ev = torch.empty(n, dtype=torch.float32, device="cuda")
+    plane = (10.0 + grad[0] * x[None, :] + grad[1] * y[:, None])
+    for k in range(nz):                                          # slice by slice: no fp64 copy of the whole grid
+        sl = slice(k * nx * ny, (k + 1) * nx * ny)
+        ref[sl] = (plane + grad[2] * k * h).reshape(-1).to(torch.float32)
+        ev[sl] = (plane + grad[2] * k * h - float(grad @ s)).reshape(-1).to(torch.float32)
+    dnorm = float(ref.max())
+    cutoff = 0.93                                                # about a tenth of the grid is evaluated
+    out = binding.gamma_eval(ref, ev, (nx, ny, nz), (h, h, h), dD / dnorm, dta, 0, cutoff)
+    torch.cuda.synchronize()
+    cnt = binding.gamma_get_counters()
+    assert cnt["n_voxels"] == n and 0 < cnt["n_evaluated"] < n
+    keep = ref >= np.float32(cutoff) * np.float32(dnorm)
+    assert int(keep.sum()) == cnt["n_evaluated"]
+    assert bool(torch.isnan(out[~keep]).all()) and not bool(torch.isnan(out[keep]).any())
+    expect = abs(grad @ s) / np.sqrt(dD ** 2 + dta ** 2 * (grad @ grad))
+    g3 = out.view(nz, ny, nx)[4:-4, 4:-4, 4:-4]
+    inner = g3[~torch.isnan(g3)]
+    assert inner.numel() > 1e6
+    # fp32 doses near 15 Gy have an ulp of 1e-6 Gy = 2e-5 dD: the tolerance of the closed form, not of the kernel
+    assert float((inner - expect).abs().max()) <= 2e-4
+    hist, summ = binding.gamma_stats(out, 32, 2.0)
+    assert summ["n_eval"] == cnt["n_evaluated"] and summ["n_nan"] == n - cnt["n_evaluated"]
+    del ref, ev, out, keep, g3, inner
+    torch.cuda.empty_cache()
+    binding.gamma_release()                                      # give the 13 GB workspace back
+
+
 def test_all_excluded_empty_work_list_and_nonfinite_inputs():
     c = phantoms.make_case("cfg2_small")
     g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.5, GammaOpts(norm_dose=100.0))
