@@ -524,47 +524,58 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
             }
         }
     }
-    // ---- beyond a truncated table: exhaustive enumeration of the remaining octant box (exact, slow)
+    // ---- beyond a truncated (prefix) table: Chebyshev shells of octant cells, sh = max(m_x, m_y, m_z) = 0, 1, 2, ...
+    // Every cell of shell sh has some m_a = sh, so nothing in it is closer than sh * hmin: the walk stops at the first
+    // shell with (sh * hmin)^2 >= gamma^2 -- it reaches as far as the running gamma, not as far as the key, and
+    // there is no radius cap.  Cells the table already covered (L^2 < Rtab^2) are skipped.
     if (c.trunc) {
         const float Rtab2 = c.Rtab2;
-        int rx = 0, ry = 0, rz = 0;
-        unsigned V = 0;
-        if (have && best2 > Rtab2) {
-            const float b = sqrtf(best2);
-            rx = g.h[0] > 0.0f ? (int)fminf((float)(g.n[0] - 1), floorf(b / g.h[0])) + 1 : 1;
-            ry = g.h[1] > 0.0f ? (int)fminf((float)(g.n[1] - 1), floorf(b / g.h[1])) + 1 : 1;
-            rz = g.h[2] > 0.0f ? (int)fminf((float)(g.n[2] - 1), floorf(b / g.h[2])) + 1 : 1;
-            V = (unsigned)(rx * ry * rz);
-        }
-        for (unsigned i0 = 0;; i0 += EPP) {
-            const bool more = i0 < V && best2 > Rtab2;
-            if (!__any_sync(FULL, more)) break;
-            if (G >= 8) {
-                const unsigned i = i0 + (unsigned)(gl >> 3);
-                float cand = best2;
-                if (more && i < V) {
-                    const int mx = i % rx, my = (i / rx) % ry, mz = i / (rx * ry);
+        const int shMax = max(g.n[0], max(g.n[1], g.n[2])) - 1;
+        for (int sh = 0; sh <= shMax; ++sh) {
+            const bool go = have && best2 > Rtab2 && (float)sh * (float)sh * g.hmin2 < best2;
+            if (!__any_sync(FULL, go)) break;
+            // the shell as three slabs: m_x = sh | m_y = sh, m_x < sh | m_z = sh, m_x < sh, m_y < sh (clipped to the grid)
+            const int ey = min(sh, g.n[1] - 1), ez = min(sh, g.n[2] - 1);
+            const int exm = min(sh - 1, g.n[0] - 1), eym = min(sh - 1, g.n[1] - 1);
+            const unsigned cX = sh <= g.n[0] - 1 ? (unsigned)((ey + 1) * (ez + 1)) : 0u;
+            const unsigned cY = (sh >= 1 && sh <= g.n[1] - 1) ? (unsigned)((exm + 1) * (ez + 1)) : 0u;
+            const unsigned cZ = (sh >= 1 && sh <= g.n[2] - 1) ? (unsigned)((exm + 1) * (eym + 1)) : 0u;
+            const unsigned V = cX + cY + cZ;
+            auto cell_of = [&](unsigned i, int& mx, int& my, int& mz) {
+                if (i < cX) { mx = sh; my = (int)(i % (unsigned)(ey + 1)); mz = (int)(i / (unsigned)(ey + 1)); }
+                else if (i < cX + cY) { const unsigned j = i - cX; my = sh; mx = (int)(j % (unsigned)(exm + 1)); mz = (int)(j / (unsigned)(exm + 1)); }
+                else { const unsigned j = i - cX - cY; mz = sh; mx = (int)(j % (unsigned)(exm + 1)); my = (int)(j / (unsigned)(exm + 1)); }
+            };
+            for (unsigned i0 = 0; i0 < V; i0 += EPP) {
+                if (G >= 8) {
+                    const unsigned i = i0 + (unsigned)(gl >> 3);
+                    float cand = best2;
+                    if (go && i < V) {
+                        int mx, my, mz;
+                        cell_of(i, mx, my, mz);
+                        const float L2 = cell_L2(mx, my, mz, g);
+                        if (L2 >= Rtab2 && L2 < best2) {
+                            const int ox = (gl & 1) ? -mx - 1 : mx;
+                            const int oy = (gl & 2) ? -my - 1 : my;
+                            const int oz = (gl & 4) ? -mz - 1 : mz;
+                            cand = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                            ++visits;
+                        }
+                    }
+                    best2 = group_min<(G >= 8 ? G : 8)>(cand);
+                } else if (go) {
+                    int mx, my, mz;
+                    cell_of(i0, mx, my, mz);
                     const float L2 = cell_L2(mx, my, mz, g);
                     if (L2 >= Rtab2 && L2 < best2) {
-                        const int ox = (gl & 1) ? -mx - 1 : mx;
-                        const int oy = (gl & 2) ? -my - 1 : my;
-                        const int oz = (gl & 4) ? -mz - 1 : mz;
-                        cand = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
-                        ++visits;
-                    }
-                }
-                best2 = group_min<(G >= 8 ? G : 8)>(cand);
-            } else if (more) {
-                const int mx = i0 % rx, my = (i0 / rx) % ry, mz = i0 / (rx * ry);
-                const float L2 = cell_L2(mx, my, mz, g);
-                if (L2 >= Rtab2 && L2 < best2) {
 #pragma unroll 1
-                    for (int var = 0; var < 8; ++var) {
-                        const int ox = (var & 1) ? -mx - 1 : mx;
-                        const int oy = (var & 2) ? -my - 1 : my;
-                        const int oz = (var & 4) ? -mz - 1 : mz;
-                        best2 = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
-                        ++visits;
+                        for (int var = 0; var < 8; ++var) {
+                            const int ox = (var & 1) ? -mx - 1 : mx;
+                            const int oy = (var & 2) ? -my - 1 : my;
+                            const int oz = (var & 4) ? -mz - 1 : mz;
+                            best2 = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                            ++visits;
+                        }
                     }
                 }
             }

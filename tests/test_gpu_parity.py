@@ -191,6 +191,21 @@ def test_rough_random_field_deep_search(oracle_mod):
 # ----------------------------------------------------------------------------------------------------
 # closed forms on the device (the same pins the oracle has, Eq. 1)
 # ----------------------------------------------------------------------------------------------------
+def test_missing_region_heavy_tail_beyond_the_prefix_table(oracle_mod):
+    """A block of the evaluation dose is missing (zero): gamma_0 = 1/DD = 33 there, far beyond the default prefix table,
+    and the nearest matching dose is several voxels away.  The search must leave the table and continue shell by
+    shell with no radius cap; every table rule and cap gives the oracle's gamma."""
+    c = phantoms.make_case("cfg2_small")
+    ev = c.eval.copy()
+    ev[6:18, 12:30, 14:34] = 0.0
+    want = cpu_gamma(oracle_mod, c.ref, ev, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    assert np.nanmax(want) > 6.0
+    for o in (GammaOpts(), GammaOpts(table_cap=27), GammaOpts(table_radius=2), GammaOpts(table_radius=2, table_cap=200),
+              GammaOpts(lanes_per_voxel=1, presort=2, table_cap=64), GammaOpts(lanes_per_voxel=8, table_cap=5)):
+        got = gpu_gamma(c.ref, ev, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
+        assert_parity(got, want, f"missing region, {o}")
+
+
 def test_identical_grids_flat_offset_and_ramp_closed_form():
     c = phantoms.make_case("cfg2_small")
     g = gpu_gamma(c.ref, c.ref, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1)
