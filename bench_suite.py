@@ -104,8 +104,8 @@ def measure(case, opts_kw, reps, dd=None, dta=None, keep_map=False):
     return res
 
 
-def oracle_sample(case, seconds, dd=None, dta=None):
-    """The oracle as it stands on a bounded seeded sample of the evaluated voxels (all host cores)."""
+def oracle_sample(case, seconds, dd=None, dta=None, nthreads=0):
+    """The oracle as it stands on a bounded seeded sample of the evaluated voxels (all host cores, or `nthreads`)."""
     if seconds <= 0:
         return None
     import oracle
@@ -119,7 +119,8 @@ def oracle_sample(case, seconds, dd=None, dta=None):
 
     def run(vox):
         t0 = time.perf_counter()
-        oracle.gamma(case.ref, case.eval, case.dims, sp, f32(dd), f32(dta), case.mode, f32(case.cutoff), voxels=vox)
+        oracle.gamma(case.ref, case.eval, case.dims, sp, f32(dd), f32(dta), case.mode, f32(case.cutoff), voxels=vox,
+                     nthreads=nthreads)
         return time.perf_counter() - t0
 
     probe = np.sort(rng.choice(keep, size=min(keep.size, 2000), replace=False))
@@ -127,7 +128,8 @@ def oracle_sample(case, seconds, dd=None, dta=None):
     n = int(min(keep.size, max(probe.size, seconds / (tp / probe.size))))
     vox = np.sort(rng.choice(keep, size=n, replace=False))
     t = run(vox)
-    return {"voxels": n, "of": int(keep.size), "seconds": t, "voxels_per_s": n / t, "cores": oracle.num_threads(),
+    return {"voxels": n, "of": int(keep.size), "seconds": t, "voxels_per_s": n / t,
+            "cores": nthreads if nthreads else oracle.num_threads(),
             "seconds_per_case_extrapolated": t / n * keep.size}
 
 
@@ -142,6 +144,8 @@ def suite_configs(args, emit):
                          ("thread per voxel, presort on", {"lanes_per_voxel": 1, "star_phase": 2, "presort": 3}),
                          ("thread per voxel, presort off", {"lanes_per_voxel": 1, "star_phase": 2, "presort": 2})]
         orc = oracle_sample(case, args.oracle_seconds)
+        if name in ("cfg1", "cfg2") and orc is not None:     # per-core figure; the paper's CPU threading is unstated
+            orc["one_core"] = oracle_sample(case, args.oracle_seconds, nthreads=1)
         for label, kw in variants:
             reps = args.reps if "thread per voxel" not in label else max(3, args.reps // 6)
             r = measure(case, kw, reps)
