@@ -77,7 +77,17 @@ k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int m
         const float4* r4 = reinterpret_cast<const float4*>(ref);
         const float4* e4 = reinterpret_cast<const float4*>(ev);
         const int n4 = N >> 2;
-        for (int i = tid; i < n4; i += nth) {
+        int i = tid;
+        for (; i + 3 * nth < n4; i += 4 * nth) {             // large grids: 8 independent 16-byte loads in flight per thread
+            const float4 x0 = __ldg(r4 + i), y0 = __ldg(e4 + i), x1 = __ldg(r4 + i + nth), y1 = __ldg(e4 + i + nth);
+            const float4 x2 = __ldg(r4 + i + 2 * nth), y2 = __ldg(e4 + i + 2 * nth);
+            const float4 x3 = __ldg(r4 + i + 3 * nth), y3 = __ldg(e4 + i + 3 * nth);
+            one(x0.x, y0.x); one(x0.y, y0.y); one(x0.z, y0.z); one(x0.w, y0.w);
+            one(x1.x, y1.x); one(x1.y, y1.y); one(x1.z, y1.z); one(x1.w, y1.w);
+            one(x2.x, y2.x); one(x2.y, y2.y); one(x2.z, y2.z); one(x2.w, y2.w);
+            one(x3.x, y3.x); one(x3.y, y3.y); one(x3.z, y3.z); one(x3.w, y3.w);
+        }
+        for (; i < n4; i += nth) {
             const float4 x = __ldg(r4 + i), y = __ldg(e4 + i);
             one(x.x, y.x); one(x.y, y.y); one(x.z, y.z); one(x.w, y.w);
         }
