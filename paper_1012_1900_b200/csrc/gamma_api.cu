@@ -97,8 +97,9 @@ struct GraphEntry {
     int kernels = 0;
 };
 constexpr int GRAPH_CACHE = 64;
-// control-block slots: 0/1 alternate between calls, 2 stand-alone entry points, 3 calls captured by the caller
-constexpr int CTL_SLOTS = 4;
+// control-block slots: 0/1/2 rotate between calls (the first kernel of call i clears the slot of call i+1 and may run
+// while call i-1 is still finishing), 3 stand-alone entry points, 4 calls captured by the caller
+constexpr int CTL_ROT = 3, CTL_STANDALONE = 3, CTL_CAPTURE = 4, CTL_SLOTS = 5;
 
 struct Workspace {
     Buf ctl;                       // Ctl
@@ -134,6 +135,10 @@ struct Workspace {
     }
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
+    cudaStream_t doneStream = nullptr;   // stream of the last work that used this workspace
+    bool chainable = false;              // that work was a pipeline ending in k_table_search (which triggers dependents)
+    const char* lastOutBegin = nullptr;  // its out_gamma range: a next call that reads it must not start early
+    const char* lastOutEnd = nullptr;
     int lastClasses = 0;           // last call used depth classes: list A holds the ring items
     long long lastN = 0;
     bool haveLast = false;
@@ -187,14 +192,20 @@ int host_key_digit(float key)
 
 int order_after_previous(cudaStream_t st)
 {
+    // Same stream as the last user of the workspace: stream order is enough (and no event sits between the last
+    // kernel of that call and the first kernel of this one).  Another stream: wait for the tail of that stream.
     if (!g_ws.done) CU_TRY(cudaEventCreateWithFlags(&g_ws.done, cudaEventDisableTiming));
-    if (g_ws.havePending) CU_TRY(cudaStreamWaitEvent(st, g_ws.done, 0));
+    if (g_ws.havePending && g_ws.doneStream != st) {
+        CU_TRY(cudaEventRecord(g_ws.done, g_ws.doneStream));
+        CU_TRY(cudaStreamWaitEvent(st, g_ws.done, 0));
+    }
     return GAMMA_OK;
 }
 int mark_done(cudaStream_t st)
 {
-    CU_TRY(cudaEventRecord(g_ws.done, st));
+    g_ws.doneStream = st;
     g_ws.havePending = true;
+    g_ws.chainable = false;
     return GAMMA_OK;
 }
 
@@ -391,7 +402,9 @@ int prepare_workspace(const GridP& g, const Resolved& r)
     CU_TRY(g_ws.key0.need(N * 4)); CU_TRY(g_ws.idx0.need(N * 4)); CU_TRY(g_ws.evalIdx.need(N * 4));
     if (r.presort) { CU_TRY(g_ws.key1.need(N * 4)); CU_TRY(g_ws.idx1.need(N * 4)); }
     if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
-    CU_TRY(g_ws.table.need((size_t)r.tableCap * 16));
+    // the small embedded table exists once per rotating control-block slot: the next call may build its own while this
+    // call's search still walks this one
+    CU_TRY(g_ws.table.need((size_t)(r.tableCap > CTL_SLOTS * TAB_EMBED_MAX_CELLS ? r.tableCap : CTL_SLOTS * TAB_EMBED_MAX_CELLS) * 16));
     CU_TRY(g_ws.tmpL.need((size_t)r.tableCap * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)r.tableCap * 4));
     if (!g_ws.aux) {
         CU_TRY(cudaStreamCreateWithFlags(&g_ws.aux, cudaStreamNonBlocking));
@@ -430,7 +443,8 @@ int prepare_workspace(const GridP& g, const Resolved& r)
 // star kernel runs.  No memset and no host synchronisation on the path: k_norm clears the control
 // block of the next call (two alternating slots; slot 2 belongs to the stand-alone entry points).
 int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
-                    const Resolved& r, float* out, cudaStream_t st, Ctl* ctl, Ctl* next, int* launched)
+                    const Resolved& r, float* out, cudaStream_t st, Ctl* ctl, Ctl* next, int* launched, bool early,
+                    int slot)
 {
     const long long N = g.N;
     int nk = 0;
@@ -482,7 +496,9 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     {                                                                    // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
-        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, ctl, next));
+        // early: the previous call on this stream ended in k_table_search, which triggers its dependents at once:
+        // k_norm then runs in the tail of that call (it touches nothing of it) and waits for its end before exiting
+        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, early, false, ref, ev, (int)N, mode, ctl, next));
         ++nk;
     }
     {                                                                    // a1: exclusion + compaction
@@ -494,7 +510,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     STAGE_MARK(1, st);
     if (r.tableMode != 1) { rc = fork_table(); if (rc) return rc; }      // paper's radius: needs k_norm's max |DD|
     {                                                                    // star phase over the compacted voxels
-        int4* tab4 = static_cast<int4*>(g_ws.table.p);
+        int4* tab4 = static_cast<int4*>(g_ws.table.p) + (embed ? (size_t)slot * (size_t)TAB_EMBED_MAX_CELLS : 0);
         unsigned *tabL = static_cast<unsigned*>(g_ws.tmpL.p), *tabI = static_cast<unsigned*>(g_ws.tmpIdx.p);
         long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
         const long long resident = (long long)sm * g_ws.occStar[r.star];
@@ -524,7 +540,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     STAGE_MARK(3, st);
     {                                                                    // a4 + a5
         const int grid = sm * (r.lanes == 0 ? 3 : 4);                    // resident blocks at 80 / 64 registers
-        const int4* tab = static_cast<const int4*>(g_ws.table.p);
+        const int4* tab = static_cast<const int4*>(g_ws.table.p) + (embed ? (size_t)slot * (size_t)TAB_EMBED_MAX_CELLS : 0);
         // adaptive lanes: an item is "deep" when its key exceeds the smallest non-zero table distance
         float hmin = 0.0f;
         for (int a = 0; a < 3; ++a)
@@ -571,18 +587,31 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         // The caller is capturing `st`: the kernels become nodes of the caller's graph.  The call must then be
         // self-contained (its replays do not pass through this function): it owns control-block slot 3 and
         // clears it with a memset node; ordering against other work is the captured stream's.
-        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + 3;
+        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_CAPTURE;
         CU_TRY(cudaMemsetAsync(ctl, 0, sizeof(Ctl), st));
         int launched = 0;
         Resolved rr = r;
         rr.profile = 0;
-        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, rr, out, st, ctl, nullptr, &launched);
+        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, rr, out, st, ctl, nullptr, &launched, false, CTL_CAPTURE);
         if (rc) return rc;
         g_ws.launches += launched;
         g_ws.haveStages = false;
+        g_ws.chainable = false;
         g_ws.lastCtl = ctl; g_ws.lastStream = nullptr; g_ws.lastN = g.N; g_ws.haveLast = true;
         return GAMMA_OK;
     }
+    // May the first kernel start while the previous call on this stream is finishing?  Only behind one of our own
+    // pipelines on the same stream, with a clean control block, the small embedded table (one per slot), no profiling,
+    // and inputs that do not overlap what that call is still writing.
+    const size_t bytes = (size_t)g.N * 4;
+    auto overlaps = [&](const void* p) {
+        const char* a = static_cast<const char*>(p);
+        return g_ws.lastOutBegin && a < g_ws.lastOutEnd && a + bytes > g_ws.lastOutBegin;
+    };
+    static const bool overlapCalls = !(std::getenv("GAMMA_OVERLAP_CALLS") && std::getenv("GAMMA_OVERLAP_CALLS")[0] == '0');
+    const bool early = overlapCalls && g_ws.pdl != 0 && g_ws.chainable && g_ws.havePending && g_ws.doneStream == st &&
+                       g_ws.ctlClean && g_ws.ctl.p == g_ws.ctlOwner && !r.profile && r.tableMode == 1 &&
+                       r.tableCap <= TAB_EMBED_MAX_CELLS && !overlaps(ref) && !overlaps(ev);
     rc = order_after_previous(st);
     if (rc) return rc;
     if (g_ws.ctl.p != g_ws.ctlOwner) { g_ws.ctlClean = false; g_ws.ctlOwner = g_ws.ctl.p; }
@@ -593,13 +622,13 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     g_ws.ctlClean = false;                                 // set again when everything below was enqueued
     Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
     Ctl* ctl = base + g_ws.slot;
-    Ctl* next = base + (g_ws.slot ^ 1);
+    Ctl* next = base + (g_ws.slot + 1) % CTL_ROT;
     g_ws.haveStages = false;
 
     const bool useGraph = g_ws.graphs != 0 && r.graph && !r.profile;
     int launched = 0;
     if (!useGraph) {
-        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, ctl, next, &launched);
+        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, ctl, next, &launched, early, g_ws.slot);
         if (rc) return rc;
     } else {
         if (g_ws.graphGen != g_allocGen) { g_ws.dropGraphs(); g_ws.graphGen = g_allocGen; }
@@ -615,7 +644,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         if (!hit) {
             cudaGraph_t graph = nullptr;
             CU_TRY(cudaStreamBeginCapture(g_ws.cap, cudaStreamCaptureModeThreadLocal));
-            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, g_ws.cap, ctl, next, &launched);
+            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, g_ws.cap, ctl, next, &launched, false, g_ws.slot);
             cudaError_t ce = cudaStreamEndCapture(g_ws.cap, &graph);
             if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
             if (ce != cudaSuccess) return fail(GAMMA_ERR_CUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(ce));
@@ -644,8 +673,11 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     CU_TRY(cudaGetLastError());
     rc = mark_done(st);
     if (rc) return rc;
+    g_ws.chainable = true;
+    g_ws.lastOutBegin = reinterpret_cast<const char*>(out);
+    g_ws.lastOutEnd = g_ws.lastOutBegin + bytes;
     g_ws.lastCtl = ctl;
-    g_ws.slot ^= 1;
+    g_ws.slot = (g_ws.slot + 1) % CTL_ROT;
     g_ws.ctlClean = true;
     g_ws.lastStream = st; g_ws.lastN = g.N; g_ws.haveLast = true;
     return GAMMA_OK;
@@ -816,7 +848,7 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
     CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
     rc = order_after_previous(st);
     if (rc) return rc;
-    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + 2;
+    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_STANDALONE;
     k_set_u32<<<1, 1, 0, st>>>(&ctl->sortN, (unsigned)n);
     unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *v1 = static_cast<unsigned*>(g_ws.idx1.p);
     int where = radix_sort_enqueue(keys, vals, k1, v1, &ctl->sortN, n, begin_bit, end_bit,
@@ -866,7 +898,7 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     CU_TRY(cudaFuncSetAttribute(k_offset_table, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TAB_DYN_SMEM));
     rc = order_after_previous(st);
     if (rc) return rc;
-    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + 2;
+    Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_STANDALONE;
     EvalP e;
     e.DD = 1.0f; e.cutoff = 0.0f; e.norm_dose = 1.0f; e.mode = 0;
     k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, st>>>(
@@ -943,7 +975,7 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
     double best = 0.0;
     for (int r = 0; r < repeats + 1; ++r) {
         CU_TRY(cudaEventRecord(a, st));
-        k_fp32_probe<<<grid, threads, 0, st>>>(reinterpret_cast<float*>(static_cast<Ctl*>(g_ws.ctl.p) + 2) + 15, 0.999f, 1e-3f);
+        k_fp32_probe<<<grid, threads, 0, st>>>(reinterpret_cast<float*>(static_cast<Ctl*>(g_ws.ctl.p) + CTL_STANDALONE) + 15, 0.999f, 1e-3f);
         ++g_ws.launches;
         CU_TRY(cudaEventRecord(b, st));
         CU_TRY(cudaEventSynchronize(b));

@@ -103,6 +103,9 @@ k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int m
         atomicMax(&cur->normOrd, float_to_ordered(m));
         if (a > 0.0f) atomicMax(&cur->maxAbsDD, __float_as_uint(a));
         if (r > 0.0f) atomicMax(&cur->maxRatio, __float_as_uint(r));
+        // Launched behind the previous call's k_table_search with programmatic dependent launch, this kernel has run
+        // in that call's tail; it must not END before that call has (the kernels after it reuse its work lists).
+        pdl_wait();
     }
 }
 
@@ -641,6 +644,7 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     const int lane = threadIdx.x & 31;
     SearchCtx c;
     pdl_wait();
+    pdl_launch_dependents();                             // the next call's k_norm may use the SMs this kernel leaves
     const unsigned nS = ctl->nSearch;
     unsigned nDeep = 0;
     if (MODE == 0 && classes) {

@@ -422,6 +422,52 @@ def test_batch_equals_single_calls_bit_for_bit():
         assert torch.equal(torch.nan_to_num(a, nan=-1.0), torch.nan_to_num(b, nan=-1.0))
 
 
+def test_back_to_back_calls_overlap_safely():
+    """Consecutive calls on one stream are pipelined (the first kernel of a call runs in the tail of the previous
+    call).  Results must be those of isolated calls: alternating geometries (the offset table differs from call to
+    call), a shared output buffer, and a call whose INPUT is the previous call's output."""
+    a, b = phantoms.make_case("cfg2_small"), phantoms.make_case("cfg4_coarse")
+    data = []
+    for c in (a, b):
+        r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+        e = torch.from_numpy(c.eval.ravel().copy()).cuda()
+        args = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+        want = binding.gamma_eval_ex(r, e, *args).clone()
+        torch.cuda.synchronize()
+        data.append((r, e, args, want))
+    outs = []
+    for i in range(40):                                          # no synchronisation in between
+        r, e, args, _ = data[i % 2]
+        outs.append(binding.gamma_eval_ex(r, e, *args))
+    torch.cuda.synchronize()
+    for i, o in enumerate(outs):
+        assert torch.equal(torch.nan_to_num(o, nan=-1.0), torch.nan_to_num(data[i % 2][3], nan=-1.0)), i
+    # one output buffer for every call of the same case
+    r, e, args, want = data[0]
+    shared = torch.empty_like(want)
+    snaps = []
+    for i in range(10):
+        binding.gamma_eval_ex(r, e, *args, None, shared)
+        snaps.append(shared.clone())
+    torch.cuda.synchronize()
+    for sn in snaps:
+        assert torch.equal(torch.nan_to_num(sn, nan=-1.0), torch.nan_to_num(want, nan=-1.0))
+    # the output of one call is the evaluation dose of the next (no cutoff, so it holds no NaN)
+    n = a.ref.size
+    args0 = (a.dims, a.spacing_mm, 0.03, 3.0, 0, 0.0)
+    rr = (r + 0.05).contiguous()
+    first = binding.gamma_eval_ex(rr, e, *args0).clone()
+    torch.cuda.synchronize()
+    want2 = binding.gamma_eval_ex(rr, first, *args0).clone()
+    torch.cuda.synchronize()
+    for _ in range(5):
+        tmp = torch.empty(n, dtype=torch.float32, device="cuda")
+        binding.gamma_eval_ex(rr, e, *args0, None, tmp)
+        got2 = binding.gamma_eval_ex(rr, tmp, *args0)
+        torch.cuda.synchronize()
+        assert torch.equal(got2, want2)
+
+
 def test_stage_times_are_reported():
     c = phantoms.make_case("cfg2_small")
     gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, GammaOpts(profile_stages=1))
