@@ -293,6 +293,15 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
         active += dims[a] > 1;
     }
     if (active == 0) return fail(GAMMA_ERR_INVALID_ARGUMENT, "at least one axis must have size > 1");
+    // the derived geometry of the last call is kept: a repeated geometry costs a compare, not 48 triangle distances
+    struct GeoKey { int d[3]; float s[3]; float dta; };
+    static thread_local GeoKey lastKey = {{0, 0, 0}, {0, 0, 0}, 0};
+    static thread_local GridP lastGrid;
+    GeoKey key;
+    std::memset(&key, 0, sizeof key);
+    for (int a = 0; a < 3; ++a) { key.d[a] = dims[a]; key.s[a] = spacing_mm[a]; }
+    key.dta = DTA_mm;
+    if (std::memcmp(&key, &lastKey, sizeof key) == 0) { g = lastGrid; return GAMMA_OK; }
     std::memset(&g, 0, sizeof g);
     double h[3], hh[3];
     for (int a = 0; a < 3; ++a) {
@@ -334,6 +343,8 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
         const double rho = star_link_distance(h) * (1.0 - 1e-5);
         g.rho_link2 = (float)(rho * rho);
     }
+    lastGrid = g;
+    lastKey = key;
     return GAMMA_OK;
 }
 
@@ -462,8 +473,13 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     // a3 on the side stream.  Default: a data-independent PREFIX of the paper's table, as large as table_cap allows,
     // forked before k_norm so that it is ready long before the search; beyond it the search enumerates (exact).
     // table_radius = 2: the paper's radius max |DD| / dD (A1 steps 1-2), forked once k_norm's maxima exist.
+    // host-side constants of the geometry (table radius / plan, ring constants): kept from the last call
+    struct HostGeo { GridP g; long long cap; float radius; TablePlan plan; GammaRingP ring; bool valid; };
+    static thread_local HostGeo geo = {};
+    const bool geoHit = geo.valid && geo.cap == r.tableCap && std::memcmp(&geo.g, &g, sizeof g) == 0;
     float radius = -1.0f;
-    if (r.tableMode == 1) {                                // largest radius whose candidate box has <= cap cells
+    if (r.tableMode == 1 && geoHit) radius = geo.radius;
+    else if (r.tableMode == 1) {                           // largest radius whose candidate box has <= cap cells
         float lo = 0.0f, hi = grid_diagonal(g);
         int bx, by, bz;
         if (table_box_cells(g, hi, bx, by, bz) <= r.tableCap) lo = hi;
@@ -478,7 +494,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     const int embed = (r.tableMode == 1 && r.tableCap <= TAB_EMBED_MAX_CELLS) ? 1 : 0;
     TablePlan plan;
     std::memset(&plan, 0, sizeof plan);
-    if (embed) plan = table_plan_make(g, radius, r.tableCap, 1, TAB_EMBED_BUCKETS);
+    if (embed) plan = geoHit ? geo.plan : table_plan_make(g, radius, r.tableCap, 1, TAB_EMBED_BUCKETS);
     auto fork_table = [&]() -> int {
         CU_TRY(cudaEventRecord(g_ws.evFork, st));
         CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
@@ -548,9 +564,14 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         const int deepDigit = (presort == 1 || presort == 3) ? host_key_digit(hmin) + 1 : KEY_DIGITS;
         GammaRingP ring;
         std::memset(&ring, 0, sizeof ring);
-        if (classes) {
+        if (classes && geoHit) {
+            ring = geo.ring;
+        } else if (classes) {
             const double hh[3] = {(double)g.h[0] * g.h[0], (double)g.h[1] * g.h[1], (double)g.h[2] * g.h[2]};
             gamma_ring_constants(hh, ring);
+        }
+        if (!geoHit && r.tableMode == 1 && g.all_active && classes) {
+            geo.g = g; geo.cap = r.tableCap; geo.radius = radius; geo.plan = plan; geo.ring = ring; geo.valid = true;
         }
         if (r.lanes == 1)
             CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
