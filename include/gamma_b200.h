@@ -57,6 +57,12 @@ extern "C" {
  *                    (reading 10; the comparison is done in double so that it is decided identically
  *                    everywhere).  Excluded voxels still serve as evaluation points of their neighbours.
  *   out_gamma        DEVICE, N fp32, written entirely
+ *   (pipelining)     consecutive calls on ONE stream overlap: the first kernel of a call (it reads ref / eval only)
+ *                    may run while the previous call on that stream is finishing.  Stream order as seen by the caller
+ *                    is kept (a call whose inputs overlap the previous call's out_gamma is not started early).  The
+ *                    one thing the library cannot see: a kernel of the caller's that writes ref / eval, sits directly
+ *                    in front of the call AND itself releases its dependents early (griddepcontrol.launch_dependents)
+ *                    must not be used; environment GAMMA_OVERLAP_CALLS=0 switches the overlap off.
  *   stream           cudaStream_t.  The offset table is built on a library-owned side stream that forks from and
  *                    joins `stream` through events (legal under stream capture).
  */
