@@ -141,8 +141,19 @@ def _dev_f32(t: torch.Tensor, name: str) -> torch.Tensor:
     return t
 
 
+_geom_cache = {}
+
+
 def _geom(dims, spacing_mm):
-    return (ctypes.c_int * 3)(*[int(d) for d in dims]), (ctypes.c_float * 3)(*[float(s) for s in spacing_mm])
+    """(int[3], float[3]) ctypes arrays; the last few geometries are kept (argument marshalling only)."""
+    key = (tuple(dims), tuple(spacing_mm))
+    hit = _geom_cache.get(key)
+    if hit is None:
+        if len(_geom_cache) > 64:
+            _geom_cache.clear()
+        hit = ((ctypes.c_int * 3)(*[int(d) for d in dims]), (ctypes.c_float * 3)(*[float(s) for s in spacing_mm]))
+        _geom_cache[key] = hit
+    return hit
 
 
 def _numel(dims) -> int:
