@@ -206,9 +206,14 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
 // first part of a4: the star phase over the compacted voxels, one voxel per thread, one warp per 32
 // consecutive list entries (first round static, later rounds fetched dynamically).
 // ------------------------------------------------------------------------------------------------
-constexpr int STAR_THREADS = 256;
+// 128 threads x 9 resident blocks = 36 warps per SM at 56 registers: 148 x 36 x 32 = 170 496 voxels are in flight at
+// once, so cases up to that many evaluated voxels (cfg2, cfg3: 160 256) finish in ONE round of items.
+#ifndef GAMMA_STAR_THREADS
+#define GAMMA_STAR_THREADS 128
+#endif
+constexpr int STAR_THREADS = GAMMA_STAR_THREADS;
 #ifndef GAMMA_STAR_MIN_BLOCKS
-#define GAMMA_STAR_MIN_BLOCKS 4
+#define GAMMA_STAR_MIN_BLOCKS 9
 #endif
 
 template <bool STAR>
@@ -227,7 +232,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     const int tid = threadIdx.x, lane = tid & 31;
     const unsigned FULL = 0xffffffffu;
     pdl_launch_dependents();
-    sHist[tid] = 0;
+    for (int d = tid; d < KEY_DIGITS; d += STAR_THREADS) sHist[d] = 0;
     // a3 inside the wait: the prefix table depends on the geometry only, so the first blocks build it (one slice of
     // buckets each) while k_classify is still running -- no side stream, no join, nothing added to the chain.
     if (buildTable) {
@@ -352,7 +357,9 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     maxKey = warp_max(maxKey);
     if (lane == 0) sMax[tid >> 5] = maxKey;
     __syncthreads();
-    if (!classes && sHist[tid]) atomicAdd(&ctl->hist[tid], sHist[tid]);
+    if (!classes)
+        for (int d = tid; d < KEY_DIGITS; d += STAR_THREADS)
+            if (sHist[d]) atomicAdd(&ctl->hist[d], sHist[d]);
     if (tid == 0) {
         float m = 0.0f;
 #pragma unroll

@@ -193,7 +193,7 @@ __device__ __forceinline__ void table_build_slice(TableSmem<ENT, NB, NS>& S, con
     const bool inSmem = cnt <= (unsigned)ENT;
     unsigned* const Ls = inSmem ? S.slice : tmpL + lo0;
     unsigned* const Is = inSmem ? S.slice + ENT : tmpIdx + lo0;
-    if (tid < TAB_SLICE) S.cursor[tid] = S.start[b0 + tid] - lo0;
+    for (unsigned b = tid; b < (unsigned)TAB_SLICE; b += NT) S.cursor[b] = S.start[b0 + b] - lo0;
     __syncthreads();
     if (cnt > 0) {
 #pragma unroll 4
