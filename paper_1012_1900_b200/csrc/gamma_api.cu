@@ -555,7 +555,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     }
     STAGE_MARK(3, st);
     {                                                                    // a4 + a5
-        const int grid = sm * (r.lanes == 0 ? 3 : 4);                    // resident blocks at 80 / 64 registers
+        const int grid = sm * (r.lanes == 0 ? SEARCH_MIN_BLOCKS : 4 * (256 / SEARCH_THREADS));   // resident blocks
         const int4* tab = static_cast<const int4*>(g_ws.table.p) + (embed ? (size_t)slot * (size_t)TAB_EMBED_MAX_CELLS : 0);
         // adaptive lanes: an item is "deep" when its key exceeds the smallest non-zero table distance
         float hmin = 0.0f;

@@ -472,7 +472,14 @@ __device__ __forceinline__ float group_min(float v)
     return v;
 }
 
-constexpr int SEARCH_THREADS = 256;
+#ifndef GAMMA_SEARCH_THREADS
+#define GAMMA_SEARCH_THREADS 128
+#endif
+#ifndef GAMMA_SEARCH_MIN_BLOCKS
+#define GAMMA_SEARCH_MIN_BLOCKS 6
+#endif
+constexpr int SEARCH_THREADS = GAMMA_SEARCH_THREADS;
+constexpr int SEARCH_MIN_BLOCKS = GAMMA_SEARCH_MIN_BLOCKS;   // adaptive-lane kernel (MODE 0)
 
 struct SearchCtx {
     const float* ref; const float* ev; float* out;
@@ -640,7 +647,7 @@ __device__ __forceinline__ void ring_items(const SearchCtx& c, const GridP& g, c
 // items only, searched one per thread (ring_items).  Work units are handed out
 // deepest first: first round static, later rounds by an atomic counter whose latency hides behind the search.
 template <int MODE>
-__global__ void __launch_bounds__(SEARCH_THREADS, MODE == 0 ? 3 : 1)
+__global__ void __launch_bounds__(SEARCH_THREADS, MODE == 0 ? SEARCH_MIN_BLOCKS : 1)
 k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
                EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
                const unsigned* __restrict__ listIdx, const unsigned* __restrict__ deepKey,
