@@ -63,8 +63,9 @@ extern "C" {
  *                    one thing the library cannot see: a kernel of the caller's that writes ref / eval, sits directly
  *                    in front of the call AND itself releases its dependents early (griddepcontrol.launch_dependents)
  *                    must not be used; environment GAMMA_OVERLAP_CALLS=0 switches the overlap off.
- *   stream           cudaStream_t.  The offset table is built on a library-owned side stream that forks from and
- *                    joins `stream` through events (legal under stream capture).
+ *   stream           cudaStream_t.  With the default options everything runs on `stream` (4 kernels).  Only with
+ *                    opts.table_radius = 2 or a table_cap above 1024 the offset table is built on a library-owned
+ *                    side stream that forks from and joins `stream` through events (legal under stream capture).
  */
 int gamma_eval(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
                float DTA_mm, int mode, float low_dose_cutoff, float* out_gamma, void* stream);
@@ -198,9 +199,10 @@ int gamma_get_counters(gamma_counters* out_host);
 typedef struct gamma_stage_times {
     float prep_ms;   /* a0 + A1 step 1 + a1: max(ref), max|DD|, cutoff + compaction (k_norm, k_classify) */
     float star_ms;   /* a1 + first part of a4: keys and the star phase (k_star)                  */
-    float table_ms;  /* a3: offset table, on the side stream, CONCURRENT with star_ms            */
+    float table_ms;  /* a3: offset table when it is built on the side stream (CONCURRENT with the main
+                        stream); ~0 by default, where the table is built inside k_star (star_ms)   */
     float sort_ms;   /* a2: presort of the search work list                                      */
-    float search_ms; /* a4 + a5: join with the side stream, table search and write-back          */
+    float search_ms; /* a4 + a5: table search (ring + deep classes) and write-back               */
     float total_ms;  /* first event to last event on `stream` = prep + star + sort + search      */
 } gamma_stage_times;
 int gamma_get_stage_times(gamma_stage_times* out_host);
