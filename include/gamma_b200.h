@@ -104,7 +104,10 @@ typedef struct gamma_opts {
                              as far as table_cap allows, built beside a0 (nothing on the critical path);
                              2: the paper's radius max |DD| / dD (A1 steps 1-2), built once
                              a0's maxima exist                                                              */
-    int pad_;
+    int interpolation;    /* 0: default (= 1); 1: the evaluation dose is the piecewise-linear surface on the Kuhn
+                             simplices (the paper's method); 2: grid vertices only -- the classical discrete
+                             gamma search (Low 1998), kept as an internal comparator: gamma_1 <= gamma_2 always
+                             (same table walk and early exit; the star phase is off)                      */
 } gamma_opts;
 
 /* Several independent cases in one call (every reference voxel and every case is independent,

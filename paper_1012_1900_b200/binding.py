@@ -39,7 +39,7 @@ class _COpts(ctypes.Structure):
     _fields_ = [("norm_dose", ctypes.c_float), ("presort", ctypes.c_int), ("star_phase", ctypes.c_int),
                 ("lanes_per_voxel", ctypes.c_int), ("sort_key_bits", ctypes.c_int), ("table_cap", ctypes.c_longlong),
                 ("profile_stages", ctypes.c_int), ("graph", ctypes.c_int), ("table_radius", ctypes.c_int),
-                ("pad_", ctypes.c_int)]
+                ("interpolation", ctypes.c_int)]
 
 
 class _CStageTimes(ctypes.Structure):
@@ -70,12 +70,13 @@ class GammaOpts:
     sort_key_bits: int = 0    # presort=3: 8, 16, 24, 32
     table_cap: int = 0
     profile_stages: int = 0   # 1: record per-stage CUDA events (gamma_get_stage_times)
+    interpolation: int = 0    # 1 Kuhn simplices (default), 2 grid vertices only (classical discrete gamma)
     table_radius: int = 0     # 1 data-independent prefix table (default), 2 the paper's radius max|DD|/dD
     graph: int = 0            # 1 replay a cached CUDA graph for repeated arguments, 2 plain launches (default)
 
     def _c(self):
         return _COpts(float(self.norm_dose), int(self.presort), int(self.star_phase), int(self.lanes_per_voxel),
-                      int(self.sort_key_bits), int(self.table_cap), int(self.profile_stages), int(self.graph), int(self.table_radius), 0)
+                      int(self.sort_key_bits), int(self.table_cap), int(self.profile_stages), int(self.graph), int(self.table_radius), int(self.interpolation))
 
 
 _lib = None

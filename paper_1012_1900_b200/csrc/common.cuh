@@ -43,6 +43,7 @@ struct EvalP {
     float cutoff;    // low-dose cutoff, fraction of D_norm
     float norm_dose; // D_norm if > 0, else taken from Ctl::normOrd
     int mode;        // 0 global, 1 local
+    int vertexOnly;  // 1: evaluation surface = grid vertices only (classical discrete gamma, comparator mode)
 };
 
 // Device control block: everything the pipeline decides on the device (no host sync on the path).

@@ -427,6 +427,7 @@ struct VoxelCtx {
     int v[3];
     int lin;
     float Dr, invdD;
+    int vertexOnly;   // comparator mode: only the grid vertex itself, no simplex
 };
 
 // All 26 faces owned by the grid vertex c = v + o; returns the new best^2.
@@ -439,6 +440,11 @@ __device__ __forceinline__ float eval_owner_vertex(const float* __restrict__ ev,
     const unsigned usable = (cx + 1 < g.n[0] ? 1u : 0u) | (cy + 1 < g.n[1] ? 2u : 0u) | (cz + 1 < g.n[2] ? 4u : 0u);
     const int sx = (usable & 1u) ? 1 : 0, sy = (usable & 2u) ? g.stride[1] : 0, sz = (usable & 4u) ? g.stride[2] : 0;
     const float* p = ev + (vc.lin + ox + oy * g.stride[1] + oz * g.stride[2]);
+    if (vc.vertexOnly) {                                       // classical discrete search (Low et al.): vertex c only
+        const float dv = (__ldg(p) - vc.Dr) * vc.invdD;
+        const float fx0 = (float)ox * g.h[0], fy0 = (float)oy * g.h[1], fz0 = (float)oz * g.h[2];
+        return fminf(best2, fmaf(dv, dv, fmaf(fx0, fx0, fmaf(fy0, fy0, fz0 * fz0))));
+    }
     float d[8];
 #pragma unroll
     for (int S = 0; S < 8; ++S)
@@ -514,9 +520,10 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
         vc.Dr = __ldg(c.ref + vc.lin);
         vc.invdD = e.mode == 0 ? c.invGlobal : criterion_inv_dD(e, c.dnorm, vc.Dr);
         voxel_coords(g, vc.lin, vc.v[0], vc.v[1], vc.v[2]);
+        vc.vertexOnly = e.vertexOnly;
         best2 = key * key;
     } else {
-        vc.lin = 0; vc.Dr = 0.0f; vc.invdD = 0.0f; vc.v[0] = vc.v[1] = vc.v[2] = 0;
+        vc.lin = 0; vc.Dr = 0.0f; vc.invdD = 0.0f; vc.v[0] = vc.v[1] = vc.v[2] = 0; vc.vertexOnly = e.vertexOnly;
     }
     // ---- Algorithm A1 step 4-b over the sorted table
     for (unsigned e0 = 0;; e0 += EPP) {

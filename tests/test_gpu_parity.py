@@ -206,6 +206,23 @@ def test_missing_region_heavy_tail_beyond_the_prefix_table(oracle_mod):
         assert_parity(got, want, f"missing region, {o}")
 
 
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_small", "cfg4_coarse"])
+def test_vertex_only_comparator_mode(oracle_mod, name):
+    """opts.interpolation = 2: the classical discrete search over grid vertices (the oracle's vertex-only form), and
+    the interpolation benefit gamma_interp <= gamma_vertex on the device maps."""
+    c = phantoms.make_case(name)
+    want = oracle_mod.gamma(c.ref, c.eval, c.dims, [f32(s) for s in c.spacing_mm], f32(c.dd), f32(c.dta_mm), c.mode,
+                            f32(c.cutoff), form="vertex")
+    for o in (GammaOpts(interpolation=2), GammaOpts(interpolation=2, lanes_per_voxel=1, presort=2),
+              GammaOpts(interpolation=2, table_cap=9), GammaOpts(interpolation=2, table_radius=2)):
+        got = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
+        assert_parity(got, want, f"{name} vertex-only {o}")
+    interp = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    m = ~np.isnan(want)
+    assert np.all(interp[m] <= got[m] + 1e-6)
+    assert np.mean(interp[m] < got[m] - 1e-4) > 0.5          # and it is a real benefit on these phantoms
+
+
 def test_identical_grids_flat_offset_and_ramp_closed_form():
     c = phantoms.make_case("cfg2_small")
     g = gpu_gamma(c.ref, c.ref, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1)
