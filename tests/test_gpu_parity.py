@@ -223,6 +223,30 @@ def test_vertex_only_comparator_mode(oracle_mod, name):
     assert np.mean(interp[m] < got[m] - 1e-4) > 0.5          # and it is a real benefit on these phantoms
 
 
+def test_unaligned_buffers_take_the_scalar_paths():
+    """ref / eval / out_gamma that start 4 or 8 bytes past a 16-byte boundary (views into larger tensors): the float4
+    streams of k_norm, k_classify and k_stats must fall back to scalar accesses and give the same result."""
+    c = phantoms.make_case("cfg2_small")
+    n = c.ref.size
+    a = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    r0 = torch.from_numpy(c.ref.ravel().copy()).cuda()
+    e0 = torch.from_numpy(c.eval.ravel().copy()).cuda()
+    want = binding.gamma_eval_ex(r0, e0, *a)
+    hist0, s0 = binding.gamma_stats(want, 64, 4.0)
+    for off_r, off_e, off_o in ((1, 0, 0), (0, 2, 0), (0, 0, 1), (1, 3, 2)):
+        rb = torch.zeros(n + 8, device="cuda"); eb = torch.zeros(n + 8, device="cuda"); ob = torch.zeros(n + 8, device="cuda")
+        r = rb[off_r:off_r + n]; e = eb[off_e:off_e + n]; o = ob[off_o:off_o + n]
+        r.copy_(r0); e.copy_(e0)
+        assert (r.data_ptr() % 16 != 0) == (off_r % 4 != 0)
+        binding.gamma_eval_ex(r, e, *a, None, o)
+        torch.cuda.synchronize()
+        assert torch.equal(torch.nan_to_num(o, nan=-1.0), torch.nan_to_num(want, nan=-1.0)), (off_r, off_e, off_o)
+        assert float(ob[:off_o].abs().sum()) == 0.0 and float(ob[off_o + n:].abs().sum()) == 0.0   # nothing outside
+        hist, s = binding.gamma_stats(o, 64, 4.0)
+        assert torch.equal(hist, hist0) and s["n_eval"] == s0["n_eval"] and s["n_pass"] == s0["n_pass"]
+        assert s["n_nan"] == s0["n_nan"] and abs(s["sum_gamma3"] - s0["sum_gamma3"]) <= 1e-9 * abs(s0["sum_gamma3"])
+
+
 def test_identical_grids_flat_offset_and_ramp_closed_form():
     c = phantoms.make_case("cfg2_small")
     g = gpu_gamma(c.ref, c.ref, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1)
