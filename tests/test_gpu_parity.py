@@ -360,6 +360,38 @@ def test_gamma_eval_host_streams_and_determinism():
     assert np.array_equal(o4.cpu().numpy().astype(np.float64), base, equal_nan=True)
 
 
+def test_calls_interleaved_over_three_streams_share_the_workspace_safely():
+    """The library has ONE workspace for single calls: a call on another stream than the previous one must wait for
+    the tail of that stream (event recorded there when the next call arrives), whatever the geometry, with the stats,
+    sort and table entry points mixed in."""
+    cases = [phantoms.make_case(n) for n in ("cfg2_small", "cfg4_coarse", "cfg1")]
+    data = []
+    for c in cases:
+        r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+        e = torch.from_numpy(c.eval.ravel().copy()).cuda()
+        a = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+        want = binding.gamma_eval_ex(r, e, *a).clone()
+        data.append((r, e, a, want))
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    outs = []
+    for i in range(45):
+        k = (i * 7) % 3                                   # case
+        s = streams[(i * 5 + i // 3) % 3]                 # stream: changes from call to call, sometimes repeats
+        r, e, a, _ = data[k]
+        o = torch.empty_like(r)
+        binding.gamma_eval_ex(r, e, *a, None, o, s)
+        if i % 6 == 5:
+            binding.gamma_stats_async(o, 32, 3.0, stream=s)
+        if i % 11 == 10:
+            keys = torch.arange(5000, 0, -1, device="cuda", dtype=torch.int32)
+            binding.gamma_sort_pairs(keys, keys.clone(), stream=s)
+        outs.append((k, o))
+    torch.cuda.synchronize()
+    for i, (k, o) in enumerate(outs):
+        assert torch.equal(torch.nan_to_num(o, nan=-1.0), torch.nan_to_num(data[k][3], nan=-1.0)), i
+
+
 def test_graph_replay_sees_new_data_and_matches_plain_launches(oracle_mod):
     """A repeated call (same pointers and arguments) replays a cached CUDA graph: the replay must read the
     buffers' CURRENT contents, agree bit for bit with kernel-by-kernel launches (opts.graph = 2), survive more
