@@ -96,6 +96,23 @@ def test_large_grids_sampled_parity(oracle_mod, name, n_random, n_top):
     print(f"{name}: max|dgamma| {err:.2e} over {vox.size} sampled voxels, max gamma {fin.max():.3f}")
 
 
+@pytest.mark.parametrize("name,cutoff", [("cfg3", 0.1), ("cfg5", 0.2)])
+def test_local_criterion_full_size_sampled_parity(oracle_mod, name, cutoff):
+    """Local gamma (dD_v = DD * D_r[v], reading 9) at full size: per-voxel criteria in every kernel (star, ring,
+    table walk), oracle on a seeded sample plus the voxels with the largest gamma_0."""
+    c = phantoms.make_case(name)
+    g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 1, cutoff)
+    ref = c.ref.ravel().astype(np.float64)
+    keep = np.flatnonzero(ref >= f32(cutoff) * ref.max())
+    rng = np.random.default_rng([0, 12])
+    g0 = np.abs(c.eval.ravel().astype(np.float64) - ref)[keep] / (f32(c.dd) * ref[keep])
+    vox = np.unique(np.concatenate([rng.choice(keep, size=30000, replace=False), keep[np.argsort(g0)[-1500:]]]))
+    o = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 1, cutoff, voxels=vox)
+    err = assert_parity(g[vox], o, f"{name} local")
+    assert np.array_equal(np.isnan(g), ref < f32(cutoff) * ref.max())
+    print(f"{name} local: max|dgamma| {err:.2e} over {vox.size} sampled voxels")
+
+
 def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
     """Config 5 is run with and without the voxel pre-sort (Table 2) and with the paper's
     thread-per-voxel mapping: the candidate set and the arithmetic of the table walk are the same, so gamma is
