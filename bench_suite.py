@@ -139,6 +139,9 @@ def suite_configs(args, emit):
     for name in ("cfg1", "cfg2", "cfg3", "cfg4_coarse", "cfg4_fine", "cfg5"):
         case = phantoms.make_case(name)
         variants = [("default", {})]
+        if name == "cfg3":       # kernel variants of SURVEY.md 8(f) 2: the paper's routine on whole cells; grid vertices only
+            variants += [("recursion variant (PAPER.md:209)", {"interpolation": 3}),
+                         ("vertices only (no interpolation)", {"interpolation": 2})]
         if name == "cfg5":
             variants += [("presort off", {"presort": 2}), ("full radix sort", {"presort": 3}),
                          ("thread per voxel, presort on", {"lanes_per_voxel": 1, "star_phase": 2, "presort": 3}),

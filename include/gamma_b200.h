@@ -107,7 +107,11 @@ typedef struct gamma_opts {
     int interpolation;    /* 0: default (= 1); 1: the evaluation dose is the piecewise-linear surface on the Kuhn
                              simplices (the paper's method); 2: grid vertices only -- the classical discrete
                              gamma search (Low 1998), kept as an internal comparator: gamma_1 <= gamma_2 always
-                             (same table walk and early exit; the star phase is off)                      */
+                             (same table walk and early exit; the star phase is off); 3: the same surface as 1,
+                             but every cell of the table walk is evaluated as its six Kuhn tetrahedra with the
+                             paper's routine: normal equations and recursion into the sub-simplices opposite
+                             negative weights -- a slow variant kept to measure that trade
+                             (3D grids; 2D / 1D grids use 1)                                              */
 } gamma_opts;
 
 /* Several independent cases in one call (every reference voxel and every case is independent,

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgamma_b200.so")
 SOURCES = ["gamma_api.cu"]
-DEPENDS = ["common.cuh", "features_generated.cuh", "gamma_search.cuh", "offset_table.cuh", "radix_sort.cuh",
+DEPENDS = ["common.cuh", "features_generated.cuh", "gamma_search.cuh", "ju_simplex.cuh", "offset_table.cuh", "radix_sort.cuh",
            "stats.cuh", os.path.join("..", "..", "include", "gamma_b200.h")]
 
 NVCC_FLAGS = [

@@ -43,7 +43,8 @@ struct EvalP {
     float cutoff;    // low-dose cutoff, fraction of D_norm
     float norm_dose; // D_norm if > 0, else taken from Ctl::normOrd
     int mode;        // 0 global, 1 local
-    int vertexOnly;  // 1: evaluation surface = grid vertices only (classical discrete gamma, comparator mode)
+    int algo;        // 0: closed form on owned faces (default); 1: grid vertices only (classical discrete gamma,
+                     // comparator); 2: the six Kuhn tetrahedra of a cell by the negative-weight recursion (ju_simplex.cuh)
 };
 
 // Device control block: everything the pipeline decides on the device (no host sync on the path).

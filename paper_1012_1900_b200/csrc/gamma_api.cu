@@ -86,7 +86,7 @@ struct GraphKey {
     void* ctl;
     GridP g;
     float DD, cutoff, normDose;
-    int mode, presort, star, lanes, keyBits, tableMode, vertexOnly;
+    int mode, presort, star, lanes, keyBits, tableMode, algo;
     long long tableCap;
     bool operator==(const GraphKey& o) const { return std::memcmp(this, &o, sizeof *this) == 0; }
 };
@@ -349,7 +349,7 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
 }
 
 struct Resolved {
-    int presort, star, lanes, keyBits, profile, graph, tableMode, vertexOnly;
+    int presort, star, lanes, keyBits, profile, graph, tableMode, algo;
     long long tableCap;
     float normDose;
 };
@@ -357,7 +357,7 @@ struct Resolved {
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
     r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 0; r.tableMode = 1; r.normDose = 0.0f;
-    r.profile = 0; r.graph = 0; r.vertexOnly = 0;
+    r.profile = 0; r.graph = 0; r.algo = 0;
     if (!o) { r.tableCap = TAB_EMBED_MAX_CELLS; return GAMMA_OK; }
     r.profile = o->profile_stages == 1;
     if (o->graph < 0 || o->graph > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.graph must be 0, 1 or 2");
@@ -384,9 +384,10 @@ int resolve_opts(const gamma_opts* o, Resolved& r)
         r.tableCap = o->table_cap;
     }
     if (r.presort == 4 && r.lanes != 0) r.presort = 1;   // depth classes only exist for the adaptive search
-    if (o->interpolation < 0 || o->interpolation > 2)
-        return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.interpolation must be 0, 1 or 2");
-    if (o->interpolation == 2) { r.vertexOnly = 1; r.star = 0; }   // the star phase is interpolation
+    if (o->interpolation < 0 || o->interpolation > 3)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.interpolation must be 0, 1, 2 or 3");
+    if (o->interpolation == 2) { r.algo = 1; r.star = 0; }   // the star phase is interpolation
+    if (o->interpolation == 3) { r.algo = 2; r.star = 0; }   // every cell through the table walk and the recursion
     if (o->table_radius < 0 || o->table_radius > 2)
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.table_radius must be 0, 1 or 2");
     if (o->table_radius == 2) r.tableMode = 2;
@@ -466,7 +467,8 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *i1 = static_cast<unsigned*>(g_ws.idx1.p);
     unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p);
     EvalP e;
-    e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode; e.vertexOnly = r.vertexOnly;
+    e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
+    e.algo = (r.algo == 2 && !g.all_active) ? 0 : r.algo;   // the recursion variant is written for 3D cells
     const int classes = (r.presort == 4 && r.star && g.all_active) ? 1 : 0;   // needs the 3D star phase
     const int presort = (r.presort == 4 && !classes) ? 1 : r.presort;
 #define STAGE_MARK(i, s) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], s)); } while (0)
@@ -576,7 +578,11 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         if (!geoHit && r.tableMode == 1 && g.all_active && classes) {
             geo.g = g; geo.cap = r.tableCap; geo.radius = radius; geo.plan = plan; geo.ring = ring; geo.valid = true;
         }
-        if (r.lanes == 1)
+        if (e.algo == 2 && r.lanes == 1)
+            CU_TRY(launch_ex(k_table_search<1, true>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
+        else if (e.algo == 2)
+            CU_TRY(launch_ex(k_table_search<0, true>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
+        else if (r.lanes == 1)
             CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
         else if (r.lanes == 8)
             CU_TRY(launch_ex(k_table_search<8>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
@@ -661,7 +667,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         key.ref = ref; key.ev = ev; key.out = out; key.ctl = ctl; key.g = g;
         key.DD = DD; key.cutoff = cutoff; key.normDose = r.normDose;
         key.mode = mode; key.presort = r.presort; key.star = r.star; key.lanes = r.lanes; key.keyBits = r.keyBits;
-        key.tableCap = r.tableCap; key.tableMode = r.tableMode; key.vertexOnly = r.vertexOnly;
+        key.tableCap = r.tableCap; key.tableMode = r.tableMode; key.algo = r.algo;
         GraphEntry* hit = nullptr;
         for (int i = 0; i < g_ws.numGraphs; ++i)
             if (g_ws.graph[i].key == key) { hit = &g_ws.graph[i]; break; }
@@ -924,7 +930,7 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     if (rc) return rc;
     Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_STANDALONE;
     EvalP e;
-    e.DD = 1.0f; e.cutoff = 0.0f; e.norm_dose = 1.0f; e.mode = 0; e.vertexOnly = 0;
+    e.DD = 1.0f; e.cutoff = 0.0f; e.norm_dose = 1.0f; e.mode = 0; e.algo = 0;
     k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, st>>>(
         g, e, ctl, radius, max_entries, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
         static_cast<unsigned*>(g_ws.tmpIdx.p), 0);

@@ -22,6 +22,7 @@
 #include "common.cuh"
 #include "features_generated.cuh"
 #include "offset_table.cuh"
+#include "ju_simplex.cuh"
 
 namespace gamma_b200 {
 
@@ -427,10 +428,11 @@ struct VoxelCtx {
     int v[3];
     int lin;
     float Dr, invdD;
-    int vertexOnly;   // comparator mode: only the grid vertex itself, no simplex
+    int algo;         // EvalP::algo
 };
 
 // All 26 faces owned by the grid vertex c = v + o; returns the new best^2.
+template <bool JU>
 __device__ __forceinline__ float eval_owner_vertex(const float* __restrict__ ev, const GridP& g, const VoxelCtx& vc,
                                                    int ox, int oy, int oz, float best2)
 {
@@ -440,7 +442,7 @@ __device__ __forceinline__ float eval_owner_vertex(const float* __restrict__ ev,
     const unsigned usable = (cx + 1 < g.n[0] ? 1u : 0u) | (cy + 1 < g.n[1] ? 2u : 0u) | (cz + 1 < g.n[2] ? 4u : 0u);
     const int sx = (usable & 1u) ? 1 : 0, sy = (usable & 2u) ? g.stride[1] : 0, sz = (usable & 4u) ? g.stride[2] : 0;
     const float* p = ev + (vc.lin + ox + oy * g.stride[1] + oz * g.stride[2]);
-    if (vc.vertexOnly) {                                       // classical discrete search (Low et al.): vertex c only
+    if (vc.algo == 1) {                                        // classical discrete search (Low et al.): vertex c only
         const float dv = (__ldg(p) - vc.Dr) * vc.invdD;
         const float fx0 = (float)ox * g.h[0], fy0 = (float)oy * g.h[1], fz0 = (float)oz * g.h[2];
         return fminf(best2, fmaf(dv, dv, fmaf(fx0, fx0, fmaf(fy0, fy0, fz0 * fz0))));
@@ -449,6 +451,10 @@ __device__ __forceinline__ float eval_owner_vertex(const float* __restrict__ ev,
 #pragma unroll
     for (int S = 0; S < 8; ++S)
         d[S] = (__ldg(p + ((S & 1) ? sx : 0) + ((S & 2) ? sy : 0) + ((S & 4) ? sz : 0)) - vc.Dr) * vc.invdD;
+    if (JU && vc.algo == 2) {                                  // variant: whole cells by the recursion of PAPER.md:209
+        if (usable != 7u) return best2;                        // only cells fully inside the grid exist (reading 11)
+        return ju_cell_min(d, g, ox, oy, oz, best2);
+    }
     const float fx = (float)ox, fy = (float)oy, fz = (float)oz;
     const float px = fx * g.h[0], py = fy * g.h[1], pz = fz * g.h[2];
     const float q[3] = {px * px, py * py, pz * pz};
@@ -498,7 +504,7 @@ struct SearchCtx {
 
 // One warp searches 32/G consecutive work items (firstItem .. firstItem + 32/G - 1, counted from the END of the
 // sorted list: deepest first), G lanes per reference voxel.  Returns the owner vertices it evaluated.
-template <int G>
+template <int G, bool JU = false>
 __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP& g, const EvalP& e,
                                                  const unsigned* __restrict__ listKey,
                                                  const unsigned* __restrict__ listIdx, unsigned nList,
@@ -520,10 +526,10 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
         vc.Dr = __ldg(c.ref + vc.lin);
         vc.invdD = e.mode == 0 ? c.invGlobal : criterion_inv_dD(e, c.dnorm, vc.Dr);
         voxel_coords(g, vc.lin, vc.v[0], vc.v[1], vc.v[2]);
-        vc.vertexOnly = e.vertexOnly;
+        vc.algo = e.algo;
         best2 = key * key;
     } else {
-        vc.lin = 0; vc.Dr = 0.0f; vc.invdD = 0.0f; vc.v[0] = vc.v[1] = vc.v[2] = 0; vc.vertexOnly = e.vertexOnly;
+        vc.lin = 0; vc.Dr = 0.0f; vc.invdD = 0.0f; vc.v[0] = vc.v[1] = vc.v[2] = 0; vc.algo = e.algo;
     }
     // ---- Algorithm A1 step 4-b over the sorted table
     for (unsigned e0 = 0;; e0 += EPP) {
@@ -539,7 +545,7 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
                     const int ox = (gl & 1) ? -t.y - 1 : t.y;
                     const int oy = (gl & 2) ? -t.z - 1 : t.z;
                     const int oz = (gl & 4) ? -t.w - 1 : t.w;
-                    cand = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                    cand = eval_owner_vertex<JU>(c.ev, g, vc, ox, oy, oz, best2);
                     ++visits;
                 }
             }
@@ -552,7 +558,7 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
                     const int ox = (var & 1) ? -t.y - 1 : t.y;
                     const int oy = (var & 2) ? -t.z - 1 : t.z;
                     const int oz = (var & 4) ? -t.w - 1 : t.w;
-                    best2 = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                    best2 = eval_owner_vertex<JU>(c.ev, g, vc, ox, oy, oz, best2);
                     ++visits;
                 }
             }
@@ -592,7 +598,7 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
                             const int ox = (gl & 1) ? -mx - 1 : mx;
                             const int oy = (gl & 2) ? -my - 1 : my;
                             const int oz = (gl & 4) ? -mz - 1 : mz;
-                            cand = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                            cand = eval_owner_vertex<JU>(c.ev, g, vc, ox, oy, oz, best2);
                             ++visits;
                         }
                     }
@@ -607,7 +613,7 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
                             const int ox = (var & 1) ? -mx - 1 : mx;
                             const int oy = (var & 2) ? -my - 1 : my;
                             const int oz = (var & 4) ? -mz - 1 : mz;
-                            best2 = eval_owner_vertex(c.ev, g, vc, ox, oy, oz, best2);
+                            best2 = eval_owner_vertex<JU>(c.ev, g, vc, ox, oy, oz, best2);
                             ++visits;
                         }
                     }
@@ -653,8 +659,10 @@ __device__ __forceinline__ void ring_items(const SearchCtx& c, const GridP& g, c
 // lists (classes != 0), the separate list (deepKey, deepIdx) that k_star filled; the other list then holds "ring"
 // items only, searched one per thread (ring_items).  Work units are handed out
 // deepest first: first round static, later rounds by an atomic counter whose latency hides behind the search.
-template <int MODE>
-__global__ void __launch_bounds__(SEARCH_THREADS, MODE == 0 ? SEARCH_MIN_BLOCKS : 1)
+// JU: the instantiation that also holds the recursion variant (ju_simplex.cuh); kept out of the default kernels, whose
+// register allocation it would disturb.
+template <int MODE, bool JU = false>
+__global__ void __launch_bounds__(SEARCH_THREADS, (MODE == 0 && !JU) ? SEARCH_MIN_BLOCKS : 1)
 k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, float* __restrict__ out, GridP g,
                EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
                const unsigned* __restrict__ listIdx, const unsigned* __restrict__ deepKey,
@@ -700,11 +708,11 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
         unsigned nextUnit = numUnits;
         if (dynamic && lane == 0) nextUnit = atomicAdd(&ctl->workCounter, 1u) + warpsTotal;
         if (MODE == 0) {
-            if (unit < nDeep) visits += search_items<32>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane);
+            if (unit < nDeep) visits += search_items<32, JU>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane);
             else if (classes) ring_items(c, g, e, ring, listKey, listIdx, nS, 32u * (unit - nDeep), lane);
-            else visits += search_items<8>(c, g, e, listKey, listIdx, nS, nDeep + 4u * (unit - nDeep), lane);
+            else visits += search_items<8, JU>(c, g, e, listKey, listIdx, nS, nDeep + 4u * (unit - nDeep), lane);
         } else {
-            visits += search_items<(MODE == 0 ? 8 : MODE)>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);
+            visits += search_items<(MODE == 0 ? 8 : MODE), JU>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);
         }
         unit = __shfl_sync(FULL, nextUnit, 0);
     }

@@ -70,7 +70,7 @@ def test_argument_errors_are_reported_without_touching_the_device(lib, kw, msg):
 def test_bad_options_and_aux_entry_points(lib):
     cd, cs = (ctypes.c_int * 3)(4, 4, 4), (ctypes.c_float * 3)(1, 1, 1)
     for bad in (dict(presort=5), dict(star_phase=-1), dict(lanes_per_voxel=4), dict(sort_key_bits=12),
-                dict(table_cap=-5), dict(norm_dose=float("inf")), dict(graph=3), dict(table_radius=3), dict(interpolation=3)):
+                dict(table_cap=-5), dict(norm_dose=float("inf")), dict(graph=3), dict(table_radius=3), dict(interpolation=4)):
         o = binding.GammaOpts(**bad)._c()
         rc = lib.gamma_eval_ex(0x1000, 0x2000, cd, cs, 0.03, 3.0, 0, 0.1, ctypes.byref(o), 0x3000, None)
         assert rc == 1, bad

@@ -264,6 +264,26 @@ def test_unaligned_buffers_take_the_scalar_paths():
         assert s["n_nan"] == s0["n_nan"] and abs(s["sum_gamma3"] - s0["sum_gamma3"]) <= 1e-9 * abs(s0["sum_gamma3"])
 
 
+@pytest.mark.parametrize("name", ["cfg2_small", "cfg4_coarse", "cfg1"])
+def test_recursion_variant_gives_the_same_gamma(oracle_mod, name):
+    """opts.interpolation = 3: every cell as six Kuhn tetrahedra through the paper's normal equations and the
+    negative-weight recursion instead of the closed form on owned faces: same surface, so the
+    oracle's gamma within the tolerance, and the default path's gamma within rounding."""
+    c = phantoms.make_case(name)
+    want = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    for o in (GammaOpts(interpolation=3), GammaOpts(interpolation=3, lanes_per_voxel=1, presort=2),
+              GammaOpts(interpolation=3, table_cap=9)):
+        got = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
+        err = assert_parity(got, want, f"{name} recursion variant {o}")
+        m = ~np.isnan(want)
+        assert np.abs(got[m] - base[m]).max() <= 2e-5
+    ref, ev = _random_case((23, 17, 9), (2.0, 3.0, 2.5), 11)
+    want = cpu_gamma(oracle_mod, ref, ev, (23, 17, 9), (2.0, 3.0, 2.5), 0.02, 4.0, 1, 0.0)
+    got = gpu_gamma(ref, ev, (23, 17, 9), (2.0, 3.0, 2.5), 0.02, 4.0, 1, 0.0, GammaOpts(interpolation=3))
+    assert_parity(got, want, "rough random field, local criterion, recursion variant")
+
+
 def test_identical_grids_flat_offset_and_ramp_closed_form():
     c = phantoms.make_case("cfg2_small")
     g = gpu_gamma(c.ref, c.ref, c.dims, c.spacing_mm, c.dd, c.dta_mm, 0, 0.1)
