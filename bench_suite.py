@@ -119,8 +119,9 @@ def oracle_sample(case, seconds, dd=None, dta=None, nthreads=0):
 
     def run(vox):
         t0 = time.perf_counter()
+        # explicit thread count: the oracle keeps the last OpenMP setting, and a one-core run may have come before
         oracle.gamma(case.ref, case.eval, case.dims, sp, f32(dd), f32(dta), case.mode, f32(case.cutoff), voxels=vox,
-                     nthreads=nthreads)
+                     nthreads=nthreads if nthreads else (os.cpu_count() or 1))
         return time.perf_counter() - t0
 
     probe = np.sort(rng.choice(keep, size=min(keep.size, 2000), replace=False))
@@ -129,7 +130,7 @@ def oracle_sample(case, seconds, dd=None, dta=None, nthreads=0):
     vox = np.sort(rng.choice(keep, size=n, replace=False))
     t = run(vox)
     return {"voxels": n, "of": int(keep.size), "seconds": t, "voxels_per_s": n / t,
-            "cores": nthreads if nthreads else oracle.num_threads(),
+            "cores": nthreads if nthreads else (os.cpu_count() or 1),
             "seconds_per_case_extrapolated": t / n * keep.size}
 
 
@@ -140,7 +141,8 @@ def suite_configs(args, emit):
         case = phantoms.make_case(name)
         variants = [("default", {})]
         if name == "cfg3":       # kernel variants of SURVEY.md 8(f) 2: the paper's routine on whole cells; grid vertices only
-            variants += [("recursion variant (PAPER.md:209)", {"interpolation": 3}),
+            variants += [("graph replay (opts.graph = 1)", {"graph": 1}),
+                         ("recursion variant (PAPER.md:209)", {"interpolation": 3}),
                          ("vertices only (no interpolation)", {"interpolation": 2})]
         if name == "cfg5":
             variants += [("presort off", {"presort": 2}), ("full radix sort", {"presort": 3}),

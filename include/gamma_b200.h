@@ -95,7 +95,8 @@ typedef struct gamma_opts {
     int profile_stages;   /* 1: record CUDA events between the stages of this call on `stream`, to be read
                              with gamma_get_stage_times (adds a few event records, no synchronisation)     */
     int graph;            /* 0: default (= 2); 1: a call whose arguments (pointers included) were seen before
-                             replays a cached CUDA graph of its kernels (up to 64 argument sets are kept):
+                             replays a cached CUDA graph of its kernels (96 graphs are kept; a call needs one per
+                             rotating control-block slot, so up to 32 argument sets replay without re-capture):
                              less host time per call, but replays do not overlap with the previous call the
                              way stream launches do; 2: launch the kernels one by one.  Ignored (= 2) while
                              `stream` is being captured by the caller (the kernels then become nodes of the

@@ -96,7 +96,7 @@ struct GraphEntry {
     unsigned long long lastUse = 0;
     int kernels = 0;
 };
-constexpr int GRAPH_CACHE = 64;
+constexpr int GRAPH_CACHE = 96;    // argument sets x 3 rotating control-block slots
 // control-block slots: 0/1/2 rotate between calls (the first kernel of call i clears the slot of call i+1 and may run
 // while call i-1 is still finishing), 3 stand-alone entry points, 4 calls captured by the caller
 constexpr int CTL_ROT = 3, CTL_STANDALONE = 3, CTL_CAPTURE = 4, CTL_SLOTS = 5;

@@ -459,14 +459,14 @@ def test_graph_replay_sees_new_data_and_matches_plain_launches(oracle_mod):
     want = cpu_gamma(oracle_mod, r.cpu().numpy(), e.cpu().numpy(), *a)
     assert_parity(got, want, "graph replay after the inputs changed in place")
     assert not torch.equal(torch.nan_to_num(first, nan=-1.0), torch.nan_to_num(out, nan=-1.0))
-    # more argument sets than the cache keeps (64): eviction, then the first set again
+    # more argument sets than the cache keeps (96 graphs): eviction, then the first set again
     outs = []
-    for k in range(70):
+    for k in range(110):
         outs.append(binding.gamma_eval_ex(r, e, c.dims, c.spacing_mm, c.dd, c.dta_mm + 0.01 * k, c.mode, c.cutoff, gr))
     again = binding.gamma_eval_ex(r, e, *a, gr, out).clone()
     torch.cuda.synchronize()
     assert torch.equal(torch.nan_to_num(again, nan=-1.0), torch.nan_to_num(outs[0], nan=-1.0))
-    assert float(torch.nan_to_num(outs[69], nan=0.0).sum()) < float(torch.nan_to_num(outs[0], nan=0.0).sum())
+    assert float(torch.nan_to_num(outs[109], nan=0.0).sum()) < float(torch.nan_to_num(outs[0], nan=0.0).sum())
     # the caller captures the stream: the library launches its kernels into that capture instead
     side = torch.cuda.Stream()
     out2 = torch.empty_like(out)
