@@ -106,7 +106,8 @@ k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int m
         if (r > 0.0f) atomicMax(&cur->maxRatio, __float_as_uint(r));
         // Launched behind the previous call's k_table_search with programmatic dependent launch, this kernel has run
         // in that call's tail; it must not END before that call has (the kernels after it reuse its work lists).
-        pdl_wait();
+        // One block holds the grid open; the others give their registers back at once.
+        if (blockIdx.x == 0) pdl_wait();
     }
 }
 
