@@ -118,6 +118,7 @@ struct Workspace {
     int slot = 0;                  // control-block slot of the next call (0/1); slot 2: stand-alone entry points
     void* lastCtl = nullptr;
     bool haveStages = false;
+    bool stageSort = false, stageTable = false;   // the last profiled call had a sort kernel / a side-stream table
     long long launches = 0;        // kernels launched so far (gamma_launch_count)
     int numSM = 0;
     int occStar[2] = {0, 0};       // resident blocks per SM of k_star<false/true>
@@ -546,7 +547,8 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     }
     STAGE_MARK(2, st);
     if (!embed) CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));   // before the presort: presort -> search stay adjacent
-    else { STAGE_MARK(5, st); STAGE_MARK(6, st); }
+    g_ws.stageTable = !embed;
+    g_ws.stageSort = presort == 1 || presort == 3;    // no sort kernel: no event either (sort_ms = 0, not a gap)
     const unsigned *lk = k0, *li = i0;
     if (presort == 1) {                                                // a2: one-pass MSD bucket presort
         CU_TRY(launch_ex(k_bucket_scatter, sm * 2, SCATTER_THREADS, 0, st, pdl, false, ctl, k0, i0, k1, i1));
@@ -558,7 +560,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         nk += 3 * (r.keyBits / 8);
         if (where) { lk = k1; li = i1; }
     }
-    STAGE_MARK(3, st);
+    if (g_ws.stageSort) STAGE_MARK(3, st);
     {                                                                    // a4 + a5
         const int grid = sm * (r.lanes == 0 ? SEARCH_MIN_BLOCKS : 4 * (256 / SEARCH_THREADS));   // resident blocks
         const int4* tab = static_cast<const int4*>(g_ws.table.p) + (embed ? (size_t)slot * (size_t)TAB_EMBED_MAX_CELLS : 0);
@@ -973,11 +975,14 @@ int gamma_get_stage_times(gamma_stage_times* out_host)
     std::lock_guard<std::mutex> lock(g_mu);
     if (!g_ws.haveStages) return fail(GAMMA_ERR_INVALID_ARGUMENT, "last gamma_eval call did not set opts.profile_stages");
     CU_TRY(cudaEventSynchronize(g_ws.stage[4]));
-    CU_TRY(cudaEventSynchronize(g_ws.stage[6]));
-    float ms[4];
-    for (int i = 0; i < 4; ++i) CU_TRY(cudaEventElapsedTime(&ms[i], g_ws.stage[i], g_ws.stage[i + 1]));
-    out_host->prep_ms = ms[0]; out_host->star_ms = ms[1]; out_host->sort_ms = ms[2]; out_host->search_ms = ms[3];
-    CU_TRY(cudaEventElapsedTime(&out_host->table_ms, g_ws.stage[5], g_ws.stage[6]));
+    if (g_ws.stageTable) CU_TRY(cudaEventSynchronize(g_ws.stage[6]));
+    CU_TRY(cudaEventElapsedTime(&out_host->prep_ms, g_ws.stage[0], g_ws.stage[1]));
+    CU_TRY(cudaEventElapsedTime(&out_host->star_ms, g_ws.stage[1], g_ws.stage[2]));
+    out_host->sort_ms = 0.0f;
+    if (g_ws.stageSort) CU_TRY(cudaEventElapsedTime(&out_host->sort_ms, g_ws.stage[2], g_ws.stage[3]));
+    CU_TRY(cudaEventElapsedTime(&out_host->search_ms, g_ws.stage[g_ws.stageSort ? 3 : 2], g_ws.stage[4]));
+    out_host->table_ms = 0.0f;
+    if (g_ws.stageTable) CU_TRY(cudaEventElapsedTime(&out_host->table_ms, g_ws.stage[5], g_ws.stage[6]));
     CU_TRY(cudaEventElapsedTime(&out_host->total_ms, g_ws.stage[0], g_ws.stage[4]));
     return GAMMA_OK;
 }

@@ -584,7 +584,12 @@ def test_stage_times_are_reported():
     t = binding.gamma_get_stage_times()
     assert t["total_ms"] > 0 and t["prep_ms"] > 0 and t["search_ms"] >= 0
     assert abs(sum(t[k] for k in ("prep_ms", "star_ms", "sort_ms", "search_ms")) - t["total_ms"]) < 0.05
-    assert t["table_ms"] > 0                         # built on the side stream, concurrent with prep
+    assert t["table_ms"] == 0 and t["sort_ms"] == 0  # default: table inside k_star, no sort kernel, no event for either
+    gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff,
+              GammaOpts(profile_stages=1, table_radius=2, presort=1))
+    t = binding.gamma_get_stage_times()
+    assert t["table_ms"] > 0 and t["sort_ms"] > 0    # side-stream table (concurrent with prep / star), bucket presort
+    assert abs(sum(t[k] for k in ("prep_ms", "star_ms", "sort_ms", "search_ms")) - t["total_ms"]) < 0.05
 
 
 # ----------------------------------------------------------------------------------------------------
