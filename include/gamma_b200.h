@@ -19,6 +19,9 @@
  *              of the calling thread.  No exceptions, no abort.
  *   threads    calls are serialised by an internal mutex; consecutive calls on different streams are
  *              ordered by an event (they share the workspace).
+ *   memory     workspace per voxel of the largest grid seen: 80 B up to 2^25 voxels (five u32 work lists x 4 rotating
+ *              sets); larger grids first count their evaluated voxels M (one 4-byte read by the host, which
+ *              SYNCHRONISES `stream` once inside the call) and take 20 B per EVALUATED voxel.
  *   no fallback: there is no CPU path; without a CUDA device every compute call returns GAMMA_ERR_CUDA.
  */
 #ifndef GAMMA_B200_H
@@ -57,20 +60,25 @@ extern "C" {
  *                    (reading 10; the comparison is done in double so that it is decided identically
  *                    everywhere).  Excluded voxels still serve as evaluation points of their neighbours.
  *   out_gamma        DEVICE, N fp32, written entirely
- *   (pipelining)     consecutive calls on ONE stream overlap: the first kernel of a call (it reads ref / eval only)
- *                    may run while the previous call on that stream is finishing.  Stream order as seen by the caller
- *                    is kept (a call whose inputs overlap the previous call's out_gamma is not started early).  The
- *                    one thing the library cannot see: a kernel of the caller's that writes ref / eval, sits directly
- *                    in front of the call AND itself releases its dependents early (griddepcontrol.launch_dependents)
- *                    must not be used; environment GAMMA_OVERLAP_CALLS=0 switches the overlap off.
  *   stream           cudaStream_t.  With the default options everything runs on `stream` (4 kernels).  Only with
  *                    opts.table_radius = 2 or a table_cap above 1024 the offset table is built on a library-owned
  *                    side stream that forks from and joins `stream` through events (legal under stream capture).
+ *   (ordering)       A call behaves like one stream operation: its first kernel waits for the operation in front of it
+ *                    before it reads ref / eval, and when its last kernel has completed, every earlier call has.
+ *                    Consecutive calls can be PIPELINED instead (the first three kernels of a call run beside the
+ *                    table search of the previous one): see gamma_opts::back_to_back.
+ *   (CUDA graphs)    A call made while the CALLER is capturing `stream` becomes four kernel nodes and one memset node
+ *                    of the caller's graph.  The graph holds addresses of a library workspace reserved for captured
+ *                    calls: that workspace never moves afterwards (a later captured call that needs a larger one fails
+ *                    with GAMMA_ERR_INVALID_ARGUMENT), gamma_release() frees it and thereby INVALIDATES every graph
+ *                    that holds such nodes, and two graphs holding captured calls must not run concurrently (they
+ *                    share that workspace; replays on one stream are ordered).  Direct calls never touch it.
  */
 int gamma_eval(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
                float DTA_mm, int mode, float low_dose_cutoff, float* out_gamma, void* stream);
 
 /* Options of gamma_eval_ex / gamma_eval_host.  Zero-initialise, then set what differs. */
+struct gamma_summary;
 typedef struct gamma_opts {
     float norm_dose;      /* D_norm; <= 0: max(ref), found on the device                                  */
     int presort;          /* pre-sort of the search work list (A2 step 3).  0: default (= 4);
@@ -113,6 +121,22 @@ typedef struct gamma_opts {
                              paper's routine: normal equations and recursion into the sub-simplices opposite
                              negative weights -- a slow variant kept to measure that trade
                              (3D grids; 2D / 1D grids use 1)                                              */
+    int back_to_back;     /* 0: default.  1: the caller ASSERTS that nothing else has been enqueued on `stream` since the
+                             library's previous gamma_eval / gamma_eval_ex call on it returned (no kernel, copy or event
+                             of the caller's).  The call is then pipelined behind that call: its k_norm, k_classify and
+                             k_star run while the previous table search is still running, each call on its own set of
+                             work lists (4 sets rotate), and calls still complete in call order.  The library checks
+                             what it can see (same stream, previous call of the same kind, no overlap between the
+                             buffers of the calls in flight: a call whose input is an earlier call's output is simply
+                             not pipelined); it cannot see foreign work on the stream, hence the assertion.  Ignored
+                             with profile_stages, graph = 1, large tables and grids above 2^25 voxels               */
+    int stats_nbins;      /* a6 fused into the call (all four stats_* fields; stats_hist = NULL: off).  The gamma
+                             kernels accumulate, where they write gamma, what gamma_stats computes from the finished map:
+                             same definition, same results (counts and histogram exact, sums in double), no second pass
+                             over gamma[N].  1 <= stats_nbins <= 1024                                              */
+    unsigned long long* stats_hist;        /* DEVICE, stats_nbins u64, overwritten                                  */
+    struct gamma_summary* stats_summary;   /* DEVICE, one gamma_summary, overwritten                                */
+    float stats_hist_max;                  /* > 0: bin b counts floor(gamma / stats_hist_max * stats_nbins) == b    */
 } gamma_opts;
 
 /* Several independent cases in one call (every reference voxel and every case is independent,
@@ -218,6 +242,9 @@ int gamma_get_stage_times(gamma_stage_times* out_host);
 /* Number of CUDA kernels this library has launched in this process so far (host counter; memsets and
  * copies are not counted). */
 long long gamma_launch_count(void);
+
+/* Device memory the library's workspaces hold right now, in bytes (host counter). */
+long long gamma_workspace_bytes(void);
 
 /*
  * gamma_fp32_probe -- measures the plain-ALU FP32 rate of the device with independent FFMA chains

@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
     "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
-    "gamma_get_stage_times", "gamma_launch_count", "gamma_fp32_probe", "gamma_release", "gamma_version",
+    "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_release", "gamma_version",
     "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
 
@@ -26,8 +26,8 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 # every symbol include/gamma_b200.h declares
 exported_symbols = (
     "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table",
-    "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_fp32_probe", "gamma_release",
-    "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
+    "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
+    "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
 
 
@@ -39,7 +39,8 @@ class _COpts(ctypes.Structure):
     _fields_ = [("norm_dose", ctypes.c_float), ("presort", ctypes.c_int), ("star_phase", ctypes.c_int),
                 ("lanes_per_voxel", ctypes.c_int), ("sort_key_bits", ctypes.c_int), ("table_cap", ctypes.c_longlong),
                 ("profile_stages", ctypes.c_int), ("graph", ctypes.c_int), ("table_radius", ctypes.c_int),
-                ("interpolation", ctypes.c_int)]
+                ("interpolation", ctypes.c_int), ("back_to_back", ctypes.c_int), ("stats_nbins", ctypes.c_int),
+                ("stats_hist", ctypes.c_void_p), ("stats_summary", ctypes.c_void_p), ("stats_hist_max", ctypes.c_float)]
 
 
 class _CStageTimes(ctypes.Structure):
@@ -73,10 +74,27 @@ class GammaOpts:
     interpolation: int = 0    # 1 Kuhn simplices (default), 2 grid vertices only (classical discrete gamma)
     table_radius: int = 0     # 1 data-independent prefix table (default), 2 the paper's radius max|DD|/dD
     graph: int = 0            # 1 replay a cached CUDA graph for repeated arguments, 2 plain launches (default)
+    back_to_back: int = 0     # 1: caller asserts nothing else was enqueued on the stream since the previous call
+    stats_hist: object = None     # int64 CUDA tensor [nbins]: a6 fused into the call (with stats_summary)
+    stats_summary: object = None  # uint8 CUDA tensor [48]: gamma_summary bytes, decode with decode_summary
+    stats_hist_max: float = 0.0
 
     def _c(self):
+        nb = int(self.stats_hist.numel()) if self.stats_hist is not None else 0
+        if (self.stats_hist is None) != (self.stats_summary is None):
+            raise GammaError("stats_hist and stats_summary must be given together")
+        if self.stats_hist is not None:
+            if not (self.stats_hist.is_cuda and self.stats_hist.dtype == torch.int64 and self.stats_hist.is_contiguous()):
+                raise GammaError("stats_hist must be a contiguous int64 CUDA tensor")
+            if not (self.stats_summary.is_cuda and self.stats_summary.is_contiguous()
+                    and self.stats_summary.numel() * self.stats_summary.element_size() >= ctypes.sizeof(_CSummary)):
+                raise GammaError("stats_summary must be a contiguous CUDA tensor of at least 48 bytes")
         return _COpts(float(self.norm_dose), int(self.presort), int(self.star_phase), int(self.lanes_per_voxel),
-                      int(self.sort_key_bits), int(self.table_cap), int(self.profile_stages), int(self.graph), int(self.table_radius), int(self.interpolation))
+                      int(self.sort_key_bits), int(self.table_cap), int(self.profile_stages), int(self.graph),
+                      int(self.table_radius), int(self.interpolation), int(self.back_to_back), nb,
+                      self.stats_hist.data_ptr() if self.stats_hist is not None else None,
+                      self.stats_summary.data_ptr() if self.stats_summary is not None else None,
+                      float(self.stats_hist_max))
 
 
 _lib = None
@@ -107,6 +125,8 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_get_stage_times.argtypes = [ctypes.POINTER(_CStageTimes)]
     lib.gamma_launch_count.argtypes = []
     lib.gamma_launch_count.restype = cll
+    lib.gamma_workspace_bytes.argtypes = []
+    lib.gamma_workspace_bytes.restype = cll
     for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
                  "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_fp32_probe"):
         getattr(lib, name).restype = ci
@@ -311,6 +331,10 @@ def gamma_get_stage_times() -> dict:
 
 def gamma_launch_count() -> int:
     return int(load_library().gamma_launch_count())
+
+
+def gamma_workspace_bytes() -> int:
+    return int(load_library().gamma_workspace_bytes())
 
 
 def gamma_fp32_probe(repeats=5, stream=None) -> float:

@@ -48,8 +48,17 @@ struct EvalP {
 };
 
 // Device control block: everything the pipeline decides on the device (no host sync on the path).
-// Two slots alternate between consecutive gamma_eval calls: the first kernel of call i clears the slot of
-// call i+1, so no memset node sits on the critical path.
+// One block per call SET.  CTL_ROT sets rotate between consecutive calls of a workspace (call number k uses set
+// k % CTL_ROT: its own control block, offset table and work lists), one more serves the stand-alone entry points and
+// one the calls captured into a caller's CUDA graph.  The invariant that makes calls in flight safe, in one place:
+//   * a block is all zero whenever no call that uses it is in flight: the LAST block of a call's last kernel
+//     (k_table_search) copies it to the set's report block (gamma_get_counters), zeroes it, and only then publishes
+//     the call as done (SeqP::done = k + 1);
+//   * calls are published in call order (that last block first waits for done == k), so "the last kernel of call k
+//     has completed" implies "every earlier call has completed": stream order as the caller sees it is kept;
+//   * the first kernel of call k (k_norm) does not write its block before done >= k + 1 - CTL_ROT, i.e. before the
+//     previous user of the set has been published, and nothing else of call k starts before k_norm has completed.
+constexpr int CTL_ROT = 4, CTL_STANDALONE = 4, CTL_CAPTURE = 5, CTL_SLOTS = 6;
 constexpr int KEY_DIGITS = 256;
 struct Ctl {
     unsigned normOrd;      // max(ref) as an order-preserving uint
@@ -66,11 +75,18 @@ struct Ctl {
     int box[3];            // table box: m_a in [0, box_a)
     unsigned sortN;        // element count for gamma_sort_pairs
     unsigned nDeep;        // depth-class lists (presort 4): items in the deep list
-    unsigned pad0_;
+    unsigned blocksDone;   // blocks of the call's last kernel that have finished (the last one publishes the call)
     float invGlobal;       // 1 / (DD * D_norm) rounded to fp32 (global criterion), written by k_classify
     unsigned long long visits;       // owner vertices evaluated by the table search
     unsigned hist[KEY_DIGITS];       // digit histogram of the search list (bucket presort)
     unsigned cursor[KEY_DIGITS];     // scatter cursors of the bucket presort
+};
+
+// Sequencing of the calls of one workspace (one word per workspace, never cleared by the kernels).
+struct SeqP {
+    unsigned* done;   // device word: number of calls published so far; nullptr = this call is not sequenced
+    unsigned seq;     // this call's number k
+    unsigned need;    // k_norm writes its control block only when done >= need (signed 32-bit difference)
 };
 
 // Monotone 8-bit quantisation of a non-negative key: 32 steps per octave over [2^-3, 2^5), clamped.

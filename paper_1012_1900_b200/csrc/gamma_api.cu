@@ -86,8 +86,10 @@ struct GraphKey {
     void* ctl;
     GridP g;
     float DD, cutoff, normDose;
-    int mode, presort, star, lanes, keyBits, tableMode, algo;
+    int mode, presort, star, lanes, keyBits, tableMode, algo, statsBins;
     long long tableCap;
+    const void *statsHist, *statsSummary;
+    float statsScale;
     bool operator==(const GraphKey& o) const { return std::memcmp(this, &o, sizeof *this) == 0; }
 };
 struct GraphEntry {
@@ -96,27 +98,52 @@ struct GraphEntry {
     unsigned long long lastUse = 0;
     int kernels = 0;
 };
-constexpr int GRAPH_CACHE = 96;    // argument sets x 3 rotating control-block slots
-// control-block slots: 0/1/2 rotate between calls (the first kernel of call i clears the slot of call i+1 and may run
-// while call i-1 is still finishing), 3 stand-alone entry points, 4 calls captured by the caller
-constexpr int CTL_ROT = 3, CTL_STANDALONE = 3, CTL_CAPTURE = 4, CTL_SLOTS = 5;
+constexpr int GRAPH_CACHE = 96;    // argument sets x CTL_ROT rotating sets
+
+// Byte ranges a call in flight reads and writes, for the hazard check of pipelined calls.
+struct Span {
+    const char *b = nullptr, *e = nullptr;
+    void set(const void* p, size_t bytes) { b = static_cast<const char*>(p); e = p ? b + bytes : b; }
+    bool hits(const Span& o) const { return b && o.b && b < o.e && o.b < e; }
+};
+struct CallSpans {
+    Span rd[2];   // ref, eval
+    Span wr[3];   // out_gamma, stats hist, stats summary
+    bool conflicts(const CallSpans& next) const     // `next` starts while this call is still running
+    {
+        for (const Span& w : wr) {
+            for (const Span& r : next.rd) if (w.hits(r)) return true;   // next reads what this call writes
+            for (const Span& x : next.wr) if (w.hits(x)) return true;   // both write
+        }
+        for (const Span& r : rd)
+            for (const Span& x : next.wr) if (r.hits(x)) return true;   // next writes what this call reads
+        return false;
+    }
+};
 
 struct Workspace {
-    Buf ctl;                       // Ctl
-    Buf evalIdx;                   // compacted indices of the evaluated voxels
-    Buf key0, idx0, key1, idx1;    // search work list, ping-pong for the sort
+    // ctl: Ctl[CTL_SLOTS] control blocks, Ctl[CTL_SLOTS] reports (copy of the block at the end of the call, for
+    // gamma_get_counters), one u32 "calls published" word (SeqP, common.cuh)
+    Buf ctl;
+    // work lists, `sets` copies of `stride` elements each (set s at element s * stride): compacted indices of the
+    // evaluated voxels; ring / sorted list (key0, idx0); deep list or sort ping-pong (key1, idx1)
+    Buf evalIdx, key0, idx0, key1, idx1;
+    long long stride = 0;
+    int sets = 0;
+    Buf sortK, sortV;              // ping-pong of gamma_sort_pairs (stand-alone)
     Buf tileHist;                  // radix sort
-    Buf table, tmpL, tmpIdx;       // offset table
-    Buf hRef, hEval, hOut;         // device staging of gamma_eval_host
+    Buf table, tmpL, tmpIdx;       // offset table: CTL_SLOTS embedded tables, then the large (side-stream) table
+    Buf hRef, hEval, hOut;         // device staging of gamma_eval_host / gamma_eval_host_batch
+    Buf count;                     // evaluated-voxel count of the two-phase path (large grids)
     cudaEvent_t done = nullptr;    // orders consecutive calls that share this workspace
     bool havePending = false;
     cudaEvent_t stage[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // opts.profile_stages
-    cudaStream_t aux = nullptr;    // side stream: the offset table is built while k_prep_star runs
+    cudaStream_t aux = nullptr;    // side stream: the large offset table is built while k_star runs
     cudaEvent_t evFork = nullptr, evJoin = nullptr;
     void* ctlOwner = nullptr;      // ctl.p the flags below refer to
-    bool ctlClean = false;         // both call slots of the control block are known to be zero / being zeroed
-    int slot = 0;                  // control-block slot of the next call (0/1); slot 2: stand-alone entry points
-    void* lastCtl = nullptr;
+    bool ctlClean = false;         // control blocks zero / being zeroed by the calls in flight, sequence word consistent
+    unsigned seq = 0;              // number of the next sequenced call (its set is seq % CTL_ROT)
+    void* lastCtl = nullptr;       // report block of the last call
     bool haveStages = false;
     bool stageSort = false, stageTable = false;   // the last profiled call had a sort kernel / a side-stream table
     long long launches = 0;        // kernels launched so far (gamma_launch_count)
@@ -124,6 +151,7 @@ struct Workspace {
     int occStar[2] = {0, 0};       // resident blocks per SM of k_star<false/true>
     int pdl = -1;                  // programmatic dependent launch between the kernels of a call (GAMMA_PDL=0 disables)
     int graphs = -1;               // replay the call as a cached CUDA graph (GAMMA_GRAPH=0 disables)
+    bool frozen = false;           // addresses of this workspace are baked into a caller's CUDA graph: it must not move
     cudaStream_t cap = nullptr;    // capture stream (the caller's may be the legacy default stream, which cannot capture)
     GraphEntry graph[GRAPH_CACHE];
     int numGraphs = 0;
@@ -137,15 +165,24 @@ struct Workspace {
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
     cudaStream_t doneStream = nullptr;   // stream of the last work that used this workspace
-    bool chainable = false;              // that work was a pipeline ending in k_table_search (which triggers dependents)
-    const char* lastOutBegin = nullptr;  // its out_gamma range: a next call that reads it must not start early
-    const char* lastOutEnd = nullptr;
+    bool chainable = false;              // that work was a sequenced pipeline ending in k_table_search
+    long long chainStride = 0;           // list layout of the calls in flight
+    CallSpans recent[CTL_ROT];           // what the last CTL_ROT - 1 calls read and write (slot = seq % CTL_ROT)
     int lastClasses = 0;           // last call used depth classes: list A holds the ring items
     long long lastN = 0;
     bool haveLast = false;
+    size_t bytes() const
+    {
+        const Buf* all[] = {&ctl, &evalIdx, &key0, &idx0, &key1, &idx1, &sortK, &sortV, &tileHist, &table, &tmpL, &tmpIdx,
+                            &hRef, &hEval, &hOut, &count};
+        size_t n = 0;
+        for (const Buf* b : all) n += b->cap;
+        return n;
+    }
     void releaseAll()
     {
-        Buf* all[] = {&ctl, &evalIdx, &key0, &idx0, &key1, &idx1, &tileHist, &table, &tmpL, &tmpIdx, &hRef, &hEval, &hOut};
+        Buf* all[] = {&ctl, &evalIdx, &key0, &idx0, &key1, &idx1, &sortK, &sortV, &tileHist, &table, &tmpL, &tmpIdx,
+                      &hRef, &hEval, &hOut, &count};
         for (Buf* b : all) b->release();
         if (done) { cudaEventDestroy(done); done = nullptr; }
         for (cudaEvent_t& ev : stage)
@@ -156,13 +193,18 @@ struct Workspace {
         if (evFork) { cudaEventDestroy(evFork); evFork = nullptr; }
         if (evJoin) { cudaEventDestroy(evJoin); evJoin = nullptr; }
         havePending = false; haveLast = false; haveStages = false; ctlClean = false; ctlOwner = nullptr;
+        chainable = false; frozen = false; stride = 0; sets = 0; seq = 0;
+        for (CallSpans& c : recent) c = CallSpans();
     }
 };
 
 // Workspace 0 serves the single-case entry points; 1 .. BATCH_LANES serve gamma_eval_batch, one per lane (own stream,
-// own control block, lists and table), so that the kernels of different cases overlap on the device.
+// own control blocks, lists and tables), so that the kernels of different cases overlap on the device; the last one
+// belongs to the calls a caller captures into its own CUDA graph (its addresses are baked into that graph, so it never
+// moves once used: gamma_release() is the only way to grow it).
 constexpr int BATCH_LANES = 4;
-Workspace g_pool[1 + BATCH_LANES];
+constexpr int WS_CAPTURE = 1 + BATCH_LANES;
+Workspace g_pool[2 + BATCH_LANES];
 Workspace* g_cur = &g_pool[0];
 #define g_ws (*g_cur)
 struct BatchLanes {
@@ -350,16 +392,30 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
 }
 
 struct Resolved {
-    int presort, star, lanes, keyBits, profile, graph, tableMode, algo;
+    int presort, star, lanes, keyBits, profile, graph, tableMode, algo, backToBack;
     long long tableCap;
     float normDose;
+    StatsP stats;      // a6 fused into the gamma kernels (hist == nullptr: off)
 };
 
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
     r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 0; r.tableMode = 1; r.normDose = 0.0f;
-    r.profile = 0; r.graph = 0; r.algo = 0;
+    r.profile = 0; r.graph = 0; r.algo = 0; r.backToBack = 0;
+    r.stats.hist = nullptr; r.stats.summary = nullptr; r.stats.nbins = 0; r.stats.binScale = 0.0f;
     if (!o) { r.tableCap = TAB_EMBED_MAX_CELLS; return GAMMA_OK; }
+    if (o->back_to_back < 0 || o->back_to_back > 1) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.back_to_back must be 0 or 1");
+    r.backToBack = o->back_to_back;
+    if (o->stats_hist || o->stats_summary) {
+        if (!o->stats_hist || !o->stats_summary)
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.stats_hist and opts.stats_summary must be given together");
+        if (o->stats_nbins < 1 || o->stats_nbins > FUSED_MAX_BINS)
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.stats_nbins must be in [1, 1024] (gamma_stats takes up to 4096)");
+        if (!(o->stats_hist_max > 0.0f) || !std::isfinite(o->stats_hist_max))
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.stats_hist_max must be > 0");
+        r.stats.hist = o->stats_hist; r.stats.summary = o->stats_summary; r.stats.nbins = o->stats_nbins;
+        r.stats.binScale = (float)o->stats_nbins / o->stats_hist_max;
+    }
     r.profile = o->profile_stages == 1;
     if (o->graph < 0 || o->graph > 2) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.graph must be 0, 1 or 2");
     r.graph = o->graph == 1;
@@ -407,20 +463,40 @@ int check_criteria(float DD, int mode, float cutoff)
     return GAMMA_OK;
 }
 
+constexpr size_t CTL_BYTES = 2 * CTL_SLOTS * sizeof(Ctl) + 16;   // control blocks, reports, sequence word
+
+// Grids up to this many voxels get their work lists sized by N, CTL_ROT sets of them (consecutive calls in flight);
+// larger grids count their evaluated voxels first (one host read of 4 bytes on a call of milliseconds) and get ONE
+// set of lists sized by M.
+constexpr long long LISTS_BY_N_MAX = 1ll << 25;
+
 // Workspace of one call: allocations, side stream, events.  Nothing is allocated once the sizes have been seen.
-int prepare_workspace(const GridP& g, const Resolved& r)
+// `sets` x `stride`: layout of the work lists this call needs.
+int prepare_workspace(const GridP& g, const Resolved& r, int sets, long long stride)
 {
     int rc = ensure_device();
     if (rc) return rc;
-    const long long N = g.N;
-    const long long maxTiles = (N + SORT_TILE - 1) / SORT_TILE;
-    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
-    CU_TRY(g_ws.key0.need(N * 4)); CU_TRY(g_ws.idx0.need(N * 4)); CU_TRY(g_ws.evalIdx.need(N * 4));
-    if (r.presort) { CU_TRY(g_ws.key1.need(N * 4)); CU_TRY(g_ws.idx1.need(N * 4)); }
+    const long long maxTiles = (stride + SORT_TILE - 1) / SORT_TILE;
+    const size_t ctlBytes = CTL_BYTES;
+    const size_t listBytes = (size_t)sets * (size_t)stride * 4;
+    const size_t tableCells = (size_t)CTL_SLOTS * TAB_EMBED_MAX_CELLS + (r.tableCap > TAB_EMBED_MAX_CELLS ? (size_t)r.tableCap : 0);
+    if (g_ws.frozen) {
+        const bool fits = ctlBytes <= g_ws.ctl.cap && listBytes <= g_ws.evalIdx.cap && listBytes <= g_ws.key1.cap &&
+                          tableCells * 16 <= g_ws.table.cap && (size_t)r.tableCap * 4 <= g_ws.tmpL.cap &&
+                          (r.presort != 3 || (size_t)maxTiles * SORT_RADIX * 4 <= g_ws.tileHist.cap);
+        if (!fits)
+            return fail(GAMMA_ERR_INVALID_ARGUMENT,
+                        "this call needs a larger capture workspace, but its addresses are part of a captured CUDA graph; "
+                        "call gamma_release() first (that invalidates the captured graphs)");
+    }
+    CU_TRY(g_ws.ctl.need(ctlBytes));
+    CU_TRY(g_ws.key0.need(listBytes)); CU_TRY(g_ws.idx0.need(listBytes)); CU_TRY(g_ws.evalIdx.need(listBytes));
+    CU_TRY(g_ws.key1.need(listBytes)); CU_TRY(g_ws.idx1.need(listBytes));
+    g_ws.stride = stride; g_ws.sets = sets;
     if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
-    // the small embedded table exists once per rotating control-block slot: the next call may build its own while this
-    // call's search still walks this one
-    CU_TRY(g_ws.table.need((size_t)(r.tableCap > CTL_SLOTS * TAB_EMBED_MAX_CELLS ? r.tableCap : CTL_SLOTS * TAB_EMBED_MAX_CELLS) * 16));
+    // the small embedded table exists once per control-block slot (the next call builds its own while this call's
+    // search still walks this one); a large table (table_radius 2, table_cap > 1024) lives BEHIND those slots
+    CU_TRY(g_ws.table.need(tableCells * 16));
     CU_TRY(g_ws.tmpL.need((size_t)r.tableCap * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)r.tableCap * 4));
     if (!g_ws.aux) {
         CU_TRY(cudaStreamCreateWithFlags(&g_ws.aux, cudaStreamNonBlocking));
@@ -450,23 +526,51 @@ int prepare_workspace(const GridP& g, const Resolved& r)
     return GAMMA_OK;
 }
 
+// The control-block buffer exists and is zero where nothing is in flight; after a call that failed half-way nothing is
+// known about the blocks or the sequence word: wait for the device and start over.
+int ensure_ctl(cudaStream_t st)
+{
+    if (g_ws.ctl.p && g_ws.ctl.p == g_ws.ctlOwner && g_ws.ctlClean) return GAMMA_OK;
+    CU_TRY(g_ws.ctl.need(CTL_BYTES));
+    if (g_ws.ctlOwner) CU_TRY(cudaDeviceSynchronize());
+    CU_TRY(cudaMemsetAsync(g_ws.ctl.p, 0, CTL_BYTES, st));
+    g_ws.ctlOwner = g_ws.ctl.p;
+    g_ws.ctlClean = true;
+    g_ws.seq = 0;
+    g_ws.chainable = false;
+    for (CallSpans& c : g_ws.recent) c = CallSpans();
+    return GAMMA_OK;
+}
+
+// What a call's kernels are told about where they run.
+struct CallSlot {
+    int slot;          // control-block / embedded-table slot
+    int set;           // work-list set
+    SeqP seq;          // sequencing of the call (done == nullptr: not sequenced)
+    int waitFirst;     // k_norm waits for the operation in front of it before it reads ref / eval
+    bool early;        // k_norm is launched as a programmatic dependent of the previous call's k_table_search
+    bool skipNorm;     // two-phase path: k_norm already ran (and the host has read the evaluated-voxel count)
+};
+
 // The kernels of one call on `st` (which may be capturing).  Returns the number of kernels in *launched.
 //
 //   st :  k_norm -> k_classify -> k_star -> [k_bucket_scatter | LSD radix sort] -> (join) -> k_table_search
-//   aux:                    \-> k_offset_table ------------------------------------/
+//   aux:                    \-> k_offset_table ------------------------------------/     (large tables only)
 //
-// The offset table only needs k_norm's maxima, so it is built on a library-owned side stream while the
-// star kernel runs.  No memset and no host synchronisation on the path: k_norm clears the control
-// block of the next call (two alternating slots; slot 2 belongs to the stand-alone entry points).
+// No memset and no host synchronisation on the path: the last block of k_table_search leaves the control block
+// zeroed for the next user of the set (common.cuh, "Device control block").
 int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
-                    const Resolved& r, float* out, cudaStream_t st, Ctl* ctl, Ctl* next, int* launched, bool early,
-                    int slot)
+                    const Resolved& r, float* out, cudaStream_t st, const CallSlot& cs, int* launched)
 {
     const long long N = g.N;
     int nk = 0;
-    unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p), *i0 = static_cast<unsigned*>(g_ws.idx0.p);
-    unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *i1 = static_cast<unsigned*>(g_ws.idx1.p);
-    unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p);
+    Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
+    Ctl* ctl = base + cs.slot;
+    Ctl* report = base + CTL_SLOTS + cs.slot;
+    const size_t off = (size_t)cs.set * (size_t)g_ws.stride;
+    unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p) + off, *i0 = static_cast<unsigned*>(g_ws.idx0.p) + off;
+    unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p) + off, *i1 = static_cast<unsigned*>(g_ws.idx1.p) + off;
+    unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p) + off;
     EvalP e;
     e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
     e.algo = (r.algo == 2 && !g.all_active) ? 0 : r.algo;   // the recursion variant is written for 3D cells
@@ -476,9 +580,9 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     const int sm = g_ws.numSM;
     const bool pdl = g_ws.pdl != 0;
     STAGE_MARK(0, st);
-    // a3 on the side stream.  Default: a data-independent PREFIX of the paper's table, as large as table_cap allows,
-    // forked before k_norm so that it is ready long before the search; beyond it the search enumerates (exact).
-    // table_radius = 2: the paper's radius max |DD| / dD (A1 steps 1-2), forked once k_norm's maxima exist.
+    // a3.  Default: a data-independent PREFIX of the paper's table, as large as table_cap allows; beyond it the search
+    // enumerates (exact).  table_radius = 2: the paper's radius max |DD| / dD (A1 steps 1-2), built on a side stream
+    // once k_norm's maxima exist.
     // host-side constants of the geometry (table radius / plan, ring constants): kept from the last call
     struct HostGeo { GridP g; long long cap; float radius; TablePlan plan; GammaRingP ring; bool valid; };
     static thread_local HostGeo geo = {};
@@ -498,6 +602,9 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     }
     // small prefix tables are built inside k_star, by its first blocks, while they wait for k_classify
     const int embed = (r.tableMode == 1 && r.tableCap <= TAB_EMBED_MAX_CELLS) ? 1 : 0;
+    int4* const tabBase = static_cast<int4*>(g_ws.table.p);
+    int4* const tab4 = embed ? tabBase + (size_t)cs.slot * (size_t)TAB_EMBED_MAX_CELLS
+                             : tabBase + (size_t)CTL_SLOTS * (size_t)TAB_EMBED_MAX_CELLS;
     TablePlan plan;
     std::memset(&plan, 0, sizeof plan);
     if (embed) plan = geoHit ? geo.plan : table_plan_make(g, radius, r.tableCap, 1, TAB_EMBED_BUCKETS);
@@ -506,7 +613,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         CU_TRY(cudaStreamWaitEvent(g_ws.aux, g_ws.evFork, 0));
         STAGE_MARK(5, g_ws.aux);
         k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, g_ws.aux>>>(
-            g, e, ctl, radius, r.tableCap, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
+            g, e, ctl, radius, r.tableCap, tab4, static_cast<unsigned*>(g_ws.tmpL.p),
             static_cast<unsigned*>(g_ws.tmpIdx.p), r.tableMode == 1 ? 1 : 0);
         ++nk;
         STAGE_MARK(6, g_ws.aux);
@@ -514,35 +621,35 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         return GAMMA_OK;
     };
     int rc = GAMMA_OK;
-    if (r.tableMode == 1 && !embed) { rc = fork_table(); if (rc) return rc; }
-    {                                                                    // a0 + A1 step 1
+    if (!cs.skipNorm) {                                                  // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
-        // early: the previous call on this stream ended in k_table_search, which triggers its dependents at once:
-        // k_norm then runs in the tail of that call (it touches nothing of it) and waits for its end before exiting
-        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, early, false, ref, ev, (int)N, mode, ctl, next));
+        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ev, (int)N, mode,
+                         ctl, cs.seq, cs.waitFirst, r.stats));
         ++nk;
     }
+    // A large prefix table does not need k_norm's maxima; it still starts after k_norm so that the control block it
+    // writes belongs to this call (the set is free once k_norm has completed).
+    if (r.tableMode == 1 && !embed) { rc = fork_table(); if (rc) return rc; }
     {                                                                    // a1: exclusion + compaction
         long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
         int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
-        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0));
+        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0, r.stats));
         ++nk;
     }
     STAGE_MARK(1, st);
     if (r.tableMode != 1) { rc = fork_table(); if (rc) return rc; }      // paper's radius: needs k_norm's max |DD|
     {                                                                    // star phase over the compacted voxels
-        int4* tab4 = static_cast<int4*>(g_ws.table.p) + (embed ? (size_t)slot * (size_t)TAB_EMBED_MAX_CELLS : 0);
         unsigned *tabL = static_cast<unsigned*>(g_ws.tmpL.p), *tabI = static_cast<unsigned*>(g_ws.tmpIdx.p);
         long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
         const long long resident = (long long)sm * g_ws.occStar[r.star];
         int grid = (int)(blocks > resident ? resident : blocks);
         if (r.star)
             CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes,
-                             embed, plan, tab4, tabL, tabI));
+                             embed, plan, tab4, tabL, tabI, r.stats));
         else
             CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes,
-                             embed, plan, tab4, tabL, tabI));
+                             embed, plan, tab4, tabL, tabI, r.stats));
         ++nk;
     }
     STAGE_MARK(2, st);
@@ -555,7 +662,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         ++nk;
         lk = k1; li = i1;
     } else if (presort == 3) {                                         // a2: full LSD radix sort of the keys
-        int where = radix_sort_enqueue(k0, i0, k1, i1, &ctl->nSearch, N, 32 - r.keyBits, 32,
+        int where = radix_sort_enqueue(k0, i0, k1, i1, &ctl->nSearch, g_ws.stride, 32 - r.keyBits, 32,
                                        static_cast<unsigned*>(g_ws.tileHist.p), st);
         nk += 3 * (r.keyBits / 8);
         if (where) { lk = k1; li = i1; }
@@ -563,7 +670,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     if (g_ws.stageSort) STAGE_MARK(3, st);
     {                                                                    // a4 + a5
         const int grid = sm * (r.lanes == 0 ? SEARCH_MIN_BLOCKS : 4 * (256 / SEARCH_THREADS));   // resident blocks
-        const int4* tab = static_cast<const int4*>(g_ws.table.p) + (embed ? (size_t)slot * (size_t)TAB_EMBED_MAX_CELLS : 0);
+        const int4* tab = tab4;
         // adaptive lanes: an item is "deep" when its key exceeds the smallest non-zero table distance
         float hmin = 0.0f;
         for (int a = 0; a < 3; ++a)
@@ -580,103 +687,206 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         if (!geoHit && r.tableMode == 1 && g.all_active && classes) {
             geo.g = g; geo.cap = r.tableCap; geo.radius = radius; geo.plan = plan; geo.ring = ring; geo.valid = true;
         }
-        if (e.algo == 2 && r.lanes == 1)
-            CU_TRY(launch_ex(k_table_search<1, true>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
-        else if (e.algo == 2)
-            CU_TRY(launch_ex(k_table_search<0, true>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
-        else if (r.lanes == 1)
-            CU_TRY(launch_ex(k_table_search<1>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
-        else if (r.lanes == 8)
-            CU_TRY(launch_ex(k_table_search<8>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
-        else if (r.lanes == 32)
-            CU_TRY(launch_ex(k_table_search<32>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
-        else
-            CU_TRY(launch_ex(k_table_search<0>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, lk, li, k1, i1, tab, deepDigit, classes, ring));
+#define LAUNCH_SEARCH(...) CU_TRY(launch_ex(k_table_search<__VA_ARGS__>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, \
+                                            ctl, lk, li, k1, i1, tab, deepDigit, classes, ring, report, cs.seq, r.stats))
+        if (e.algo == 2 && r.lanes == 1) LAUNCH_SEARCH(1, true);
+        else if (e.algo == 2) LAUNCH_SEARCH(0, true);
+        else if (r.lanes == 1) LAUNCH_SEARCH(1);
+        else if (r.lanes == 8) LAUNCH_SEARCH(8);
+        else if (r.lanes == 32) LAUNCH_SEARCH(32);
+        else LAUNCH_SEARCH(0);
+#undef LAUNCH_SEARCH
         ++nk;
     }
     STAGE_MARK(4, st);
 #undef STAGE_MARK
     *launched = nk;
     g_ws.lastClasses = classes;
+    g_ws.lastCtl = report;
     return GAMMA_OK;
 }
 
+// a0 + count of the evaluated voxels for the two-phase path of large grids: k_norm, then k_count, then 4 bytes to the
+// host.  SYNCHRONISES `st`.
+__global__ void __launch_bounds__(256)
+k_count_eval(const float* __restrict__ ref, int N, EvalP e, const Ctl* __restrict__ ctl, unsigned* __restrict__ count)
+{
+    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
+    const double dnorm = (double)dnormF;
+    const double thr = (double)e.cutoff * dnorm;
+    const bool globalOk = (double)e.DD * dnorm > 0.0;
+    unsigned c = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        const float Dr = __ldg(ref + i);
+        const bool excluded = ((double)Dr < thr) || (e.mode == 0 ? !globalOk : !((double)e.DD * (double)Dr > 0.0));
+        c += excluded ? 0u : 1u;
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) c += __shfl_xor_sync(0xffffffffu, c, s);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(count, c);
+}
+
 // Enqueue the whole hot path on `st` (device pointers).  Caller holds g_mu.
-// A call with arguments seen before (same pointers, geometry, criteria, options, control-block slot) replays a cached
-// CUDA graph of its kernels -- one driver call instead of five launches plus the fork/join of the side stream; the
-// graph is captured on a library-owned stream on first sight.  Not used when the caller's stream is itself being
-// captured, with opts.profile_stages, or GAMMA_GRAPH=0.  Opt-in (opts.graph = 1): measured on B200, a replay costs
-// less host time (24 vs 31 us per call) but back-to-back replays do not overlap their ramp-up with the previous call's
-// tail the way stream launches do (0.055 vs 0.045 ms per cfg3 case), so stream launches stay the default.
+//
+// Calls of one workspace are SEQUENCED (common.cuh): call k uses set k % CTL_ROT and is published, in call order, by
+// the last block of its last kernel.  A call may be PIPELINED behind the previous one -- its k_norm is launched as a
+// programmatic dependent of that call's k_table_search and does not wait for it, so k_norm, k_classify and k_star run
+// beside the previous search -- when the caller asserted that nothing else was enqueued on the stream in between
+// (gamma_opts::back_to_back; the library cannot see foreign work), the previous call on this workspace was a
+// sequenced pipeline on the same stream with the same list layout, the table is the small per-set one, and nothing
+// this call reads or writes overlaps what the calls still in flight write or read.  Every other call waits, in its
+// first kernel, for the operation in front of it (and so, by the in-order publication, for every earlier call).
+//
+// opts.graph = 1: a call with arguments seen before (same pointers, geometry, criteria, options, set) replays a cached
+// CUDA graph of its kernels; not sequenced, never pipelined.  A stream that the CALLER is capturing gets the kernels
+// as nodes of the caller's graph, on the capture workspace.
 int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
                      const Resolved& r, float* out, cudaStream_t st)
 {
-    int rc = prepare_workspace(g, r);
-    if (rc) return rc;
     cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
     CU_TRY(cudaStreamIsCapturing(st, &capStatus));
-    if (capStatus != cudaStreamCaptureStatusNone) {
-        // The caller is capturing `st`: the kernels become nodes of the caller's graph.  The call must then be
-        // self-contained (its replays do not pass through this function): it owns control-block slot 3 and
-        // clears it with a memset node; ordering against other work is the captured stream's.
-        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_CAPTURE;
-        CU_TRY(cudaMemsetAsync(ctl, 0, sizeof(Ctl), st));
+    const bool capturing = capStatus != cudaStreamCaptureStatusNone;
+    const long long N = g.N;
+    int rc;
+    if (capturing) {
+        // The kernels become nodes of the caller's graph.  The call must be self-contained (its replays do not pass
+        // through this function): its own workspace (never moved afterwards), its own control block cleared by a
+        // memset node, no sequencing; ordering against other work is the captured stream's.
+        Workspace* keep = g_cur;
+        g_cur = &g_pool[WS_CAPTURE];
+        {   // cudaMalloc is not a stream operation, but a capture in "global" mode forbids it: relax for the allocation
+            cudaStreamCaptureMode cm = cudaStreamCaptureModeRelaxed;
+            cudaThreadExchangeStreamCaptureMode(&cm);
+            rc = prepare_workspace(g, r, 1, N);
+            cudaThreadExchangeStreamCaptureMode(&cm);
+        }
+        if (rc == GAMMA_OK) {
+            g_ws.frozen = true;
+            Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_CAPTURE;
+            cudaError_t ce = cudaMemsetAsync(ctl, 0, sizeof(Ctl), st);
+            if (ce != cudaSuccess) rc = fail(GAMMA_ERR_CUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(ce));
+        }
         int launched = 0;
-        Resolved rr = r;
-        rr.profile = 0;
-        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, rr, out, st, ctl, nullptr, &launched, false, CTL_CAPTURE);
-        if (rc) return rc;
-        g_ws.launches += launched;
-        g_ws.haveStages = false;
-        g_ws.chainable = false;
-        g_ws.lastCtl = ctl; g_ws.lastStream = nullptr; g_ws.lastN = g.N; g_ws.haveLast = true;
-        return GAMMA_OK;
+        if (rc == GAMMA_OK) {
+            Resolved rr = r;
+            rr.profile = 0;
+            CallSlot cs;
+            cs.slot = CTL_CAPTURE; cs.set = 0; cs.seq.done = nullptr; cs.seq.seq = 0; cs.seq.need = 0;
+            cs.waitFirst = 1; cs.early = false; cs.skipNorm = false;
+            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, rr, out, st, cs, &launched);
+        }
+        if (rc == GAMMA_OK) {
+            g_ws.launches += launched;
+            g_ws.haveStages = false;
+            g_ws.lastStream = nullptr; g_ws.lastN = g.N; g_ws.haveLast = true;
+        }
+        Workspace* used = g_cur;
+        g_cur = keep;
+        if (rc == GAMMA_OK) {                       // gamma_get_counters reports on the captured call
+            g_ws.haveLast = true; g_ws.lastCtl = used->lastCtl; g_ws.lastStream = nullptr; g_ws.lastN = g.N;
+            g_ws.lastClasses = used->lastClasses; g_ws.haveStages = false;
+        }
+        return rc;
     }
-    // May the first kernel start while the previous call on this stream is finishing?  Only behind one of our own
-    // pipelines on the same stream, with a clean control block, the small embedded table (one per slot), no profiling,
-    // and inputs that do not overlap what that call is still writing.
-    const size_t bytes = (size_t)g.N * 4;
-    auto overlaps = [&](const void* p) {
-        const char* a = static_cast<const char*>(p);
-        return g_ws.lastOutBegin && a < g_ws.lastOutEnd && a + bytes > g_ws.lastOutBegin;
-    };
-    static const bool overlapCalls = !(std::getenv("GAMMA_OVERLAP_CALLS") && std::getenv("GAMMA_OVERLAP_CALLS")[0] == '0');
-    const bool early = overlapCalls && g_ws.pdl != 0 && g_ws.chainable && g_ws.havePending && g_ws.doneStream == st &&
-                       g_ws.ctlClean && g_ws.ctl.p == g_ws.ctlOwner && !r.profile && r.tableMode == 1 &&
-                       r.tableCap <= TAB_EMBED_MAX_CELLS && !overlaps(ref) && !overlaps(ev);
+    // ---- layout of the work lists
+    long long byNMax = LISTS_BY_N_MAX;
+    if (const char* env = std::getenv("GAMMA_LISTS_BY_N_MAX")) byNMax = std::atoll(env);   // tests: two-phase path on small grids
+    const bool twoPhase = N > byNMax;
+    const bool useGraph = g_ws.graphs != 0 && r.graph && !r.profile && !twoPhase;
+    int sets = CTL_ROT;
+    long long stride = N;
+    EvalP e0p;
+    e0p.DD = DD; e0p.cutoff = cutoff; e0p.norm_dose = r.normDose; e0p.mode = mode; e0p.algo = 0;
     rc = order_after_previous(st);
     if (rc) return rc;
-    if (g_ws.ctl.p != g_ws.ctlOwner) { g_ws.ctlClean = false; g_ws.ctlOwner = g_ws.ctl.p; }
-    if (!g_ws.ctlClean) {                                  // first call, or a previous call failed half-way
-        CU_TRY(cudaMemsetAsync(g_ws.ctl.p, 0, CTL_SLOTS * sizeof(Ctl), st));
-        g_ws.slot = 0;
-    }
+    // control blocks: zero at the start, and again whenever a previous call failed half-way (then nothing is known
+    // about the sequence word either: wait for the device, start over)
+    rc = ensure_device();
+    if (rc) return rc;
+    rc = ensure_ctl(st);
+    if (rc) return rc;
     g_ws.ctlClean = false;                                 // set again when everything below was enqueued
-    Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
-    Ctl* ctl = base + g_ws.slot;
-    Ctl* next = base + (g_ws.slot + 1) % CTL_ROT;
+    unsigned* doneWord = reinterpret_cast<unsigned*>(static_cast<char*>(g_ws.ctl.p) + 2 * CTL_SLOTS * sizeof(Ctl));
+    CallSlot cs;
+    cs.skipNorm = false;
+    if (twoPhase) {
+        // a0, then the count of evaluated voxels, read by the host: the lists are sized by M, one set, no pipelining
+        rc = ensure_device();
+        if (rc) return rc;
+        CU_TRY(g_ws.count.need(16));
+        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + (g_ws.seq % CTL_ROT);
+        CU_TRY(cudaMemsetAsync(g_ws.count.p, 0, 16, st));
+        SeqP sq;
+        sq.done = doneWord; sq.seq = g_ws.seq; sq.need = g_ws.seq;     // every earlier call has been published
+        const int sm = g_ws.numSM;
+        CU_TRY(launch_ex(k_norm, sm * 4, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, ctl, sq, 1, r.stats));
+        k_count_eval<<<sm * 8, 256, 0, st>>>(ref, (int)N, e0p, ctl, static_cast<unsigned*>(g_ws.count.p));
+        unsigned M = 0;
+        CU_TRY(cudaMemcpyAsync(&M, g_ws.count.p, 4, cudaMemcpyDeviceToHost, st));
+        CU_TRY(cudaStreamSynchronize(st));
+        g_ws.launches += 2;
+        sets = 1;
+        stride = (long long)M + 1024;
+        cs.skipNorm = true;
+    }
+    if ((long long)g_ws.sets * g_ws.stride >= (long long)sets * stride && g_ws.stride >= stride && !twoPhase &&
+        g_ws.sets >= sets) {
+        sets = g_ws.sets; stride = g_ws.stride;            // the layout in place is large enough: keep it (pipelining)
+    }
+    rc = prepare_workspace(g, r, sets, stride);
+    if (rc) return rc;
+    const int slot = (int)(g_ws.seq % CTL_ROT);
+    cs.slot = slot;
+    cs.set = sets == 1 ? 0 : slot;
+    // ---- may this call be pipelined behind the previous one?
+    CallSpans mine;
+    const size_t bytes = (size_t)N * 4;
+    mine.rd[0].set(ref, bytes); mine.rd[1].set(ev, bytes); mine.wr[0].set(out, bytes);
+    mine.wr[1].set(r.stats.hist, (size_t)r.stats.nbins * 8); mine.wr[2].set(r.stats.summary, sizeof(gamma_summary));
+    static const bool overlapCalls = !(std::getenv("GAMMA_OVERLAP_CALLS") && std::getenv("GAMMA_OVERLAP_CALLS")[0] == '0');
+    const bool embed = r.tableMode == 1 && r.tableCap <= TAB_EMBED_MAX_CELLS;
+    bool early = overlapCalls && r.backToBack && g_ws.pdl != 0 && g_ws.chainable && g_ws.havePending &&
+                 g_ws.doneStream == st && !r.profile && !useGraph && !twoPhase && embed && sets == CTL_ROT &&
+                 g_ws.chainStride == stride;
+    if (early)
+        for (int back = 1; back < CTL_ROT && early; ++back) {
+            if (g_ws.seq < (unsigned)back) break;
+            if (g_ws.recent[(g_ws.seq - back) % CTL_ROT].conflicts(mine)) early = false;
+        }
+    cs.early = early;
+    cs.waitFirst = early ? 0 : 1;
+    const bool sequenced = !useGraph;
+    cs.seq.done = sequenced ? doneWord : nullptr;
+    cs.seq.seq = g_ws.seq;
+    // pipelined: the set must be free (call seq - CTL_ROT published).  Not pipelined: k_norm has waited for the
+    // previous kernel, hence for every earlier call: nothing to poll (need = 0 is always met: done - 0 >= 0 ... the
+    // comparison is a signed 32-bit difference, so pass the value that is certainly reached).
+    cs.seq.need = early ? g_ws.seq - (unsigned)(CTL_ROT - 1) : g_ws.seq;
+    if (early && g_ws.seq < (unsigned)(CTL_ROT - 1)) cs.seq.need = 0;
     g_ws.haveStages = false;
 
-    const bool useGraph = g_ws.graphs != 0 && r.graph && !r.profile;
     int launched = 0;
     if (!useGraph) {
-        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, ctl, next, &launched, early, g_ws.slot);
+        rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, cs, &launched);
         if (rc) return rc;
     } else {
         if (g_ws.graphGen != g_allocGen) { g_ws.dropGraphs(); g_ws.graphGen = g_allocGen; }
+        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + slot;
         GraphKey key;
         std::memset(&key, 0, sizeof key);
         key.ref = ref; key.ev = ev; key.out = out; key.ctl = ctl; key.g = g;
         key.DD = DD; key.cutoff = cutoff; key.normDose = r.normDose;
         key.mode = mode; key.presort = r.presort; key.star = r.star; key.lanes = r.lanes; key.keyBits = r.keyBits;
         key.tableCap = r.tableCap; key.tableMode = r.tableMode; key.algo = r.algo;
+        key.statsHist = r.stats.hist; key.statsSummary = r.stats.summary; key.statsBins = r.stats.nbins;
+        key.statsScale = r.stats.binScale;
         GraphEntry* hit = nullptr;
         for (int i = 0; i < g_ws.numGraphs; ++i)
             if (g_ws.graph[i].key == key) { hit = &g_ws.graph[i]; break; }
         if (!hit) {
             cudaGraph_t graph = nullptr;
             CU_TRY(cudaStreamBeginCapture(g_ws.cap, cudaStreamCaptureModeThreadLocal));
-            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, g_ws.cap, ctl, next, &launched, false, g_ws.slot);
+            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, g_ws.cap, cs, &launched);
             cudaError_t ce = cudaStreamEndCapture(g_ws.cap, &graph);
             if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
             if (ce != cudaSuccess) return fail(GAMMA_ERR_CUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(ce));
@@ -698,6 +908,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         }
         hit->lastUse = ++g_ws.useClock;
         launched = hit->kernels;
+        g_ws.lastCtl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_SLOTS + slot;
         CU_TRY(cudaGraphLaunch(hit->exec, st));
     }
     g_ws.launches += launched;
@@ -705,11 +916,12 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     CU_TRY(cudaGetLastError());
     rc = mark_done(st);
     if (rc) return rc;
-    g_ws.chainable = true;
-    g_ws.lastOutBegin = reinterpret_cast<const char*>(out);
-    g_ws.lastOutEnd = g_ws.lastOutBegin + bytes;
-    g_ws.lastCtl = ctl;
-    g_ws.slot = (g_ws.slot + 1) % CTL_ROT;
+    g_ws.chainable = sequenced && sets == CTL_ROT;
+    g_ws.chainStride = stride;
+    if (sequenced) {
+        g_ws.recent[g_ws.seq % CTL_ROT] = mine;
+        ++g_ws.seq;
+    }
     g_ws.ctlClean = true;
     g_ws.lastStream = st; g_ws.lastN = g.N; g_ws.haveLast = true;
     return GAMMA_OK;
@@ -783,11 +995,16 @@ int gamma_eval_batch(int n_cases, const float* const* ref, const float* const* e
     CU_TRY(cudaEventRecord(g_lanes.start, st));                       // the lanes start after what is already on `stream`
     for (int l = 0; l < lanes; ++l) CU_TRY(cudaStreamWaitEvent(g_lanes.stream[l], g_lanes.start, 0));
     rc = GAMMA_OK;
+    r.stats.hist = nullptr; r.stats.summary = nullptr;                // one pair of buffers cannot serve n cases
     for (int i = 0; i < n_cases && rc == GAMMA_OK; ++i) {
         const int l = i % lanes;
         GridP g;
         make_grid(dims + 3 * i, spacing_mm + 3 * i, DTA_mm, g);
         g_cur = &g_pool[1 + l];
+        // The lane streams are the library's own: behind the first case of a lane (which waits for `stream`) its
+        // calls are back to back by construction, so they are pipelined (hazards between the cases' buffers are
+        // checked as for any pipelined call).
+        r.backToBack = i >= lanes ? 1 : 0;
         rc = enqueue_pipeline(ref[i], eval[i], g, DD, mode, low_dose_cutoff, r, out_gamma[i], g_lanes.stream[l]);
         g_cur = &g_pool[0];
     }
@@ -815,6 +1032,7 @@ int gamma_eval_host(const float* ref_host, const float* eval_host, const int dim
     Resolved r;
     rc = resolve_opts(opts, r);
     if (rc) return rc;
+    r.backToBack = 0;                                    // the copies sit between consecutive calls
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::lock_guard<std::mutex> lock(g_mu);
     const size_t bytes = (size_t)g.N * 4;
@@ -875,14 +1093,15 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const long long maxTiles = (n + SORT_TILE - 1) / SORT_TILE;
-    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
-    CU_TRY(g_ws.key1.need(n * 4)); CU_TRY(g_ws.idx1.need(n * 4));
+    rc = ensure_ctl(st);
+    if (rc) return rc;
+    CU_TRY(g_ws.sortK.need(n * 4)); CU_TRY(g_ws.sortV.need(n * 4));
     CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
     rc = order_after_previous(st);
     if (rc) return rc;
     Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_STANDALONE;
     k_set_u32<<<1, 1, 0, st>>>(&ctl->sortN, (unsigned)n);
-    unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *v1 = static_cast<unsigned*>(g_ws.idx1.p);
+    unsigned *k1 = static_cast<unsigned*>(g_ws.sortK.p), *v1 = static_cast<unsigned*>(g_ws.sortV.p);
     int where = radix_sort_enqueue(keys, vals, k1, v1, &ctl->sortN, n, begin_bit, end_bit,
                                    static_cast<unsigned*>(g_ws.tileHist.p), st);
     g_ws.launches += 1 + 3 * ((end_bit - begin_bit) / 8);
@@ -924,7 +1143,8 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
+    rc = ensure_ctl(st);
+    if (rc) return rc;
     CU_TRY(g_ws.table.need((size_t)max_entries * 16));
     CU_TRY(g_ws.tmpL.need((size_t)max_entries * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)max_entries * 4));
     CU_TRY(cudaFuncSetAttribute(k_offset_table, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TAB_DYN_SMEM));
@@ -995,6 +1215,14 @@ long long gamma_launch_count(void)
     return n;
 }
 
+long long gamma_workspace_bytes(void)
+{
+    std::lock_guard<std::mutex> lock(g_mu);
+    size_t n = 0;
+    for (const Workspace& w : g_pool) n += w.bytes();
+    return (long long)n;
+}
+
 int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
 {
     g_err.clear();
@@ -1003,7 +1231,8 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
     int rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    CU_TRY(g_ws.ctl.need(CTL_SLOTS * sizeof(Ctl)));
+    rc = ensure_ctl(st);
+    if (rc) return rc;
     cudaEvent_t a, b;
     CU_TRY(cudaEventCreate(&a)); CU_TRY(cudaEventCreate(&b));
     const int grid = g_ws.numSM * 8 * 4, threads = 256;

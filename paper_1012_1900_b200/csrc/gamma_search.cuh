@@ -2,7 +2,8 @@
 //
 //   k_norm           a0 + A1 step 1: D_norm = max(ref) (reading 8) and max |D_r - D_e|,
 //                    which bounds every key and so fixes the radius of the offset table before the search
-//                    list exists; also clears the control block of the NEXT call.
+//                    list exists; zeroes the caller's fused-statistics buffers; holds the call back until its
+//                    set of work lists is free (SeqP, common.cuh).
 //   k_classify       a1: cutoff decision, NaN for excluded voxels, compaction of the evaluated voxels.
 // Consecutive kernels of a call are chained by programmatic dependent launch (pdl_wait / pdl_launch_dependents).
 //   k_prep_star      a1 + first part of a4: per voxel DD, cutoff, key (Algorithm A2 step 2 / CUDA Kernel 1,
@@ -23,6 +24,7 @@
 #include "features_generated.cuh"
 #include "offset_table.cuh"
 #include "ju_simplex.cuh"
+#include "stats.cuh"
 
 namespace gamma_b200 {
 
@@ -58,13 +60,22 @@ __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepc
 
 
 __global__ void __launch_bounds__(NORM_THREADS)
-k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur,
-       Ctl* __restrict__ next)
+k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur, SeqP seq,
+       int waitFirst, StatsP st)
 {
     pdl_launch_dependents();
-    if (blockIdx.x == gridDim.x - 1 && next != nullptr) {      // the next call finds its control block cleared
-        unsigned* w = reinterpret_cast<unsigned*>(next);
-        for (int i = threadIdx.x; i < (int)(sizeof(Ctl) / 4); i += NORM_THREADS) w[i] = 0u;
+    // waitFirst: ref / eval may be results of the operation in front of this call: nothing is read before that
+    // operation has completed.  Otherwise (the caller asserted back-to-back library calls, gamma_opts::back_to_back)
+    // this kernel runs beside the previous call's table search: it reads this call's inputs only and touches the
+    // control block of its own set once that set is free.
+    if (waitFirst) pdl_wait();
+    if (st.hist) {                                              // a6 fused: the caller's buffers start from zero
+        for (int b = blockIdx.x * NORM_THREADS + threadIdx.x; b < st.nbins; b += gridDim.x * NORM_THREADS) st.hist[b] = 0ull;
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            gamma_summary z;
+            z.n_eval = 0; z.n_pass = 0; z.sum_gamma = 0.0; z.sum_gamma3 = 0.0; z.max_gamma = 0.0f; z.n_nan = 0; z.pad_ = 0;
+            *st.summary = z;
+        }
     }
     float m = -INFINITY, a = 0.0f, r = 0.0f;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
@@ -101,13 +112,14 @@ k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int m
     a = block_max_256(a, sm8);
     if (mode == 1) r = block_max_256(r, sm8);
     if (threadIdx.x == 0) {
+        // The set (control block, table, work lists) this call uses was last used by call seq - CTL_ROT: wait until
+        // that call has been published (its last block has zeroed the control block).  Every block of an earlier
+        // kernel in the stream is resident or done when this kernel starts, so the wait cannot deadlock.
+        if (seq.done)
+            while ((int)(ld_acquire_u32(seq.done) - seq.need) < 0) __nanosleep(64);
         atomicMax(&cur->normOrd, float_to_ordered(m));
         if (a > 0.0f) atomicMax(&cur->maxAbsDD, __float_as_uint(a));
         if (r > 0.0f) atomicMax(&cur->maxRatio, __float_as_uint(r));
-        // Launched behind the previous call's k_table_search with programmatic dependent launch, this kernel has run
-        // in that call's tail; it must not END before that call has (the kernels after it reuse its work lists).
-        // One block holds the grid open; the others give their registers back at once.
-        if (blockIdx.x == 0) pdl_wait();
     }
 }
 
@@ -127,10 +139,13 @@ __device__ __forceinline__ float criterion_inv_dD(const EvalP& e, double dnorm, 
 
 __global__ void __launch_bounds__(PREP_THREADS)
 k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, EvalP e, Ctl* __restrict__ ctl,
-           unsigned* __restrict__ evalIdx)
+           unsigned* __restrict__ evalIdx, StatsP st)
 {
     __shared__ unsigned sWarp[PREP_THREADS / 32];
     __shared__ unsigned sBase;
+    __shared__ unsigned sNan;
+    unsigned nExcluded = 0;                           // a6 fused: excluded voxels of this thread
+    if (threadIdx.x == 0) sNan = 0;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned FULL = 0xffffffffu;
     const int numChunks = (g.N + PREP_CHUNK - 1) / PREP_CHUNK;
@@ -181,6 +196,7 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
                 if (j < nval && !(keepMask & (1u << j))) out[lin0 + j] = qnan;
         }
         const int c = __popc(keepMask);
+        nExcluded += (unsigned)(nval - c);
         int incl = c;
 #pragma unroll
         for (int s = 1; s < 32; s <<= 1) {
@@ -201,6 +217,13 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
         for (int j = 0; j < 4; ++j)
             if (keepMask & (1u << j)) evalIdx[pos++] = (unsigned)(lin0 + j);
         __syncthreads();
+    }
+    if (st.hist) {
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) nExcluded += __shfl_xor_sync(FULL, nExcluded, s);
+        if (lane == 0 && nExcluded) atomicAdd(&sNan, nExcluded);
+        __syncthreads();
+        if (tid == 0 && sNan) atomicAdd(&st.summary->n_nan, sNan);
     }
 }
 
@@ -224,7 +247,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
        Ctl* __restrict__ ctl, const unsigned* __restrict__ evalIdx, unsigned* __restrict__ listKey,
        unsigned* __restrict__ listIdx, unsigned* __restrict__ deepKey, unsigned* __restrict__ deepIdx, int classes,
        int buildTable, const __grid_constant__ TablePlan tabPlan, int4* __restrict__ table,
-       unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx)
+       unsigned* __restrict__ tmpL, unsigned* __restrict__ tmpIdx, StatsP st)
 {
     // classes != 0: the work list is split by depth class at append time instead of being sorted afterwards --
     // "deep" items (key beyond the first non-zero table distance: the walk will pass table entry 0) go to
@@ -237,8 +260,14 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     for (int d = tid; d < KEY_DIGITS; d += STAR_THREADS) sHist[d] = 0;
     // a3 inside the wait: the prefix table depends on the geometry only, so the first blocks build it (one slice of
     // buckets each) while k_classify is still running -- no side stream, no join, nothing added to the chain.
+    // the table builder's working set and the fused-statistics slots share one piece of shared memory: the table is
+    // finished (table_build_slice ends with a barrier) before the first voxel is looked at
+    using TabS = TableSmem<TAB_EMBED_ENTRIES, TAB_EMBED_BUCKETS, TAB_EMBED_BLOCKS>;
+    using StatS = FusedStats<STAR_THREADS>;
+    __shared__ __align__(16) unsigned char sRaw[sizeof(TabS) > sizeof(StatS) ? sizeof(TabS) : sizeof(StatS)];
+    StatS& sStat = *reinterpret_cast<StatS*>(sRaw);
     if (buildTable) {
-        __shared__ TableSmem<TAB_EMBED_ENTRIES, TAB_EMBED_BUCKETS, TAB_EMBED_BLOCKS> sTab;
+        TabS& sTab = *reinterpret_cast<TabS*>(sRaw);
         for (int slice = blockIdx.x; slice < TAB_EMBED_BLOCKS; slice += gridDim.x)
             table_build_slice<STAR_THREADS, TAB_EMBED_ENTRIES, TAB_EMBED_BUCKETS, TAB_EMBED_BLOCKS>(
                 sTab, g, e, ctl, &tabPlan, 0.0f, TAB_EMBED_MAX_CELLS, table, tmpL, tmpIdx, slice);
@@ -262,6 +291,8 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
 #pragma unroll
     for (int T = 1; T < 8; ++T) A[T] = ((T & 1) ? g.hh[0] : 0.0f) + ((T & 2) ? g.hh[1] : 0.0f) + ((T & 4) ? g.hh[2] : 0.0f);
     float maxKey = 0.0f;
+    fused_stats_init(sStat, st);
+    unsigned nNanKey = 0;
     __syncthreads();
 
     while (item < numItems) {
@@ -312,6 +343,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
                     const float outside2 = fminf(g.hmin2, fmaf(dr, dr, g.rho_link2));
                     if (key * key <= outside2) {          // nothing outside the star can be closer
                         out[lin] = key;
+                        fused_stats_add(sStat, st, key);
                         toSearch = false;
                     } else {
                         key = fminf(key, sqrtf(vb));      // the 26 neighbour grid points also bound gamma from above
@@ -320,6 +352,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
             }
             if (!(key == key)) {                          // non-finite doses: no search, NaN out
                 out[lin] = qnan;
+                ++nNanKey;
                 toSearch = false;
             }
         }
@@ -368,6 +401,8 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
         for (int w = 0; w < STAR_THREADS / 32; ++w) m = fmaxf(m, sMax[w]);
         if (m > 0.0f) atomicMax(&ctl->maxKeyBits, __float_as_uint(m));
     }
+    if (st.hist && nNanKey) atomicAdd(&st.summary->n_nan, nNanKey);
+    fused_stats_flush(sStat, st);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -501,6 +536,8 @@ struct SearchCtx {
     bool trunc;
     float Rtab2, invGlobal;
     double dnorm;
+    FusedStats<SEARCH_THREADS>* stat;   // a6 fused (gamma_opts::stats_*)
+    StatsP st;
 };
 
 // One warp searches 32/G consecutive work items (firstItem .. firstItem + 32/G - 1, counted from the END of the
@@ -622,7 +659,11 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
             }
         }
     }
-    if (have && gl == 0) c.out[vc.lin] = fminf(key, sqrtf(best2));   // a5: write at the voxel's own place
+    if (have && gl == 0) {
+        const float gam = fminf(key, sqrtf(best2));
+        c.out[vc.lin] = gam;                                         // a5: write at the voxel's own place
+        fused_stats_add(*c.stat, c.st, gam);
+    }
     return visits;
 }
 
@@ -651,7 +692,9 @@ __device__ __forceinline__ void ring_items(const SearchCtx& c, const GridP& g, c
                 d[(ox + 1) + 3 * (oy + 1) + 9 * (oz + 1)] =
                     (__ldg(p + ox + oy * g.stride[1] + oz * g.stride[2]) - Dr) * invdD;
     const float best2 = gamma_ring_min(d, g.invA, R, key * key);
-    c.out[lin] = fminf(key, sqrtf(best2));                 // a5: write at the voxel's own place
+    const float gam = fminf(key, sqrtf(best2));
+    c.out[lin] = gam;                                      // a5: write at the voxel's own place
+    fused_stats_add(*c.stat, c.st, gam);
 }
 
 // MODE = lanes per reference voxel: 1 (thread per voxel), 8, 32, or 0 = adaptive: deep items (the
@@ -668,11 +711,14 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
                EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
                const unsigned* __restrict__ listIdx, const unsigned* __restrict__ deepKey,
                const unsigned* __restrict__ deepIdx, const int4* __restrict__ table, int deepDigit, int classes,
-               const __grid_constant__ GammaRingP ring)
+               const __grid_constant__ GammaRingP ring, Ctl* __restrict__ report, SeqP seq, StatsP st)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
+    __shared__ FusedStats<SEARCH_THREADS> sStat;
+    __shared__ unsigned sLast;
     SearchCtx c;
+    fused_stats_init(sStat, st);
     pdl_wait();
     pdl_launch_dependents();                             // the next call's k_norm may use the SMs this kernel leaves
     const unsigned nS = ctl->nSearch;
@@ -688,38 +734,65 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     // shallow items: all of the list with depth classes, else what is left of the sorted list before its deep tail
     const unsigned nShallow = (MODE == 0 && classes) ? nS : nS - nDeep;
     const unsigned nDeepList = (MODE == 0 && classes) ? nDeep : nS;   // deep item i is entry nDeepList - 1 - i
-    if (nS + nDeep == 0) return;
     constexpr unsigned VPW = MODE == 0 ? 4u : 32u / (unsigned)(MODE == 0 ? 8 : MODE);
     const unsigned numUnits = MODE != 0 ? (nS + VPW - 1u) / VPW
                               : classes ? nDeep + (nShallow + 31u) / 32u : nDeep + (nShallow + 3u) / 4u;
     const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
     unsigned unit = blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5);
-    if (unit >= numUnits) return;
-    const bool dynamic = numUnits > warpsTotal;
-    c.ref = ref; c.ev = ev; c.out = out; c.table = table;
-    c.T = ctl->tableCount;
-    c.trunc = ctl->tableTrunc != 0;
-    c.Rtab2 = ctl->Rtab2;
-    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
-    c.dnorm = (double)dnormF;
-    c.invGlobal = ctl->invGlobal;
-    unsigned visits = 0;
+    if (unit < numUnits) {
+        const bool dynamic = numUnits > warpsTotal;
+        c.ref = ref; c.ev = ev; c.out = out; c.table = table;
+        c.T = ctl->tableCount;
+        c.trunc = ctl->tableTrunc != 0;
+        c.Rtab2 = ctl->Rtab2;
+        const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
+        c.dnorm = (double)dnormF;
+        c.invGlobal = ctl->invGlobal;
+        c.stat = &sStat; c.st = st;
+        unsigned visits = 0;
 
-    while (unit < numUnits) {
-        unsigned nextUnit = numUnits;
-        if (dynamic && lane == 0) nextUnit = atomicAdd(&ctl->workCounter, 1u) + warpsTotal;
-        if (MODE == 0) {
-            if (unit < nDeep) visits += search_items<32, JU>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane);
-            else if (classes) ring_items(c, g, e, ring, listKey, listIdx, nS, 32u * (unit - nDeep), lane);
-            else visits += search_items<8, JU>(c, g, e, listKey, listIdx, nS, nDeep + 4u * (unit - nDeep), lane);
-        } else {
-            visits += search_items<(MODE == 0 ? 8 : MODE), JU>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);
+        while (unit < numUnits) {
+            unsigned nextUnit = numUnits;
+            if (dynamic && lane == 0) nextUnit = atomicAdd(&ctl->workCounter, 1u) + warpsTotal;
+            if (MODE == 0) {
+                if (unit < nDeep) visits += search_items<32, JU>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane);
+                else if (classes) ring_items(c, g, e, ring, listKey, listIdx, nS, 32u * (unit - nDeep), lane);
+                else visits += search_items<8, JU>(c, g, e, listKey, listIdx, nS, nDeep + 4u * (unit - nDeep), lane);
+            } else {
+                visits += search_items<(MODE == 0 ? 8 : MODE), JU>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);
+            }
+            unit = __shfl_sync(FULL, nextUnit, 0);
         }
-        unit = __shfl_sync(FULL, nextUnit, 0);
+        // diagnostic counter: one atomic per warp
+        for (int s = 16; s > 0; s >>= 1) visits += __shfl_xor_sync(FULL, visits, s);
+        if (lane == 0 && visits) atomicAdd(&ctl->visits, (unsigned long long)visits);
     }
-    // diagnostic counter: one atomic per warp
-    for (int s = 16; s > 0; s >>= 1) visits += __shfl_xor_sync(FULL, visits, s);
-    if (lane == 0 && visits) atomicAdd(&ctl->visits, (unsigned long long)visits);
+    fused_stats_flush(sStat, st);
+    // ---- end of the call (common.cuh, "Device control block"): the last block to finish copies the control block to
+    // the set's report, zeroes it and publishes the call -- in call order, so that the end of this kernel implies the
+    // end of every earlier call on the workspace.
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        sLast = atomicAdd(&ctl->blocksDone, 1u) == gridDim.x - 1u ? 1u : 0u;
+    }
+    __syncthreads();
+    if (sLast) {
+        __threadfence();
+        if (threadIdx.x == 0 && seq.done)
+            while ((int)(ld_acquire_u32(seq.done) - seq.seq) < 0) __nanosleep(64);
+        unsigned* w = reinterpret_cast<unsigned*>(ctl);
+        unsigned* r = reinterpret_cast<unsigned*>(report);
+        for (int i = threadIdx.x; i < (int)(sizeof(Ctl) / 4); i += SEARCH_THREADS) {
+            r[i] = __ldcg(w + i);
+            w[i] = 0u;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0 && seq.done) {
+            __threadfence();
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(seq.done), "r"(seq.seq + 1u) : "memory");
+        }
+    }
 }
 
 }  // namespace gamma_b200

@@ -117,6 +117,113 @@ k_stats(const float* __restrict__ gam, long long n, int nbins, float binScale,
 }
 
 // ------------------------------------------------------------------------------------------------
+// a6 fused into the gamma kernels (gamma_opts::stats_*): gamma is in a register when k_star / k_table_search write it,
+// so the reduction costs a few shared-memory updates per voxel instead of a second pass over gamma[N].
+// Every thread owns one slot in shared memory (no registers are held across the search), the histogram is a block-wide
+// shared array; a block flushes once, at its end.  The caller's hist / summary are zeroed by k_norm, the first kernel
+// of the call, which completes before any other kernel of the call starts.
+// ------------------------------------------------------------------------------------------------
+constexpr int FUSED_MAX_BINS = 1024;
+
+struct StatsP {
+    unsigned long long* hist;   // DEVICE, nbins u64; nullptr = no fused statistics
+    gamma_summary* summary;     // DEVICE
+    int nbins;
+    float binScale;             // nbins / hist_max
+};
+
+struct StatSlot {
+    double s1, s3;
+    unsigned nEval, nPass;
+    float mx;
+    unsigned pad_;
+};
+
+template <int THREADS>
+struct FusedStats {
+    StatSlot slot[THREADS];
+    unsigned hist[FUSED_MAX_BINS];
+    double wSum[THREADS / 32][2];
+    unsigned wCnt[THREADS / 32][2];
+    float wMax[THREADS / 32];
+};
+
+// all threads of the block must call (contains a barrier when statistics are on)
+template <int THREADS>
+__device__ __forceinline__ void fused_stats_init(FusedStats<THREADS>& S, const StatsP& st)
+{
+    if (!st.hist) return;
+    StatSlot z;
+    z.s1 = 0.0; z.s3 = 0.0; z.nEval = 0; z.nPass = 0; z.mx = 0.0f; z.pad_ = 0;
+    S.slot[threadIdx.x] = z;
+    for (int b = threadIdx.x; b < st.nbins; b += THREADS) S.hist[b] = 0;
+    __syncthreads();                                     // st.hist is uniform over the block
+}
+
+// one finite gamma value written by this thread (same bin rule as k_stats: decided in fp32)
+template <int THREADS>
+__device__ __forceinline__ void fused_stats_add(FusedStats<THREADS>& S, const StatsP& st, float v)
+{
+    if (!st.hist) return;
+    if (!(v == v)) { atomicAdd(&st.summary->n_nan, 1u); return; }   // non-finite neighbourhood: counted as excluded
+    StatSlot& z = S.slot[threadIdx.x];
+    const double dv = (double)v;
+    z.s1 += dv;
+    z.s3 += dv * dv * dv;
+    z.nEval += 1u;
+    z.nPass += v <= 1.0f ? 1u : 0u;
+    z.mx = fmaxf(z.mx, v);
+    const float fb = v * st.binScale;
+    const int b = fb >= (float)(st.nbins - 1) ? st.nbins - 1 : (fb > 0.0f ? (int)fb : 0);
+    atomicAdd(&S.hist[b], 1u);
+}
+
+// block-wide flush: all threads of the block must call (contains __syncthreads)
+template <int THREADS>
+__device__ __forceinline__ void fused_stats_flush(FusedStats<THREADS>& S, const StatsP& st)
+{
+    if (!st.hist) return;
+    __syncthreads();
+    StatSlot z = S.slot[threadIdx.x];
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        z.s1 += __shfl_xor_sync(0xffffffffu, z.s1, s);
+        z.s3 += __shfl_xor_sync(0xffffffffu, z.s3, s);
+        z.nEval += __shfl_xor_sync(0xffffffffu, z.nEval, s);
+        z.nPass += __shfl_xor_sync(0xffffffffu, z.nPass, s);
+        z.mx = fmaxf(z.mx, __shfl_xor_sync(0xffffffffu, z.mx, s));
+    }
+    const int warp = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) {
+        S.wSum[warp][0] = z.s1; S.wSum[warp][1] = z.s3;
+        S.wCnt[warp][0] = z.nEval; S.wCnt[warp][1] = z.nPass;
+        S.wMax[warp] = z.mx;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long cE = 0, cP = 0;
+        double a1 = 0.0, a3 = 0.0;
+        float m = 0.0f;
+        for (int w = 0; w < THREADS / 32; ++w) {
+            cE += S.wCnt[w][0]; cP += S.wCnt[w][1];
+            a1 += S.wSum[w][0]; a3 += S.wSum[w][1];
+            m = fmaxf(m, S.wMax[w]);
+        }
+        if (cE) {
+            atomicAdd(&st.summary->n_eval, cE);
+            atomicAdd(&st.summary->sum_gamma, a1);
+            atomicAdd(&st.summary->sum_gamma3, a3);
+            atomicMax(reinterpret_cast<unsigned*>(&st.summary->max_gamma), __float_as_uint(m));   // m >= 0
+        }
+        if (cP) atomicAdd(&st.summary->n_pass, cP);
+    }
+    for (int b = threadIdx.x; b < st.nbins; b += THREADS) {
+        const unsigned c = S.hist[b];
+        if (c) atomicAdd(&st.hist[b], (unsigned long long)c);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // FP32 ALU rate probe: 16 independent FFMA chains per thread (the "alu" roofline denominator).
 // ------------------------------------------------------------------------------------------------
 constexpr int PROBE_ITERS = 2048;

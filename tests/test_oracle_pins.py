@@ -397,6 +397,66 @@ def test_visit_counts_scale_as_gamma_cubed(oracle_mod):
     assert 6.0 < counts[1] / counts[0] < 10.0      # (2x gamma)^3 = 8
 
 
+@pytest.mark.parametrize("shape,spacing,dd,dta,mode", [
+    ((3, 3, 3), (2.0, 2.5, 3.0), 0.03, 3.0, 0),
+    ((5, 4, 6), (3.0, 1.5, 2.0), 0.02, 2.5, 0),
+    ((7, 7, 7), (1.0, 1.0, 1.0), 0.01, 1.0, 1),        # deep: gamma_0 of several voxels, box clipped by the grid
+    ((6, 9), (2.5, 2.0, 1.0), 0.03, 2.0, 0),
+])
+def test_vertex_only_form_equals_bruteforce_over_every_grid_vertex(oracle_mod, shape, spacing, dd, dta, mode):
+    """The classical discrete gamma (Low et al.; the comparator of PAPER.md:135-137): the minimum of Gamma (Eq. 1,
+    PAPER.md:149-162) over EVERY evaluation grid point, no radius, no pruning -- numpy over the whole grid."""
+    rng = np.random.default_rng([31, len(shape), shape[0]])
+    n = len(shape)
+    ref_xyz = rng.uniform(0.9, 2.0, size=shape)
+    ev_xyz = ref_xyz * rng.uniform(0.95, 1.05) + rng.normal(0, 0.08, size=shape)
+    ref = to_xyz_order(ref_xyz)[None] if n == 2 else to_xyz_order(ref_xyz)
+    ev = to_xyz_order(ev_xyz)[None] if n == 2 else to_xyz_order(ev_xyz)
+    out = run_oracle(oracle_mod, ref, ev, spacing, dd, dta, mode=mode, cutoff=0.0, form="vertex")
+    out_xyz = to_xyz_order(out[0] if n == 2 else out)
+    idx = np.stack(np.meshgrid(*[np.arange(k) for k in shape], indexing="ij"), axis=-1).astype(np.float64)
+    hn = np.array(spacing[:n]) / dta
+    for v in itertools.product(*[range(k) for k in shape]):
+        dD = dd * (ref_xyz.max() if mode == 0 else ref_xyz[v])
+        spatial2 = (((idx - np.array(v, dtype=np.float64)) * hn) ** 2).sum(axis=-1)
+        brute = np.sqrt(spatial2 + ((ev_xyz - ref_xyz[v]) / dD) ** 2).min()
+        assert out_xyz[v] == pytest.approx(brute, abs=1e-12)
+
+
+@pytest.mark.parametrize("shape,spacing,dd,dta", [
+    ((7, 7, 7), (1.0, 1.0, 1.0), 0.02, 1.0),
+    ((7, 6, 5), (2.0, 1.0, 1.5), 0.02, 1.5),
+    ((8, 7), (1.0, 2.0, 1.0), 0.01, 1.5),
+])
+def test_visit_counts_equal_explicit_enumeration(oracle_mod, shape, spacing, dd, dta):
+    """N_s(v) = #{in-grid cells c : L_cell(c - v) < gamma[v]} ("search length L ~ gamma"; DESIGN.md
+    reading 4 for L_cell): counted here by a plain loop over every CELL of the grid, exact integers."""
+    rng = np.random.default_rng([37, len(shape), shape[1]])
+    n = len(shape)
+    ref_xyz = rng.uniform(0.9, 2.0, size=shape)
+    ev_xyz = ref_xyz * 1.03 + rng.normal(0, 0.10, size=shape)
+    ref = to_xyz_order(ref_xyz)[None] if n == 2 else to_xyz_order(ref_xyz)
+    ev = to_xyz_order(ev_xyz)[None] if n == 2 else to_xyz_order(ev_xyz)
+    dims = tuple(shape) + (1,) * (3 - n)
+    gam, vis = oracle_mod.gamma(ref, ev, dims, spacing, dd, dta, cutoff=0.0, return_visits=True)
+    full = ref.shape if n == 3 else ref.shape[1:]
+    gam_xyz, vis_xyz = to_xyz_order(gam.reshape(full)), to_xyz_order(vis.reshape(full))
+    hn = [spacing[a] / dta for a in range(n)]
+    total = 0
+    for v in itertools.product(*[range(k) for k in shape]):
+        cnt = 0
+        for c in itertools.product(*[range(k - 1) for k in shape]):
+            s = 0.0
+            for a in range(n):
+                o = c[a] - v[a]
+                d = float(max(o, -o - 1, 0)) * hn[a]
+                s += d * d
+            cnt += np.sqrt(s) < gam_xyz[v]
+        assert vis_xyz[v] == cnt, (v, vis_xyz[v], cnt)
+        total += cnt
+    assert total > 2 * np.prod(shape)            # the case is not trivial: more than the touching cells are counted
+
+
 # ----------------------------------------------------------------------------
 # conventions the paper does not pin (DESIGN.md readings 8-12): checked as stated
 # ----------------------------------------------------------------------------
