@@ -8,6 +8,9 @@ configs   every BASELINE.json config (cfg1, cfg2, cfg3, cfg4 coarse/fine, cfg5):
           the resolution exponent of cfg4 (Fig. 2) and cfg5 with the voxel pre-sort on / off and
           with the paper's thread-per-voxel mapping (Table 2)
 batch     independent cfg3 cases per call through gamma_eval_batch against the same cases one by one
+trace     device timeline of consecutive calls (library built with -DGAMMA_TRACE: GAMMA_NVCC_EXTRA=-DGAMMA_TRACE python -m
+          paper_1012_1900_b200.build --force): when each kernel of a call starts, passes its dependency wait and ends,
+          relative to the call's first kernel, one call after the other with and without opts.back_to_back
 criteria  the 9 DD x DTA combinations of Table 3 on the cfg3 phantom: time against sum gamma^3
           (Fig. 1) and the exact law gamma(k DD, k DTA) = gamma(DD, DTA) / k checked on the device maps
 
@@ -66,13 +69,15 @@ def measure(case, opts_kw, reps, dd=None, dta=None, keep_map=False):
         e1.record(stream)
         e1.synchronize()
         times.append(e0.elapsed_time(e1))
-    # back-to-back rate (what bench.py reports): the launches of consecutive calls overlap
+    # back-to-back rate (what bench.py reports): consecutive calls pipelined (opts.back_to_back: nothing else is
+    # enqueued on the stream between them)
     torch.cuda.synchronize()
+    bopts = GammaOpts(back_to_back=1, **opts_kw)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for i in range(reps):
         k = i % nsets
-        binding.gamma_eval_ex(refs[k], evs[k], *a, opts, outs[k], stream)
+        binding.gamma_eval_ex(refs[k], evs[k], *a, bopts, outs[k], stream)
     e1.record(stream)
     torch.cuda.synchronize()
     ms_stream = e0.elapsed_time(e1) / reps
@@ -189,7 +194,8 @@ def suite_batch(args, emit):
                           ("batch, graph replay", lambda: binding.gamma_eval_batch(refs, evs, dims, sps, *a, gopts, outs,
                                                                                    stream)),
                           ("one by one", lambda: [binding.gamma_eval_ex(refs[i], evs[i], case.dims, case.spacing_mm, *a,
-                                                                        None, outs[i], stream) for i in range(nb)])):
+                                                                        binding.GammaOpts(back_to_back=1), outs[i], stream)
+                                                  for i in range(nb)])):
             for _ in range(3):
                 fn()
             torch.cuda.synchronize()
@@ -240,6 +246,51 @@ def suite_criteria(args, emit):
     return rows
 
 
+def suite_trace(args, emit):
+    """Where the time of a call goes: %globaltimer stamps of every kernel (first thread in, dependency wait passed,
+    last block out), median over the calls of a back-to-back run; needs a -DGAMMA_TRACE build of the library."""
+    import torch
+    from paper_1012_1900_b200 import binding, phantoms
+    from paper_1012_1900_b200.binding import GammaOpts
+    case = phantoms.make_case(args.trace_case)
+    dev = torch.device("cuda", 0)
+    N = case.ref.size
+    nsets = max(2, min(24, int(np.ceil(2.0 * L2_BYTES / (12.0 * N))) + 1))
+    refs = [torch.from_numpy(case.ref.ravel().copy()).to(dev) for _ in range(nsets)]
+    evs = [torch.from_numpy(case.eval.ravel().copy()).to(dev) for _ in range(nsets)]
+    outs = [torch.empty(N, dtype=torch.float32, device=dev) for _ in range(nsets)]
+    a = (case.dims, case.spacing_mm, case.dd, case.dta_mm, case.mode, case.cutoff)
+    stream = torch.cuda.current_stream()
+    names = ("k_norm", "k_classify", "k_star", "k_table_search")
+    for label, opts in (("back_to_back", GammaOpts(back_to_back=1)), ("serial (default)", GammaOpts())):
+        for i in range(8):
+            binding.gamma_eval_ex(refs[i % nsets], evs[i % nsets], *a, opts, outs[i % nsets], stream)
+        torch.cuda.synchronize()
+        binding.gamma_trace_reset()
+        _, first_call = binding.gamma_trace_read()
+        ncalls = 120
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(ncalls):
+            binding.gamma_eval_ex(refs[i % nsets], evs[i % nsets], *a, opts, outs[i % nsets], stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        rec, nxt = binding.gamma_trace_read()
+        assert nxt - first_call == ncalls
+        idx = [(first_call + i) % 256 for i in range(20, ncalls)]          # steady state
+        t = rec[idx].astype(np.float64)                                      # [call, kernel, (first, waited, last, 0)]
+        origin = t[:, 0, 0][:, None, None]
+        rel = (t[:, :, :3] - origin) / 1e3                                   # us after the call's k_norm started
+        med = np.median(rel, axis=0)
+        period = np.median(np.diff(t[:, 0, 0])) / 1e3
+        prev_search_end = np.median((t[:-1, 3, 2] - t[1:, 0, 0]) / 1e3)      # previous call's search end after this norm start
+        emit({"suite": "trace", "case": args.trace_case, "mode": label, "ms_per_case_events": e0.elapsed_time(e1) / ncalls,
+              "period_us": float(period), "previous_search_ends_after_this_norm_starts_us": float(prev_search_end),
+              "kernels_us_after_norm_start": {n: {"first": float(med[k, 0]), "waited": float(med[k, 1]),
+                                                 "last": float(med[k, 2])} for k, n in enumerate(names)},
+              "pipelined_calls": binding.gamma_get_counters()["calls_pipelined"]})
+
+
 def write_md(path, rows):
     with open(path, "w") as f:
         f.write("| suite | case | variant | criteria | N | M | ms/case (median) | ms/case (back to back) | t_p ms | "
@@ -263,7 +314,8 @@ def write_md(path, rows):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--suite", default="all", choices=["configs", "criteria", "batch", "all"])
+    ap.add_argument("--suite", default="all", choices=["configs", "criteria", "batch", "trace", "all"])
+    ap.add_argument("--trace-case", default="cfg3")
     ap.add_argument("--reps", type=int, default=30)
     ap.add_argument("--oracle-seconds", type=float, default=8.0)
     ap.add_argument("--md", default=None)
@@ -284,6 +336,8 @@ def main():
         suite_criteria(args, emit)
     if args.suite in ("batch", "all"):
         suite_batch(args, emit)
+    if args.suite == "trace":
+        suite_trace(args, emit)
     if args.md:
         write_md(args.md, rows)
 

@@ -19,9 +19,10 @@
  *              of the calling thread.  No exceptions, no abort.
  *   threads    calls are serialised by an internal mutex; consecutive calls on different streams are
  *              ordered by an event (they share the workspace).
- *   memory     workspace per voxel of the largest grid seen: 80 B up to 2^25 voxels (five u32 work lists x 4 rotating
- *              sets); larger grids first count their evaluated voxels M (one 4-byte read by the host, which
- *              SYNCHRONISES `stream` once inside the call) and take 20 B per EVALUATED voxel.
+ *   memory     workspace per voxel of the largest grid seen: 20 B up to 2^25 voxels (five u32 work lists), once for
+ *              calls on the caller's stream and once per lane used by back-to-back / batched calls; larger grids first
+ *              count their evaluated voxels M (one 4-byte read by the host, which SYNCHRONISES `stream` once inside
+ *              the call) and take 20 B per EVALUATED voxel.
  *   no fallback: there is no CPU path; without a CUDA device every compute call returns GAMMA_ERR_CUDA.
  */
 #ifndef GAMMA_B200_H
@@ -65,8 +66,7 @@ extern "C" {
  *                    side stream that forks from and joins `stream` through events (legal under stream capture).
  *   (ordering)       A call behaves like one stream operation: its first kernel waits for the operation in front of it
  *                    before it reads ref / eval, and when its last kernel has completed, every earlier call has.
- *                    Consecutive calls can be PIPELINED instead (the first three kernels of a call run beside the
- *                    table search of the previous one): see gamma_opts::back_to_back.
+ *                    Consecutive calls can be OVERLAPPED instead: see gamma_opts::back_to_back.
  *   (CUDA graphs)    A call made while the CALLER is capturing `stream` becomes four kernel nodes and one memset node
  *                    of the caller's graph.  The graph holds addresses of a library workspace reserved for captured
  *                    calls: that workspace never moves afterwards (a later captured call that needs a larger one fails
@@ -122,14 +122,18 @@ typedef struct gamma_opts {
                              negative weights -- a slow variant kept to measure that trade
                              (3D grids; 2D / 1D grids use 1)                                              */
     int back_to_back;     /* 0: default.  1: the caller ASSERTS that nothing else has been enqueued on `stream` since the
-                             library's previous gamma_eval / gamma_eval_ex call on it returned (no kernel, copy or event
-                             of the caller's).  The call is then pipelined behind that call: its k_norm, k_classify and
-                             k_star run while the previous table search is still running, each call on its own set of
-                             work lists (4 sets rotate), and calls still complete in call order.  The library checks
-                             what it can see (same stream, previous call of the same kind, no overlap between the
-                             buffers of the calls in flight: a call whose input is an earlier call's output is simply
-                             not pipelined); it cannot see foreign work on the stream, hence the assertion.  Ignored
-                             with profile_stages, graph = 1, large tables and grids above 2^25 voxels               */
+                             library's previous call on it returned (no kernel, copy or event of the caller's, no other
+                             library entry point).  Consecutive such calls are then run round-robin on 4 library-owned
+                             streams, each with its own workspace, so that their kernels overlap on the device (one
+                             stream cannot do that: its operations complete in order).  `stream` stays the ordering
+                             point: the first call of such a sequence starts after what is on `stream`, and `stream`
+                             waits for every call, so whatever the caller enqueues afterwards sees all results.  Calls of
+                             a sequence may COMPLETE out of order; a call that reads or writes a buffer an earlier call
+                             of the sequence still writes (or writes one it reads) waits for that call -- the library
+                             checks the ranges of ref / eval / out_gamma / stats_* -- so results are those of calls made
+                             one after the other.  What the library cannot see is foreign work on `stream` between two
+                             calls, hence the assertion.  Ignored (the call runs on `stream` itself) with
+                             profile_stages, graph = 1, large tables, grids above 2^25 voxels and under stream capture */
     int stats_nbins;      /* a6 fused into the call (all four stats_* fields; stats_hist = NULL: off).  The gamma
                              kernels accumulate, where they write gamma, what gamma_stats computes from the finished map:
                              same definition, same results (counts and histogram exact, sums in double), no second pass
@@ -141,10 +145,11 @@ typedef struct gamma_opts {
 
 /* Several independent cases in one call (every reference voxel and every case is independent,
  * PAPER.md:141).  One case is tens of microseconds of dependent kernels that cannot fill 148 SMs; the batch spreads
- * the cases over 4 library-owned streams, each with its own workspace, so that their kernels overlap on the device.
+ * the cases over 4 library-owned streams, each with its own workspace, so that their kernels overlap on the device
+ * (the same mechanism as gamma_opts::back_to_back, for which the batch is shorthand).
  * Results are those of n_cases gamma_eval_ex calls, bit for bit.
  *   ref, eval, out_gamma   HOST arrays of n_cases DEVICE pointers (fp32, layout as in gamma_eval); the outputs must
- *                          not alias each other or any input
+ *                          not alias each other or any input (cases whose buffers overlap are run one after the other)
  *   dims, spacing_mm       HOST, n_cases x 3 (case-major); the criteria and options are shared by all cases
  *   stream                 the batch starts after the work already on `stream` and `stream` continues after the last
  *                          case; asynchronous.  Cannot be captured into a CUDA graph (INVALID_ARGUMENT).
@@ -223,6 +228,9 @@ typedef struct gamma_counters {
     float norm_dose;         /* D_norm used                                                    */
     int table_truncated;
     int n_ring_search;    /* of n_table_search: voxels finished by the ring search (depth classes), no table walk */
+    int pipelined;        /* 1: the call ran on a library lane stream (gamma_opts::back_to_back honoured, or a batch) */
+    int pad_;
+    long long calls_pipelined; /* such calls so far in this process                                               */
 } gamma_counters;
 int gamma_get_counters(gamma_counters* out_host);
 
@@ -242,6 +250,17 @@ int gamma_get_stage_times(gamma_stage_times* out_host);
 /* Number of CUDA kernels this library has launched in this process so far (host counter; memsets and
  * copies are not counted). */
 long long gamma_launch_count(void);
+
+/*
+ * Device timeline of the kernels (diagnostic; only in a library built with -DGAMMA_TRACE, otherwise both calls return
+ * GAMMA_ERR_INVALID_ARGUMENT).  gamma_trace_reset clears the records and switches the stamps on (SYNCHRONISES the
+ * device); gamma_trace_read (SYNCHRONISES) copies them out: out_host HOST, 256 calls x 4 kernels (k_norm, k_classify,
+ * k_star, k_table_search) x 4 u64 = (first thread started, dependency wait passed, last block ended, 0), nanoseconds
+ * of %globaltimer, record of call number c (as counted on the single-call workspace) at index c % 256; *next_call =
+ * number of the next call.  The timeline in profiles/ is made with bench_suite.py --suite trace.
+ */
+int gamma_trace_reset(void);
+int gamma_trace_read(unsigned long long* out_host, long long* next_call);
 
 /* Device memory the library's workspaces hold right now, in bytes (host counter). */
 long long gamma_workspace_bytes(void);

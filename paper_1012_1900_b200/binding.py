@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
     "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
-    "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_release", "gamma_version",
+    "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_version",
     "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
 
@@ -27,7 +27,7 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 exported_symbols = (
     "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table",
     "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
-    "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
+    "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
 
 
@@ -58,7 +58,8 @@ class _CCounters(ctypes.Structure):
     _fields_ = [("n_voxels", ctypes.c_longlong), ("n_evaluated", ctypes.c_longlong),
                 ("n_table_search", ctypes.c_longlong), ("table_entries", ctypes.c_longlong),
                 ("vertex_visits", ctypes.c_longlong), ("max_key", ctypes.c_float), ("norm_dose", ctypes.c_float),
-                ("table_truncated", ctypes.c_int), ("n_ring_search", ctypes.c_int)]
+                ("table_truncated", ctypes.c_int), ("n_ring_search", ctypes.c_int), ("pipelined", ctypes.c_int),
+                ("pad_", ctypes.c_int), ("calls_pipelined", ctypes.c_longlong)]
 
 
 @dataclass
@@ -125,6 +126,10 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_get_stage_times.argtypes = [ctypes.POINTER(_CStageTimes)]
     lib.gamma_launch_count.argtypes = []
     lib.gamma_launch_count.restype = cll
+    lib.gamma_trace_reset.argtypes = []
+    lib.gamma_trace_reset.restype = ci
+    lib.gamma_trace_read.argtypes = [vp, ctypes.POINTER(cll)]
+    lib.gamma_trace_read.restype = ci
     lib.gamma_workspace_bytes.argtypes = []
     lib.gamma_workspace_bytes.restype = cll
     for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
@@ -331,6 +336,20 @@ def gamma_get_stage_times() -> dict:
 
 def gamma_launch_count() -> int:
     return int(load_library().gamma_launch_count())
+
+
+def gamma_trace_reset():
+    """Clear the device timeline and switch the stamps on (library built with -DGAMMA_TRACE only)."""
+    _check(load_library().gamma_trace_reset())
+
+
+def gamma_trace_read():
+    """(records uint64 numpy [256, 4, 4] = call x kernel x (first, waited, last, 0) in ns, number of the next call)."""
+    import numpy as np
+    buf = np.zeros((256, 4, 4), dtype=np.uint64)
+    nxt = ctypes.c_longlong(0)
+    _check(load_library().gamma_trace_read(buf.ctypes.data_as(ctypes.c_void_p), ctypes.byref(nxt)))
+    return buf, int(nxt.value)
 
 
 def gamma_workspace_bytes() -> int:

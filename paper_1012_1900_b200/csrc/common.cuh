@@ -3,6 +3,7 @@
 // criterion, L the normalised spatial distance of the offset table (Algorithm A1).
 #pragma once
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 namespace gamma_b200 {
@@ -45,20 +46,18 @@ struct EvalP {
     int mode;        // 0 global, 1 local
     int algo;        // 0: closed form on owned faces (default); 1: grid vertices only (classical discrete gamma,
                      // comparator); 2: the six Kuhn tetrahedra of a cell by the negative-weight recursion (ju_simplex.cuh)
+    unsigned call;   // number of the call on its workspace (device timeline, GAMMA_TRACE)
 };
 
 // Device control block: everything the pipeline decides on the device (no host sync on the path).
-// One block per call SET.  CTL_ROT sets rotate between consecutive calls of a workspace (call number k uses set
-// k % CTL_ROT: its own control block, offset table and work lists), one more serves the stand-alone entry points and
-// one the calls captured into a caller's CUDA graph.  The invariant that makes calls in flight safe, in one place:
-//   * a block is all zero whenever no call that uses it is in flight: the LAST block of a call's last kernel
-//     (k_table_search) copies it to the set's report block (gamma_get_counters), zeroes it, and only then publishes
-//     the call as done (SeqP::done = k + 1);
-//   * calls are published in call order (that last block first waits for done == k), so "the last kernel of call k
-//     has completed" implies "every earlier call has completed": stream order as the caller sees it is kept;
-//   * the first kernel of call k (k_norm) does not write its block before done >= k + 1 - CTL_ROT, i.e. before the
-//     previous user of the set has been published, and nothing else of call k starts before k_norm has completed.
-constexpr int CTL_ROT = 4, CTL_STANDALONE = 4, CTL_CAPTURE = 5, CTL_SLOTS = 6;
+// Slots 0 .. CTL_ROT-1 rotate between the consecutive calls of a workspace, slot CTL_STANDALONE serves the stand-alone
+// entry points, slot CTL_CAPTURE the calls captured into a caller's CUDA graph (cleared by a memset node).  Each slot
+// has its own small offset table.  The invariant, in one place: k_norm of call i zeroes slot (i + 1) % CTL_ROT for
+// call i + 1; that slot was last used by call i - 2, which has completed before k_norm(i) writes anything: k_norm(i)
+// either waits for the operation in front of it before doing anything (default), or -- started early, in the tail of
+// call i - 1 on a library-owned stream -- is launched only after k_star(i - 1) has completed, which is after
+// k_classify(i - 1) passed its wait for k_norm(i - 1), whose last act is to wait for the end of call i - 2.
+constexpr int CTL_ROT = 3, CTL_STANDALONE = 3, CTL_CAPTURE = 4, CTL_SLOTS = 5;
 constexpr int KEY_DIGITS = 256;
 struct Ctl {
     unsigned normOrd;      // max(ref) as an order-preserving uint
@@ -75,19 +74,50 @@ struct Ctl {
     int box[3];            // table box: m_a in [0, box_a)
     unsigned sortN;        // element count for gamma_sort_pairs
     unsigned nDeep;        // depth-class lists (presort 4): items in the deep list
-    unsigned blocksDone;   // blocks of the call's last kernel that have finished (the last one publishes the call)
+    unsigned pad0_;
     float invGlobal;       // 1 / (DD * D_norm) rounded to fp32 (global criterion), written by k_classify
     unsigned long long visits;       // owner vertices evaluated by the table search
     unsigned hist[KEY_DIGITS];       // digit histogram of the search list (bucket presort)
     unsigned cursor[KEY_DIGITS];     // scatter cursors of the bucket presort
 };
 
-// Sequencing of the calls of one workspace (one word per workspace, never cleared by the kernels).
-struct SeqP {
-    unsigned* done;   // device word: number of calls published so far; nullptr = this call is not sequenced
-    unsigned seq;     // this call's number k
-    unsigned need;    // k_norm writes its control block only when done >= need (signed 32-bit difference)
+// ------------------------------------------------------------------------------------------------
+// Device timeline (build with -DGAMMA_TRACE, e.g. GAMMA_NVCC_EXTRA=-DGAMMA_TRACE python -m paper_1012_1900_b200.build
+// --force; read with gamma_trace_read / bench_suite.py --suite trace).  Every kernel of a call stamps %globaltimer when
+// its first thread starts, when it passes its griddepcontrol.wait, and when its last block ends, into the record of the
+// call (call number modulo TRACE_CALLS).  Without the macro nothing is compiled into the kernels.
+// ------------------------------------------------------------------------------------------------
+constexpr int TRACE_CALLS = 256;
+constexpr int TRACE_KERNELS = 4;      // 0 k_norm, 1 k_classify, 2 k_star, 3 k_table_search
+struct TraceRec {
+    unsigned long long first, waited, last;   // ns: earliest start, latest "dependency met", latest block end
+    unsigned long long pad_;
 };
+#ifdef GAMMA_TRACE
+__device__ TraceRec* g_trace_buf = nullptr;   // TRACE_CALLS x TRACE_KERNELS records, set by the host
+__device__ __forceinline__ unsigned long long trace_now()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void trace_first(unsigned call, int k)
+{
+    if (threadIdx.x == 0 && g_trace_buf) atomicMin(&g_trace_buf[(call % TRACE_CALLS) * TRACE_KERNELS + k].first, trace_now());
+}
+__device__ __forceinline__ void trace_waited(unsigned call, int k)
+{
+    if (threadIdx.x == 0 && g_trace_buf) atomicMax(&g_trace_buf[(call % TRACE_CALLS) * TRACE_KERNELS + k].waited, trace_now());
+}
+__device__ __forceinline__ void trace_last(unsigned call, int k)
+{
+    if (threadIdx.x == 0 && g_trace_buf) atomicMax(&g_trace_buf[(call % TRACE_CALLS) * TRACE_KERNELS + k].last, trace_now());
+}
+#else
+__device__ __forceinline__ void trace_first(unsigned, int) {}
+__device__ __forceinline__ void trace_waited(unsigned, int) {}
+__device__ __forceinline__ void trace_last(unsigned, int) {}
+#endif
 
 // Monotone 8-bit quantisation of a non-negative key: 32 steps per octave over [2^-3, 2^5), clamped.
 // This is the digit of the one-pass MSD radix presort of the search work list.

@@ -122,18 +122,15 @@ struct CallSpans {
 };
 
 struct Workspace {
-    // ctl: Ctl[CTL_SLOTS] control blocks, Ctl[CTL_SLOTS] reports (copy of the block at the end of the call, for
-    // gamma_get_counters), one u32 "calls published" word (SeqP, common.cuh)
-    Buf ctl;
-    // work lists, `sets` copies of `stride` elements each (set s at element s * stride): compacted indices of the
-    // evaluated voxels; ring / sorted list (key0, idx0); deep list or sort ping-pong (key1, idx1)
+    Buf ctl;                       // Ctl[CTL_SLOTS]
+    // work lists, `stride` elements each: compacted indices of the evaluated voxels; ring / sorted list (key0, idx0);
+    // deep list or sort ping-pong (key1, idx1)
     Buf evalIdx, key0, idx0, key1, idx1;
     long long stride = 0;
-    int sets = 0;
     Buf sortK, sortV;              // ping-pong of gamma_sort_pairs (stand-alone)
     Buf tileHist;                  // radix sort
     Buf table, tmpL, tmpIdx;       // offset table: CTL_SLOTS embedded tables, then the large (side-stream) table
-    Buf hRef, hEval, hOut;         // device staging of gamma_eval_host / gamma_eval_host_batch
+    Buf hRef, hEval, hOut;         // device staging of gamma_eval_host
     Buf count;                     // evaluated-voxel count of the two-phase path (large grids)
     cudaEvent_t done = nullptr;    // orders consecutive calls that share this workspace
     bool havePending = false;
@@ -141,9 +138,10 @@ struct Workspace {
     cudaStream_t aux = nullptr;    // side stream: the large offset table is built while k_star runs
     cudaEvent_t evFork = nullptr, evJoin = nullptr;
     void* ctlOwner = nullptr;      // ctl.p the flags below refer to
-    bool ctlClean = false;         // control blocks zero / being zeroed by the calls in flight, sequence word consistent
-    unsigned seq = 0;              // number of the next sequenced call (its set is seq % CTL_ROT)
-    void* lastCtl = nullptr;       // report block of the last call
+    bool ctlClean = false;         // the rotating slots are known to be zero / being zeroed by the calls in flight
+    int slot = 0;                  // control-block slot of the next call (0 .. CTL_ROT-1)
+    unsigned calls = 0;            // calls so far (device timeline)
+    void* lastCtl = nullptr;       // control block of the last call
     bool haveStages = false;
     bool stageSort = false, stageTable = false;   // the last profiled call had a sort kernel / a side-stream table
     long long launches = 0;        // kernels launched so far (gamma_launch_count)
@@ -165,9 +163,10 @@ struct Workspace {
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
     cudaStream_t doneStream = nullptr;   // stream of the last work that used this workspace
-    bool chainable = false;              // that work was a sequenced pipeline ending in k_table_search
-    long long chainStride = 0;           // list layout of the calls in flight
-    CallSpans recent[CTL_ROT];           // what the last CTL_ROT - 1 calls read and write (slot = seq % CTL_ROT)
+    bool chainable = false;              // that work was a pipeline ending in k_table_search (which triggers dependents)
+    CallSpans lastSpans;                 // what that pipeline reads and writes
+    int lastEarly = 0;                   // the last call started in the tail of its predecessor
+    long long numEarly = 0;
     int lastClasses = 0;           // last call used depth classes: list A holds the ring items
     long long lastN = 0;
     bool haveLast = false;
@@ -193,23 +192,42 @@ struct Workspace {
         if (evFork) { cudaEventDestroy(evFork); evFork = nullptr; }
         if (evJoin) { cudaEventDestroy(evJoin); evJoin = nullptr; }
         havePending = false; haveLast = false; haveStages = false; ctlClean = false; ctlOwner = nullptr;
-        chainable = false; frozen = false; stride = 0; sets = 0; seq = 0;
-        for (CallSpans& c : recent) c = CallSpans();
+        chainable = false; frozen = false; stride = 0; slot = 0;
+        lastSpans = CallSpans();
     }
 };
 
-// Workspace 0 serves the single-case entry points; 1 .. BATCH_LANES serve gamma_eval_batch, one per lane (own stream,
-// own control blocks, lists and tables), so that the kernels of different cases overlap on the device; the last one
-// belongs to the calls a caller captures into its own CUDA graph (its addresses are baked into that graph, so it never
-// moves once used: gamma_release() is the only way to grow it).
-constexpr int BATCH_LANES = 4;
-constexpr int WS_CAPTURE = 1 + BATCH_LANES;
-Workspace g_pool[2 + BATCH_LANES];
+// Workspace 0 serves calls on the caller's stream; 1 .. LANES belong to the library's own lane streams, on which
+// back-to-back calls (gamma_opts::back_to_back) and the cases of gamma_eval_batch run so that the kernels of
+// consecutive calls overlap on the device; the last one belongs to the calls a caller captures into its own CUDA graph
+// (its addresses are baked into that graph, so it never moves once used: gamma_release() is the only way to grow it).
+constexpr int LANES = 4;
+constexpr int WS_CAPTURE = 1 + LANES;
+Workspace g_pool[2 + LANES];
 Workspace* g_cur = &g_pool[0];
+Workspace* g_lastWs = &g_pool[0];      // workspace of the last gamma_eval* call (gamma_get_counters)
+unsigned g_callNo = 0;                 // gamma_eval* calls so far, all workspaces (device timeline)
 #define g_ws (*g_cur)
-struct BatchLanes {
-    cudaStream_t stream[BATCH_LANES] = {};
-    cudaEvent_t start = nullptr, done[BATCH_LANES] = {};
+
+// Back-to-back calls.  A programmatic dependent that never waits is still not reported complete before its primary
+// (measured: profiles/r2_trace.md), so consecutive calls cannot run ahead of each other on ONE stream.  They are
+// spread round-robin over LANES library-owned streams instead, each with its own workspace: the lane waits for what
+// was on the caller's stream when the sequence of back-to-back calls began (one event), the caller's stream waits for
+// every call (one event per call, so later work of the caller's sees all results), calls on one lane are in stream
+// order, and a call that touches a buffer of one of the last B2B_WINDOW - 1 calls on another lane waits for that call.
+constexpr int B2B_WINDOW = 8;          // calls whose buffers are remembered; call j waits (host) for call j - B2B_WINDOW
+struct LaneState {
+    cudaStream_t stream[LANES] = {};
+    cudaEvent_t fork = nullptr;
+    unsigned long long forkGen = 0, laneFork[LANES] = {};
+    bool laneDirty[LANES] = {};        // something other than a library pipeline is the last operation on the lane
+    cudaEvent_t done[B2B_WINDOW] = {};
+    CallSpans spans[B2B_WINDOW];
+    int laneOf[B2B_WINDOW] = {};
+    bool used[B2B_WINDOW] = {};
+    unsigned long long next = 0;       // number of the next back-to-back call
+    cudaStream_t user = nullptr;       // caller's stream of the sequence in progress
+    bool active = false;               // the library's last operation was a back-to-back call on `user`
     bool ready = false;
 } g_lanes;
 
@@ -463,25 +481,24 @@ int check_criteria(float DD, int mode, float cutoff)
     return GAMMA_OK;
 }
 
-constexpr size_t CTL_BYTES = 2 * CTL_SLOTS * sizeof(Ctl) + 16;   // control blocks, reports, sequence word
+constexpr size_t CTL_BYTES = CTL_SLOTS * sizeof(Ctl);
 
-// Grids up to this many voxels get their work lists sized by N, CTL_ROT sets of them (consecutive calls in flight);
-// larger grids count their evaluated voxels first (one host read of 4 bytes on a call of milliseconds) and get ONE
-// set of lists sized by M.
+// Grids up to this many voxels get their work lists sized by N; larger grids count their evaluated voxels first (one
+// host read of 4 bytes on a call of milliseconds) and get lists sized by M.
 constexpr long long LISTS_BY_N_MAX = 1ll << 25;
 
 // Workspace of one call: allocations, side stream, events.  Nothing is allocated once the sizes have been seen.
-// `sets` x `stride`: layout of the work lists this call needs.
-int prepare_workspace(const GridP& g, const Resolved& r, int sets, long long stride)
+// `stride`: elements each work list must hold.
+int prepare_workspace(const GridP& g, const Resolved& r, long long stride)
 {
     int rc = ensure_device();
     if (rc) return rc;
+    if (stride < g_ws.stride) stride = g_ws.stride;            // grow-only
     const long long maxTiles = (stride + SORT_TILE - 1) / SORT_TILE;
-    const size_t ctlBytes = CTL_BYTES;
-    const size_t listBytes = (size_t)sets * (size_t)stride * 4;
+    const size_t listBytes = (size_t)stride * 4;
     const size_t tableCells = (size_t)CTL_SLOTS * TAB_EMBED_MAX_CELLS + (r.tableCap > TAB_EMBED_MAX_CELLS ? (size_t)r.tableCap : 0);
     if (g_ws.frozen) {
-        const bool fits = ctlBytes <= g_ws.ctl.cap && listBytes <= g_ws.evalIdx.cap && listBytes <= g_ws.key1.cap &&
+        const bool fits = CTL_BYTES <= g_ws.ctl.cap && listBytes <= g_ws.evalIdx.cap && listBytes <= g_ws.key1.cap &&
                           tableCells * 16 <= g_ws.table.cap && (size_t)r.tableCap * 4 <= g_ws.tmpL.cap &&
                           (r.presort != 3 || (size_t)maxTiles * SORT_RADIX * 4 <= g_ws.tileHist.cap);
         if (!fits)
@@ -489,13 +506,14 @@ int prepare_workspace(const GridP& g, const Resolved& r, int sets, long long str
                         "this call needs a larger capture workspace, but its addresses are part of a captured CUDA graph; "
                         "call gamma_release() first (that invalidates the captured graphs)");
     }
-    CU_TRY(g_ws.ctl.need(ctlBytes));
+    CU_TRY(g_ws.ctl.need(CTL_BYTES));
     CU_TRY(g_ws.key0.need(listBytes)); CU_TRY(g_ws.idx0.need(listBytes)); CU_TRY(g_ws.evalIdx.need(listBytes));
     CU_TRY(g_ws.key1.need(listBytes)); CU_TRY(g_ws.idx1.need(listBytes));
-    g_ws.stride = stride; g_ws.sets = sets;
+    g_ws.stride = stride;
     if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
     // the small embedded table exists once per control-block slot (the next call builds its own while this call's
-    // search still walks this one); a large table (table_radius 2, table_cap > 1024) lives BEHIND those slots
+    // search still walks this one); a large table (table_radius 2, table_cap > 1024) lives BEHIND those slots, so a
+    // following call's embedded table never aliases it
     CU_TRY(g_ws.table.need(tableCells * 16));
     CU_TRY(g_ws.tmpL.need((size_t)r.tableCap * 4)); CU_TRY(g_ws.tmpIdx.need((size_t)r.tableCap * 4));
     if (!g_ws.aux) {
@@ -526,29 +544,11 @@ int prepare_workspace(const GridP& g, const Resolved& r, int sets, long long str
     return GAMMA_OK;
 }
 
-// The control-block buffer exists and is zero where nothing is in flight; after a call that failed half-way nothing is
-// known about the blocks or the sequence word: wait for the device and start over.
-int ensure_ctl(cudaStream_t st)
-{
-    if (g_ws.ctl.p && g_ws.ctl.p == g_ws.ctlOwner && g_ws.ctlClean) return GAMMA_OK;
-    CU_TRY(g_ws.ctl.need(CTL_BYTES));
-    if (g_ws.ctlOwner) CU_TRY(cudaDeviceSynchronize());
-    CU_TRY(cudaMemsetAsync(g_ws.ctl.p, 0, CTL_BYTES, st));
-    g_ws.ctlOwner = g_ws.ctl.p;
-    g_ws.ctlClean = true;
-    g_ws.seq = 0;
-    g_ws.chainable = false;
-    for (CallSpans& c : g_ws.recent) c = CallSpans();
-    return GAMMA_OK;
-}
-
 // What a call's kernels are told about where they run.
 struct CallSlot {
     int slot;          // control-block / embedded-table slot
-    int set;           // work-list set
-    SeqP seq;          // sequencing of the call (done == nullptr: not sequenced)
+    int nextSlot;      // slot k_norm zeroes for the next call (-1: none)
     int waitFirst;     // k_norm waits for the operation in front of it before it reads ref / eval
-    bool early;        // k_norm is launched as a programmatic dependent of the previous call's k_table_search
     bool skipNorm;     // two-phase path: k_norm already ran (and the host has read the evaluated-voxel count)
 };
 
@@ -557,8 +557,8 @@ struct CallSlot {
 //   st :  k_norm -> k_classify -> k_star -> [k_bucket_scatter | LSD radix sort] -> (join) -> k_table_search
 //   aux:                    \-> k_offset_table ------------------------------------/     (large tables only)
 //
-// No memset and no host synchronisation on the path: the last block of k_table_search leaves the control block
-// zeroed for the next user of the set (common.cuh, "Device control block").
+// No memset and no host synchronisation on the path: k_norm zeroes the control block of the next call
+// (common.cuh, "Device control block").
 int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
                     const Resolved& r, float* out, cudaStream_t st, const CallSlot& cs, int* launched)
 {
@@ -566,14 +566,14 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     int nk = 0;
     Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
     Ctl* ctl = base + cs.slot;
-    Ctl* report = base + CTL_SLOTS + cs.slot;
-    const size_t off = (size_t)cs.set * (size_t)g_ws.stride;
-    unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p) + off, *i0 = static_cast<unsigned*>(g_ws.idx0.p) + off;
-    unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p) + off, *i1 = static_cast<unsigned*>(g_ws.idx1.p) + off;
-    unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p) + off;
+    Ctl* next = cs.nextSlot >= 0 ? base + cs.nextSlot : nullptr;
+    unsigned *k0 = static_cast<unsigned*>(g_ws.key0.p), *i0 = static_cast<unsigned*>(g_ws.idx0.p);
+    unsigned *k1 = static_cast<unsigned*>(g_ws.key1.p), *i1 = static_cast<unsigned*>(g_ws.idx1.p);
+    unsigned* e0 = static_cast<unsigned*>(g_ws.evalIdx.p);
     EvalP e;
     e.DD = DD; e.cutoff = cutoff; e.norm_dose = r.normDose; e.mode = mode;
     e.algo = (r.algo == 2 && !g.all_active) ? 0 : r.algo;   // the recursion variant is written for 3D cells
+    e.call = g_callNo;
     const int classes = (r.presort == 4 && r.star && g.all_active) ? 1 : 0;   // needs the 3D star phase
     const int presort = (r.presort == 4 && !classes) ? 1 : r.presort;
 #define STAGE_MARK(i, s) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], s)); } while (0)
@@ -621,16 +621,16 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         return GAMMA_OK;
     };
     int rc = GAMMA_OK;
+    // a large prefix table needs nothing of this call: forked in front of it (a call with a large table is never
+    // started early, so the previous call on the workspace has ended by the time the fork event fires)
+    if (r.tableMode == 1 && !embed) { rc = fork_table(); if (rc) return rc; }
     if (!cs.skipNorm) {                                                  // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
-        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ev, (int)N, mode,
-                         ctl, cs.seq, cs.waitFirst, r.stats));
+        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ev, (int)N, mode, ctl, next, cs.waitFirst,
+                         e.call, r.stats));
         ++nk;
     }
-    // A large prefix table does not need k_norm's maxima; it still starts after k_norm so that the control block it
-    // writes belongs to this call (the set is free once k_norm has completed).
-    if (r.tableMode == 1 && !embed) { rc = fork_table(); if (rc) return rc; }
     {                                                                    // a1: exclusion + compaction
         long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
         int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
@@ -669,7 +669,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     }
     if (g_ws.stageSort) STAGE_MARK(3, st);
     {                                                                    // a4 + a5
-        const int grid = sm * (r.lanes == 0 ? SEARCH_MIN_BLOCKS : 4 * (256 / SEARCH_THREADS));   // resident blocks
+        const int grid = sm * (r.lanes == 0 ? SEARCH_GRID_BLOCKS : 4 * (256 / SEARCH_THREADS));   // resident blocks
         const int4* tab = tab4;
         // adaptive lanes: an item is "deep" when its key exceeds the smallest non-zero table distance
         float hmin = 0.0f;
@@ -688,7 +688,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
             geo.g = g; geo.cap = r.tableCap; geo.radius = radius; geo.plan = plan; geo.ring = ring; geo.valid = true;
         }
 #define LAUNCH_SEARCH(...) CU_TRY(launch_ex(k_table_search<__VA_ARGS__>, grid, SEARCH_THREADS, 0, st, pdl, false, ref, ev, out, g, e, \
-                                            ctl, lk, li, k1, i1, tab, deepDigit, classes, ring, report, cs.seq, r.stats))
+                                            ctl, lk, li, k1, i1, tab, deepDigit, classes, ring, r.stats))
         if (e.algo == 2 && r.lanes == 1) LAUNCH_SEARCH(1, true);
         else if (e.algo == 2) LAUNCH_SEARCH(0, true);
         else if (r.lanes == 1) LAUNCH_SEARCH(1);
@@ -702,12 +702,11 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
 #undef STAGE_MARK
     *launched = nk;
     g_ws.lastClasses = classes;
-    g_ws.lastCtl = report;
+    g_ws.lastCtl = ctl;
     return GAMMA_OK;
 }
 
-// a0 + count of the evaluated voxels for the two-phase path of large grids: k_norm, then k_count, then 4 bytes to the
-// host.  SYNCHRONISES `st`.
+// Count of the evaluated voxels for the two-phase path of large grids (same decision as k_classify).
 __global__ void __launch_bounds__(256)
 k_count_eval(const float* __restrict__ ref, int N, EvalP e, const Ctl* __restrict__ ctl, unsigned* __restrict__ count)
 {
@@ -726,22 +725,32 @@ k_count_eval(const float* __restrict__ ref, int N, EvalP e, const Ctl* __restric
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(count, c);
 }
 
-// Enqueue the whole hot path on `st` (device pointers).  Caller holds g_mu.
+// The rotating control blocks exist and are zero where nothing is in flight; after a call that failed half-way nothing
+// is known about them: zero them behind whatever is still running.
+int ensure_ctl(cudaStream_t st)
+{
+    if (g_ws.ctl.p && g_ws.ctl.p == g_ws.ctlOwner && g_ws.ctlClean) return GAMMA_OK;
+    CU_TRY(g_ws.ctl.need(CTL_BYTES));
+    CU_TRY(cudaMemsetAsync(g_ws.ctl.p, 0, CTL_BYTES, st));
+    g_ws.ctlOwner = g_ws.ctl.p;
+    g_ws.ctlClean = true;
+    g_ws.slot = 0;
+    g_ws.chainable = false;
+    return GAMMA_OK;
+}
+
+// Enqueue the whole hot path on `st` (device pointers) with the current workspace.  Caller holds g_mu.
 //
-// Calls of one workspace are SEQUENCED (common.cuh): call k uses set k % CTL_ROT and is published, in call order, by
-// the last block of its last kernel.  A call may be PIPELINED behind the previous one -- its k_norm is launched as a
-// programmatic dependent of that call's k_table_search and does not wait for it, so k_norm, k_classify and k_star run
-// beside the previous search -- when the caller asserted that nothing else was enqueued on the stream in between
-// (gamma_opts::back_to_back; the library cannot see foreign work), the previous call on this workspace was a
-// sequenced pipeline on the same stream with the same list layout, the table is the small per-set one, and nothing
-// this call reads or writes overlaps what the calls still in flight write or read.  Every other call waits, in its
-// first kernel, for the operation in front of it (and so, by the in-order publication, for every earlier call).
+// allowEarly: `st` is a library-owned lane stream whose last operation is the previous pipeline of this workspace:
+// k_norm may then start in the tail of that call (it is launched as a programmatic dependent of its k_table_search,
+// reads this call's inputs only and ends after that call).  On a caller's stream the first kernel always waits for the
+// operation in front of it: the library cannot see what that operation is.
 //
-// opts.graph = 1: a call with arguments seen before (same pointers, geometry, criteria, options, set) replays a cached
-// CUDA graph of its kernels; not sequenced, never pipelined.  A stream that the CALLER is capturing gets the kernels
-// as nodes of the caller's graph, on the capture workspace.
+// opts.graph = 1: a call with arguments seen before (same pointers, geometry, criteria, options, slot) replays a cached
+// CUDA graph of its kernels.  A stream that the CALLER is capturing gets the kernels as nodes of the caller's graph, on
+// the capture workspace.
 int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
-                     const Resolved& r, float* out, cudaStream_t st)
+                     const Resolved& r, float* out, cudaStream_t st, bool allowEarly)
 {
     cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
     CU_TRY(cudaStreamIsCapturing(st, &capStatus));
@@ -751,118 +760,85 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     if (capturing) {
         // The kernels become nodes of the caller's graph.  The call must be self-contained (its replays do not pass
         // through this function): its own workspace (never moved afterwards), its own control block cleared by a
-        // memset node, no sequencing; ordering against other work is the captured stream's.
+        // memset node; ordering against other work is the captured stream's.
         Workspace* keep = g_cur;
         g_cur = &g_pool[WS_CAPTURE];
         {   // cudaMalloc is not a stream operation, but a capture in "global" mode forbids it: relax for the allocation
             cudaStreamCaptureMode cm = cudaStreamCaptureModeRelaxed;
             cudaThreadExchangeStreamCaptureMode(&cm);
-            rc = prepare_workspace(g, r, 1, N);
+            rc = prepare_workspace(g, r, N);
             cudaThreadExchangeStreamCaptureMode(&cm);
         }
+        int launched = 0;
         if (rc == GAMMA_OK) {
             g_ws.frozen = true;
             Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_CAPTURE;
             cudaError_t ce = cudaMemsetAsync(ctl, 0, sizeof(Ctl), st);
             if (ce != cudaSuccess) rc = fail(GAMMA_ERR_CUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(ce));
         }
-        int launched = 0;
         if (rc == GAMMA_OK) {
             Resolved rr = r;
             rr.profile = 0;
             CallSlot cs;
-            cs.slot = CTL_CAPTURE; cs.set = 0; cs.seq.done = nullptr; cs.seq.seq = 0; cs.seq.need = 0;
-            cs.waitFirst = 1; cs.early = false; cs.skipNorm = false;
+            cs.slot = CTL_CAPTURE; cs.nextSlot = -1; cs.waitFirst = 1; cs.skipNorm = false;
             rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, rr, out, st, cs, &launched);
         }
         if (rc == GAMMA_OK) {
             g_ws.launches += launched;
             g_ws.haveStages = false;
-            g_ws.lastStream = nullptr; g_ws.lastN = g.N; g_ws.haveLast = true;
+            g_ws.lastStream = nullptr; g_ws.lastN = g.N; g_ws.haveLast = true; g_ws.lastEarly = 0;
+            g_lastWs = g_cur;
         }
-        Workspace* used = g_cur;
         g_cur = keep;
-        if (rc == GAMMA_OK) {                       // gamma_get_counters reports on the captured call
-            g_ws.haveLast = true; g_ws.lastCtl = used->lastCtl; g_ws.lastStream = nullptr; g_ws.lastN = g.N;
-            g_ws.lastClasses = used->lastClasses; g_ws.haveStages = false;
-        }
         return rc;
     }
-    // ---- layout of the work lists
     long long byNMax = LISTS_BY_N_MAX;
     if (const char* env = std::getenv("GAMMA_LISTS_BY_N_MAX")) byNMax = std::atoll(env);   // tests: two-phase path on small grids
     const bool twoPhase = N > byNMax;
     const bool useGraph = g_ws.graphs != 0 && r.graph && !r.profile && !twoPhase;
-    int sets = CTL_ROT;
-    long long stride = N;
-    EvalP e0p;
-    e0p.DD = DD; e0p.cutoff = cutoff; e0p.norm_dose = r.normDose; e0p.mode = mode; e0p.algo = 0;
-    rc = order_after_previous(st);
-    if (rc) return rc;
-    // control blocks: zero at the start, and again whenever a previous call failed half-way (then nothing is known
-    // about the sequence word either: wait for the device, start over)
     rc = ensure_device();
+    if (rc) return rc;
+    rc = order_after_previous(st);
     if (rc) return rc;
     rc = ensure_ctl(st);
     if (rc) return rc;
     g_ws.ctlClean = false;                                 // set again when everything below was enqueued
-    unsigned* doneWord = reinterpret_cast<unsigned*>(static_cast<char*>(g_ws.ctl.p) + 2 * CTL_SLOTS * sizeof(Ctl));
     CallSlot cs;
+    cs.slot = g_ws.slot;
+    cs.nextSlot = (g_ws.slot + 1) % CTL_ROT;
     cs.skipNorm = false;
+    long long stride = N;
     if (twoPhase) {
-        // a0, then the count of evaluated voxels, read by the host: the lists are sized by M, one set, no pipelining
-        rc = ensure_device();
-        if (rc) return rc;
+        // a0, then the count of evaluated voxels, read by the host: the lists are sized by M
         CU_TRY(g_ws.count.need(16));
-        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + (g_ws.seq % CTL_ROT);
+        Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
+        EvalP e0p;
+        e0p.DD = DD; e0p.cutoff = cutoff; e0p.norm_dose = r.normDose; e0p.mode = mode; e0p.algo = 0; e0p.call = g_callNo;
         CU_TRY(cudaMemsetAsync(g_ws.count.p, 0, 16, st));
-        SeqP sq;
-        sq.done = doneWord; sq.seq = g_ws.seq; sq.need = g_ws.seq;     // every earlier call has been published
         const int sm = g_ws.numSM;
-        CU_TRY(launch_ex(k_norm, sm * 4, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, ctl, sq, 1, r.stats));
-        k_count_eval<<<sm * 8, 256, 0, st>>>(ref, (int)N, e0p, ctl, static_cast<unsigned*>(g_ws.count.p));
+        CU_TRY(launch_ex(k_norm, sm * 4, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, base + cs.slot,
+                         base + cs.nextSlot, 1, g_callNo, r.stats));
+        k_count_eval<<<sm * 8, 256, 0, st>>>(ref, (int)N, e0p, base + cs.slot, static_cast<unsigned*>(g_ws.count.p));
         unsigned M = 0;
         CU_TRY(cudaMemcpyAsync(&M, g_ws.count.p, 4, cudaMemcpyDeviceToHost, st));
         CU_TRY(cudaStreamSynchronize(st));
         g_ws.launches += 2;
-        sets = 1;
         stride = (long long)M + 1024;
         cs.skipNorm = true;
     }
-    if ((long long)g_ws.sets * g_ws.stride >= (long long)sets * stride && g_ws.stride >= stride && !twoPhase &&
-        g_ws.sets >= sets) {
-        sets = g_ws.sets; stride = g_ws.stride;            // the layout in place is large enough: keep it (pipelining)
-    }
-    rc = prepare_workspace(g, r, sets, stride);
+    rc = prepare_workspace(g, r, stride);
     if (rc) return rc;
-    const int slot = (int)(g_ws.seq % CTL_ROT);
-    cs.slot = slot;
-    cs.set = sets == 1 ? 0 : slot;
-    // ---- may this call be pipelined behind the previous one?
+    // ---- may k_norm start in the tail of the previous call?
     CallSpans mine;
     const size_t bytes = (size_t)N * 4;
     mine.rd[0].set(ref, bytes); mine.rd[1].set(ev, bytes); mine.wr[0].set(out, bytes);
     mine.wr[1].set(r.stats.hist, (size_t)r.stats.nbins * 8); mine.wr[2].set(r.stats.summary, sizeof(gamma_summary));
     static const bool overlapCalls = !(std::getenv("GAMMA_OVERLAP_CALLS") && std::getenv("GAMMA_OVERLAP_CALLS")[0] == '0');
     const bool embed = r.tableMode == 1 && r.tableCap <= TAB_EMBED_MAX_CELLS;
-    bool early = overlapCalls && r.backToBack && g_ws.pdl != 0 && g_ws.chainable && g_ws.havePending &&
-                 g_ws.doneStream == st && !r.profile && !useGraph && !twoPhase && embed && sets == CTL_ROT &&
-                 g_ws.chainStride == stride;
-    if (early)
-        for (int back = 1; back < CTL_ROT && early; ++back) {
-            if (g_ws.seq < (unsigned)back) break;
-            if (g_ws.recent[(g_ws.seq - back) % CTL_ROT].conflicts(mine)) early = false;
-        }
-    cs.early = early;
+    const bool early = allowEarly && overlapCalls && g_ws.pdl != 0 && g_ws.chainable && g_ws.havePending &&
+                       g_ws.doneStream == st && !r.profile && !useGraph && !twoPhase && embed &&
+                       !g_ws.lastSpans.conflicts(mine);
     cs.waitFirst = early ? 0 : 1;
-    const bool sequenced = !useGraph;
-    cs.seq.done = sequenced ? doneWord : nullptr;
-    cs.seq.seq = g_ws.seq;
-    // pipelined: the set must be free (call seq - CTL_ROT published).  Not pipelined: k_norm has waited for the
-    // previous kernel, hence for every earlier call: nothing to poll (need = 0 is always met: done - 0 >= 0 ... the
-    // comparison is a signed 32-bit difference, so pass the value that is certainly reached).
-    cs.seq.need = early ? g_ws.seq - (unsigned)(CTL_ROT - 1) : g_ws.seq;
-    if (early && g_ws.seq < (unsigned)(CTL_ROT - 1)) cs.seq.need = 0;
     g_ws.haveStages = false;
 
     int launched = 0;
@@ -871,7 +847,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         if (rc) return rc;
     } else {
         if (g_ws.graphGen != g_allocGen) { g_ws.dropGraphs(); g_ws.graphGen = g_allocGen; }
-        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + slot;
+        Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + cs.slot;
         GraphKey key;
         std::memset(&key, 0, sizeof key);
         key.ref = ref; key.ev = ev; key.out = out; key.ctl = ctl; key.g = g;
@@ -908,7 +884,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         }
         hit->lastUse = ++g_ws.useClock;
         launched = hit->kernels;
-        g_ws.lastCtl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_SLOTS + slot;
+        g_ws.lastCtl = ctl;
         CU_TRY(cudaGraphLaunch(hit->exec, st));
     }
     g_ws.launches += launched;
@@ -916,16 +892,78 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     CU_TRY(cudaGetLastError());
     rc = mark_done(st);
     if (rc) return rc;
-    g_ws.chainable = sequenced && sets == CTL_ROT;
-    g_ws.chainStride = stride;
-    if (sequenced) {
-        g_ws.recent[g_ws.seq % CTL_ROT] = mine;
-        ++g_ws.seq;
-    }
+    g_ws.chainable = true;
+    g_ws.lastSpans = mine;
+    g_ws.slot = (g_ws.slot + 1) % CTL_ROT;
+    ++g_ws.calls;
+    ++g_callNo;
     g_ws.ctlClean = true;
     g_ws.lastStream = st; g_ws.lastN = g.N; g_ws.haveLast = true;
+    g_ws.lastEarly = early ? 1 : 0;
+    g_ws.numEarly += early ? 1 : 0;
+    g_lastWs = g_cur;
     return GAMMA_OK;
 }
+
+int lanes_init()
+{
+    if (g_lanes.ready) return GAMMA_OK;
+    CU_TRY(cudaEventCreateWithFlags(&g_lanes.fork, cudaEventDisableTiming));
+    for (int l = 0; l < LANES; ++l) CU_TRY(cudaStreamCreateWithFlags(&g_lanes.stream[l], cudaStreamNonBlocking));
+    for (int w = 0; w < B2B_WINDOW; ++w) CU_TRY(cudaEventCreateWithFlags(&g_lanes.done[w], cudaEventDisableTiming));
+    g_lanes.ready = true;
+    return GAMMA_OK;
+}
+
+// One back-to-back call (see LaneState).  `fresh`: the sequence starts here -- the lanes wait for what is on `user` now.
+int enqueue_on_lane(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
+                    const Resolved& r, float* out, cudaStream_t user, bool fresh)
+{
+    int rc = lanes_init();
+    if (rc) return rc;
+    LaneState& L = g_lanes;
+    if (fresh || !L.active || L.user != user) {
+        CU_TRY(cudaEventRecord(L.fork, user));
+        ++L.forkGen;
+        L.user = user;
+    }
+    L.active = false;                                      // set again on success
+    const unsigned long long j = L.next;
+    const int w = (int)(j % B2B_WINDOW), lane = (int)(j % LANES);
+    if (L.used[w]) CU_TRY(cudaEventSynchronize(L.done[w]));           // call j - B2B_WINDOW has ended (back-pressure)
+    cudaStream_t st = L.stream[lane];
+    if (L.laneFork[lane] != L.forkGen) {
+        CU_TRY(cudaStreamWaitEvent(st, L.fork, 0));
+        L.laneFork[lane] = L.forkGen;
+        L.laneDirty[lane] = true;
+    }
+    CallSpans mine;
+    const size_t bytes = (size_t)g.N * 4;
+    mine.rd[0].set(ref, bytes); mine.rd[1].set(ev, bytes); mine.wr[0].set(out, bytes);
+    mine.wr[1].set(r.stats.hist, (size_t)r.stats.nbins * 8); mine.wr[2].set(r.stats.summary, sizeof(gamma_summary));
+    for (int back = 1; back < B2B_WINDOW && (unsigned long long)back <= j; ++back) {
+        const int wi = (int)((j - back) % B2B_WINDOW);
+        if (L.used[wi] && L.laneOf[wi] != lane && L.spans[wi].conflicts(mine)) {
+            CU_TRY(cudaStreamWaitEvent(st, L.done[wi], 0));           // that call writes what this one touches, or reads what it writes
+            L.laneDirty[lane] = true;
+        }
+    }
+    Workspace* keep = g_cur;
+    g_cur = &g_pool[1 + lane];
+    rc = enqueue_pipeline(ref, ev, g, DD, mode, cutoff, r, out, st, !L.laneDirty[lane]);
+    g_cur = keep;
+    if (rc) { L.laneDirty[lane] = true; return rc; }
+    L.laneDirty[lane] = false;
+    CU_TRY(cudaEventRecord(L.done[w], st));
+    CU_TRY(cudaStreamWaitEvent(user, L.done[w], 0));                  // the caller's stream sees the result
+    L.spans[w] = mine; L.laneOf[w] = lane; L.used[w] = true;
+    ++L.next;
+    L.active = true;
+    return GAMMA_OK;
+}
+
+// any other library operation ends a sequence of back-to-back calls: the next one forks from the caller's stream again
+void end_b2b_sequence() { g_lanes.active = false; }
 
 }  // namespace
 
@@ -946,7 +984,20 @@ int gamma_eval_ex(const float* ref, const float* eval, const int dims[3], const 
     rc = resolve_opts(opts, r);
     if (rc) return rc;
     std::lock_guard<std::mutex> lock(g_mu);
-    return enqueue_pipeline(ref, eval, g, DD, mode, low_dose_cutoff, r, out_gamma, static_cast<cudaStream_t>(stream));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (r.backToBack) {
+        // honoured for the default kind of call only; everything else runs on the caller's stream, in stream order
+        cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
+        CU_TRY(cudaStreamIsCapturing(st, &capStatus));
+        long long byNMax = LISTS_BY_N_MAX;
+        if (const char* env = std::getenv("GAMMA_LISTS_BY_N_MAX")) byNMax = std::atoll(env);
+        static const bool overlapCalls = !(std::getenv("GAMMA_OVERLAP_CALLS") && std::getenv("GAMMA_OVERLAP_CALLS")[0] == '0');
+        if (overlapCalls && capStatus == cudaStreamCaptureStatusNone && !r.profile && !r.graph && g.N <= byNMax &&
+            r.tableMode == 1 && r.tableCap <= TAB_EMBED_MAX_CELLS)
+            return enqueue_on_lane(ref, eval, g, DD, mode, low_dose_cutoff, r, out_gamma, st, false);
+    }
+    end_b2b_sequence();
+    return enqueue_pipeline(ref, eval, g, DD, mode, low_dose_cutoff, r, out_gamma, st, false);
 }
 
 int gamma_eval(const float* ref, const float* eval, const int dims[3], const float spacing_mm[3], float DD,
@@ -983,36 +1034,15 @@ int gamma_eval_batch(int n_cases, const float* const* ref, const float* const* e
     CU_TRY(cudaStreamIsCapturing(st, &capStatus));
     if (capStatus != cudaStreamCaptureStatusNone)
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_batch cannot be captured into a CUDA graph; capture gamma_eval calls");
-    if (!g_lanes.ready) {
-        CU_TRY(cudaEventCreateWithFlags(&g_lanes.start, cudaEventDisableTiming));
-        for (int l = 0; l < BATCH_LANES; ++l) {
-            CU_TRY(cudaStreamCreateWithFlags(&g_lanes.stream[l], cudaStreamNonBlocking));
-            CU_TRY(cudaEventCreateWithFlags(&g_lanes.done[l], cudaEventDisableTiming));
-        }
-        g_lanes.ready = true;
-    }
-    const int lanes = n_cases < BATCH_LANES ? n_cases : BATCH_LANES;
-    CU_TRY(cudaEventRecord(g_lanes.start, st));                       // the lanes start after what is already on `stream`
-    for (int l = 0; l < lanes; ++l) CU_TRY(cudaStreamWaitEvent(g_lanes.stream[l], g_lanes.start, 0));
-    rc = GAMMA_OK;
     r.stats.hist = nullptr; r.stats.summary = nullptr;                // one pair of buffers cannot serve n cases
-    for (int i = 0; i < n_cases && rc == GAMMA_OK; ++i) {
-        const int l = i % lanes;
+    // The cases run like back-to-back calls: round-robin over the library's lane streams, the first one after what is
+    // already on `stream`, `stream` continues after the last; hazards between the cases' buffers are checked.
+    for (int i = 0; i < n_cases; ++i) {
         GridP g;
         make_grid(dims + 3 * i, spacing_mm + 3 * i, DTA_mm, g);
-        g_cur = &g_pool[1 + l];
-        // The lane streams are the library's own: behind the first case of a lane (which waits for `stream`) its
-        // calls are back to back by construction, so they are pipelined (hazards between the cases' buffers are
-        // checked as for any pipelined call).
-        r.backToBack = i >= lanes ? 1 : 0;
-        rc = enqueue_pipeline(ref[i], eval[i], g, DD, mode, low_dose_cutoff, r, out_gamma[i], g_lanes.stream[l]);
-        g_cur = &g_pool[0];
+        rc = enqueue_on_lane(ref[i], eval[i], g, DD, mode, low_dose_cutoff, r, out_gamma[i], st, i == 0);
+        if (rc) return rc;
     }
-    for (int l = 0; l < lanes; ++l) {                                 // `stream` continues when every lane is done
-        cudaEventRecord(g_lanes.done[l], g_lanes.stream[l]);
-        cudaStreamWaitEvent(st, g_lanes.done[l], 0);
-    }
-    if (rc) return rc;
     CU_TRY(cudaGetLastError());
     return GAMMA_OK;
 }
@@ -1032,9 +1062,9 @@ int gamma_eval_host(const float* ref_host, const float* eval_host, const int dim
     Resolved r;
     rc = resolve_opts(opts, r);
     if (rc) return rc;
-    r.backToBack = 0;                                    // the copies sit between consecutive calls
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::lock_guard<std::mutex> lock(g_mu);
+    end_b2b_sequence();
     const size_t bytes = (size_t)g.N * 4;
     CU_TRY(g_ws.hRef.need(bytes)); CU_TRY(g_ws.hEval.need(bytes)); CU_TRY(g_ws.hOut.need(bytes));
     rc = order_after_previous(st);
@@ -1042,7 +1072,7 @@ int gamma_eval_host(const float* ref_host, const float* eval_host, const int dim
     CU_TRY(cudaMemcpyAsync(g_ws.hRef.p, ref_host, bytes, cudaMemcpyHostToDevice, st));     // A2 step 1
     CU_TRY(cudaMemcpyAsync(g_ws.hEval.p, eval_host, bytes, cudaMemcpyHostToDevice, st));
     rc = enqueue_pipeline(static_cast<const float*>(g_ws.hRef.p), static_cast<const float*>(g_ws.hEval.p), g, DD, mode,
-                          low_dose_cutoff, r, static_cast<float*>(g_ws.hOut.p), st);
+                          low_dose_cutoff, r, static_cast<float*>(g_ws.hOut.p), st, false);
     if (rc) return rc;
     CU_TRY(cudaMemcpyAsync(out_gamma_host, g_ws.hOut.p, bytes, cudaMemcpyDeviceToHost, st)); // A2 step 8
     rc = mark_done(st);
@@ -1061,6 +1091,7 @@ int gamma_stats(const float* gamma, long long n, int nbins, float hist_max, unsi
     if (nbins < 1 || nbins > STATS_MAX_BINS) return fail(GAMMA_ERR_INVALID_ARGUMENT, "nbins must be in [1, 4096]");
     if (!(hist_max > 0.0f) || !std::isfinite(hist_max)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "hist_max must be > 0");
     std::lock_guard<std::mutex> lock(g_mu);
+    end_b2b_sequence();
     int rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -1089,6 +1120,7 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "need 0 <= begin_bit < end_bit <= 32, multiples of 8");
     if (n == 0) return GAMMA_OK;
     std::lock_guard<std::mutex> lock(g_mu);
+    end_b2b_sequence();
     int rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -1140,6 +1172,7 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     int rc = make_grid(dims, spacing_mm, DTA_mm, g);
     if (rc) return rc;
     std::lock_guard<std::mutex> lock(g_mu);
+    end_b2b_sequence();
     rc = ensure_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -1152,7 +1185,7 @@ int gamma_offset_table(const int dims[3], const float spacing_mm[3], float DTA_m
     if (rc) return rc;
     Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_STANDALONE;
     EvalP e;
-    e.DD = 1.0f; e.cutoff = 0.0f; e.norm_dose = 1.0f; e.mode = 0; e.algo = 0;
+    e.DD = 1.0f; e.cutoff = 0.0f; e.norm_dose = 1.0f; e.mode = 0; e.algo = 0; e.call = 0;
     k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, st>>>(
         g, e, ctl, radius, max_entries, static_cast<int4*>(g_ws.table.p), static_cast<unsigned*>(g_ws.tmpL.p),
         static_cast<unsigned*>(g_ws.tmpIdx.p), 0);
@@ -1168,13 +1201,14 @@ int gamma_get_counters(gamma_counters* out_host)
     g_err.clear();
     if (!out_host) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_host is NULL");
     std::lock_guard<std::mutex> lock(g_mu);
-    if (!g_ws.haveLast || !g_ws.ctl.p) return fail(GAMMA_ERR_INVALID_ARGUMENT, "no gamma_eval call to report on");
-    if (g_ws.lastStream) CU_TRY(cudaStreamSynchronize(g_ws.lastStream));
+    const Workspace& w = *g_lastWs;                  // the workspace the last gamma_eval* call ran on
+    if (!w.haveLast || !w.ctl.p) return fail(GAMMA_ERR_INVALID_ARGUMENT, "no gamma_eval call to report on");
+    if (w.lastStream) CU_TRY(cudaStreamSynchronize(w.lastStream));
     else CU_TRY(cudaDeviceSynchronize());            // last call was captured by the caller: no stream to wait on
     Ctl c;
-    CU_TRY(cudaMemcpy(&c, g_ws.lastCtl, sizeof c, cudaMemcpyDeviceToHost));
+    CU_TRY(cudaMemcpy(&c, w.lastCtl, sizeof c, cudaMemcpyDeviceToHost));
     std::memset(out_host, 0, sizeof *out_host);
-    out_host->n_voxels = g_ws.lastN;
+    out_host->n_voxels = w.lastN;
     out_host->n_evaluated = c.nEval;
     out_host->n_table_search = (long long)c.nSearch + (long long)c.nDeep;
     out_host->table_entries = c.tableCount;
@@ -1184,7 +1218,9 @@ int gamma_get_counters(gamma_counters* out_host)
     out_host->max_key = cv.f;
     out_host->norm_dose = ordered_to_float(c.normOrd);
     out_host->table_truncated = (int)c.tableTrunc;
-    out_host->n_ring_search = g_ws.lastClasses ? (int)c.nSearch : 0;
+    out_host->n_ring_search = w.lastClasses ? (int)c.nSearch : 0;
+    out_host->pipelined = (&w != &g_pool[0] && &w != &g_pool[WS_CAPTURE]) ? 1 : 0;
+    out_host->calls_pipelined = (long long)g_lanes.next;
     return GAMMA_OK;
 }
 
@@ -1213,6 +1249,45 @@ long long gamma_launch_count(void)
     long long n = 0;
     for (const Workspace& w : g_pool) n += w.launches;
     return n;
+}
+
+// ---- device timeline (GAMMA_TRACE builds; common.cuh)
+#ifdef GAMMA_TRACE
+namespace { TraceRec* g_traceDev = nullptr; }
+#endif
+int gamma_trace_reset(void)
+{
+    g_err.clear();
+#ifdef GAMMA_TRACE
+    std::lock_guard<std::mutex> lock(g_mu);
+    CU_TRY(cudaDeviceSynchronize());
+    const size_t n = (size_t)TRACE_CALLS * TRACE_KERNELS;
+    if (!g_traceDev) CU_TRY(cudaMalloc(&g_traceDev, n * sizeof(TraceRec)));
+    static TraceRec init[TRACE_CALLS * TRACE_KERNELS];
+    for (size_t i = 0; i < n; ++i) { init[i].first = ~0ull; init[i].waited = 0; init[i].last = 0; init[i].pad_ = 0; }
+    CU_TRY(cudaMemcpy(g_traceDev, init, n * sizeof(TraceRec), cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpyToSymbol(g_trace_buf, &g_traceDev, sizeof g_traceDev));
+    return GAMMA_OK;
+#else
+    return fail(GAMMA_ERR_INVALID_ARGUMENT, "libgamma_b200 was built without -DGAMMA_TRACE");
+#endif
+}
+
+int gamma_trace_read(unsigned long long* out_host, long long* next_call)
+{
+    g_err.clear();
+#ifdef GAMMA_TRACE
+    if (!out_host || !next_call) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_host / next_call is NULL");
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (!g_traceDev) return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_trace_reset has not been called");
+    CU_TRY(cudaDeviceSynchronize());
+    CU_TRY(cudaMemcpy(out_host, g_traceDev, (size_t)TRACE_CALLS * TRACE_KERNELS * sizeof(TraceRec), cudaMemcpyDeviceToHost));
+    *next_call = (long long)g_callNo;
+    return GAMMA_OK;
+#else
+    (void)out_host; (void)next_call;
+    return fail(GAMMA_ERR_INVALID_ARGUMENT, "libgamma_b200 was built without -DGAMMA_TRACE");
+#endif
 }
 
 long long gamma_workspace_bytes(void)
@@ -1257,13 +1332,15 @@ int gamma_fp32_probe(int repeats, double* out_tflops, void* stream)
 void gamma_release(void)
 {
     std::lock_guard<std::mutex> lock(g_mu);
+    cudaDeviceSynchronize();
     for (Workspace& w : g_pool) w.releaseAll();
-    for (int l = 0; l < BATCH_LANES; ++l) {
+    for (int l = 0; l < LANES; ++l)
         if (g_lanes.stream[l]) { cudaStreamDestroy(g_lanes.stream[l]); g_lanes.stream[l] = nullptr; }
-        if (g_lanes.done[l]) { cudaEventDestroy(g_lanes.done[l]); g_lanes.done[l] = nullptr; }
-    }
-    if (g_lanes.start) { cudaEventDestroy(g_lanes.start); g_lanes.start = nullptr; }
-    g_lanes.ready = false;
+    for (int w = 0; w < B2B_WINDOW; ++w)
+        if (g_lanes.done[w]) { cudaEventDestroy(g_lanes.done[w]); g_lanes.done[w] = nullptr; }
+    if (g_lanes.fork) { cudaEventDestroy(g_lanes.fork); g_lanes.fork = nullptr; }
+    g_lanes = LaneState();
+    g_lastWs = &g_pool[0];
 }
 
 void gamma_abi_sizes(int out_host[4])

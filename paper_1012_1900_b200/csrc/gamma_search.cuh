@@ -2,8 +2,7 @@
 //
 //   k_norm           a0 + A1 step 1: D_norm = max(ref) (reading 8) and max |D_r - D_e|,
 //                    which bounds every key and so fixes the radius of the offset table before the search
-//                    list exists; zeroes the caller's fused-statistics buffers; holds the call back until its
-//                    set of work lists is free (SeqP, common.cuh).
+//                    list exists; zeroes the caller's fused-statistics buffers and the control block of the NEXT call.
 //   k_classify       a1: cutoff decision, NaN for excluded voxels, compaction of the evaluated voxels.
 // Consecutive kernels of a call are chained by programmatic dependent launch (pdl_wait / pdl_launch_dependents).
 //   k_prep_star      a1 + first part of a4: per voxel DD, cutoff, key (Algorithm A2 step 2 / CUDA Kernel 1,
@@ -60,15 +59,22 @@ __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepc
 
 
 __global__ void __launch_bounds__(NORM_THREADS)
-k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur, SeqP seq,
-       int waitFirst, StatsP st)
+k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur,
+       Ctl* __restrict__ next, int waitFirst, unsigned call, StatsP st)
 {
     pdl_launch_dependents();
+    trace_first(call, 0);
     // waitFirst: ref / eval may be results of the operation in front of this call: nothing is read before that
-    // operation has completed.  Otherwise (the caller asserted back-to-back library calls, gamma_opts::back_to_back)
-    // this kernel runs beside the previous call's table search: it reads this call's inputs only and touches the
-    // control block of its own set once that set is free.
+    // operation has completed.  Otherwise (library-owned stream, the operation in front is the previous call's
+    // k_table_search, which triggers its dependents at once) this kernel runs in the tail of that call: it reads this
+    // call's inputs only, writes control blocks that call does not use, and waits for its end as its LAST act, so that
+    // nothing after it can overtake the previous call.
     if (waitFirst) pdl_wait();
+    trace_waited(call, 0);
+    if (blockIdx.x == gridDim.x - 1 && next != nullptr) {      // the next call finds its control block cleared
+        unsigned* w = reinterpret_cast<unsigned*>(next);
+        for (int i = threadIdx.x; i < (int)(sizeof(Ctl) / 4); i += NORM_THREADS) w[i] = 0u;
+    }
     if (st.hist) {                                              // a6 fused: the caller's buffers start from zero
         for (int b = blockIdx.x * NORM_THREADS + threadIdx.x; b < st.nbins; b += gridDim.x * NORM_THREADS) st.hist[b] = 0ull;
         if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -112,15 +118,14 @@ k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int m
     a = block_max_256(a, sm8);
     if (mode == 1) r = block_max_256(r, sm8);
     if (threadIdx.x == 0) {
-        // The set (control block, table, work lists) this call uses was last used by call seq - CTL_ROT: wait until
-        // that call has been published (its last block has zeroed the control block).  Every block of an earlier
-        // kernel in the stream is resident or done when this kernel starts, so the wait cannot deadlock.
-        if (seq.done)
-            while ((int)(ld_acquire_u32(seq.done) - seq.need) < 0) __nanosleep(64);
         atomicMax(&cur->normOrd, float_to_ordered(m));
         if (a > 0.0f) atomicMax(&cur->maxAbsDD, __float_as_uint(a));
         if (r > 0.0f) atomicMax(&cur->maxRatio, __float_as_uint(r));
+        // started early: one block holds the grid open until the previous call has ended (the kernels after this one
+        // reuse its work lists); the other blocks give their registers back at once
+        if (!waitFirst && blockIdx.x == 0) pdl_wait();
     }
+    trace_last(call, 0);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -165,11 +170,13 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
         return nval;
     };
     pdl_launch_dependents();
+    trace_first(e.call, 1);
     // ref is an input of the call, not a result of k_norm: the first chunk is fetched while k_norm drains
     float Dr[4] = {0.0f, 0.0f, 0.0f, 0.0f};
     int nval = 0;
     if ((int)blockIdx.x < numChunks) nval = load_chunk(blockIdx.x, Dr);
     pdl_wait();                                       // k_norm's maxima from here on
+    trace_waited(e.call, 1);
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
     const double dnorm = (double)dnormF;
     const double thr = (double)e.cutoff * dnorm;      // decided in double (include/gamma_b200.h)
@@ -225,6 +232,7 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
         __syncthreads();
         if (tid == 0 && sNan) atomicAdd(&st.summary->n_nan, sNan);
     }
+    trace_last(e.call, 1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -257,6 +265,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     const int tid = threadIdx.x, lane = tid & 31;
     const unsigned FULL = 0xffffffffu;
     pdl_launch_dependents();
+    trace_first(e.call, 2);
     for (int d = tid; d < KEY_DIGITS; d += STAR_THREADS) sHist[d] = 0;
     // a3 inside the wait: the prefix table depends on the geometry only, so the first blocks build it (one slice of
     // buckets each) while k_classify is still running -- no side stream, no join, nothing added to the chain.
@@ -273,6 +282,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
                 sTab, g, e, ctl, &tabPlan, 0.0f, TAB_EMBED_MAX_CELLS, table, tmpL, tmpIdx, slice);
     }
     pdl_wait();                                           // k_classify's results from here on
+    trace_waited(e.call, 2);
     // The index of the warp's first voxel is fetched together with the control block, not after it: one L2 round
     // trip less in front of the first round.  Entries at or beyond M are never used (and never dereferenced).
     unsigned item = blockIdx.x * (STAR_THREADS / 32) + (tid >> 5);
@@ -403,6 +413,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     }
     if (st.hist && nNanKey) atomicAdd(&st.summary->n_nan, nNanKey);
     fused_stats_flush(sStat, st);
+    trace_last(e.call, 2);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -527,7 +538,11 @@ __device__ __forceinline__ float group_min(float v)
 #define GAMMA_SEARCH_MIN_BLOCKS 6
 #endif
 constexpr int SEARCH_THREADS = GAMMA_SEARCH_THREADS;
-constexpr int SEARCH_MIN_BLOCKS = GAMMA_SEARCH_MIN_BLOCKS;   // adaptive-lane kernel (MODE 0)
+constexpr int SEARCH_MIN_BLOCKS = GAMMA_SEARCH_MIN_BLOCKS;   // adaptive-lane kernel (MODE 0): register budget
+#ifndef GAMMA_SEARCH_GRID_BLOCKS
+#define GAMMA_SEARCH_GRID_BLOCKS GAMMA_SEARCH_MIN_BLOCKS
+#endif
+constexpr int SEARCH_GRID_BLOCKS = GAMMA_SEARCH_GRID_BLOCKS; // blocks per SM actually launched (<= SEARCH_MIN_BLOCKS)
 
 struct SearchCtx {
     const float* ref; const float* ev; float* out;
@@ -711,16 +726,17 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
                EvalP e, Ctl* __restrict__ ctl, const unsigned* __restrict__ listKey,
                const unsigned* __restrict__ listIdx, const unsigned* __restrict__ deepKey,
                const unsigned* __restrict__ deepIdx, const int4* __restrict__ table, int deepDigit, int classes,
-               const __grid_constant__ GammaRingP ring, Ctl* __restrict__ report, SeqP seq, StatsP st)
+               const __grid_constant__ GammaRingP ring, StatsP st)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     __shared__ FusedStats<SEARCH_THREADS> sStat;
-    __shared__ unsigned sLast;
     SearchCtx c;
     fused_stats_init(sStat, st);
+    trace_first(e.call, 3);
     pdl_wait();
     pdl_launch_dependents();                             // the next call's k_norm may use the SMs this kernel leaves
+    trace_waited(e.call, 3);
     const unsigned nS = ctl->nSearch;
     unsigned nDeep = 0;
     if (MODE == 0 && classes) {
@@ -768,31 +784,7 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
         if (lane == 0 && visits) atomicAdd(&ctl->visits, (unsigned long long)visits);
     }
     fused_stats_flush(sStat, st);
-    // ---- end of the call (common.cuh, "Device control block"): the last block to finish copies the control block to
-    // the set's report, zeroes it and publishes the call -- in call order, so that the end of this kernel implies the
-    // end of every earlier call on the workspace.
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        sLast = atomicAdd(&ctl->blocksDone, 1u) == gridDim.x - 1u ? 1u : 0u;
-    }
-    __syncthreads();
-    if (sLast) {
-        __threadfence();
-        if (threadIdx.x == 0 && seq.done)
-            while ((int)(ld_acquire_u32(seq.done) - seq.seq) < 0) __nanosleep(64);
-        unsigned* w = reinterpret_cast<unsigned*>(ctl);
-        unsigned* r = reinterpret_cast<unsigned*>(report);
-        for (int i = threadIdx.x; i < (int)(sizeof(Ctl) / 4); i += SEARCH_THREADS) {
-            r[i] = __ldcg(w + i);
-            w[i] = 0u;
-        }
-        __syncthreads();
-        if (threadIdx.x == 0 && seq.done) {
-            __threadfence();
-            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(seq.done), "r"(seq.seq + 1u) : "memory");
-        }
-    }
+    trace_last(e.call, 3);
 }
 
 }  // namespace gamma_b200

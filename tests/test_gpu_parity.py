@@ -655,6 +655,16 @@ def test_pipelined_calls_mixed_with_large_tables_and_other_entry_points():
                 GammaOpts(back_to_back=1, table_cap=4096), GammaOpts(back_to_back=1), GammaOpts(back_to_back=1),
                 GammaOpts(back_to_back=1, graph=1), GammaOpts(back_to_back=1), GammaOpts(back_to_back=1, profile_stages=1),
                 GammaOpts(back_to_back=1), GammaOpts(back_to_back=1, presort=3), GammaOpts(back_to_back=1, lanes_per_voxel=1)]
+    # what each variant returns on its own (the ring search of the default path rounds its constants on the host: the
+    # other search variants agree with it to an ulp, not bit for bit)
+    import dataclasses
+    alone = {}
+    for k, (r, e, args, _) in enumerate(data):
+        for v, o in enumerate(variants):
+            kind = dataclasses.astuple(dataclasses.replace(o, back_to_back=0, graph=0, profile_stages=0))
+            if (k, kind) not in alone:
+                alone[(k, kind)] = binding.gamma_eval_ex(r, e, *args, dataclasses.replace(o, back_to_back=0)).clone()
+                torch.cuda.synchronize()
     outs = []
     for i in range(72):
         k = (i + i // 5) % 2
@@ -666,7 +676,10 @@ def test_pipelined_calls_mixed_with_large_tables_and_other_entry_points():
             binding.gamma_offset_table((40, 30, 20), (2.0, 2.0, 2.0), 2.0, 6.0)
     torch.cuda.synchronize()
     for i, (k, o) in enumerate(outs):
-        assert torch.equal(_nn(o), _nn(data[k][3])), (i, variants[i % len(variants)])
+        v = variants[i % len(variants)]
+        kind = dataclasses.astuple(dataclasses.replace(v, back_to_back=0, graph=0, profile_stages=0))
+        assert torch.equal(_nn(o), _nn(alone[(k, kind)])), (i, v)
+        assert float((_nn(o) - _nn(data[k][3])).abs().max()) <= 2e-6
 
 
 @pytest.mark.parametrize("name,nbins,hmax", [("cfg2_small", 64, 4.0), ("cfg1", 17, 1.5), ("cfg3", 1024, 3.0),
