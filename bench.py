@@ -34,12 +34,18 @@ sys.path.insert(0, ROOT)
 SM_COUNT, FP32_LANES, SM_MAX_MHZ_NOMINAL = 148, 128, 1965.0
 F_CELL_3D, F_CELL_2D = 1911.0, 190.0       # canonical flops per visited cell, frozen in BASELINE.md
 L2_BYTES = 126e6
-# executed FP32 flops per unit (ncu smsp__sass_thread_inst_executed_op_{fadd,fmul,ffma}; profiles/)
-# r1e: k_star 65.7 Mflop / 160 256 voxels; k_table_search = 379 per owner-vertex visit + 1210 per ring item (solved from
-# the cfg2 and cfg3 launches, checked on cfg5 and cfg4_fine to 0.1 %)
-FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT, FLOP_PER_RING_ITEM = 410.0, 379.0, 1210.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on cfg3 from the same ncu --set full capture
-TRAFFIC_BYTES = {"k_star": 2.68e6, "k_table_search": 1.83e6}
+# executed FP32 flops per unit (ncu smsp__sass_thread_inst_executed_op_{fadd,fmul,ffma}_pred_on, FFMA counted twice),
+# re-measured on the round-2 kernels (profiles/r2_mix_<case>.csv, profiles/r2_profile.md): k_star 65.55 Mflop / 160 256
+# voxels; k_table_search = 379 per owner-vertex visit + 1 211 per ring item (solved from the cfg2 and cfg3 launches,
+# reproduces cfg5 and cfg4_fine to 0.1 %)
+FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT, FLOP_PER_RING_ITEM = 409.0, 379.0, 1211.0
+# executed WARP instructions per unit (smsp__inst_executed.sum of the same capture): k_norm and k_classify per grid voxel,
+# k_star per evaluated voxel, k_table_search per owner-vertex visit / per ring item / fixed part per launch
+WINST = {"norm_per_voxel": 0.748, "classify_per_voxel": 1.74, "star_per_voxel": 36.76, "visit": 21.85, "ring_item": 44.4,
+         "search_fixed": 0.268e6}
+SCHEDULERS = 4 * SM_COUNT                   # one warp instruction per scheduler per cycle
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on cfg3 from the ncu --set full capture (profiles/r2_full_summary.csv)
+TRAFFIC_BYTES = {"k_star": 2.69e6, "k_table_search": 1.83e6}
 
 
 def f32(x):
@@ -192,7 +198,8 @@ def main():
     ap.add_argument("--presort", type=int, default=0)
     ap.add_argument("--star-phase", type=int, default=0)
     ap.add_argument("--lanes", type=int, default=0)
-    ap.add_argument("--serial-calls", action="store_true", help="do not pipeline consecutive calls (opts.back_to_back = 0)")
+    ap.add_argument("--serial-calls", action="store_true", help="do not overlap consecutive calls (opts.back_to_back = 0)")
+    ap.add_argument("--star-load", type=int, default=0, help="opts.star_load: 1 compacted list (default), 2 TMA tiles, 3 tiles by loads")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -221,7 +228,7 @@ def main():
 
     N = case.ref.size
     # back_to_back: the timed loop enqueues nothing but gamma_eval_ex calls on the stream, which is what the flag asserts
-    okw = dict(presort=args.presort, star_phase=args.star_phase, lanes_per_voxel=args.lanes)
+    okw = dict(presort=args.presort, star_phase=args.star_phase, lanes_per_voxel=args.lanes, star_load=args.star_load)
     opts = GammaOpts(back_to_back=0 if args.serial_calls else 1, **okw)
     popts = GammaOpts(profile_stages=1, **okw)
     # Rotating input sets larger than L2 (126 MB): every timed step reads buffers that the previous steps have
@@ -360,6 +367,16 @@ def main():
             "algorithmic_flops_per_launch": alg,
             "achieved": alg / (kernel_ms[dom] * 1e-3) / 1e12}
     roof["frac"] = roof["achieved"] / peak
+    roof["frac_of_ffma_chain_probe"] = roof["achieved"] / probe_tflops if probe_tflops > 0 else None
+    # the bound that actually limits this path: issue slots.  Warp instructions of one step (per-unit constants above x
+    # the units the library counted) / (592 schedulers x 1 instruction per cycle x the SM clock)
+    winst = (N * (WINST["norm_per_voxel"] + WINST["classify_per_voxel"]) + M * WINST["star_per_voxel"]
+             + cnt["vertex_visits"] * WINST["visit"] + cnt["n_ring_search"] * WINST["ring_item"] + WINST["search_fixed"])
+    clk_hz = (clk.get("sm_mhz") or SM_MAX_MHZ_NOMINAL) * 1e6
+    issue_us = winst / SCHEDULERS / clk_hz * 1e6
+    roof["issue"] = {"warp_inst": winst, "bound_us": issue_us, "frac": issue_us / (ms_step * 1e3),
+                     "note": "executed warp instructions / (592 schedulers x 1 per cycle x SM clock) over the step time; "
+                             "3D grids (per-unit constants measured on cfg2 / cfg3 / cfg5 / cfg4_fine)"}
     exec_total = units["k_star"] * flop_per_unit["k_star"] + units["k_table_search"] * flop_per_unit["k_table_search"]
     roof["whole_path"] = {"executed_fp32_flops": exec_total, "achieved": exec_total / (ms_step * 1e-3) / 1e12,
                           "frac": exec_total / (ms_step * 1e-3) / 1e12 / peak}

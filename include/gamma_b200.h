@@ -134,6 +134,15 @@ typedef struct gamma_opts {
                              one after the other.  What the library cannot see is foreign work on `stream` between two
                              calls, hence the assertion.  Ignored (the call runs on `stream` itself) with
                              profile_stages, graph = 1, large tables, grids above 2^25 voxels and under stream capture */
+    int star_load;        /* how the star phase gets its evaluation doses (BASELINE.json north_star (4)).
+                             0: default (= 1); 1: compacted list -- k_classify writes the list of evaluated voxels,
+                             k_star reads each voxel's 27 doses through L1 / L2, every evaluated voxel in flight at once
+                             (4 kernels per call); 2: spatial tiles of 8 x 4 x 4 voxels plus a halo of one voxel staged
+                             by the TMA into shared memory, two tiles in flight, classification, compaction and star
+                             phase in ONE kernel (3 kernels per call; 3D grids with the default presort / star_phase;
+                             needs nx % 4 == 0 and 16-byte aligned ref / eval, else it behaves as 3); 3: the same tile
+                             kernel with the tiles filled by cooperative loads.  Same gamma, bit for bit; measured on
+                             B200 the list is faster (profiles/r2_star_load.md), hence the default                  */
     int stats_nbins;      /* a6 fused into the call (all four stats_* fields; stats_hist = NULL: off).  The gamma
                              kernels accumulate, where they write gamma, what gamma_stats computes from the finished map:
                              same definition, same results (counts and histogram exact, sums in double), no second pass

@@ -39,7 +39,7 @@ class _COpts(ctypes.Structure):
     _fields_ = [("norm_dose", ctypes.c_float), ("presort", ctypes.c_int), ("star_phase", ctypes.c_int),
                 ("lanes_per_voxel", ctypes.c_int), ("sort_key_bits", ctypes.c_int), ("table_cap", ctypes.c_longlong),
                 ("profile_stages", ctypes.c_int), ("graph", ctypes.c_int), ("table_radius", ctypes.c_int),
-                ("interpolation", ctypes.c_int), ("back_to_back", ctypes.c_int), ("stats_nbins", ctypes.c_int),
+                ("interpolation", ctypes.c_int), ("back_to_back", ctypes.c_int), ("star_load", ctypes.c_int), ("stats_nbins", ctypes.c_int),
                 ("stats_hist", ctypes.c_void_p), ("stats_summary", ctypes.c_void_p), ("stats_hist_max", ctypes.c_float)]
 
 
@@ -76,11 +76,25 @@ class GammaOpts:
     table_radius: int = 0     # 1 data-independent prefix table (default), 2 the paper's radius max|DD|/dD
     graph: int = 0            # 1 replay a cached CUDA graph for repeated arguments, 2 plain launches (default)
     back_to_back: int = 0     # 1: caller asserts nothing else was enqueued on the stream since the previous call
+    star_load: int = 0        # 1 compacted list + __ldg (default), 2 TMA-staged tiles, 3 tiles by cooperative loads
     stats_hist: object = None     # int64 CUDA tensor [nbins]: a6 fused into the call (with stats_summary)
     stats_summary: object = None  # uint8 CUDA tensor [48]: gamma_summary bytes, decode with decode_summary
     stats_hist_max: float = 0.0
 
     def _c(self):
+        # the ctypes struct of the last field values is kept (argument marshalling only)
+        key = (self.norm_dose, self.presort, self.star_phase, self.lanes_per_voxel, self.sort_key_bits, self.table_cap,
+               self.profile_stages, self.interpolation, self.table_radius, self.graph, self.back_to_back, self.star_load,
+               None if self.stats_hist is None else (self.stats_hist.data_ptr(), self.stats_hist.numel()),
+               None if self.stats_summary is None else self.stats_summary.data_ptr(), self.stats_hist_max)
+        hit = self.__dict__.get("_cached")
+        if hit is not None and hit[0] == key:
+            return hit[1]
+        c = self._build()
+        self.__dict__["_cached"] = (key, c)
+        return c
+
+    def _build(self):
         nb = int(self.stats_hist.numel()) if self.stats_hist is not None else 0
         if (self.stats_hist is None) != (self.stats_summary is None):
             raise GammaError("stats_hist and stats_summary must be given together")
@@ -92,7 +106,7 @@ class GammaOpts:
                 raise GammaError("stats_summary must be a contiguous CUDA tensor of at least 48 bytes")
         return _COpts(float(self.norm_dose), int(self.presort), int(self.star_phase), int(self.lanes_per_voxel),
                       int(self.sort_key_bits), int(self.table_cap), int(self.profile_stages), int(self.graph),
-                      int(self.table_radius), int(self.interpolation), int(self.back_to_back), nb,
+                      int(self.table_radius), int(self.interpolation), int(self.back_to_back), int(self.star_load), nb,
                       self.stats_hist.data_ptr() if self.stats_hist is not None else None,
                       self.stats_summary.data_ptr() if self.stats_summary is not None else None,
                       float(self.stats_hist_max))

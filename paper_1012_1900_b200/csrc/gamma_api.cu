@@ -16,6 +16,7 @@
 #include "offset_table.cuh"
 #include "radix_sort.cuh"
 #include "stats.cuh"
+#include "tile_star.cuh"
 
 using namespace gamma_b200;
 
@@ -86,7 +87,7 @@ struct GraphKey {
     void* ctl;
     GridP g;
     float DD, cutoff, normDose;
-    int mode, presort, star, lanes, keyBits, tableMode, algo, statsBins;
+    int mode, presort, star, lanes, keyBits, tableMode, algo, statsBins, starLoad;
     long long tableCap;
     const void *statsHist, *statsSummary;
     float statsScale;
@@ -147,6 +148,7 @@ struct Workspace {
     long long launches = 0;        // kernels launched so far (gamma_launch_count)
     int numSM = 0;
     int occStar[2] = {0, 0};       // resident blocks per SM of k_star<false/true>
+    int occTile[2] = {0, 0};       // resident blocks per SM of k_tile_star<false/true>
     int pdl = -1;                  // programmatic dependent launch between the kernels of a call (GAMMA_PDL=0 disables)
     int graphs = -1;               // replay the call as a cached CUDA graph (GAMMA_GRAPH=0 disables)
     bool frozen = false;           // addresses of this workspace are baked into a caller's CUDA graph: it must not move
@@ -410,7 +412,7 @@ int make_grid(const int dims[3], const float spacing_mm[3], float DTA_mm, GridP&
 }
 
 struct Resolved {
-    int presort, star, lanes, keyBits, profile, graph, tableMode, algo, backToBack;
+    int presort, star, lanes, keyBits, profile, graph, tableMode, algo, backToBack, starLoad;
     long long tableCap;
     float normDose;
     StatsP stats;      // a6 fused into the gamma kernels (hist == nullptr: off)
@@ -419,10 +421,12 @@ struct Resolved {
 int resolve_opts(const gamma_opts* o, Resolved& r)
 {
     r.presort = 4; r.star = 1; r.lanes = 0; r.keyBits = 16; r.tableCap = 0; r.tableMode = 1; r.normDose = 0.0f;
-    r.profile = 0; r.graph = 0; r.algo = 0; r.backToBack = 0;
+    r.profile = 0; r.graph = 0; r.algo = 0; r.backToBack = 0; r.starLoad = 0;
     r.stats.hist = nullptr; r.stats.summary = nullptr; r.stats.nbins = 0; r.stats.binScale = 0.0f;
     if (!o) { r.tableCap = TAB_EMBED_MAX_CELLS; return GAMMA_OK; }
     if (o->back_to_back < 0 || o->back_to_back > 1) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.back_to_back must be 0 or 1");
+    if (o->star_load < 0 || o->star_load > 3) return fail(GAMMA_ERR_INVALID_ARGUMENT, "opts.star_load must be 0, 1, 2 or 3");
+    r.starLoad = o->star_load;
     r.backToBack = o->back_to_back;
     if (o->stats_hist || o->stats_summary) {
         if (!o->stats_hist || !o->stats_summary)
@@ -482,6 +486,65 @@ int check_criteria(float DD, int mode, float cutoff)
 }
 
 constexpr size_t CTL_BYTES = CTL_SLOTS * sizeof(Ctl);
+
+// ---- TMA descriptors of k_tile_star (tile_star.cuh).  cuTensorMapEncodeTiled is fetched through the runtime (the
+// library does not link libcuda); the last few (pointer, dims, box) descriptors are kept.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encodeTiled = nullptr;
+bool g_encodeTried = false;
+
+bool tma_usable(const void* ref, const void* ev, const GridP& g)
+{
+    if (!g_encodeTried) {
+        g_encodeTried = true;
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            g_encodeTiled = reinterpret_cast<EncodeTiledFn>(fn);
+        else
+            cudaGetLastError();
+    }
+    return g_encodeTiled != nullptr && g.n[0] % 4 == 0 &&
+           ((reinterpret_cast<uintptr_t>(ref) | reinterpret_cast<uintptr_t>(ev)) & 15u) == 0;
+}
+
+struct MapKey { const void* p; int n[3]; unsigned box[3]; };
+struct MapEntry { MapKey key; CUtensorMap map; unsigned long long use; };
+constexpr int MAP_CACHE = 64;
+MapEntry g_maps[MAP_CACHE];
+int g_numMaps = 0;
+unsigned long long g_mapClock = 0;
+
+int tensor_map(const float* p, const GridP& g, unsigned bx, unsigned by, unsigned bz, CUtensorMap& out)
+{
+    MapKey key;
+    std::memset(&key, 0, sizeof key);
+    key.p = p; key.n[0] = g.n[0]; key.n[1] = g.n[1]; key.n[2] = g.n[2]; key.box[0] = bx; key.box[1] = by; key.box[2] = bz;
+    for (int i = 0; i < g_numMaps; ++i)
+        if (std::memcmp(&g_maps[i].key, &key, sizeof key) == 0) { g_maps[i].use = ++g_mapClock; out = g_maps[i].map; return GAMMA_OK; }
+    const cuuint64_t dims[3] = {(cuuint64_t)g.n[0], (cuuint64_t)g.n[1], (cuuint64_t)g.n[2]};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.n[0] * 4u, (cuuint64_t)g.n[0] * (cuuint64_t)g.n[1] * 4u};
+    const cuuint32_t box[3] = {bx, by, bz}, estr[3] = {1, 1, 1};
+    CUtensorMap m;
+    const CUresult cr = g_encodeTiled(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(p), dims, strides, box, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) return fail(GAMMA_ERR_CUDA, "cuTensorMapEncodeTiled failed with code " + std::to_string((int)cr));
+    int victim = g_numMaps;
+    if (victim == MAP_CACHE) {
+        victim = 0;
+        for (int i = 1; i < MAP_CACHE; ++i)
+            if (g_maps[i].use < g_maps[victim].use) victim = i;
+    } else {
+        ++g_numMaps;
+    }
+    g_maps[victim].key = key; g_maps[victim].map = m; g_maps[victim].use = ++g_mapClock;
+    out = m;
+    return GAMMA_OK;
+}
 
 // Grids up to this many voxels get their work lists sized by N; larger grids count their evaluated voxels first (one
 // host read of 4 bytes on a call of milliseconds) and get lists sized by M.
@@ -631,6 +694,52 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
                          e.call, r.stats));
         ++nk;
     }
+    // a1 + a2 + star phase.  Default: the compacted-list pipeline k_classify -> k_star (doses through L1 / L2).
+    // opts.star_load = 2 / 3 (3D grids with depth classes): ONE kernel over spatial tiles, evaluation doses staged by
+    // the TMA (tile_star.cuh) or by cooperative loads (what grids whose nx is not a multiple of 4 get anyway).
+    // Measured (profiles/r2_star_load.md): the list wins, because every evaluated voxel is in flight at once there,
+    // while a block works through its hot tiles one after the other.
+    const bool tiles = classes && r.starLoad >= 2;
+    if (tiles) {
+        STAGE_MARK(1, st);
+        if (r.tableMode != 1) { rc = fork_table(); if (rc) return rc; }  // paper's radius: needs k_norm's max |DD|
+        const bool tma = r.starLoad != 3 && tma_usable(ref, ev, g);
+        CUtensorMap mapRef, mapEv;
+        std::memset(&mapRef, 0, sizeof mapRef);
+        std::memset(&mapEv, 0, sizeof mapEv);
+        if (tma) {
+            rc = tensor_map(ref, g, TILE_X, TILE_Y, TILE_Z, mapRef);
+            if (rc) return rc;
+            rc = tensor_map(ev, g, HALO_PX, HALO_Y, HALO_Z, mapEv);
+            if (rc) return rc;
+        }
+        TileGrid tg;
+        tg.tx = (g.n[0] + TILE_X - 1) / TILE_X; tg.ty = (g.n[1] + TILE_Y - 1) / TILE_Y; tg.tz = (g.n[2] + TILE_Z - 1) / TILE_Z;
+        const unsigned dv[2] = {(unsigned)tg.tx, (unsigned)tg.tx * (unsigned)tg.ty};
+        for (int k = 0; k < 2; ++k) {
+            unsigned l = 0;
+            while ((1ull << l) < dv[k]) ++l;
+            tg.divMul[k] = (unsigned)((1ull << (31 + l)) / dv[k] + 1ull);
+            tg.divSh[k] = 31 + l;
+        }
+        const long long numTiles = (long long)tg.tx * tg.ty * tg.tz;
+        if (g_ws.occTile[tma] == 0) {
+            int occ = 0;
+            if (tma) CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tile_star<true>, TILE_VOX, 0));
+            else CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tile_star<false>, TILE_VOX, 0));
+            g_ws.occTile[tma] = occ > 0 ? occ : 1;
+        }
+        const long long resident = (long long)sm * g_ws.occTile[tma];
+        const int grid = (int)(numTiles > resident ? resident : numTiles);
+        unsigned *tabL = static_cast<unsigned*>(g_ws.tmpL.p), *tabI = static_cast<unsigned*>(g_ws.tmpIdx.p);
+        if (tma)
+            CU_TRY(launch_ex(k_tile_star<true>, grid, TILE_VOX, 0, st, pdl, false, mapRef, mapEv, ref, ev, out, g, e, ctl, k0, i0,
+                             k1, i1, embed, plan, tab4, tabL, tabI, r.stats, tg));
+        else
+            CU_TRY(launch_ex(k_tile_star<false>, grid, TILE_VOX, 0, st, pdl, false, mapRef, mapEv, ref, ev, out, g, e, ctl, k0, i0,
+                             k1, i1, embed, plan, tab4, tabL, tabI, r.stats, tg));
+        ++nk;
+    } else {
     {                                                                    // a1: exclusion + compaction
         long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
         int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
@@ -651,6 +760,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
             CU_TRY(launch_ex(k_star<false>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes,
                              embed, plan, tab4, tabL, tabI, r.stats));
         ++nk;
+    }
     }
     STAGE_MARK(2, st);
     if (!embed) CU_TRY(cudaStreamWaitEvent(st, g_ws.evJoin, 0));   // before the presort: presort -> search stay adjacent
@@ -753,7 +863,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
                      const Resolved& r, float* out, cudaStream_t st, bool allowEarly)
 {
     cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
-    CU_TRY(cudaStreamIsCapturing(st, &capStatus));
+    if (!allowEarly) CU_TRY(cudaStreamIsCapturing(st, &capStatus));      // lane streams are never captured
     const bool capturing = capStatus != cudaStreamCaptureStatusNone;
     const long long N = g.N;
     int rc;
@@ -855,7 +965,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         key.mode = mode; key.presort = r.presort; key.star = r.star; key.lanes = r.lanes; key.keyBits = r.keyBits;
         key.tableCap = r.tableCap; key.tableMode = r.tableMode; key.algo = r.algo;
         key.statsHist = r.stats.hist; key.statsSummary = r.stats.summary; key.statsBins = r.stats.nbins;
-        key.statsScale = r.stats.binScale;
+        key.statsScale = r.stats.binScale; key.starLoad = r.starLoad;
         GraphEntry* hit = nullptr;
         for (int i = 0; i < g_ws.numGraphs; ++i)
             if (g_ws.graph[i].key == key) { hit = &g_ws.graph[i]; break; }

@@ -62,14 +62,15 @@ __global__ void __launch_bounds__(NORM_THREADS)
 k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur,
        Ctl* __restrict__ next, int waitFirst, unsigned call, StatsP st)
 {
-    pdl_launch_dependents();
     trace_first(call, 0);
     // waitFirst: ref / eval may be results of the operation in front of this call: nothing is read before that
-    // operation has completed.  Otherwise (library-owned stream, the operation in front is the previous call's
-    // k_table_search, which triggers its dependents at once) this kernel runs in the tail of that call: it reads this
-    // call's inputs only, writes control blocks that call does not use, and waits for its end as its LAST act, so that
-    // nothing after it can overtake the previous call.
+    // operation has completed -- and the dependents (k_classify fetches ref before its own wait) are released only
+    // after that.  Otherwise (library-owned stream, the operation in front is the previous call's k_table_search,
+    // which triggers its dependents at once) this kernel runs in the tail of that call: it reads this call's inputs
+    // only, writes control blocks that call does not use, and waits for its end as its LAST act, so that nothing
+    // after it can overtake the previous call.
     if (waitFirst) pdl_wait();
+    pdl_launch_dependents();
     trace_waited(call, 0);
     if (blockIdx.x == gridDim.x - 1 && next != nullptr) {      // the next call finds its control block cleared
         unsigned* w = reinterpret_cast<unsigned*>(next);

@@ -130,6 +130,25 @@ def test_criteria_sweep_table3(oracle_mod):
     print(f"criteria sweep: max|dgamma| {worst:.2e} over 9 full maps; scaling law residual k=2 {law2:.1e}, k=3 {law3:.1e}")
 
 
+@pytest.mark.parametrize("name", ["cfg4_fine", "cfg5", "cfg2_small"])
+def test_star_load_paths_agree_bit_for_bit(name):
+    """opts.star_load: compacted list + __ldg (1), TMA-staged tiles (2, default) and tiles filled by cooperative loads (3)
+    evaluate the same faces with the same arithmetic: identical maps, identical counters."""
+    c = phantoms.make_case(name)
+    r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+    e = torch.from_numpy(c.eval.ravel().copy()).cuda()
+    args = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    got, cnts = [], []
+    for sl in (1, 2, 3):
+        got.append(binding.gamma_eval_ex(r, e, *args, GammaOpts(star_load=sl)).clone())
+        cnts.append(binding.gamma_get_counters())
+    for g in got[1:]:
+        assert torch.equal(torch.nan_to_num(g, nan=-1.0), torch.nan_to_num(got[0], nan=-1.0))
+    for c2 in cnts[1:]:
+        for k in ("n_evaluated", "n_table_search", "n_ring_search", "vertex_visits"):
+            assert c2[k] == cnts[0][k], k
+
+
 def test_cfg5_presort_on_off_and_thread_per_voxel_agree(oracle_mod):
     """Config 5 is run with and without the voxel pre-sort (Table 2) and with the paper's
     thread-per-voxel mapping: the candidate set and the arithmetic of the table walk are the same, so gamma is
@@ -159,6 +178,7 @@ VARIANTS = [
     GammaOpts(presort=3, sort_key_bits=8), GammaOpts(presort=3, sort_key_bits=32), GammaOpts(table_cap=1),
     GammaOpts(table_cap=7, star_phase=2), GammaOpts(table_cap=40, lanes_per_voxel=32),
     GammaOpts(table_cap=3, lanes_per_voxel=1),
+    GammaOpts(star_load=2), GammaOpts(star_load=3), GammaOpts(star_load=2, table_cap=2), GammaOpts(star_load=2, table_radius=2),
 ]
 
 
@@ -171,7 +191,7 @@ def test_option_variants_small_cases(oracle_mod, name, vi):
     assert_parity(g, o, f"{name} {VARIANTS[vi]}")
 
 
-@pytest.mark.parametrize("vi", [1, 3, 4, 5, 8, 10])
+@pytest.mark.parametrize("vi", [1, 3, 4, 5, 8, 10, 17, 18])
 def test_option_variants_cfg3(oracle_mod, vi):
     c = phantoms.make_case("cfg3")
     g = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, VARIANTS[vi])
@@ -203,7 +223,8 @@ def _random_case(shape_xyz, sp, seed, smooth=True, amp=0.15):
     ((1, 1, 17), (1.0, 1.0, 0.7), 0.05, 1.0, 0, 0.0, 8),          # 1D along z
     ((130, 3, 2), (0.5, 4.0, 4.0), 0.03, 3.0, 0, 0.05, 9),        # thin slab, strongly anisotropic
 ])
-@pytest.mark.parametrize("opts", [GammaOpts(), GammaOpts(star_phase=2, lanes_per_voxel=1), GammaOpts(table_cap=5)])
+@pytest.mark.parametrize("opts", [GammaOpts(), GammaOpts(star_phase=2, lanes_per_voxel=1), GammaOpts(table_cap=5),
+                                  GammaOpts(star_load=2)])
 def test_random_grids_edge_shapes(oracle_mod, dims, sp, dd, dta, mode, cutoff, seed, opts):
     ref, ev = _random_case(dims, sp, seed)
     g = gpu_gamma(ref, ev, dims, sp, dd, dta, mode, cutoff, opts)
@@ -235,7 +256,8 @@ def test_missing_region_heavy_tail_beyond_the_prefix_table(oracle_mod):
     want = cpu_gamma(oracle_mod, c.ref, ev, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
     assert np.nanmax(want) > 6.0
     for o in (GammaOpts(), GammaOpts(table_cap=27), GammaOpts(table_radius=2), GammaOpts(table_radius=2, table_cap=200),
-              GammaOpts(lanes_per_voxel=1, presort=2, table_cap=64), GammaOpts(lanes_per_voxel=8, table_cap=5)):
+              GammaOpts(lanes_per_voxel=1, presort=2, table_cap=64), GammaOpts(lanes_per_voxel=8, table_cap=5),
+              GammaOpts(star_load=2), GammaOpts(star_load=3, table_radius=2)):
         got = gpu_gamma(c.ref, ev, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, o)
         assert_parity(got, want, f"missing region, {o}")
 
@@ -583,9 +605,9 @@ def _nn(t):
 
 
 def test_back_to_back_calls_overlap_safely(oracle_mod):
-    """Consecutive calls on one stream with opts.back_to_back = 1 are pipelined: k_norm / k_classify / k_star of a call
-    run beside the table search of the previous one, each call on its own set of work lists (4 sets rotate), calls are
-    published in call order.  Results must be those of isolated calls: three alternating geometries over 60 calls (the
+    """Consecutive calls on one stream with opts.back_to_back = 1 run round-robin on the library's lane streams (own
+    workspace each), so that their kernels overlap; the caller's stream waits for every call.  Results must be those of
+    isolated calls: three alternating geometries over 60 calls (the
     offset table and the list sizes differ from call to call), a shared output buffer, a call whose INPUT is the
     previous call's output, and a call whose OUTPUT is the previous call's input."""
     b2b = GammaOpts(back_to_back=1)
@@ -607,6 +629,8 @@ def test_back_to_back_calls_overlap_safely(oracle_mod):
     torch.cuda.synchronize()
     for i, o in enumerate(outs):
         assert torch.equal(_nn(o), _nn(data[(i * 2) % 3][3])), i
+    cnt = binding.gamma_get_counters()
+    assert cnt["pipelined"] == 1 and cnt["calls_pipelined"] >= 60        # the flag was honoured: lane streams
     # one output buffer for every call of the same case: consecutive calls write the same range -> not pipelined, but
     # the flag stays set; nothing of the caller's sits between the calls
     r, e, args, want = data[0]
