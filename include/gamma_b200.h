@@ -173,6 +173,34 @@ int gamma_eval_ex(const float* ref, const float* eval, const int dims[3], const 
                   void* stream);
 
 /*
+ * gamma_eval_general -- gamma with the evaluation dose on ITS OWN grid, and the closest point of the evaluation surface
+ * (SURVEY.md 8(f) item 3).  Eq. 1 does not need the two doses on one grid (the paper's data were,
+ * PAPER.md:312), and the refinements it cites (Stock et al. 2005: the "gamma angle" that tells a
+ * dose-difference failure from a distance failure) need the point where the minimum is attained.
+ *   The centre of reference voxel (i, j, k) is ref_origin_mm + (i, j, k) * ref_spacing_mm, evaluation vertex (i, j, k)
+ *   sits at eval_origin_mm + (i, j, k) * eval_spacing_mm; the surface is the Kuhn interpolant of `eval` on its grid
+ *   (readings 5, 6); gamma[v] = min over that surface of the distance of Eq. 1, exact (no radius cap, reading 18);
+ *   a reference point outside the evaluation grid is compared with the surface as it is (no extrapolation, reading 11).
+ *   ref            DEVICE, Nr = product of ref_dims fp32; ref_dims each >= 1
+ *   eval           DEVICE, product of eval_dims fp32; every eval_dims >= 2 (three active axes)
+ *   *_dims, *_spacing_mm (> 0), *_origin_mm (finite)   HOST, 3 values each (x, y, z)
+ *   DD, DTA_mm, mode, low_dose_cutoff   as gamma_eval (D_norm = max(ref) unless opts->norm_dose > 0)
+ *   opts           NULL or gamma_opts of which norm_dose and table_cap are used
+ *   out_gamma      DEVICE, Nr fp32, written entirely (NaN = excluded)
+ *   out_closest    DEVICE, Nr x 4 fp32 or NULL: (x, y, z in mm, evaluation dose) of one point of the surface at distance
+ *                  gamma[v] (the minimiser need not be unique); NaN for excluded voxels.  The gamma angle follows as
+ *                  atan2(|r - r_v| / DTA, |D - D_r[v]| / dD).
+ *   stream         everything runs on `stream` (4 kernels + one memset), in stream order; cannot be captured.
+ * With identical geometry the result equals gamma_eval's (other kernels, same surface); this path has no star / ring
+ * shortcut because the reference point is not an evaluation vertex: every evaluated voxel walks the offset table,
+ * 8 lanes per voxel.
+ */
+int gamma_eval_general(const float* ref, const int ref_dims[3], const float ref_spacing_mm[3], const float ref_origin_mm[3],
+                       const float* eval, const int eval_dims[3], const float eval_spacing_mm[3],
+                       const float eval_origin_mm[3], float DD, float DTA_mm, int mode, float low_dose_cutoff,
+                       const gamma_opts* opts, float* out_gamma, float* out_closest, void* stream);
+
+/*
  * gamma_eval_host -- the same computation for HOST buffers (A2 steps 1 and 8):
  * copies ref and eval to the device, runs gamma_eval_ex, copies gamma back and SYNCHRONISES `stream`
  * before returning.  ref_host, eval_host, out_gamma_host: HOST, N fp32 each (pinned memory makes the

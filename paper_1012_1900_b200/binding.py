@@ -16,7 +16,7 @@ from . import build as _build
 
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
-    "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
+    "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
     "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_version",
     "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
@@ -25,8 +25,8 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 
 # every symbol include/gamma_b200.h declares
 exported_symbols = (
-    "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs", "gamma_offset_table",
-    "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
+    "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
+    "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
     "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
 
@@ -132,6 +132,8 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_eval_ex.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
     lib.gamma_eval_batch.argtypes = [ci, vp, vp, vp, vp, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
     lib.gamma_eval_host.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
+    lib.gamma_eval_general.argtypes = [vp, i3, f3, f3, vp, i3, f3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp, vp]
+    lib.gamma_eval_general.restype = ci
     lib.gamma_stats.argtypes = [vp, cll, ci, cf, vp, vp, vp]
     lib.gamma_sort_pairs.argtypes = [vp, vp, cll, ci, ci, vp]
     lib.gamma_offset_table.argtypes = [i3, f3, cf, cf, cll, vp, vp, vp]
@@ -146,7 +148,7 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_trace_read.restype = ci
     lib.gamma_workspace_bytes.argtypes = []
     lib.gamma_workspace_bytes.restype = cll
-    for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
+    for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
                  "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_fp32_probe"):
         getattr(lib, name).restype = ci
     lib.gamma_release.restype = None
@@ -258,6 +260,38 @@ def gamma_eval_batch(refs, evals, dims_list, spacing_list, DD, DTA_mm, mode=GAMM
     _check(lib.gamma_eval_batch(n, pr, pe, cd, cs, float(DD), float(DTA_mm), int(mode), float(low_dose_cutoff),
                                 ctypes.byref(o) if o is not None else None, po, _stream(stream)))
     return outs
+
+
+def gamma_eval_general(ref, ref_dims, ref_spacing_mm, ref_origin_mm, eval, eval_dims, eval_spacing_mm, eval_origin_mm, DD,
+                       DTA_mm, mode=GAMMA_MODE_GLOBAL, low_dose_cutoff=0.1, opts=None, out_gamma=None, want_closest=False,
+                       out_closest=None, stream=None):
+    """``gamma_eval_general``: evaluation dose on its own grid.  Returns gamma (float32 CUDA tensor, Nr elements), or
+    (gamma, closest [Nr, 4] = x, y, z in mm and evaluation dose of the closest surface point) with ``want_closest``."""
+    lib = load_library()
+    ref, eval = _dev_f32(ref, "ref"), _dev_f32(eval, "eval")
+    nr, ne = _numel(ref_dims), _numel(eval_dims)
+    if ref.numel() != nr or eval.numel() != ne:
+        raise GammaError("ref / eval size does not match its dims")
+    if out_gamma is None:
+        out_gamma = torch.empty(nr, dtype=torch.float32, device=ref.device)
+    _dev_f32(out_gamma, "out_gamma")
+    if want_closest and out_closest is None:
+        out_closest = torch.empty((nr, 4), dtype=torch.float32, device=ref.device)
+    if out_closest is not None:
+        _dev_f32(out_closest, "out_closest")
+        if out_closest.numel() != 4 * nr:
+            raise GammaError("out_closest must hold Nr x 4 values")
+    if out_gamma.numel() != nr:
+        raise GammaError("out_gamma size does not match ref_dims")
+    rd, rs = _geom(ref_dims, ref_spacing_mm)
+    ed, es = _geom(eval_dims, eval_spacing_mm)
+    ro = (ctypes.c_float * 3)(*[float(x) for x in ref_origin_mm])
+    eo = (ctypes.c_float * 3)(*[float(x) for x in eval_origin_mm])
+    co = opts._c() if opts is not None else None
+    _check(lib.gamma_eval_general(ref.data_ptr(), rd, rs, ro, eval.data_ptr(), ed, es, eo, float(DD), float(DTA_mm), int(mode),
+                                  float(low_dose_cutoff), ctypes.byref(co) if co is not None else None, out_gamma.data_ptr(),
+                                  out_closest.data_ptr() if out_closest is not None else None, _stream(stream)))
+    return (out_gamma, out_closest) if out_closest is not None else out_gamma
 
 
 def gamma_eval_host(ref_host, eval_host, dims, spacing_mm, DD, DTA_mm, mode=GAMMA_MODE_GLOBAL, low_dose_cutoff=0.1,

@@ -17,6 +17,7 @@
 #include "radix_sort.cuh"
 #include "stats.cuh"
 #include "tile_star.cuh"
+#include "general.cuh"
 
 using namespace gamma_b200;
 
@@ -149,6 +150,7 @@ struct Workspace {
     int numSM = 0;
     int occStar[2] = {0, 0};       // resident blocks per SM of k_star<false/true>
     int occTile[2] = {0, 0};       // resident blocks per SM of k_tile_star<false/true>
+    int occGeneral = 0;            // resident blocks per SM of k_general_search
     int pdl = -1;                  // programmatic dependent launch between the kernels of a call (GAMMA_PDL=0 disables)
     int graphs = -1;               // replay the call as a cached CUDA graph (GAMMA_GRAPH=0 disables)
     bool frozen = false;           // addresses of this workspace are baked into a caller's CUDA graph: it must not move
@@ -1154,6 +1156,137 @@ int gamma_eval_batch(int n_cases, const float* const* ref, const float* const* e
         if (rc) return rc;
     }
     CU_TRY(cudaGetLastError());
+    return GAMMA_OK;
+}
+
+int gamma_eval_general(const float* ref, const int ref_dims[3], const float ref_spacing_mm[3], const float ref_origin_mm[3],
+                       const float* eval, const int eval_dims[3], const float eval_spacing_mm[3],
+                       const float eval_origin_mm[3], float DD, float DTA_mm, int mode, float low_dose_cutoff,
+                       const gamma_opts* opts, float* out_gamma, float* out_closest, void* stream)
+{
+    g_err.clear();
+    if (!ref || !eval || !out_gamma) return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref / eval / out_gamma is NULL");
+    if (!ref_dims || !ref_spacing_mm || !ref_origin_mm || !eval_origin_mm)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "a geometry argument is NULL");
+    GridP g;
+    int rc = make_grid(eval_dims, eval_spacing_mm, DTA_mm, g);
+    if (rc) return rc;
+    if (!g.all_active) return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_general needs every evaluation axis >= 2 voxels");
+    rc = check_criteria(DD, mode, low_dose_cutoff);
+    if (rc) return rc;
+    Resolved r;
+    rc = resolve_opts(opts, r);
+    if (rc) return rc;
+    GeneralP gp;
+    std::memset(&gp, 0, sizeof gp);
+    long long Nr = 1;
+    for (int a = 0; a < 3; ++a) {
+        if (ref_dims[a] < 1) return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref_dims must be >= 1");
+        if (!(ref_spacing_mm[a] > 0.0f) || !std::isfinite(ref_spacing_mm[a]))
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref_spacing_mm must be > 0");
+        if (!std::isfinite(ref_origin_mm[a]) || !std::isfinite(eval_origin_mm[a]))
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "origins must be finite");
+        Nr *= ref_dims[a];
+        if (Nr >= (1ll << 31)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "reference voxels must be < 2^31");
+        gp.rn[a] = ref_dims[a];
+        gp.off[a] = ((double)ref_origin_mm[a] - (double)eval_origin_mm[a]) / (double)eval_spacing_mm[a];
+        gp.scale[a] = (double)ref_spacing_mm[a] / (double)eval_spacing_mm[a];
+        gp.eorg[a] = eval_origin_mm[a];
+        gp.esp[a] = eval_spacing_mm[a];
+    }
+    {
+        const unsigned dv[2] = {(unsigned)ref_dims[0], (unsigned)ref_dims[0] * (unsigned)ref_dims[1]};
+        for (int k = 0; k < 2; ++k) {
+            unsigned l = 0;
+            while ((1ull << l) < dv[k]) ++l;
+            gp.rDivMul[k] = (unsigned)((1ull << (31 + l)) / dv[k] + 1ull);
+            gp.rDivSh[k] = 31 + l;
+        }
+    }
+    GridP gr;                                   // the reference grid as k_classify sees it: a run of Nr voxels
+    std::memset(&gr, 0, sizeof gr);
+    gr.n[0] = ref_dims[0]; gr.n[1] = ref_dims[1]; gr.n[2] = ref_dims[2];
+    gr.stride[0] = 1; gr.stride[1] = ref_dims[0]; gr.stride[2] = ref_dims[0] * ref_dims[1];
+    gr.N = (int)Nr;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::lock_guard<std::mutex> lock(g_mu);
+    end_b2b_sequence();
+    cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
+    CU_TRY(cudaStreamIsCapturing(st, &capStatus));
+    if (capStatus != cudaStreamCaptureStatusNone)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_general cannot be captured into a CUDA graph");
+    rc = ensure_device();
+    if (rc) return rc;
+    rc = order_after_previous(st);
+    if (rc) return rc;
+    rc = ensure_ctl(st);
+    if (rc) return rc;
+    g_ws.ctlClean = false;
+    rc = prepare_workspace(g, r, Nr);
+    if (rc) return rc;
+    Ctl* base = static_cast<Ctl*>(g_ws.ctl.p);
+    Ctl* ctl = base + g_ws.slot;
+    Ctl* next = base + (g_ws.slot + 1) % CTL_ROT;
+    EvalP e;
+    e.DD = DD; e.cutoff = low_dose_cutoff; e.norm_dose = r.normDose; e.mode = mode; e.algo = 0; e.call = g_callNo;
+    const int sm = g_ws.numSM;
+    const bool pdl = g_ws.pdl != 0;
+    StatsP noStats;
+    noStats.hist = nullptr; noStats.summary = nullptr; noStats.nbins = 0; noStats.binScale = 0.0f;
+    {                                                                    // a0 on the reference grid
+        long long blocks = (Nr + 1023) / 1024;
+        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
+        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ref, (int)Nr, mode, ctl, next, 1, e.call, noStats));
+    }
+    {                                                                    // a1 on the reference grid
+        long long chunks = (Nr + PREP_CHUNK - 1) / PREP_CHUNK;
+        int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
+        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out_gamma, gr, e, ctl,
+                         static_cast<unsigned*>(g_ws.evalIdx.p), noStats));
+    }
+    // a3 on the evaluation grid: the same data-independent prefix table as gamma_eval (table_cap cells), here by the
+    // stand-alone builder; beyond it the search enumerates
+    const bool embed = r.tableCap <= TAB_EMBED_MAX_CELLS;
+    int4* tab = static_cast<int4*>(g_ws.table.p) + (embed ? (size_t)g_ws.slot * TAB_EMBED_MAX_CELLS : (size_t)CTL_SLOTS * TAB_EMBED_MAX_CELLS);
+    {
+        float lo = 0.0f, hi = grid_diagonal(g);
+        int bx, by, bz;
+        if (table_box_cells(g, hi, bx, by, bz) <= r.tableCap) lo = hi;
+        else
+            for (int it = 0; it < 48; ++it) {
+                const float mid = 0.5f * (lo + hi);
+                if (table_box_cells(g, mid, bx, by, bz) <= r.tableCap) lo = mid; else hi = mid;
+            }
+        k_offset_table<<<TAB_BLOCKS, TAB_THREADS, TAB_DYN_SMEM, st>>>(g, e, ctl, lo, r.tableCap, tab, static_cast<unsigned*>(g_ws.tmpL.p),
+                                                                      static_cast<unsigned*>(g_ws.tmpIdx.p), 1);
+    }
+    if (out_closest) CU_TRY(cudaMemsetAsync(out_closest, 0xff, (size_t)Nr * 16, st));   // NaN where nothing is evaluated
+    {
+        long long units = (Nr + 3) / 4, blocks = (units + GENERAL_THREADS / 32 - 1) / (GENERAL_THREADS / 32);
+        if (g_ws.occGeneral == 0) {
+            int occ = 0;
+            CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_general_search, GENERAL_THREADS, 0));
+            g_ws.occGeneral = occ > 0 ? occ : 1;
+        }
+        const long long resident = (long long)sm * g_ws.occGeneral;
+        const int grid = (int)(blocks > resident ? resident : (blocks < 1 ? 1 : blocks));
+        CU_TRY(launch_ex(k_general_search, grid, GENERAL_THREADS, 0, st, false, false, ref, eval, out_gamma,
+                         reinterpret_cast<float4*>(out_closest), g, gp, e, ctl, static_cast<const unsigned*>(g_ws.evalIdx.p),
+                         static_cast<const int4*>(tab)));
+    }
+    g_ws.launches += 4;
+    CU_TRY(cudaGetLastError());
+    rc = mark_done(st);
+    if (rc) return rc;
+    g_ws.lastSpans = CallSpans();
+    g_ws.lastCtl = ctl;
+    g_ws.lastClasses = 0;
+    g_ws.slot = (g_ws.slot + 1) % CTL_ROT;
+    ++g_ws.calls;
+    ++g_callNo;
+    g_ws.ctlClean = true;
+    g_ws.lastStream = st; g_ws.lastN = Nr; g_ws.haveLast = true; g_ws.haveStages = false;
+    g_lastWs = g_cur;
     return GAMMA_OK;
 }
 

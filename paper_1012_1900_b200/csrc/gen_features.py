@@ -21,6 +21,7 @@ Three routines are emitted:
                          lam in {0,1}):  gamma_star^2 = d0^2 / max feasible G1, no division per face;
   * gamma_owned_min   -- the 26 faces owned by a grid vertex c (= faces whose lowest vertex is c),
                          any offset, with per-face validity (faces that would leave the grid);
+  * gamma_owned_argmin -- gamma_owned_min that also returns the foot point (closest-point output, general geometry);
   * gamma_ring_min    -- the 72 faces of the 2x2x2 block of cells around an interior reference voxel that neither
                          contain the voxel (those are the star) nor lie on the block's boundary (those are at least
                          one voxel spacing away): together with the star, everything closer than min_a h_a.  The
@@ -195,6 +196,87 @@ def emit_owned(w):
     w("    return best2;\n}\n")
 
 
+def emit_owned_arg(w):
+    """gamma_owned_argmin: gamma_owned_min that also reports WHERE the minimum is (general geometry: closest point)."""
+    w("\n// gamma_owned_min with the foot point: when a face improves best2, loc[a] (a = 0..2) receives the cell-local\n")
+    w("// coordinate of the foot along axis a (0..1 from the owner vertex c) and loc[3] the normalised dose of the surface\n")
+    w("// there, (D_e(foot) - D_r[v]) / dD.  Same faces, same arithmetic as gamma_owned_min; run once per voxel, on the\n")
+    w("// owner vertex that won the search (closest-point output of the general-geometry path).\n")
+    w("GAMMA_HD float gamma_owned_argmin(const float (&d)[8], const float (&invA)[8], const float (&lam)[8],\n")
+    w("                                  const float (&q)[3], const float (&X)[8], unsigned usable, float best2,\n")
+    w("                                  float (&loc)[4])\n{\n")
+    w("    {\n        const float dv = (q[0] + q[1]) + (q[2] + d[0] * d[0]);   // the vertex c itself\n")
+    w("        if (dv < best2) { best2 = dv; loc[0] = 0.0f; loc[1] = 0.0f; loc[2] = 0.0f; loc[3] = d[0]; }\n    }\n")
+    done_e, done_n, done_g = set(), set(), set()
+    for s in range(1, 8):
+        w("    const bool ok%d = (usable & %du) == %du;\n" % (s, s, s))
+
+    def edge(a, b):
+        nm = "%d_%d" % (a, b)
+        if nm not in done_e:
+            w("    const float dl%s = d[%d] - d[%d];\n" % (nm, b, a))
+            w("    const float w%s = dl%s * invA[%d];\n" % (nm, nm, a ^ b))
+            done_e.add(nm)
+        return nm
+
+    def nsum(full):
+        nm = "N" + "_".join(str(s) for s in full)
+        if nm not in done_n:
+            e = edge(full[-2], full[-1])
+            prev = "d[0]" if len(full) == 2 else nsum(full[:-1])
+            w("    const float %s = fmaf(dl%s, lam[%d], %s);\n" % (nm, e, full[-1] ^ full[-2], prev))
+            done_n.add(nm)
+        return nm
+
+    def gsum(full):
+        nm = "G" + "_".join(str(s) for s in full)
+        if nm not in done_g:
+            e = edge(full[-2], full[-1])
+            prev = "1.0f" if len(full) == 2 else gsum(full[:-1])
+            w("    const float %s = fmaf(dl%s, w%s, %s);\n" % (nm, e, e, prev))
+            done_g.add(nm)
+        return nm
+
+    def cval(ch):
+        full = (0,) + ch
+        steps = [full[i] ^ full[i - 1] for i in range(1, len(full))]
+        terms = ["X[%d]" % t for t in steps if bin(t).count("1") >= 2]
+        terms += ["q[%d]" % a for a in range(3) if not (ch[-1] & AX[a])]
+        return " + ".join(terms) if terms else None
+
+    for ch in chains():
+        full = (0,) + ch
+        k = len(ch)
+        names = [edge(full[i - 1], full[i]) for i in range(1, k + 1)]
+        N, G = nsum(full), gsum(full)
+        w("    {   // chain %s\n" % "<".join(str(s) for s in full))
+        w("        const float r = GAMMA_FDIV(%s, %s);\n" % (N, G))
+        ts = []
+        for i in range(k):
+            w("        const float t%d = fmaf(-r, w%s, lam[%d]);\n" % (i + 1, names[i], full[i + 1] ^ full[i]))
+            ts.append("t%d" % (i + 1))
+        conds = ["ok%d" % ch[-1], "1.0f >= t1"]
+        conds += ["%s >= %s" % (ts[i], ts[i + 1]) for i in range(k - 1)]
+        conds.append("%s >= 0.0f" % ts[-1])
+        c = cval(ch)
+        dist = "fmaf(%s, r, %s)" % (N, c) if c else "%s * r" % N
+        w("        const float dist = %s;\n" % dist)
+        locs = []
+        for a in range(3):
+            val = "0.0f"
+            for i in range(k):
+                if (full[i + 1] ^ full[i]) & AX[a]:
+                    val = ts[i]
+            locs.append("loc[%d] = %s;" % (a, val))
+        dose = "d[0]"
+        for i in range(k):
+            dose = "fmaf(%s, dl%s, %s)" % (ts[i], names[i], dose)
+        w("        if ((%s) && dist < best2) { best2 = dist; %s loc[3] = %s; }\n"
+          % (" & ".join("(%s)" % x for x in conds), " ".join(locs), dose))
+        w("    }\n")
+    w("    return best2;\n}\n")
+
+
 def ring_faces():
     """(owner o, neg mask, chain) of the 72 ring faces, in emission order."""
     out = []
@@ -309,6 +391,7 @@ def main():
           "#define GAMMA_FDIV(a, b) gamma_fdiv((a), (b))\n#else\n#define GAMMA_FDIV(a, b) ((a) / (b))\n#endif\n\n")
         emit_star(w)
         emit_owned(w)
+        emit_owned_arg(w)
         emit_ring(w)
     print("wrote", path)
 

@@ -26,7 +26,8 @@ import numpy as np
 from scipy.ndimage import map_coordinates
 from scipy.special import erf, ndtr
 
-__all__ = ["Case", "make_case", "CASE_NAMES", "resample_shifted", "beam_phantom", "blob_phantom_2d"]
+__all__ = ["Case", "GeneralCase", "make_case", "make_general_case", "CASE_NAMES", "resample_shifted", "beam_phantom",
+           "blob_phantom_2d"]
 
 
 @dataclass
@@ -159,6 +160,45 @@ def _perturb(ref64, spacing, shift_mm, scale, noise_frac, rng):
     ev = scale * resample_shifted(ref64, spacing, shift_mm)
     ev = ev + rng.normal(0.0, noise_frac * ref64.max(), size=ref64.shape)
     return ev
+
+
+@dataclass
+class GeneralCase:
+    """A gamma-index problem whose evaluation dose lives on its own grid."""
+
+    name: str
+    ref: np.ndarray
+    ref_dims: tuple
+    ref_spacing_mm: tuple
+    ref_origin_mm: tuple            # position of the centre of reference voxel (0, 0, 0)
+    eval: np.ndarray
+    eval_dims: tuple
+    eval_spacing_mm: tuple
+    eval_origin_mm: tuple
+    dd: float
+    dta_mm: float
+    mode: int = 0
+    cutoff: float = 0.10
+
+
+def make_general_case(name: str, seed: int = 0) -> GeneralCase:
+    """"cfg3_general": the cfg3 reference (128x128x64 at 2.5 mm) against the same beam phantom computed analytically on
+    a 2 mm grid (160x160x80) whose origin is displaced by a fraction of a voxel, with cfg3's perturbation (shift, scale,
+    noise) and criteria.  "general_small": the same construction on grids the oracle finishes in a second."""
+    if name == "cfg3_general":
+        rd, rs, ed, es, off = (128, 128, 64), (2.5, 2.5, 2.5), (160, 160, 80), (2.0, 2.0, 2.0), (0.37, -0.81, 0.55)
+    elif name == "general_small":
+        rd, rs, ed, es, off = (40, 36, 20), (7.5, 7.0, 8.0), (50, 42, 27), (6.0, 6.0, 6.0), (1.3, -2.2, 0.9)
+    else:
+        raise KeyError(name)
+    ref = beam_phantom(rd, rs, seed, 3)
+    ev0 = beam_phantom(ed, es, seed, 3)
+    ev0 *= 1.0                                   # same analytic phantom: both normalised to 2.0 Gy at their own maximum
+    rng = np.random.default_rng([seed, 13, 1])
+    ev = _perturb(ev0, es, (2.0, 1.5, -1.0), 0.97, 0.02, rng)
+    ro = tuple(-(n - 1) / 2.0 * h for n, h in zip(rd, rs))
+    eo = tuple(-(n - 1) / 2.0 * h + o for n, h, o in zip(ed, es, off))
+    return GeneralCase(name, ref.astype(np.float32), rd, rs, ro, ev.astype(np.float32), ed, es, eo, 0.02, 2.0, 0, 0.10)
 
 
 CASE_NAMES = ("cfg1", "cfg2", "cfg3", "cfg4_fine", "cfg4_coarse", "cfg5", "cfg2_small")
