@@ -292,6 +292,38 @@ def main():
         e2e_s = (time.perf_counter() - t0) / ne2e
     e2e_s = max_over_ranks(e2e_s)
 
+    # ---- end to end, a stream of cases: gamma_eval_host_batch overlaps the copies of consecutive cases with compute
+    nhb = 12
+    hb_refs = [ref_h] + [ref_h.clone().pin_memory() for _ in range(nhb - 1)]
+    hb_evs = [ev_h] + [ev_h.clone().pin_memory() for _ in range(nhb - 1)]
+    hb_outs = [torch.empty(N, dtype=torch.float32).pin_memory() for _ in range(nhb)]
+    hb_dims, hb_sp = [case.dims] * nhb, [case.spacing_mm] * nhb
+    hb_args = (case.dd, case.dta_mm, case.mode, case.cutoff)
+    binding.gamma_eval_host_batch(hb_refs, hb_evs, hb_dims, hb_sp, *hb_args, None, hb_outs, stream)
+    barrier()
+    nrep_hb = 3
+    with clocks:
+        t0 = time.perf_counter()
+        for _ in range(nrep_hb):
+            binding.gamma_eval_host_batch(hb_refs, hb_evs, hb_dims, hb_sp, *hb_args, None, hb_outs, stream)   # synchronises
+        e2e_pipe_s = (time.perf_counter() - t0) / (nrep_hb * nhb)
+    e2e_pipe_s = max_over_ranks(e2e_pipe_s)
+    e2e_pipe_ok = bool(torch.equal(torch.nan_to_num(hb_outs[nhb - 1], nan=-1.0), torch.nan_to_num(out_h, nan=-1.0)))
+    del hb_refs, hb_evs, hb_outs
+    # what the PCIe link of this box gives for the same buffers (plain pinned copies, nothing else running): the bound
+    # of any host-buffer path is 8N bytes / this host-to-device rate
+    tc0, tc1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dst = torch.empty(2 * N, dtype=torch.float32, device=dev)
+    dst[:N].copy_(ref_h, non_blocking=True)
+    tc0.record(stream)
+    for _ in range(10):
+        dst[:N].copy_(ref_h, non_blocking=True)
+        dst[N:].copy_(ev_h, non_blocking=True)
+    tc1.record(stream)
+    torch.cuda.synchronize()
+    h2d_gbs = 10 * 8 * N / (tc0.elapsed_time(tc1) * 1e-3) / 1e9
+    del dst
+
     # ---- stats on the result (not timed: a6 is reported separately) ---------------------------------
     hist, summ = binding.gamma_stats(outs[0], 64, 4.0)
     torch.cuda.synchronize()
@@ -398,7 +430,13 @@ def main():
                    "options": {"presort": args.presort, "star_phase": args.star_phase, "lanes": args.lanes}},
         "grid_voxels_per_s": world * N / (ms_step * 1e-3), "ms_per_case": ms_step,
         "e2e": {"value": world * M / e2e_s, "unit": "evaluated reference voxels/s", "ms_per_case": e2e_s * 1e3,
-                "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N},
+                "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N,
+                "pipelined": {"value": world * M / e2e_pipe_s, "unit": "evaluated reference voxels/s",
+                              "ms_per_case": e2e_pipe_s * 1e3, "cases_per_call": nhb, "same_result_as_single_call": e2e_pipe_ok,
+                              "h2d_bytes_per_case": 8 * N, "d2h_bytes_per_case": 4 * N,
+                              "h2d_gbs_of_this_box": h2d_gbs, "h2d_bound_ms_per_case": 8 * N / (h2d_gbs * 1e9) * 1e3,
+                              "note": "gamma_eval_host_batch: pinned HOST buffers in and out, H2D of case i+1 and D2H of "
+                                      "case i-1 overlapped with the kernels of case i; wall time of the synchronising call"}},
         "gpu_launches": int(launches), "host_submit_us_per_step": t_sub * 1e6,
         "clocks": clk, "roofline": roof,
         "counters": cnt, "stats": summ, "stats_ms": stats_ms,

@@ -210,6 +210,18 @@ int gamma_eval_host(const float* ref_host, const float* eval_host, const int dim
                     float DD, float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts,
                     float* out_gamma_host, void* stream);
 
+/*
+ * gamma_eval_host_batch -- n_cases independent cases from HOST buffers with the transfers of A2 steps 1 and 8
+ * overlapped with the computation: while case i is computed, the doses of case i + 1 travel to the
+ * device and the gamma map of case i - 1 travels back (three rotating sets of device staging buffers, one library
+ * stream per direction, the kernels on a third).  Arguments as gamma_eval_batch with HOST pointers (pinned memory makes
+ * the copies asynchronous; pageable memory works, more slowly).  Starts after what is on `stream`, SYNCHRONISES before
+ * returning; cannot be captured.  Results are those of gamma_eval_host case by case, bit for bit.
+ */
+int gamma_eval_host_batch(int n_cases, const float* const* ref_host, const float* const* eval_host, const int* dims,
+                          const float* spacing_mm, float DD, float DTA_mm, int mode, float low_dose_cutoff,
+                          const gamma_opts* opts, float* const* out_gamma_host, void* stream);
+
 /* Summary written by gamma_stats (layout fixed, 48 bytes). */
 typedef struct gamma_summary {
     unsigned long long n_eval; /* voxels with a finite gamma                                  */

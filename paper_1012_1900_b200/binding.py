@@ -16,7 +16,7 @@ from . import build as _build
 
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
-    "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
+    "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
     "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_version",
     "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
@@ -25,8 +25,8 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 
 # every symbol include/gamma_b200.h declares
 exported_symbols = (
-    "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
-    "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
+    "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats",
+    "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
     "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
 
@@ -132,6 +132,8 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_eval_ex.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
     lib.gamma_eval_batch.argtypes = [ci, vp, vp, vp, vp, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
     lib.gamma_eval_host.argtypes = [vp, vp, i3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
+    lib.gamma_eval_host_batch.argtypes = [ci, vp, vp, vp, vp, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp]
+    lib.gamma_eval_host_batch.restype = ci
     lib.gamma_eval_general.argtypes = [vp, i3, f3, f3, vp, i3, f3, f3, cf, cf, ci, cf, ctypes.POINTER(_COpts), vp, vp, vp]
     lib.gamma_eval_general.restype = ci
     lib.gamma_stats.argtypes = [vp, cll, ci, cf, vp, vp, vp]
@@ -148,7 +150,7 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_trace_read.restype = ci
     lib.gamma_workspace_bytes.argtypes = []
     lib.gamma_workspace_bytes.restype = cll
-    for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_stats", "gamma_sort_pairs",
+    for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats", "gamma_sort_pairs",
                  "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_fp32_probe"):
         getattr(lib, name).restype = ci
     lib.gamma_release.restype = None
@@ -314,6 +316,33 @@ def gamma_eval_host(ref_host, eval_host, dims, spacing_mm, DD, DTA_mm, mode=GAMM
                              out_gamma_host.data_ptr(), _stream(stream))
     _check(rc)
     return out_gamma_host
+
+
+def gamma_eval_host_batch(refs_host, evals_host, dims_list, spacing_list, DD, DTA_mm, mode=GAMMA_MODE_GLOBAL,
+                          low_dose_cutoff=0.1, opts=None, outs_host=None, stream=None):
+    """``gamma_eval_host_batch``: lists of CPU float32 tensors in (pinned for speed), list of CPU float32 tensors out;
+    copies and kernels of consecutive cases overlap; synchronises."""
+    lib = load_library()
+    n = len(refs_host)
+    if not (len(evals_host) == len(dims_list) == len(spacing_list) == n):
+        raise ValueError("refs_host, evals_host, dims_list and spacing_list must have the same length")
+    if outs_host is None:
+        outs_host = [torch.empty(_numel(d), dtype=torch.float32).pin_memory() for d in dims_list]
+    for i in range(n):
+        for t, name in ((refs_host[i], "ref_host"), (evals_host[i], "eval_host"), (outs_host[i], "out_gamma_host")):
+            if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+                    and t.numel() == _numel(dims_list[i])):
+                raise GammaError(f"case {i}: {name} must be a contiguous float32 CPU tensor with nx*ny*nz elements")
+    ptr = ctypes.c_void_p * max(n, 1)
+    pr = ptr(*[t.data_ptr() for t in refs_host])
+    pe = ptr(*[t.data_ptr() for t in evals_host])
+    po = ptr(*[t.data_ptr() for t in outs_host])
+    cd = (ctypes.c_int * (3 * max(n, 1)))(*[int(x) for d in dims_list for x in d])
+    cs = (ctypes.c_float * (3 * max(n, 1)))(*[float(x) for sp in spacing_list for x in sp])
+    o = opts._c() if opts is not None else None
+    _check(lib.gamma_eval_host_batch(n, pr, pe, cd, cs, float(DD), float(DTA_mm), int(mode), float(low_dose_cutoff),
+                                     ctypes.byref(o) if o is not None else None, po, _stream(stream)))
+    return outs_host
 
 
 def gamma_stats_async(gamma, nbins=64, hist_max=4.0, hist=None, summary_buf=None, stream=None):

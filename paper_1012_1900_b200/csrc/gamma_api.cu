@@ -1074,6 +1074,29 @@ int enqueue_on_lane(const float* ref, const float* ev, const GridP& g, float DD,
     return GAMMA_OK;
 }
 
+// gamma_eval_host_batch: copy engines and compute overlapped.  Three sets of device staging buffers rotate; the
+// host-to-device copies run on one library stream, the kernels on lane 0, the device-to-host copies on another stream.
+constexpr int HB_DEPTH = 3;
+struct HostBatchState {
+    Buf ref[HB_DEPTH], ev[HB_DEPTH], out[HB_DEPTH];
+    cudaStream_t h2d = nullptr, d2h = nullptr;
+    cudaEvent_t start = nullptr, copied[HB_DEPTH] = {}, computed[HB_DEPTH] = {}, freed[HB_DEPTH] = {};
+    bool ready = false;
+    void release()
+    {
+        for (int k = 0; k < HB_DEPTH; ++k) {
+            ref[k].release(); ev[k].release(); out[k].release();
+            if (copied[k]) { cudaEventDestroy(copied[k]); copied[k] = nullptr; }
+            if (computed[k]) { cudaEventDestroy(computed[k]); computed[k] = nullptr; }
+            if (freed[k]) { cudaEventDestroy(freed[k]); freed[k] = nullptr; }
+        }
+        if (start) { cudaEventDestroy(start); start = nullptr; }
+        if (h2d) { cudaStreamDestroy(h2d); h2d = nullptr; }
+        if (d2h) { cudaStreamDestroy(d2h); d2h = nullptr; }
+        ready = false;
+    }
+} g_hb;
+
 // any other library operation ends a sequence of back-to-back calls: the next one forks from the caller's stream again
 void end_b2b_sequence() { g_lanes.active = false; }
 
@@ -1321,6 +1344,87 @@ int gamma_eval_host(const float* ref_host, const float* eval_host, const int dim
     rc = mark_done(st);
     if (rc) return rc;
     CU_TRY(cudaStreamSynchronize(st));
+    return GAMMA_OK;
+}
+
+int gamma_eval_host_batch(int n_cases, const float* const* ref_host, const float* const* eval_host, const int* dims,
+                          const float* spacing_mm, float DD, float DTA_mm, int mode, float low_dose_cutoff,
+                          const gamma_opts* opts, float* const* out_gamma_host, void* stream)
+{
+    g_err.clear();
+    if (n_cases < 0) return fail(GAMMA_ERR_INVALID_ARGUMENT, "n_cases must be >= 0");
+    if (n_cases == 0) return GAMMA_OK;
+    if (!ref_host || !eval_host || !out_gamma_host || !dims || !spacing_mm)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref_host / eval_host / out_gamma_host / dims / spacing_mm is NULL");
+    int rc = check_criteria(DD, mode, low_dose_cutoff);
+    if (rc) return rc;
+    Resolved r;
+    rc = resolve_opts(opts, r);
+    if (rc) return rc;
+    r.profile = 0; r.graph = 0;
+    r.stats.hist = nullptr; r.stats.summary = nullptr;
+    long long maxN = 0;
+    for (int i = 0; i < n_cases; ++i) {                  // every case is checked before anything is enqueued
+        if (!ref_host[i] || !eval_host[i] || !out_gamma_host[i])
+            return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref_host[i] / eval_host[i] / out_gamma_host[i] is NULL");
+        GridP g;
+        rc = make_grid(dims + 3 * i, spacing_mm + 3 * i, DTA_mm, g);
+        if (rc) return rc;
+        if (g.N > maxN) maxN = g.N;
+    }
+    cudaStream_t user = static_cast<cudaStream_t>(stream);
+    std::lock_guard<std::mutex> lock(g_mu);
+    end_b2b_sequence();
+    cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
+    CU_TRY(cudaStreamIsCapturing(user, &capStatus));
+    if (capStatus != cudaStreamCaptureStatusNone)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_host_batch synchronises and cannot be captured into a CUDA graph");
+    rc = lanes_init();
+    if (rc) return rc;
+    HostBatchState& H = g_hb;
+    if (!H.ready) {
+        CU_TRY(cudaStreamCreateWithFlags(&H.h2d, cudaStreamNonBlocking));
+        CU_TRY(cudaStreamCreateWithFlags(&H.d2h, cudaStreamNonBlocking));
+        CU_TRY(cudaEventCreateWithFlags(&H.start, cudaEventDisableTiming));
+        for (int k = 0; k < HB_DEPTH; ++k) {
+            CU_TRY(cudaEventCreateWithFlags(&H.copied[k], cudaEventDisableTiming));
+            CU_TRY(cudaEventCreateWithFlags(&H.computed[k], cudaEventDisableTiming));
+            CU_TRY(cudaEventCreateWithFlags(&H.freed[k], cudaEventDisableTiming));
+        }
+        H.ready = true;
+    }
+    const int depth = n_cases < HB_DEPTH ? n_cases : HB_DEPTH;
+    for (int k = 0; k < depth; ++k) {
+        CU_TRY(H.ref[k].need((size_t)maxN * 4)); CU_TRY(H.ev[k].need((size_t)maxN * 4)); CU_TRY(H.out[k].need((size_t)maxN * 4));
+    }
+    cudaStream_t comp = g_lanes.stream[0];
+    CU_TRY(cudaEventRecord(H.start, user));              // everything starts after what is already on `stream`
+    CU_TRY(cudaStreamWaitEvent(H.h2d, H.start, 0));
+    g_lanes.laneDirty[0] = true;
+    for (int i = 0; i < n_cases; ++i) {
+        const int k = i % HB_DEPTH;
+        GridP g;
+        make_grid(dims + 3 * i, spacing_mm + 3 * i, DTA_mm, g);
+        const size_t bytes = (size_t)g.N * 4;
+        if (i >= HB_DEPTH) CU_TRY(cudaStreamWaitEvent(H.h2d, H.freed[k], 0));          // set k has been read back
+        CU_TRY(cudaMemcpyAsync(H.ref[k].p, ref_host[i], bytes, cudaMemcpyHostToDevice, H.h2d));      // A2 step 1
+        CU_TRY(cudaMemcpyAsync(H.ev[k].p, eval_host[i], bytes, cudaMemcpyHostToDevice, H.h2d));
+        CU_TRY(cudaEventRecord(H.copied[k], H.h2d));
+        CU_TRY(cudaStreamWaitEvent(comp, H.copied[k], 0));
+        Workspace* keep = g_cur;
+        g_cur = &g_pool[1];
+        rc = enqueue_pipeline(static_cast<const float*>(H.ref[k].p), static_cast<const float*>(H.ev[k].p), g, DD, mode,
+                              low_dose_cutoff, r, static_cast<float*>(H.out[k].p), comp, false);
+        g_cur = keep;
+        if (rc) break;
+        CU_TRY(cudaEventRecord(H.computed[k], comp));
+        CU_TRY(cudaStreamWaitEvent(H.d2h, H.computed[k], 0));
+        CU_TRY(cudaMemcpyAsync(out_gamma_host[i], H.out[k].p, bytes, cudaMemcpyDeviceToHost, H.d2h));  // A2 step 8
+        CU_TRY(cudaEventRecord(H.freed[k], H.d2h));
+    }
+    cudaError_t e1 = cudaStreamSynchronize(H.d2h), e2 = cudaStreamSynchronize(comp), e3 = cudaStreamSynchronize(H.h2d);
+    if (rc) return rc;
+    CU_TRY(e1); CU_TRY(e2); CU_TRY(e3);
     return GAMMA_OK;
 }
 
@@ -1583,6 +1687,7 @@ void gamma_release(void)
         if (g_lanes.done[w]) { cudaEventDestroy(g_lanes.done[w]); g_lanes.done[w] = nullptr; }
     if (g_lanes.fork) { cudaEventDestroy(g_lanes.fork); g_lanes.fork = nullptr; }
     g_lanes = LaneState();
+    g_hb.release();
     g_lastWs = &g_pool[0];
 }
 

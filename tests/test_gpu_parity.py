@@ -461,6 +461,35 @@ def test_gamma_eval_host_streams_and_determinism():
     assert np.array_equal(o4.cpu().numpy().astype(np.float64), base, equal_nan=True)
 
 
+def test_host_batch_equals_host_calls_bit_for_bit(oracle_mod):
+    """gamma_eval_host_batch (copies and kernels of consecutive cases overlapped, three rotating staging sets) returns
+    what gamma_eval_host returns case by case; more cases than staging sets, mixed geometries, pinned and pageable
+    host memory; one case also against the oracle."""
+    names = ["cfg2_small", "cfg1", "cfg4_coarse", "cfg2_small", "cfg4_coarse", "cfg1", "cfg2_small"]
+    cases = [phantoms.make_case(n) for n in names]
+    rng = np.random.default_rng([0, 55])
+    refs, evs = [], []
+    for i, c in enumerate(cases):
+        r = torch.from_numpy((c.ref.ravel() * np.float32(1.0 + 0.01 * i)).copy())
+        e = torch.from_numpy((c.eval.ravel() + rng.normal(0, 0.01, c.eval.size).astype(np.float32)).copy())
+        refs.append(r.pin_memory() if i % 2 == 0 else r)
+        evs.append(e.pin_memory() if i % 3 != 1 else e)
+    dims, sps = [c.dims for c in cases], [c.spacing_mm for c in cases]
+    single = [binding.gamma_eval_host(r, e, d, sp, 0.03, 3.0, 0, 0.1).clone() for r, e, d, sp in zip(refs, evs, dims, sps)]
+    outs = binding.gamma_eval_host_batch(refs, evs, dims, sps, 0.03, 3.0, 0, 0.1)
+    assert len(outs) == len(cases)
+    for a, b in zip(outs, single):
+        assert torch.equal(torch.nan_to_num(a, nan=-1.0), torch.nan_to_num(b, nan=-1.0))
+    want = cpu_gamma(oracle_mod, refs[4].numpy(), evs[4].numpy(), dims[4], sps[4], 0.03, 3.0, 0, 0.1)
+    assert_parity(outs[4].numpy().astype(np.float64), want, "host batch, case 4")
+    again = binding.gamma_eval_host_batch(refs[:2], evs[:2], dims[:2], sps[:2], 0.03, 3.0, 0, 0.1)     # fewer cases than sets
+    for a, b in zip(again, single[:2]):
+        assert torch.equal(torch.nan_to_num(a, nan=-1.0), torch.nan_to_num(b, nan=-1.0))
+    assert binding.gamma_eval_host_batch([], [], [], [], 0.03, 3.0) == []
+    with pytest.raises(binding.GammaError):                     # nothing is launched on an argument error
+        binding.gamma_eval_host_batch(refs[:2], evs[:2], [dims[0], (1, 1, dims[1][0] * dims[1][1] * dims[1][2])], sps[:2], -1.0, 3.0)
+
+
 def test_calls_interleaved_over_three_streams_share_the_workspace_safely():
     """The library has ONE workspace for single calls: a call on another stream than the previous one must wait for
     the tail of that stream (event recorded there when the next call arrives), whatever the geometry, with the stats,
