@@ -8,6 +8,9 @@ configs   every BASELINE.json config (cfg1, cfg2, cfg3, cfg4 coarse/fine, cfg5):
           the resolution exponent of cfg4 (Fig. 2) and cfg5 with the voxel pre-sort on / off and
           with the paper's thread-per-voxel mapping (Table 2)
 batch     independent cfg3 cases per call through gamma_eval_batch against the same cases one by one
+sort      subsystem (3) stand-alone: gamma_sort_pairs on 2^20 / 2^24 (key, value) pairs, 16 and 32 key bits, GB/s against
+          the algorithmic 20 B per pair per 8-bit pass and the measured HBM copy rate
+general   gamma_eval_general on the cfg3 reference against a 2 mm evaluation grid: ms per case, with / without closest point
 trace     device timeline of consecutive calls (library built with -DGAMMA_TRACE: GAMMA_NVCC_EXTRA=-DGAMMA_TRACE python -m
           paper_1012_1900_b200.build --force): when each kernel of a call starts, passes its dependency wait and ends,
           relative to the call's first kernel, one call after the other with and without opts.back_to_back
@@ -246,6 +249,72 @@ def suite_criteria(args, emit):
     return rows
 
 
+def suite_sort(args, emit):
+    """Hand-written LSD radix sort (csrc/radix_sort.cuh): per 8-bit pass it reads the keys twice and the values once and
+    writes both (20 B per pair); an odd number of passes costs one more copy back (16 B per pair)."""
+    import torch
+    from paper_1012_1900_b200 import binding
+    hbm = 6551.4
+    try:
+        hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:  # noqa: BLE001
+        pass
+    stream = torch.cuda.current_stream()
+    for n in (1 << 20, 1 << 24):
+        rng = np.random.default_rng([n, 3])
+        keys0 = torch.from_numpy(np.abs(rng.normal(0, 3, size=n)).astype(np.float32).view(np.int32)).cuda()
+        vals0 = torch.arange(n, dtype=torch.int32, device="cuda")
+        for bits in ((16, 32), (0, 32)):
+            passes = (bits[1] - bits[0]) // 8
+            k, v = keys0.clone(), vals0.clone()
+            binding.gamma_sort_pairs(k, v, *bits)
+            torch.cuda.synchronize()
+            ok = bool((k[1:].view(torch.int32) >> bits[0] >= k[:-1].view(torch.int32) >> bits[0]).all())
+            times = []
+            for _ in range(max(5, args.reps // 3)):
+                k.copy_(keys0); v.copy_(vals0)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                binding.gamma_sort_pairs(k, v, *bits)
+                e1.record(stream)
+                e1.synchronize()
+                times.append(e0.elapsed_time(e1))
+            ms = float(np.median(times))
+            alg = passes * 20.0 * n
+            emit({"suite": "sort", "pairs": n, "key_bits": bits[1] - bits[0], "passes": passes, "ms": ms, "sorted": ok,
+                  "pairs_per_s": n / (ms * 1e-3), "algorithmic_GBs": alg / (ms * 1e-3) / 1e9,
+                  "frac_of_hbm_copy_peak": alg / (ms * 1e-3) / 1e9 / hbm, "hbm_peak_GBs": hbm})
+
+
+def suite_general(args, emit):
+    import torch
+    from paper_1012_1900_b200 import binding, phantoms
+    c = phantoms.make_general_case("cfg3_general")
+    r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+    e = torch.from_numpy(c.eval.ravel().copy()).cuda()
+    a = (c.ref_dims, c.ref_spacing_mm, c.ref_origin_mm)
+    b = (c.eval_dims, c.eval_spacing_mm, c.eval_origin_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    stream = torch.cuda.current_stream()
+    out = torch.empty(r.numel(), device="cuda")
+    clo = torch.empty((r.numel(), 4), device="cuda")
+    res = {}
+    for label, oc in (("gamma only", None), ("gamma + closest point", clo)):
+        for _ in range(3):
+            binding.gamma_eval_general(r, *a, e, *b, None, out, False, oc, stream)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.reps):
+            binding.gamma_eval_general(r, *a, e, *b, None, out, False, oc, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        res[label] = e0.elapsed_time(e1) / args.reps
+    m = int((~torch.isnan(out)).sum().item())
+    emit({"suite": "general", "case": "cfg3_general: cfg3 reference (128x128x64 at 2.5 mm) against a 160x160x80 evaluation grid "
+          "at 2 mm, fractional origin offset", "M": m, "ms_per_case": res,
+          "evaluated_voxels_per_s": m / (res["gamma only"] * 1e-3)})
+
+
 def suite_trace(args, emit):
     """Where the time of a call goes: %globaltimer stamps of every kernel (first thread in, dependency wait passed,
     last block out), median over the calls of a back-to-back run; needs a -DGAMMA_TRACE build of the library."""
@@ -314,7 +383,7 @@ def write_md(path, rows):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--suite", default="all", choices=["configs", "criteria", "batch", "trace", "all"])
+    ap.add_argument("--suite", default="all", choices=["configs", "criteria", "batch", "sort", "general", "trace", "all"])
     ap.add_argument("--trace-case", default="cfg3")
     ap.add_argument("--reps", type=int, default=30)
     ap.add_argument("--oracle-seconds", type=float, default=8.0)
@@ -336,6 +405,10 @@ def main():
         suite_criteria(args, emit)
     if args.suite in ("batch", "all"):
         suite_batch(args, emit)
+    if args.suite in ("sort", "all"):
+        suite_sort(args, emit)
+    if args.suite in ("general", "all"):
+        suite_general(args, emit)
     if args.suite == "trace":
         suite_trace(args, emit)
     if args.md:

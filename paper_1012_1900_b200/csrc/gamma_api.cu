@@ -565,7 +565,7 @@ int prepare_workspace(const GridP& g, const Resolved& r, long long stride)
     if (g_ws.frozen) {
         const bool fits = CTL_BYTES <= g_ws.ctl.cap && listBytes <= g_ws.evalIdx.cap && listBytes <= g_ws.key1.cap &&
                           tableCells * 16 <= g_ws.table.cap && (size_t)r.tableCap * 4 <= g_ws.tmpL.cap &&
-                          (r.presort != 3 || (size_t)maxTiles * SORT_RADIX * 4 <= g_ws.tileHist.cap);
+                          (r.presort != 3 || (size_t)(maxTiles + 1) * SORT_RADIX * 4 <= g_ws.tileHist.cap);
         if (!fits)
             return fail(GAMMA_ERR_INVALID_ARGUMENT,
                         "this call needs a larger capture workspace, but its addresses are part of a captured CUDA graph; "
@@ -575,7 +575,7 @@ int prepare_workspace(const GridP& g, const Resolved& r, long long stride)
     CU_TRY(g_ws.key0.need(listBytes)); CU_TRY(g_ws.idx0.need(listBytes)); CU_TRY(g_ws.evalIdx.need(listBytes));
     CU_TRY(g_ws.key1.need(listBytes)); CU_TRY(g_ws.idx1.need(listBytes));
     g_ws.stride = stride;
-    if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
+    if (r.presort == 3) CU_TRY(g_ws.tileHist.need((size_t)(maxTiles + 1) * SORT_RADIX * 4));   // + the 256 digit totals
     // the small embedded table exists once per control-block slot (the next call builds its own while this call's
     // search still walks this one); a large table (table_radius 2, table_cap > 1024) lives BEHIND those slots, so a
     // following call's embedded table never aliases it
@@ -1475,7 +1475,7 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
     rc = ensure_ctl(st);
     if (rc) return rc;
     CU_TRY(g_ws.sortK.need(n * 4)); CU_TRY(g_ws.sortV.need(n * 4));
-    CU_TRY(g_ws.tileHist.need((size_t)maxTiles * SORT_RADIX * 4));
+    CU_TRY(g_ws.tileHist.need((size_t)(maxTiles + 1) * SORT_RADIX * 4));             // + the 256 digit totals
     rc = order_after_previous(st);
     if (rc) return rc;
     Ctl* ctl = static_cast<Ctl*>(g_ws.ctl.p) + CTL_STANDALONE;

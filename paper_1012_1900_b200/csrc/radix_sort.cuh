@@ -7,7 +7,7 @@
 // One pass per 8-bit digit, three kernels per pass, all reading the element count from device memory so
 // that the pipeline never synchronises with the host:
 //   k_radix_hist    per-tile digit histogram            -> tileHist[digit][tile]
-//   k_radix_scan    exclusive scan in digit-major order -> global base of every (digit, tile)
+//   k_radix_scan    exclusive scan along the tiles of every digit (one block per digit) + digit totals
 //   k_radix_scatter stable ranking inside the tile (warp match + per-warp counters) and scatter
 // Tile = 256 threads x 8 keys; a warp owns 256 consecutive keys and ranks them 32 at a time, which keeps
 // the sort stable.  Algorithmic traffic per pass: read keys twice + values once, write both: 20 B/pair.
@@ -40,62 +40,77 @@ k_radix_hist(const unsigned* __restrict__ keys, const unsigned* __restrict__ nPt
             if (i < n) atomicAdd(&hist[(keys[i] >> shift) & 0xffu], 1u);
         }
         __syncthreads();
-        tileHist[threadIdx.x * numTiles + tile] = hist[threadIdx.x];
+        tileHist[(size_t)threadIdx.x * numTiles + tile] = hist[threadIdx.x];
         __syncthreads();
     }
 }
 
-// exclusive scan of tileHist[0 .. 256*numTiles) in place; one block of 1024 threads.
-__global__ void __launch_bounds__(1024)
-k_radix_scan(unsigned* __restrict__ tileHist, const unsigned* __restrict__ nPtr)
+// Exclusive scan ALONG THE TILES of every digit's row tileHist[d][0 .. numTiles), in place, one block per digit
+// (256 independent, coalesced scans instead of one scan over 256 * numTiles values: the single-block version of round 1
+// took 3.5 ms of a 3.8 ms pass at 2^24 pairs, profiles/r2_sort.md); the row's total goes to digitTotal[d], from which
+// every scatter block derives the digit's global base.
+__global__ void __launch_bounds__(SORT_THREADS)
+k_radix_scan(unsigned* __restrict__ tileHist, const unsigned* __restrict__ nPtr, unsigned* __restrict__ digitTotal)
 {
-    const unsigned n = *nPtr;
-    const unsigned total = sort_num_tiles(n) * SORT_RADIX;
-    if (total == 0) return;
-    const unsigned per = (total + 1023u) / 1024u;
-    const unsigned lo = min(threadIdx.x * per, total), hi = min(lo + per, total);
-    unsigned sum = 0;
-    for (unsigned i = lo; i < hi; ++i) sum += tileHist[i];
-    // block exclusive scan of the 1024 partial sums
-    __shared__ unsigned warpSums[32];
+    const unsigned numTiles = sort_num_tiles(*nPtr);
+    unsigned* row = tileHist + (size_t)blockIdx.x * numTiles;
+    __shared__ unsigned warpSums[SORT_THREADS / 32];
+    __shared__ unsigned carry;
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    unsigned incl = sum;
-#pragma unroll
-    for (int s = 1; s < 32; s <<= 1) {
-        const unsigned t = __shfl_up_sync(0xffffffffu, incl, s);
-        if (lane >= (unsigned)s) incl += t;
-    }
-    if (lane == 31) warpSums[warp] = incl;
+    if (threadIdx.x == 0) carry = 0;
     __syncthreads();
-    if (warp == 0) {
-        unsigned w = warpSums[lane], wi = w;
+    for (unsigned base = 0; base < numTiles; base += SORT_THREADS) {
+        const unsigned i = base + threadIdx.x;
+        const unsigned v = i < numTiles ? row[i] : 0u;
+        unsigned incl = v;
 #pragma unroll
         for (int s = 1; s < 32; s <<= 1) {
-            const unsigned t = __shfl_up_sync(0xffffffffu, wi, s);
-            if (lane >= (unsigned)s) wi += t;
+            const unsigned t = __shfl_up_sync(0xffffffffu, incl, s);
+            if (lane >= (unsigned)s) incl += t;
         }
-        warpSums[lane] = wi - w;
+        if (lane == 31) warpSums[warp] = incl;
+        __syncthreads();
+        unsigned off = carry;
+#pragma unroll
+        for (int w = 0; w < SORT_THREADS / 32; ++w) off += (unsigned)w < warp ? warpSums[w] : 0u;
+        if (i < numTiles) row[i] = off + incl - v;
+        __syncthreads();
+        if (threadIdx.x == SORT_THREADS - 1) carry = off + incl;
+        __syncthreads();
     }
-    __syncthreads();
-    unsigned run = warpSums[warp] + incl - sum;
-    for (unsigned i = lo; i < hi; ++i) {
-        const unsigned t = tileHist[i];
-        tileHist[i] = run;
-        run += t;
-    }
+    if (threadIdx.x == 0) digitTotal[blockIdx.x] = carry;
 }
 
 __global__ void __launch_bounds__(SORT_THREADS)
 k_radix_scatter(const unsigned* __restrict__ keysIn, const unsigned* __restrict__ valsIn,
                 unsigned* __restrict__ keysOut, unsigned* __restrict__ valsOut,
-                const unsigned* __restrict__ nPtr, int shift, const unsigned* __restrict__ tileHist)
+                const unsigned* __restrict__ nPtr, int shift, const unsigned* __restrict__ tileHist,
+                const unsigned* __restrict__ digitTotal)
 {
     const unsigned n = *nPtr;
     const unsigned numTiles = sort_num_tiles(n);
     constexpr int WARPS = SORT_THREADS / 32;
     __shared__ unsigned wc[WARPS][SORT_RADIX];
+    __shared__ unsigned digitBase[SORT_RADIX];
+    __shared__ unsigned baseWarp[WARPS];
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const unsigned ltMask = (1u << lane) - 1u;
+    {   // global base of digit d = exclusive scan of the 256 digit totals (thread d)
+        const unsigned v = digitTotal[threadIdx.x];
+        unsigned incl = v;
+#pragma unroll
+        for (int s = 1; s < 32; s <<= 1) {
+            const unsigned t = __shfl_up_sync(0xffffffffu, incl, s);
+            if (lane >= (unsigned)s) incl += t;
+        }
+        if (lane == 31) baseWarp[warp] = incl;
+        __syncthreads();
+        unsigned off = 0;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) off += (unsigned)w < warp ? baseWarp[w] : 0u;
+        digitBase[threadIdx.x] = off + incl - v;
+        __syncthreads();
+    }
     for (unsigned tile = blockIdx.x; tile < numTiles; tile += gridDim.x) {
 #pragma unroll
         for (int w = 0; w < WARPS; ++w) wc[w][threadIdx.x] = 0;
@@ -118,7 +133,7 @@ k_radix_scatter(const unsigned* __restrict__ keysIn, const unsigned* __restrict_
         }
         __syncthreads();
         {   // thread d turns the per-warp counts of digit d into global base positions
-            unsigned run = tileHist[threadIdx.x * numTiles + tile];
+            unsigned run = digitBase[threadIdx.x] + tileHist[(size_t)threadIdx.x * numTiles + tile];
 #pragma unroll
             for (int w = 0; w < WARPS; ++w) {
                 const unsigned t = wc[w][threadIdx.x];
@@ -151,9 +166,10 @@ inline int radix_sort_enqueue(unsigned* k0, unsigned* v0, unsigned* k1, unsigned
     for (int bit = beginBit; bit < endBit; bit += 8) {
         unsigned* ki = cur ? k1 : k0; unsigned* vi = cur ? v1 : v0;
         unsigned* ko = cur ? k0 : k1; unsigned* vo = cur ? v0 : v1;
+        unsigned* digitTotal = tileHist + (size_t)tiles * SORT_RADIX;     // 256 words behind the tile histograms
         k_radix_hist<<<grid, SORT_THREADS, 0, st>>>(ki, nPtr, bit, tileHist);
-        k_radix_scan<<<1, 1024, 0, st>>>(tileHist, nPtr);
-        k_radix_scatter<<<grid, SORT_THREADS, 0, st>>>(ki, vi, ko, vo, nPtr, bit, tileHist);
+        k_radix_scan<<<SORT_RADIX, SORT_THREADS, 0, st>>>(tileHist, nPtr, digitTotal);
+        k_radix_scatter<<<grid, SORT_THREADS, 0, st>>>(ki, vi, ko, vo, nPtr, bit, tileHist, digitTotal);
         cur ^= 1;
     }
     return cur;
