@@ -26,6 +26,32 @@ namespace {
 thread_local std::string g_err;
 std::mutex g_mu;
 
+// Host-side time of the submission path (build with -DGAMMA_HOSTPROF; printed to stderr by gamma_release()).
+#ifdef GAMMA_HOSTPROF
+}  // namespace
+#include <chrono>
+namespace {
+struct HostProf {
+    double us[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long n[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+} g_hp;
+const char* const HP_NAMES[8] = {"gamma_eval_ex total", "back-pressure wait", "kernel launches", "events", "prepare/order/ctl",
+                                 "argument checks", "getenv", "enqueue_kernels"};
+struct HpScope {
+    int k;
+    std::chrono::steady_clock::time_point t0;
+    explicit HpScope(int k_) : k(k_), t0(std::chrono::steady_clock::now()) {}
+    ~HpScope()
+    {
+        g_hp.us[k] += std::chrono::duration<double, std::micro>(std::chrono::steady_clock::now() - t0).count();
+        ++g_hp.n[k];
+    }
+};
+#define HP(k) HpScope hp_scope_##k(k)
+#else
+#define HP(k) do { } while (0)
+#endif
+
 int fail(int code, const std::string& msg)
 {
     g_err = msg;
@@ -55,6 +81,7 @@ cudaError_t launch_ex(void (*kernel)(KArgs...), int grid, int block, size_t smem
     if (pdl) { at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[n].val.programmaticStreamSerializationAllowed = 1; ++n; }
     if (coop) { at[n].id = cudaLaunchAttributeCooperative; at[n].val.cooperative = 1; ++n; }
     cfg.attrs = at; cfg.numAttrs = n;
+    HP(2);
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
@@ -219,7 +246,10 @@ unsigned g_callNo = 0;                 // gamma_eval* calls so far, all workspac
 // was on the caller's stream when the sequence of back-to-back calls began (one event), the caller's stream waits for
 // every call (one event per call, so later work of the caller's sees all results), calls on one lane are in stream
 // order, and a call that touches a buffer of one of the last B2B_WINDOW - 1 calls on another lane waits for that call.
-constexpr int B2B_WINDOW = 8;          // calls whose buffers are remembered; call j waits (host) for call j - B2B_WINDOW
+#ifndef GAMMA_B2B_WINDOW
+#define GAMMA_B2B_WINDOW 8
+#endif
+constexpr int B2B_WINDOW = GAMMA_B2B_WINDOW;   // calls whose buffers are remembered; call j waits (host) for call j - B2B_WINDOW
 struct LaneState {
     cudaStream_t stream[LANES] = {};
     cudaEvent_t fork = nullptr;
@@ -905,15 +935,18 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         return rc;
     }
     long long byNMax = LISTS_BY_N_MAX;
-    if (const char* env = std::getenv("GAMMA_LISTS_BY_N_MAX")) byNMax = std::atoll(env);   // tests: two-phase path on small grids
+    { HP(6); if (const char* env = std::getenv("GAMMA_LISTS_BY_N_MAX")) byNMax = std::atoll(env); }  // tests: two-phase path on small grids
     const bool twoPhase = N > byNMax;
     const bool useGraph = g_ws.graphs != 0 && r.graph && !r.profile && !twoPhase;
-    rc = ensure_device();
-    if (rc) return rc;
-    rc = order_after_previous(st);
-    if (rc) return rc;
-    rc = ensure_ctl(st);
-    if (rc) return rc;
+    {
+        HP(4);
+        rc = ensure_device();
+        if (rc) return rc;
+        rc = order_after_previous(st);
+        if (rc) return rc;
+        rc = ensure_ctl(st);
+        if (rc) return rc;
+    }
     g_ws.ctlClean = false;                                 // set again when everything below was enqueued
     CallSlot cs;
     cs.slot = g_ws.slot;
@@ -938,7 +971,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         stride = (long long)M + 1024;
         cs.skipNorm = true;
     }
-    rc = prepare_workspace(g, r, stride);
+    { HP(4); rc = prepare_workspace(g, r, stride); }
     if (rc) return rc;
     // ---- may k_norm start in the tail of the previous call?
     CallSpans mine;
@@ -955,6 +988,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
 
     int launched = 0;
     if (!useGraph) {
+        HP(7);
         rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, cs, &launched);
         if (rc) return rc;
     } else {
@@ -1042,7 +1076,7 @@ int enqueue_on_lane(const float* ref, const float* ev, const GridP& g, float DD,
     L.active = false;                                      // set again on success
     const unsigned long long j = L.next;
     const int w = (int)(j % B2B_WINDOW), lane = (int)(j % LANES);
-    if (L.used[w]) CU_TRY(cudaEventSynchronize(L.done[w]));           // call j - B2B_WINDOW has ended (back-pressure)
+    if (L.used[w]) { HP(1); CU_TRY(cudaEventSynchronize(L.done[w])); }   // call j - B2B_WINDOW has ended (back-pressure)
     cudaStream_t st = L.stream[lane];
     if (L.laneFork[lane] != L.forkGen) {
         CU_TRY(cudaStreamWaitEvent(st, L.fork, 0));
@@ -1066,8 +1100,11 @@ int enqueue_on_lane(const float* ref, const float* ev, const GridP& g, float DD,
     g_cur = keep;
     if (rc) { L.laneDirty[lane] = true; return rc; }
     L.laneDirty[lane] = false;
-    CU_TRY(cudaEventRecord(L.done[w], st));
-    CU_TRY(cudaStreamWaitEvent(user, L.done[w], 0));                  // the caller's stream sees the result
+    {
+        HP(3);
+        CU_TRY(cudaEventRecord(L.done[w], st));
+        CU_TRY(cudaStreamWaitEvent(user, L.done[w], 0));              // the caller's stream sees the result
+    }
     L.spans[w] = mine; L.laneOf[w] = lane; L.used[w] = true;
     ++L.next;
     L.active = true;
@@ -1108,16 +1145,21 @@ int gamma_eval_ex(const float* ref, const float* eval, const int dims[3], const 
                   float DTA_mm, int mode, float low_dose_cutoff, const gamma_opts* opts, float* out_gamma,
                   void* stream)
 {
+    HP(0);
     g_err.clear();
     if (!ref || !eval || !out_gamma) return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref / eval / out_gamma is NULL");
     GridP g;
-    int rc = make_grid(dims, spacing_mm, DTA_mm, g);
-    if (rc) return rc;
-    rc = check_criteria(DD, mode, low_dose_cutoff);
-    if (rc) return rc;
     Resolved r;
-    rc = resolve_opts(opts, r);
-    if (rc) return rc;
+    int rc;
+    {
+        HP(5);
+        rc = make_grid(dims, spacing_mm, DTA_mm, g);
+        if (rc) return rc;
+        rc = check_criteria(DD, mode, low_dose_cutoff);
+        if (rc) return rc;
+        rc = resolve_opts(opts, r);
+        if (rc) return rc;
+    }
     std::lock_guard<std::mutex> lock(g_mu);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (r.backToBack) {
@@ -1680,6 +1722,13 @@ void gamma_release(void)
 {
     std::lock_guard<std::mutex> lock(g_mu);
     cudaDeviceSynchronize();
+#ifdef GAMMA_HOSTPROF
+    for (int k = 0; k < 8; ++k)
+        if (g_hp.n[k])
+            std::fprintf(stderr, "[gamma hostprof] %-22s %10lld x %8.3f us = %10.1f us\n", HP_NAMES[k], g_hp.n[k],
+                         g_hp.us[k] / (double)g_hp.n[k], g_hp.us[k]);
+    g_hp = HostProf();
+#endif
     for (Workspace& w : g_pool) w.releaseAll();
     for (int l = 0; l < LANES; ++l)
         if (g_lanes.stream[l]) { cudaStreamDestroy(g_lanes.stream[l]); g_lanes.stream[l] = nullptr; }

@@ -479,6 +479,32 @@ struct VoxelCtx {
     int algo;         // EvalP::algo
 };
 
+// Offset-dependent terms of the 26 faces owned by the vertex at (real-valued) offset (fx, fy, fz) voxels from the
+// reference point (features_generated.cuh, gamma_owned_min): lam[T] = -(p . h_T) / A_T, q[a] = p_a^2, X[T].
+// usable: bit a set when the owner's neighbour along +a is inside the grid.  A face that steps along an unusable axis
+// does not exist (reading 11): lam[T] is NaN for every T holding such an axis, which fails the face's first comparison.
+__device__ __forceinline__ void owned_face_terms(const GridP& g, float fx, float fy, float fz, unsigned usable,
+                                                 float (&lam)[8], float (&q)[3], float (&X)[8])
+{
+    const float qnan = __int_as_float(0x7fc00000);
+    const float px = fx * g.h[0], py = fy * g.h[1], pz = fz * g.h[2];
+    q[0] = px * px; q[1] = py * py; q[2] = pz * pz;
+    const float gx = (usable & 1u) ? fx : qnan, gy = (usable & 2u) ? fy : qnan, gz = (usable & 4u) ? fz : qnan;
+    const float bxh = gx * g.hh[0], byh = gy * g.hh[1], bzh = gz * g.hh[2];
+    lam[0] = 0.0f;
+    lam[1] = -gx; lam[2] = -gy; lam[4] = -gz;
+    lam[3] = -(bxh + byh) * g.invA[3];
+    lam[5] = -(bxh + bzh) * g.invA[5];
+    lam[6] = -(byh + bzh) * g.invA[6];
+    lam[7] = -(bxh + byh + bzh) * g.invA[7];
+    const float dxy = fx - fy, dxz = fx - fz, dyz = fy - fz;
+    X[0] = X[1] = X[2] = X[4] = 0.0f;
+    X[3] = g.K3 * dxy * dxy;
+    X[5] = g.K5 * dxz * dxz;
+    X[6] = g.K6 * dyz * dyz;
+    X[7] = g.Kxy7 * dxy * dxy + g.Kyz7 * dyz * dyz + g.Kzx7 * dxz * dxz;
+}
+
 // All 26 faces owned by the grid vertex c = v + o; returns the new best^2.
 template <bool JU>
 __device__ __forceinline__ float eval_owner_vertex(const float* __restrict__ ev, const GridP& g, const VoxelCtx& vc,
@@ -497,31 +523,15 @@ __device__ __forceinline__ float eval_owner_vertex(const float* __restrict__ ev,
     }
     float d[8];
 #pragma unroll
-    for (int S = 0; S < 8; ++S)
-        d[S] = (__ldg(p + ((S & 1) ? sx : 0) + ((S & 2) ? sy : 0) + ((S & 4) ? sz : 0)) - vc.Dr) * vc.invdD;
+    for (int S = 0; S < 8; ++S)                                // 32-bit offsets from one base pointer
+        d[S] = (__ldg(p + (((S & 1) ? sx : 0) + ((S & 2) ? sy : 0) + ((S & 4) ? sz : 0))) - vc.Dr) * vc.invdD;
     if (JU && vc.algo == 2) {                                  // variant: whole cells by the recursion of PAPER.md:209
         if (usable != 7u) return best2;                        // only cells fully inside the grid exist (reading 11)
         return ju_cell_min(d, g, ox, oy, oz, best2);
     }
-    const float fx = (float)ox, fy = (float)oy, fz = (float)oz;
-    const float px = fx * g.h[0], py = fy * g.h[1], pz = fz * g.h[2];
-    const float q[3] = {px * px, py * py, pz * pz};
-    const float bxh = fx * g.hh[0], byh = fy * g.hh[1], bzh = fz * g.hh[2];
-    float lam[8];
-    lam[0] = 0.0f;
-    lam[1] = -fx; lam[2] = -fy; lam[4] = -fz;
-    lam[3] = -(bxh + byh) * g.invA[3];
-    lam[5] = -(bxh + bzh) * g.invA[5];
-    lam[6] = -(byh + bzh) * g.invA[6];
-    lam[7] = -(bxh + byh + bzh) * g.invA[7];
-    const float dxy = fx - fy, dxz = fx - fz, dyz = fy - fz;
-    float X[8];
-    X[0] = X[1] = X[2] = X[4] = 0.0f;
-    X[3] = g.K3 * dxy * dxy;
-    X[5] = g.K5 * dxz * dxz;
-    X[6] = g.K6 * dyz * dyz;
-    X[7] = g.Kxy7 * dxy * dxy + g.Kyz7 * dyz * dyz + g.Kzx7 * dxz * dxz;
-    return gamma_owned_min(d, g.invA, lam, q, X, usable, best2);
+    float lam[8], q[3], X[8];
+    owned_face_terms(g, (float)ox, (float)oy, (float)oz, usable, lam, q, X);
+    return gamma_owned_min(d, g.invA, lam, q, X, best2);
 }
 
 template <int G>

@@ -59,6 +59,37 @@ def add(o, mask):
     return tuple(o[a] + (1 if mask & AX[a] else 0) for a in range(3))
 
 
+
+def emit_select_helpers(w):
+    """gamma_min_if<n> / gamma_max_if<n>: best = min / max(best, x) when a_1 >= b_1 && ... && a_n >= b_n.
+
+    The feasibility test of a face is a chain of ordered comparisons (1 >= t_1 >= ... >= t_k >= 0).  Written as C++
+    the compiler turns every comparison into an FSETP plus an FSEL on the candidate; here the comparisons feed one
+    predicate (setp.ge.and takes the previous predicate as its third operand) that guards a single FMNMX: k + 2
+    instructions per face instead of 2k + 3.  NaN operands fail every comparison (ordered compare), which is how faces
+    that would leave the grid are rejected (gamma_owned_min)."""
+    w("// best = min(best, x) / max(best, x) when every a_i >= b_i: one predicate through a chain of FSETPs (each takes\n")
+    w("// the previous predicate as an input) guarding ONE predicated FMNMX; a NaN operand fails its comparison.\n")
+    for op in ("min", "max"):
+        for n in range(1, 5):
+            args = ", ".join("float a%d, float b%d" % (i, i) for i in range(n))
+            w("GAMMA_HD void gamma_%s_if%d(float& best, float x, %s)\n{\n" % (op, n, args))
+            w("#if defined(__CUDA_ARCH__)\n")
+            lines = ["{", ".reg .pred p;", "setp.ge.f32 p, %2, %3;"]
+            for i in range(1, n):
+                lines.append("setp.ge.and.f32 p, %%%d, %%%d, p;" % (2 + 2 * i, 3 + 2 * i))
+            lines.append("@p %s.f32 %%0, %%0, %%1;" % op)
+            lines.append("}")
+            body = "\\n\\t".join(lines)
+            ins = ", ".join(['"f"(x)'] + ['"f"(a%d), "f"(b%d)' % (i, i) for i in range(n)])
+            w('    asm("%s" : "+f"(best) : %s);\n' % (body, ins))
+            w("#else\n")
+            cond = " && ".join("(a%d >= b%d)" % (i, i) for i in range(n))
+            w("    if (%s) best = f%sf(best, x);\n" % (cond, op))
+            w("#endif\n}\n")
+    w("\n")
+
+
 def emit_star(w):
     w("// The 75 faces of the Kuhn mesh that contain the reference voxel (its star), generated.\n")
     w("// d[27]: (D_e[v+o] - D_r[v]) / dD for o in {-1,0,1}^3, index (ox+1) + 3(oy+1) + 9(oz+1).\n")
@@ -77,7 +108,6 @@ def emit_star(w):
             b_off = add(a_off, tmask)
             lines.append("    const float dl_%s = d[%d] - d[%d];\n" % (nm, vid(b_off), vid(a_off)))
             lines.append("    const float w_%s = dl_%s * invA[%d];\n" % (nm, nm, tmask))
-            lines.append("    const float g_%s = dl_%s * w_%s;\n" % (nm, nm, nm))
             lines.append("    const float u_%s = d0 * w_%s;\n" % (nm, nm))
             edges[key] = nm
         return edges[key]
@@ -86,11 +116,8 @@ def emit_star(w):
         key = tuple(names)
         if key not in sums:
             nm = "s_" + "_".join(names)
-            if len(names) == 1:
-                lines.append("    const float %s = 1.0f + g_%s;\n" % (nm, names[0]))
-            else:
-                prev = gsum(names[:-1])
-                lines.append("    const float %s = %s + g_%s;\n" % (nm, prev, names[-1]))
+            prev = "1.0f" if len(names) == 1 else gsum(names[:-1])
+            lines.append("    const float %s = fmaf(dl_%s, w_%s, %s);\n" % (nm, names[-1], names[-1], prev))
             sums[key] = nm
         return sums[key]
 
@@ -108,18 +135,18 @@ def emit_star(w):
                 names.append(edge(add(o, full[i - 1]), full[i] ^ full[i - 1]))
             G1 = gsum(names)
             u = ["u_" + n for n in names]
-            conds = []
+            conds = []                                        # (a, b): a >= b
             # cond_0: G1 >= T_1
-            conds.append("%s >= 0.0f" % u[0] if jstar >= 1 else "%s >= -%s" % (G1, u[0]))
+            conds.append((u[0], "0.0f") if jstar >= 1 else (G1, "-" + u[0]))
             for i in range(1, k):                             # T_i >= T_{i+1}
                 if (i <= jstar) == (i + 1 <= jstar):
-                    conds.append("%s >= %s" % (u[i], u[i - 1]))
+                    conds.append((u[i], u[i - 1]))
                 else:
-                    conds.append("%s >= %s - %s" % (G1, u[i - 1], u[i]))
-            conds.append("%s >= %s" % (G1, u[k - 1]) if jstar == k else "%s <= 0.0f" % u[k - 1])
+                    conds.append((G1, "%s - %s" % (u[i - 1], u[i])))
+            conds.append((G1, u[k - 1]) if jstar == k else ("0.0f", u[k - 1]))
             lines.append("    // owner (%d,%d,%d) chain %s, reference voxel is chain vertex %d\n"
                          % (o[0], o[1], o[2], "<".join(str(s) for s in full), jstar))
-            lines.append("    if (%s) gmax = fmaxf(gmax, %s);\n" % (" && ".join("(%s)" % c for c in conds), G1))
+            lines.append("    gamma_max_if%d(gmax, %s, %s);\n" % (len(conds), G1, ", ".join("%s, %s" % c for c in conds)))
             nfeat += 1
     assert nfeat == 74, nfeat       # + the vertex itself = 75
     for ln in lines:
@@ -132,14 +159,15 @@ def emit_owned(w):
     w("// (vertex, 7 edges, 12 triangles, 6 tetrahedra whose lowest corner is c), generated.\n")
     w("// d[S]:   (D_e[c+S] - D_r[v]) / dD for the 8 corners S (bit0 = +x, bit1 = +y, bit2 = +z);\n")
     w("// lam[T]: -(p . h_T)/A_T, p = o*h;  q[a] = p_a^2;  X[T] (T = 3,5,6,7): squared distance of p's\n")
-    w("//         T-components to the line along h_T;  usable: bit a set when c_a + 1 is inside the grid.\n")
+    w("//         T-components to the line along h_T.\n")
+    w("// A face that would leave the grid (its chain steps along an axis a with c_a + 1 outside) must be rejected by the\n")
+    w("// caller's lam: lam[T] = NaN for every T that holds such an axis (owned_face_terms) -- N, r and every t_i of the\n")
+    w("// face are then NaN and its first comparison fails.\n")
     w("// Returns min(best2, squared distance to every feasible, valid owned face).\n")
     w("GAMMA_HD float gamma_owned_min(const float (&d)[8], const float (&invA)[8], const float (&lam)[8],\n")
-    w("                               const float (&q)[3], const float (&X)[8], unsigned usable, float best2)\n{\n")
+    w("                               const float (&q)[3], const float (&X)[8], float best2)\n{\n")
     w("    best2 = fminf(best2, (q[0] + q[1]) + (q[2] + d[0] * d[0]));   // the vertex c itself\n")
     done_e, done_n, done_g, done_c = set(), set(), set(), set()
-    for s in range(1, 8):
-        w("    const bool ok%d = (usable & %du) == %du;\n" % (s, s, s))
 
     def edge(a, b):
         nm = "%d_%d" % (a, b)
@@ -186,12 +214,10 @@ def emit_owned(w):
         for i in range(k):
             w("        const float t%d = fmaf(-r, w%s, lam[%d]);\n" % (i + 1, names[i], full[i + 1] ^ full[i]))
             ts.append("t%d" % (i + 1))
-        conds = ["ok%d" % ch[-1], "1.0f >= t1"]
-        conds += ["%s >= %s" % (ts[i], ts[i + 1]) for i in range(k - 1)]
-        conds.append("%s >= 0.0f" % ts[-1])
+        conds = [("1.0f", "t1")] + [(ts[i], ts[i + 1]) for i in range(k - 1)] + [(ts[-1], "0.0f")]
         c = cval(ch)
         dist = "fmaf(%s, r, %s)" % (N, c) if c else "%s * r" % N
-        w("        best2 = (%s) ? fminf(best2, %s) : best2;\n" % (" & ".join("(%s)" % x for x in conds), dist))
+        w("        gamma_min_if%d(best2, %s, %s);\n" % (len(conds), dist, ", ".join("%s, %s" % x for x in conds)))
         w("    }\n")
     w("    return best2;\n}\n")
 
@@ -365,11 +391,9 @@ def emit_ring(w):
         for i in range(k):
             w("        const float t%d = fmaf(-r, w%s, R.lam[%d][%d]);\n" % (i + 1, names[i], neg, full[i + 1] ^ full[i]))
             ts.append("t%d" % (i + 1))
-        conds = ["1.0f >= t1"]
-        conds += ["%s >= %s" % (ts[i], ts[i + 1]) for i in range(k - 1)]
-        conds.append("%s >= 0.0f" % ts[-1])
-        w("        best2 = (%s) ? fminf(best2, fmaf(%s, r, R.C[%d])) : best2;\n"
-          % (" & ".join("(%s)" % x for x in conds), N, f))
+        conds = [("1.0f", "t1")] + [(ts[i], ts[i + 1]) for i in range(k - 1)] + [(ts[-1], "0.0f")]
+        w("        gamma_min_if%d(best2, fmaf(%s, r, R.C[%d]), %s);\n"
+          % (len(conds), N, f, ", ".join("%s, %s" % x for x in conds)))
         w("    }\n")
     w("    return best2;\n}\n")
 
@@ -389,6 +413,7 @@ def main():
         w("#if defined(__CUDA_ARCH__)\n__device__ __forceinline__ float gamma_fdiv(float a, float b)\n{\n"
           "    float r;\n    asm(\"rcp.approx.ftz.f32 %0, %1;\" : \"=f\"(r) : \"f\"(b));\n    return a * r;\n}\n"
           "#define GAMMA_FDIV(a, b) gamma_fdiv((a), (b))\n#else\n#define GAMMA_FDIV(a, b) ((a) / (b))\n#endif\n\n")
+        emit_select_helpers(w)
         emit_star(w)
         emit_owned(w)
         emit_owned_arg(w)

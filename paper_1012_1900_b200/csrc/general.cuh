@@ -43,27 +43,11 @@ __device__ __forceinline__ float general_owner_vertex(const float* __restrict__ 
     float d[8];
 #pragma unroll
     for (int S = 0; S < 8; ++S)
-        d[S] = (__ldg(p + ((S & 1) ? sx : 0) + ((S & 2) ? sy : 0) + ((S & 4) ? sz : 0)) - Dr) * invdD;
-    const float fx = (float)ox - f[0], fy = (float)oy - f[1], fz = (float)oz - f[2];
-    const float px = fx * g.h[0], py = fy * g.h[1], pz = fz * g.h[2];
-    const float q[3] = {px * px, py * py, pz * pz};
-    const float bxh = fx * g.hh[0], byh = fy * g.hh[1], bzh = fz * g.hh[2];
-    float lam[8];
-    lam[0] = 0.0f;
-    lam[1] = -fx; lam[2] = -fy; lam[4] = -fz;
-    lam[3] = -(bxh + byh) * g.invA[3];
-    lam[5] = -(bxh + bzh) * g.invA[5];
-    lam[6] = -(byh + bzh) * g.invA[6];
-    lam[7] = -(bxh + byh + bzh) * g.invA[7];
-    const float dxy = fx - fy, dxz = fx - fz, dyz = fy - fz;
-    float X[8];
-    X[0] = X[1] = X[2] = X[4] = 0.0f;
-    X[3] = g.K3 * dxy * dxy;
-    X[5] = g.K5 * dxz * dxz;
-    X[6] = g.K6 * dyz * dyz;
-    X[7] = g.Kxy7 * dxy * dxy + g.Kyz7 * dyz * dyz + g.Kzx7 * dxz * dxz;
+        d[S] = (__ldg(p + (((S & 1) ? sx : 0) + ((S & 2) ? sy : 0) + ((S & 4) ? sz : 0))) - Dr) * invdD;
+    float lam[8], q[3], X[8];
+    owned_face_terms(g, (float)ox - f[0], (float)oy - f[1], (float)oz - f[2], usable, lam, q, X);
     if (wantLoc) return gamma_owned_argmin(d, g.invA, lam, q, X, usable, best2, loc);
-    return gamma_owned_min(d, g.invA, lam, q, X, usable, best2);
+    return gamma_owned_min(d, g.invA, lam, q, X, best2);
 }
 
 // exact squared minimum spatial distance (normalised) from the point c0 + f to the cell [c0 + o, c0 + o + 1]
