@@ -77,6 +77,7 @@ struct Ctl {
     unsigned pad0_;
     float invGlobal;       // 1 / (DD * D_norm) rounded to fp32 (global criterion), written by k_classify
     unsigned long long visits;       // owner vertices evaluated by the table search
+    unsigned zeros[32];              // always zero (ticket_one)
     unsigned hist[KEY_DIGITS];       // digit histogram of the search list (bucket presort)
     unsigned cursor[KEY_DIGITS];     // scatter cursors of the bucket presort
 };
@@ -119,6 +120,8 @@ __device__ __forceinline__ void trace_waited(unsigned, int) {}
 __device__ __forceinline__ void trace_last(unsigned, int) {}
 #endif
 
+__device__ __forceinline__ unsigned ticket_one(const Ctl* ctl) { return 1u + ctl->zeros[threadIdx.x & 31]; }
+
 // Monotone 8-bit quantisation of a non-negative key: 32 steps per octave over [2^-3, 2^5), clamped.
 // This is the digit of the one-pass MSD radix presort of the search work list.
 __device__ __forceinline__ unsigned key_digit(float key)
@@ -152,6 +155,20 @@ __device__ __forceinline__ float cell_L2(int mx, int my, int mz, const GridP& g)
 {
     const float ax = (float)mx * g.h[0], ay = (float)my * g.h[1], az = (float)mz * g.h[2];
     return fmaf(ax, ax, fmaf(ay, ay, az * az));
+}
+
+// Work ticket: a counter incremented by one whose old value is not needed before the end of the current work item.
+// ptxas aggregates an integer atomicAdd (or PTX atom.add / atom.inc, 32 or 64 bit) with a warp-uniform addend over the
+// active lanes -- vote, popc, the leader's ATOMG, SHFL of the result -- and that shuffle waits for the atomic right
+// where it was issued (measured: the largest single stall of k_table_search, 19 % of its warp samples; fp32 atomics are
+// not aggregated but serialise on one address: 5 us slower).  With an addend it cannot prove uniform (1 + a zero word
+// loaded per lane from the control block) a partially active warp gets a plain ATOMG per lane, whose result is consumed
+// where the program uses it.  Call from ONE lane of the warp with `one` = ticket_one(ctl).
+__device__ __forceinline__ unsigned ticket_next(unsigned* p, unsigned one)
+{
+    unsigned r;
+    asm volatile("atom.global.add.u32 %0, [%1], %2;" : "=r"(r) : "l"(p), "r"(one));
+    return r;
 }
 
 __device__ __forceinline__ float warp_max(float v)

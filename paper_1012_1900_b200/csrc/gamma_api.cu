@@ -232,7 +232,10 @@ struct Workspace {
 // back-to-back calls (gamma_opts::back_to_back) and the cases of gamma_eval_batch run so that the kernels of
 // consecutive calls overlap on the device; the last one belongs to the calls a caller captures into its own CUDA graph
 // (its addresses are baked into that graph, so it never moves once used: gamma_release() is the only way to grow it).
-constexpr int LANES = 4;
+#ifndef GAMMA_LANES
+#define GAMMA_LANES 4
+#endif
+constexpr int LANES = GAMMA_LANES;
 constexpr int WS_CAPTURE = 1 + LANES;
 Workspace g_pool[2 + LANES];
 Workspace* g_cur = &g_pool[0];

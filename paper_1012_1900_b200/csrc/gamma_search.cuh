@@ -238,7 +238,7 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
 
 // ------------------------------------------------------------------------------------------------
 // first part of a4: the star phase over the compacted voxels, one voxel per thread, one warp per 32
-// consecutive list entries (first round static, later rounds fetched dynamically).
+// consecutive list entries (whole rounds static, the last partial round fetched dynamically).
 // ------------------------------------------------------------------------------------------------
 // 128 threads x 9 resident blocks = 36 warps per SM at 56 registers: 148 x 36 x 32 = 170 496 voxels are in flight at
 // once, so cases up to that many evaluated voxels (cfg2, cfg3: 160 256) finish in ONE round of items.
@@ -291,7 +291,12 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     const unsigned M = ctl->nEval;
     const unsigned warpsTotal = gridDim.x * (STAR_THREADS / 32);
     const unsigned numItems = (M + 31u) / 32u;
-    const bool dynamic = numItems > warpsTotal;
+    // Items are handed out in static rounds (item = warp + round * warps) while whole rounds are left; only the last,
+    // partial round goes through the ticket counter: 5 000 warps asking one address for a ticket at the same moment
+    // queue up for microseconds (same-address atomics are served one at a time).
+    const unsigned staticRounds = numItems / warpsTotal;
+    const unsigned one = ticket_one(ctl);
+    unsigned round = 1;
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
     const double dnorm = (double)dnormF;
     const float invGlobal = ctl->invGlobal;
@@ -308,7 +313,9 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
 
     while (item < numItems) {
         unsigned nextItem = numItems;
-        if (dynamic && lane == 0) nextItem = atomicAdd(&ctl->tileCounter, 1u) + warpsTotal;
+        if (round < staticRounds) nextItem = item + warpsTotal;
+        else if (staticRounds && lane == 0) nextItem = ticket_next(&ctl->tileCounter, one) + staticRounds * warpsTotal;
+        ++round;
         const unsigned j = item * 32u + lane;
         bool toSearch = false, starDone = false;
         float key = 0.0f;
@@ -572,8 +579,10 @@ template <int G, bool JU = false>
 __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP& g, const EvalP& e,
                                                  const unsigned* __restrict__ listKey,
                                                  const unsigned* __restrict__ listIdx, unsigned nList,
-                                                 unsigned firstItem, int lane)
+                                                 unsigned firstItem, int lane, bool pre = false, unsigned preIdx = 0u,
+                                                 unsigned preKey = 0u)
 {
+    // pre: (preIdx, preKey) is this lane's list entry, fetched while the previous work item was searched
     constexpr int EPP = G >= 8 ? G / 8 : 1;     // table entries per pass
     const unsigned FULL = 0xffffffffu;
     const int gid = lane / G, gl = lane % G;
@@ -585,8 +594,8 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
     float key = 0.0f, best2 = 0.0f;
     if (have) {
         const unsigned idx = nList - 1u - item;
-        vc.lin = (int)listIdx[idx];
-        key = __uint_as_float(listKey[idx]);
+        vc.lin = (int)(pre ? preIdx : listIdx[idx]);
+        key = __uint_as_float(pre ? preKey : listKey[idx]);
         vc.Dr = __ldg(c.ref + vc.lin);
         vc.invdD = e.mode == 0 ? c.invGlobal : criterion_inv_dD(e, c.dnorm, vc.Dr);
         voxel_coords(g, vc.lin, vc.v[0], vc.v[1], vc.v[2]);
@@ -699,12 +708,12 @@ __device__ __forceinline__ unsigned search_items(const SearchCtx& c, const GridP
 __device__ __forceinline__ void ring_items(const SearchCtx& c, const GridP& g, const EvalP& e, const GammaRingP& R,
                                            const unsigned* __restrict__ listKey,
                                            const unsigned* __restrict__ listIdx, unsigned nList, unsigned firstItem,
-                                           int lane)
+                                           int lane, bool pre = false, unsigned preIdx = 0u, unsigned preKey = 0u)
 {
     const unsigned item = firstItem + (unsigned)lane;
     if (item >= nList) return;
-    const int lin = (int)listIdx[item];
-    const float key = __uint_as_float(listKey[item]);
+    const int lin = (int)(pre ? preIdx : listIdx[item]);
+    const float key = __uint_as_float(pre ? preKey : listKey[item]);
     const float Dr = __ldg(c.ref + lin);
     const float invdD = e.mode == 0 ? c.invGlobal : criterion_inv_dD(e, c.dnorm, Dr);
     const float* p = c.ev + lin;
@@ -767,7 +776,9 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
     unsigned unit = blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5);
     if (unit < numUnits) {
-        const bool dynamic = numUnits > warpsTotal;
+        const unsigned staticRounds = numUnits / warpsTotal;      // whole rounds are static, the rest by tickets (k_star)
+        const unsigned one = ticket_one(ctl);
+        unsigned round = 1;
         c.ref = ref; c.ev = ev; c.out = out; c.table = table;
         c.T = ctl->tableCount;
         c.trunc = ctl->tableTrunc != 0;
@@ -777,13 +788,32 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
         c.invGlobal = ctl->invGlobal;
         c.stat = &sStat; c.st = st;
         unsigned visits = 0;
+        bool pre = false;
+        unsigned preIdx = 0u, preKey = 0u;
 
         while (unit < numUnits) {
             unsigned nextUnit = numUnits;
-            if (dynamic && lane == 0) nextUnit = atomicAdd(&ctl->workCounter, 1u) + warpsTotal;
+            const bool staticNext = round < staticRounds;
+            if (staticNext) nextUnit = unit + warpsTotal;
+            else if (staticRounds && lane == 0) nextUnit = ticket_next(&ctl->workCounter, one) + staticRounds * warpsTotal;
+            ++round;
+            // the list entry of a statically known next unit is fetched now and used after this unit's search
+            const bool havePre = pre;
+            const unsigned curIdx = preIdx, curKey = preKey;
+            pre = false;
+            if (MODE == 0 && classes && staticNext) {
+                if (nextUnit < nDeep) {
+                    const unsigned idx = nDeepList - 1u - nextUnit;
+                    preIdx = deepIdx[idx]; preKey = deepKey[idx]; pre = true;
+                } else {
+                    const unsigned item = 32u * (nextUnit - nDeep) + (unsigned)lane;
+                    if (item < nS) { preIdx = listIdx[item]; preKey = listKey[item]; }
+                    pre = true;
+                }
+            }
             if (MODE == 0) {
-                if (unit < nDeep) visits += search_items<32, JU>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane);
-                else if (classes) ring_items(c, g, e, ring, listKey, listIdx, nS, 32u * (unit - nDeep), lane);
+                if (unit < nDeep) visits += search_items<32, JU>(c, g, e, deepKey, deepIdx, nDeepList, unit, lane, havePre, curIdx, curKey);
+                else if (classes) ring_items(c, g, e, ring, listKey, listIdx, nS, 32u * (unit - nDeep), lane, havePre, curIdx, curKey);
                 else visits += search_items<8, JU>(c, g, e, listKey, listIdx, nS, nDeep + 4u * (unit - nDeep), lane);
             } else {
                 visits += search_items<(MODE == 0 ? 8 : MODE), JU>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);
