@@ -81,17 +81,20 @@ class GammaOpts:
     stats_summary: object = None  # uint8 CUDA tensor [48]: gamma_summary bytes, decode with decode_summary
     stats_hist_max: float = 0.0
 
+    def __setattr__(self, name, value):
+        # any field change drops the cached ctypes struct (argument marshalling only)
+        self.__dict__[name] = value
+        self.__dict__["_cached"] = None
+
     def _c(self):
-        # the ctypes struct of the last field values is kept (argument marshalling only)
-        key = (self.norm_dose, self.presort, self.star_phase, self.lanes_per_voxel, self.sort_key_bits, self.table_cap,
-               self.profile_stages, self.interpolation, self.table_radius, self.graph, self.back_to_back, self.star_load,
-               None if self.stats_hist is None else (self.stats_hist.data_ptr(), self.stats_hist.numel()),
-               None if self.stats_summary is None else self.stats_summary.data_ptr(), self.stats_hist_max)
-        hit = self.__dict__.get("_cached")
-        if hit is not None and hit[0] == key:
-            return hit[1]
-        c = self._build()
-        self.__dict__["_cached"] = (key, c)
+        c = self.__dict__.get("_cached")
+        if c is not None and self.stats_hist is not None and (
+                c.stats_hist != self.stats_hist.data_ptr() or c.stats_nbins != self.stats_hist.numel()
+                or c.stats_summary != self.stats_summary.data_ptr()):
+            c = None                                   # the tensors were resized or moved in place
+        if c is None:
+            c = self._build()
+            self.__dict__["_cached"] = c
         return c
 
     def _build(self):

@@ -9,6 +9,8 @@
 #include <cstring>
 #include <mutex>
 #include <string>
+#include <tuple>
+#include <utility>
 
 #include "../../include/gamma_b200.h"
 #include "common.cuh"
@@ -66,6 +68,29 @@ int fail(int code, const std::string& msg)
     } while (0)
 
 
+// A call's kernels as an instantiated CUDA graph whose kernel-node parameters are rewritten for every call
+// (cudaGraphExecKernelNodeSetParams: 0.4 us per node, one graph launch of 1.3 us -- against 3.3 us per stream launch,
+// measured on the B200 box): the host cost of a call on a lane stream.  While `g_upd` is set, launch_ex() does not
+// launch: it checks that the kernel is the one the node was built from and stores the new grid and arguments.
+// While `g_rec` is set (the capture that builds such a graph) it notes the kernels in launch order.
+constexpr int UPD_MAX_NODES = 8;
+struct GraphUpdate {
+    cudaGraphExec_t exec;
+    const cudaGraphNode_t* nodes;
+    void* const* funcs;
+    int count, idx;
+    bool ok;
+};
+GraphUpdate* g_upd = nullptr;
+struct LaunchRecord { void* funcs[UPD_MAX_NODES]; int count; bool overflow; };
+LaunchRecord* g_rec = nullptr;
+
+template <typename Tuple, size_t... I>
+void tuple_pointers(Tuple& t, void** p, std::index_sequence<I...>)
+{
+    ((p[I] = const_cast<void*>(static_cast<const void*>(&std::get<I>(t)))), ...);
+}
+
 // Kernel launch with attributes: `pdl` = programmatic dependent launch (the kernel may start while its predecessor
 // in the stream drains; it calls pdl_wait() before touching the predecessor's results), `coop` = cooperative
 // (all blocks co-resident: required by the grid barrier of k_norm).
@@ -73,6 +98,23 @@ template <typename... KArgs, typename... Args>
 cudaError_t launch_ex(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, bool pdl, bool coop,
                       Args... args)
 {
+    if (g_upd) {
+        GraphUpdate& u = *g_upd;
+        if (u.idx >= u.count || u.funcs[u.idx] != reinterpret_cast<void*>(kernel)) { u.ok = false; return cudaSuccess; }
+        std::tuple<std::remove_cv_t<KArgs>...> vals(static_cast<KArgs>(args)...);
+        void* ptrs[sizeof...(KArgs)];
+        tuple_pointers(vals, ptrs, std::index_sequence_for<KArgs...>{});
+        cudaKernelNodeParams kp = {};
+        kp.func = reinterpret_cast<void*>(kernel);
+        kp.gridDim = dim3((unsigned)grid); kp.blockDim = dim3((unsigned)block);
+        kp.sharedMemBytes = (unsigned)smem; kp.kernelParams = ptrs; kp.extra = nullptr;
+        HP(2);
+        return cudaGraphExecKernelNodeSetParams(u.exec, u.nodes[u.idx++], &kp);
+    }
+    if (g_rec) {
+        if (g_rec->count < UPD_MAX_NODES) g_rec->funcs[g_rec->count++] = reinterpret_cast<void*>(kernel);
+        else g_rec->overflow = true;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block);
     cfg.dynamicSmemBytes = smem; cfg.stream = st;
@@ -129,6 +171,22 @@ struct GraphEntry {
 };
 constexpr int GRAPH_CACHE = 96;    // argument sets x CTL_ROT rotating sets
 
+// One updatable graph per kernel sequence (GraphUpdate): the options that decide WHICH kernels a call launches.
+struct UpdKey {
+    int star, lanes, algoJu, classes, presort;
+    bool operator==(const UpdKey& o) const { return std::memcmp(this, &o, sizeof *this) == 0; }
+};
+struct UpdGraph {
+    UpdKey key;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaGraphNode_t nodes[UPD_MAX_NODES];
+    void* funcs[UPD_MAX_NODES];
+    int count = 0;
+    bool unusable = false;         // this sequence cannot be updated in place (a kernel twice, too many kernels)
+};
+constexpr int UPD_CACHE = 4;
+
 // Byte ranges a call in flight reads and writes, for the hazard check of pipelined calls.
 struct Span {
     const char *b = nullptr, *e = nullptr;
@@ -184,12 +242,19 @@ struct Workspace {
     cudaStream_t cap = nullptr;    // capture stream (the caller's may be the legacy default stream, which cannot capture)
     GraphEntry graph[GRAPH_CACHE];
     int numGraphs = 0;
+    UpdGraph upd[UPD_CACHE];
+    int numUpd = 0;
     unsigned long long graphGen = 0, useClock = 0;
     void dropGraphs()
     {
         for (int i = 0; i < numGraphs; ++i)
             if (graph[i].exec) { cudaGraphExecDestroy(graph[i].exec); graph[i].exec = nullptr; }
         numGraphs = 0;
+        for (int i = 0; i < numUpd; ++i) {
+            if (upd[i].exec) { cudaGraphExecDestroy(upd[i].exec); upd[i].exec = nullptr; }
+            if (upd[i].graph) { cudaGraphDestroy(upd[i].graph); upd[i].graph = nullptr; }
+        }
+        numUpd = 0;
     }
     // last call, for gamma_get_counters
     cudaStream_t lastStream = nullptr;
@@ -250,9 +315,13 @@ unsigned g_callNo = 0;                 // gamma_eval* calls so far, all workspac
 // every call (one event per call, so later work of the caller's sees all results), calls on one lane are in stream
 // order, and a call that touches a buffer of one of the last B2B_WINDOW - 1 calls on another lane waits for that call.
 #ifndef GAMMA_B2B_WINDOW
-#define GAMMA_B2B_WINDOW 8
+#define GAMMA_B2B_WINDOW 16
 #endif
-constexpr int B2B_WINDOW = GAMMA_B2B_WINDOW;   // calls whose buffers are remembered; call j waits (host) for call j - B2B_WINDOW
+constexpr int B2B_WINDOW = GAMMA_B2B_WINDOW;   // calls whose buffers are remembered (a multiple of 2 * LANES)
+// Back-pressure: every call is also joined into the library's own stream `join`; every B2B_PERIOD calls an event is
+// recorded there and the host waits for the event of the period before, so that call j - B2B_WINDOW has ended when call
+// j takes over its slot -- one host wait per period instead of one per call.
+constexpr int B2B_PERIOD = B2B_WINDOW / 2;
 struct LaneState {
     cudaStream_t stream[LANES] = {};
     cudaEvent_t fork = nullptr;
@@ -263,6 +332,9 @@ struct LaneState {
     int laneOf[B2B_WINDOW] = {};
     bool used[B2B_WINDOW] = {};
     unsigned long long next = 0;       // number of the next back-to-back call
+    cudaStream_t join = nullptr;       // waits for every call; carries the back-pressure events
+    cudaEvent_t joined = nullptr;      // recorded on `join` at the start of a period: all earlier calls have ended
+    bool haveJoined = false;
     cudaStream_t user = nullptr;       // caller's stream of the sequence in progress
     bool active = false;               // the library's last operation was a back-to-back call on `user`
     bool ready = false;
@@ -644,6 +716,7 @@ int prepare_workspace(const GridP& g, const Resolved& r, long long stride)
 
 // What a call's kernels are told about where they run.
 struct CallSlot {
+    bool shared;       // the call runs on a lane stream beside the calls of the other lanes: grids that leave room
     int slot;          // control-block / embedded-table slot
     int nextSlot;      // slot k_norm zeroes for the next call (-1: none)
     int waitFirst;     // k_norm waits for the operation in front of it before it reads ref / eval
@@ -677,6 +750,23 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
 #define STAGE_MARK(i, s) do { if (r.profile) CU_TRY(cudaEventRecord(g_ws.stage[i], s)); } while (0)
     const int sm = g_ws.numSM;
     const bool pdl = g_ws.pdl != 0;
+    // Resident blocks per SM each kernel asks for.  A call on its own gets grids that fill the GPU.  Calls on the lane
+    // streams get grids of about half an SM's registers (k_star 4 x 128 x 56 + k_table_search 3 x 128 x 80 = 59 K of
+    // 64 K), so that the star phase of one call and the search of another are RESIDENT TOGETHER and fill each other's
+    // stalls: every kernel here is latency-bound on its own (issue slots 45 - 50 % busy), and with full-size grids the
+    // device timeline shows the kernels of different calls strictly one after the other (profiles/r2_profile.md).
+    // GAMMA_LANE_GRIDS=norm,classify,star,search overrides the lane figures (tuning).
+    static int laneBlocks[4] = {0, 0, 0, 0};
+    if (laneBlocks[0] == 0) {
+        laneBlocks[0] = 2; laneBlocks[1] = 4; laneBlocks[2] = 4; laneBlocks[3] = 3;
+        if (const char* env = std::getenv("GAMMA_LANE_GRIDS")) {
+            int v[4];
+            if (std::sscanf(env, "%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3]) == 4)
+                for (int k = 0; k < 4; ++k) if (v[k] >= 1 && v[k] <= 16) laneBlocks[k] = v[k];
+        }
+    }
+    const int normBlocks = cs.shared ? laneBlocks[0] : 4, classifyBlocks = cs.shared ? laneBlocks[1] : 8;
+    const int starBlocks = cs.shared ? laneBlocks[2] : 1 << 20, searchBlocks = cs.shared ? laneBlocks[3] : SEARCH_GRID_BLOCKS;
     STAGE_MARK(0, st);
     // a3.  Default: a data-independent PREFIX of the paper's table, as large as table_cap allows; beyond it the search
     // enumerates (exact).  table_radius = 2: the paper's radius max |DD| / dD (A1 steps 1-2), built on a side stream
@@ -724,7 +814,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     if (r.tableMode == 1 && !embed) { rc = fork_table(); if (rc) return rc; }
     if (!cs.skipNorm) {                                                  // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
-        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
+        int grid = (int)(blocks < 1 ? 1 : (blocks > sm * normBlocks ? sm * normBlocks : blocks));
         CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ev, (int)N, mode, ctl, next, cs.waitFirst,
                          e.call, r.stats));
         ++nk;
@@ -777,7 +867,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     } else {
     {                                                                    // a1: exclusion + compaction
         long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
-        int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
+        int grid = (int)(chunks > sm * classifyBlocks ? sm * classifyBlocks : chunks);
         CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0, r.stats));
         ++nk;
     }
@@ -786,7 +876,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     {                                                                    // star phase over the compacted voxels
         unsigned *tabL = static_cast<unsigned*>(g_ws.tmpL.p), *tabI = static_cast<unsigned*>(g_ws.tmpIdx.p);
         long long warps = (N + 31) / 32, blocks = (warps + STAR_THREADS / 32 - 1) / (STAR_THREADS / 32);
-        const long long resident = (long long)sm * g_ws.occStar[r.star];
+        const long long resident = (long long)sm * (g_ws.occStar[r.star] < starBlocks ? g_ws.occStar[r.star] : starBlocks);
         int grid = (int)(blocks > resident ? resident : blocks);
         if (r.star)
             CU_TRY(launch_ex(k_star<true>, grid, STAR_THREADS, 0, st, pdl, false, ref, ev, out, g, e, ctl, e0, k0, i0, k1, i1, classes,
@@ -814,7 +904,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     }
     if (g_ws.stageSort) STAGE_MARK(3, st);
     {                                                                    // a4 + a5
-        const int grid = sm * (r.lanes == 0 ? SEARCH_GRID_BLOCKS : 4 * (256 / SEARCH_THREADS));   // resident blocks
+        const int grid = sm * (r.lanes == 0 ? searchBlocks : 4 * (256 / SEARCH_THREADS));   // resident blocks
         const int4* tab = tab4;
         // adaptive lanes: an item is "deep" when its key exceeds the smallest non-zero table distance
         float hmin = 0.0f;
@@ -895,7 +985,7 @@ int ensure_ctl(cudaStream_t st)
 // CUDA graph of its kernels.  A stream that the CALLER is capturing gets the kernels as nodes of the caller's graph, on
 // the capture workspace.
 int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD, int mode, float cutoff,
-                     const Resolved& r, float* out, cudaStream_t st, bool allowEarly)
+                     const Resolved& r, float* out, cudaStream_t st, bool allowEarly, bool shared = false)
 {
     cudaStreamCaptureStatus capStatus = cudaStreamCaptureStatusNone;
     if (!allowEarly) CU_TRY(cudaStreamIsCapturing(st, &capStatus));      // lane streams are never captured
@@ -925,7 +1015,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             Resolved rr = r;
             rr.profile = 0;
             CallSlot cs;
-            cs.slot = CTL_CAPTURE; cs.nextSlot = -1; cs.waitFirst = 1; cs.skipNorm = false;
+            cs.slot = CTL_CAPTURE; cs.nextSlot = -1; cs.waitFirst = 1; cs.skipNorm = false; cs.shared = false;
             rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, rr, out, st, cs, &launched);
         }
         if (rc == GAMMA_OK) {
@@ -955,6 +1045,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     cs.slot = g_ws.slot;
     cs.nextSlot = (g_ws.slot + 1) % CTL_ROT;
     cs.skipNorm = false;
+    cs.shared = shared;
     long long stride = N;
     if (twoPhase) {
         // a0, then the count of evaluated voxels, read by the host: the lists are sized by M
@@ -983,14 +1074,90 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     mine.wr[1].set(r.stats.hist, (size_t)r.stats.nbins * 8); mine.wr[2].set(r.stats.summary, sizeof(gamma_summary));
     static const bool overlapCalls = !(std::getenv("GAMMA_OVERLAP_CALLS") && std::getenv("GAMMA_OVERLAP_CALLS")[0] == '0');
     const bool embed = r.tableMode == 1 && r.tableCap <= TAB_EMBED_MAX_CELLS;
+    // Calls on a lane stream (and opts.graph = 1 calls) go out as ONE graph launch whose kernel nodes get this call's
+    // arguments (GraphUpdate): 4 x 0.4 us + 1.3 us of host time instead of 4 x 3.3 us.  Only for kernel sequences without
+    // side stream, events or repeated kernels; everything else is launched kernel by kernel.
+    static const bool updGraphs = !(std::getenv("GAMMA_UPDATE_GRAPHS") && std::getenv("GAMMA_UPDATE_GRAPHS")[0] == '0');
+    bool useUpd = updGraphs && g_ws.graphs != 0 && (shared || r.graph) && !r.profile && !twoPhase && embed &&
+                  r.starLoad <= 1 && r.presort != 3;
     const bool early = allowEarly && overlapCalls && g_ws.pdl != 0 && g_ws.chainable && g_ws.havePending &&
-                       g_ws.doneStream == st && !r.profile && !useGraph && !twoPhase && embed &&
+                       g_ws.doneStream == st && !r.profile && !useGraph && !useUpd && !twoPhase && embed &&
                        !g_ws.lastSpans.conflicts(mine);
     cs.waitFirst = early ? 0 : 1;
     g_ws.haveStages = false;
 
     int launched = 0;
-    if (!useGraph) {
+    bool launchedByUpdate = false;
+    if (useUpd) {
+        if (g_ws.graphGen != g_allocGen) { g_ws.dropGraphs(); g_ws.graphGen = g_allocGen; }
+        UpdKey uk;
+        std::memset(&uk, 0, sizeof uk);
+        uk.star = r.star; uk.lanes = r.lanes; uk.algoJu = r.algo == 2; uk.classes = g.all_active; uk.presort = r.presort;
+        UpdGraph* hit = nullptr;
+        for (int i = 0; i < g_ws.numUpd; ++i)
+            if (g_ws.upd[i].key == uk) { hit = &g_ws.upd[i]; break; }
+        if (!hit) {                                        // build: capture this call once, keep graph, exec and nodes
+            int victim = g_ws.numUpd < UPD_CACHE ? g_ws.numUpd++ : 0;
+            UpdGraph& ug = g_ws.upd[victim];
+            if (ug.exec) { cudaGraphExecDestroy(ug.exec); ug.exec = nullptr; }
+            if (ug.graph) { cudaGraphDestroy(ug.graph); ug.graph = nullptr; }
+            ug.key = uk; ug.count = 0; ug.unusable = false;
+            LaunchRecord rec;
+            std::memset(&rec, 0, sizeof rec);
+            CU_TRY(cudaStreamBeginCapture(g_ws.cap, cudaStreamCaptureModeThreadLocal));
+            g_rec = &rec;
+            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, g_ws.cap, cs, &launched);
+            g_rec = nullptr;
+            cudaError_t ce = cudaStreamEndCapture(g_ws.cap, &ug.graph);
+            if (rc) { if (ug.graph) { cudaGraphDestroy(ug.graph); ug.graph = nullptr; } ug.unusable = true; return rc; }
+            if (ce != cudaSuccess) { ug.unusable = true; return fail(GAMMA_ERR_CUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(ce)); }
+            ug.unusable = rec.overflow || rec.count == 0;
+            for (int a = 0; a < rec.count && !ug.unusable; ++a)
+                for (int b = a + 1; b < rec.count; ++b)
+                    if (rec.funcs[a] == rec.funcs[b]) ug.unusable = true;       // a node is found by its kernel
+            if (!ug.unusable) {
+                cudaGraphNode_t all[4 * UPD_MAX_NODES];
+                size_t nAll = 0;
+                CU_TRY(cudaGraphGetNodes(ug.graph, nullptr, &nAll));
+                if (nAll > 4 * UPD_MAX_NODES) ug.unusable = true;
+                else CU_TRY(cudaGraphGetNodes(ug.graph, all, &nAll));
+                for (int a = 0; a < rec.count && !ug.unusable; ++a) {
+                    bool found = false;
+                    for (size_t i = 0; i < nAll && !found; ++i) {
+                        cudaGraphNodeType ty;
+                        CU_TRY(cudaGraphNodeGetType(all[i], &ty));
+                        if (ty != cudaGraphNodeTypeKernel) continue;
+                        cudaKernelNodeParams kp;
+                        CU_TRY(cudaGraphKernelNodeGetParams(all[i], &kp));
+                        if (kp.func == rec.funcs[a]) { ug.nodes[a] = all[i]; ug.funcs[a] = rec.funcs[a]; found = true; }
+                    }
+                    if (!found) ug.unusable = true;
+                }
+                ug.count = rec.count;
+            }
+            if (!ug.unusable) {
+                ce = cudaGraphInstantiate(&ug.exec, ug.graph, 0);
+                if (ce != cudaSuccess) { ug.unusable = true; cudaGetLastError(); }
+            }
+            hit = &ug;
+        }
+        if (!hit->unusable) {
+            GraphUpdate u = {hit->exec, hit->nodes, hit->funcs, hit->count, 0, true};
+            g_upd = &u;
+            rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, cs, &launched);
+            g_upd = nullptr;
+            if (rc) return rc;
+            if (u.ok && u.idx == u.count) {
+                HP(2);
+                CU_TRY(cudaGraphLaunch(hit->exec, st));
+                launchedByUpdate = true;
+            } else {
+                hit->unusable = true;                      // not the kernels the graph was built from: launch them one by one
+            }
+        }
+    }
+    if (launchedByUpdate) {
+    } else if (!useGraph) {
         HP(7);
         rc = enqueue_kernels(ref, ev, g, DD, mode, cutoff, r, out, st, cs, &launched);
         if (rc) return rc;
@@ -1060,6 +1227,8 @@ int lanes_init()
     CU_TRY(cudaEventCreateWithFlags(&g_lanes.fork, cudaEventDisableTiming));
     for (int l = 0; l < LANES; ++l) CU_TRY(cudaStreamCreateWithFlags(&g_lanes.stream[l], cudaStreamNonBlocking));
     for (int w = 0; w < B2B_WINDOW; ++w) CU_TRY(cudaEventCreateWithFlags(&g_lanes.done[w], cudaEventDisableTiming));
+    CU_TRY(cudaStreamCreateWithFlags(&g_lanes.join, cudaStreamNonBlocking));
+    CU_TRY(cudaEventCreateWithFlags(&g_lanes.joined, cudaEventDisableTiming));
     g_lanes.ready = true;
     return GAMMA_OK;
 }
@@ -1079,7 +1248,12 @@ int enqueue_on_lane(const float* ref, const float* ev, const GridP& g, float DD,
     L.active = false;                                      // set again on success
     const unsigned long long j = L.next;
     const int w = (int)(j % B2B_WINDOW), lane = (int)(j % LANES);
-    if (L.used[w]) { HP(1); CU_TRY(cudaEventSynchronize(L.done[w])); }   // call j - B2B_WINDOW has ended (back-pressure)
+    if (j % B2B_PERIOD == 0) {                             // back-pressure: calls up to j - B2B_PERIOD - 1 have ended
+        HP(1);
+        if (L.haveJoined) CU_TRY(cudaEventSynchronize(L.joined));
+        CU_TRY(cudaEventRecord(L.joined, L.join));         // covers every call before this one
+        L.haveJoined = true;
+    }
     cudaStream_t st = L.stream[lane];
     if (L.laneFork[lane] != L.forkGen) {
         CU_TRY(cudaStreamWaitEvent(st, L.fork, 0));
@@ -1099,7 +1273,7 @@ int enqueue_on_lane(const float* ref, const float* ev, const GridP& g, float DD,
     }
     Workspace* keep = g_cur;
     g_cur = &g_pool[1 + lane];
-    rc = enqueue_pipeline(ref, ev, g, DD, mode, cutoff, r, out, st, !L.laneDirty[lane]);
+    rc = enqueue_pipeline(ref, ev, g, DD, mode, cutoff, r, out, st, !L.laneDirty[lane], true);
     g_cur = keep;
     if (rc) { L.laneDirty[lane] = true; return rc; }
     L.laneDirty[lane] = false;
@@ -1107,6 +1281,7 @@ int enqueue_on_lane(const float* ref, const float* ev, const GridP& g, float DD,
         HP(3);
         CU_TRY(cudaEventRecord(L.done[w], st));
         CU_TRY(cudaStreamWaitEvent(user, L.done[w], 0));              // the caller's stream sees the result
+        CU_TRY(cudaStreamWaitEvent(L.join, L.done[w], 0));
     }
     L.spans[w] = mine; L.laneOf[w] = lane; L.used[w] = true;
     ++L.next;
@@ -1738,6 +1913,8 @@ void gamma_release(void)
     for (int w = 0; w < B2B_WINDOW; ++w)
         if (g_lanes.done[w]) { cudaEventDestroy(g_lanes.done[w]); g_lanes.done[w] = nullptr; }
     if (g_lanes.fork) { cudaEventDestroy(g_lanes.fork); g_lanes.fork = nullptr; }
+    if (g_lanes.joined) { cudaEventDestroy(g_lanes.joined); g_lanes.joined = nullptr; }
+    if (g_lanes.join) { cudaStreamDestroy(g_lanes.join); g_lanes.join = nullptr; }
     g_lanes = LaneState();
     g_hb.release();
     g_lastWs = &g_pool[0];
