@@ -446,7 +446,7 @@ def main():
                         "note": "gamma_opts::stats_*: a6 accumulated inside the gamma kernels; stats_ms is the separate gamma_stats call"},
         "batched": {"cases_per_call": nbatch, "ms_per_case": batch_ms_case,
                     "value": world * M / (batch_ms_case * 1e-3), "unit": "evaluated reference voxels/s",
-                    "note": "gamma_eval_batch: independent cases spread over 4 library-owned streams"},
+                    "note": "gamma_eval_batch: independent cases spread over 6 library-owned streams"},
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(case)

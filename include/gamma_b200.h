@@ -123,10 +123,11 @@ typedef struct gamma_opts {
                              (3D grids; 2D / 1D grids use 1)                                              */
     int back_to_back;     /* 0: default.  1: the caller ASSERTS that nothing else has been enqueued on `stream` since the
                              library's previous call on it returned (no kernel, copy or event of the caller's, no other
-                             library entry point).  Consecutive such calls are then run round-robin on 4 library-owned
-                             streams, each with its own workspace, so that their kernels overlap on the device (one
-                             stream cannot do that: its operations complete in order).  `stream` stays the ordering
-                             point: the first call of such a sequence starts after what is on `stream`, and `stream`
+                             library entry point).  Consecutive such calls are then run round-robin on 6 library-owned
+                             streams, each with its own workspace and with grids of about half an SM's registers, so that
+                             the kernels of different calls are resident together (one stream cannot do that: its
+                             operations complete in order); each call goes out as one CUDA-graph launch.  `stream` stays the
+                             ordering point: the first call of such a sequence starts after what is on `stream`, and `stream`
                              waits for every call, so whatever the caller enqueues afterwards sees all results.  Calls of
                              a sequence may COMPLETE out of order; a call that reads or writes a buffer an earlier call
                              of the sequence still writes (or writes one it reads) waits for that call -- the library
@@ -154,7 +155,7 @@ typedef struct gamma_opts {
 
 /* Several independent cases in one call (every reference voxel and every case is independent,
  * PAPER.md:141).  One case is tens of microseconds of dependent kernels that cannot fill 148 SMs; the batch spreads
- * the cases over 4 library-owned streams, each with its own workspace, so that their kernels overlap on the device
+ * the cases over 6 library-owned streams, each with its own workspace, so that their kernels overlap on the device
  * (the same mechanism as gamma_opts::back_to_back, for which the batch is shorthand).
  * Results are those of n_cases gamma_eval_ex calls, bit for bit.
  *   ref, eval, out_gamma   HOST arrays of n_cases DEVICE pointers (fp32, layout as in gamma_eval); the outputs must

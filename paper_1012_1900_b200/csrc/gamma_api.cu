@@ -298,7 +298,7 @@ struct Workspace {
 // consecutive calls overlap on the device; the last one belongs to the calls a caller captures into its own CUDA graph
 // (its addresses are baked into that graph, so it never moves once used: gamma_release() is the only way to grow it).
 #ifndef GAMMA_LANES
-#define GAMMA_LANES 4
+#define GAMMA_LANES 6
 #endif
 constexpr int LANES = GAMMA_LANES;
 constexpr int WS_CAPTURE = 1 + LANES;
@@ -315,7 +315,7 @@ unsigned g_callNo = 0;                 // gamma_eval* calls so far, all workspac
 // every call (one event per call, so later work of the caller's sees all results), calls on one lane are in stream
 // order, and a call that touches a buffer of one of the last B2B_WINDOW - 1 calls on another lane waits for that call.
 #ifndef GAMMA_B2B_WINDOW
-#define GAMMA_B2B_WINDOW 16
+#define GAMMA_B2B_WINDOW 24
 #endif
 constexpr int B2B_WINDOW = GAMMA_B2B_WINDOW;   // calls whose buffers are remembered (a multiple of 2 * LANES)
 // Back-pressure: every call is also joined into the library's own stream `join`; every B2B_PERIOD calls an event is
@@ -816,7 +816,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * normBlocks ? sm * normBlocks : blocks));
         CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ev, (int)N, mode, ctl, next, cs.waitFirst,
-                         e.call, r.stats));
+                         e.call, r.stats, r.tableMode != 1 ? 1 : 0));
         ++nk;
     }
     // a1 + a2 + star phase.  Default: the compacted-list pipeline k_classify -> k_star (doses through L1 / L2).
@@ -947,12 +947,12 @@ k_count_eval(const float* __restrict__ ref, int N, EvalP e, const Ctl* __restric
 {
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
     const double dnorm = (double)dnormF;
-    const double thr = (double)e.cutoff * dnorm;
+    const float thrUp = __double2float_ru((double)e.cutoff * dnorm);     // same decision as k_classify
     const bool globalOk = (double)e.DD * dnorm > 0.0;
     unsigned c = 0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         const float Dr = __ldg(ref + i);
-        const bool excluded = ((double)Dr < thr) || (e.mode == 0 ? !globalOk : !((double)e.DD * (double)Dr > 0.0));
+        const bool excluded = (Dr < thrUp) || (e.mode == 0 ? !globalOk : !(Dr > 0.0f));
         c += excluded ? 0u : 1u;
     }
 #pragma unroll
@@ -1056,7 +1056,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         CU_TRY(cudaMemsetAsync(g_ws.count.p, 0, 16, st));
         const int sm = g_ws.numSM;
         CU_TRY(launch_ex(k_norm, sm * 4, NORM_THREADS, 0, st, false, false, ref, ev, (int)N, mode, base + cs.slot,
-                         base + cs.nextSlot, 1, g_callNo, r.stats));
+                         base + cs.nextSlot, 1, g_callNo, r.stats, r.tableMode != 1 ? 1 : 0));
         k_count_eval<<<sm * 8, 256, 0, st>>>(ref, (int)N, e0p, base + cs.slot, static_cast<unsigned*>(g_ws.count.p));
         unsigned M = 0;
         CU_TRY(cudaMemcpyAsync(&M, g_ws.count.p, 4, cudaMemcpyDeviceToHost, st));
@@ -1479,7 +1479,7 @@ int gamma_eval_general(const float* ref, const int ref_dims[3], const float ref_
     {                                                                    // a0 on the reference grid
         long long blocks = (Nr + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * 4 ? sm * 4 : blocks));
-        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ref, (int)Nr, mode, ctl, next, 1, e.call, noStats));
+        CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ref, (int)Nr, mode, ctl, next, 1, e.call, noStats, 0));
     }
     {                                                                    // a1 on the reference grid
         long long chunks = (Nr + PREP_CHUNK - 1) / PREP_CHUNK;

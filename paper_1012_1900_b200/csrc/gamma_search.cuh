@@ -60,8 +60,10 @@ __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepc
 
 __global__ void __launch_bounds__(NORM_THREADS)
 k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int mode, Ctl* __restrict__ cur,
-       Ctl* __restrict__ next, int waitFirst, unsigned call, StatsP st)
+       Ctl* __restrict__ next, int waitFirst, unsigned call, StatsP st, int needDD)
 {
+    // needDD == 0: only max(ref) is wanted -- the default prefix table does not depend on max |DD| (A1 step 1 sizes the
+    // PAPER's table, opts.table_radius = 2), so the evaluation dose is not read here at all: 4 instead of 8 bytes per voxel
     trace_first(call, 0);
     // waitFirst: ref / eval may be results of the operation in front of this call: nothing is read before that
     // operation has completed -- and the dependents (k_classify fetches ref before its own wait) are released only
@@ -92,7 +94,26 @@ k_norm(const float* __restrict__ ref, const float* __restrict__ ev, int N, int m
         a = fmaxf(a, ad);                                       // fmaxf drops NaN
         if (mode == 1 && Dr > 0.0f) r = fmaxf(r, ad / Dr);
     };
-    if (((reinterpret_cast<uintptr_t>(ref) | reinterpret_cast<uintptr_t>(ev)) & 15u) == 0) {
+    if (!needDD) {
+        if ((reinterpret_cast<uintptr_t>(ref) & 15u) == 0) {
+            const float4* r4 = reinterpret_cast<const float4*>(ref);
+            const int n4 = N >> 2;
+            int i = tid;
+            for (; i + 3 * nth < n4; i += 4 * nth) {         // 4 independent 16-byte loads in flight per thread
+                const float4 x0 = __ldg(r4 + i), x1 = __ldg(r4 + i + nth), x2 = __ldg(r4 + i + 2 * nth), x3 = __ldg(r4 + i + 3 * nth);
+                m = fmaxf(fmaxf(fmaxf(m, x0.x), fmaxf(x0.y, x0.z)), fmaxf(fmaxf(x0.w, x1.x), fmaxf(x1.y, x1.z)));
+                m = fmaxf(fmaxf(fmaxf(m, x1.w), fmaxf(x2.x, x2.y)), fmaxf(fmaxf(x2.z, x2.w), fmaxf(x3.x, x3.y)));
+                m = fmaxf(m, fmaxf(x3.z, x3.w));
+            }
+            for (; i < n4; i += nth) {
+                const float4 x = __ldg(r4 + i);
+                m = fmaxf(fmaxf(m, x.x), fmaxf(fmaxf(x.y, x.z), x.w));
+            }
+            for (int k = (n4 << 2) + tid; k < N; k += nth) m = fmaxf(m, __ldg(ref + k));
+        } else {
+            for (int i = tid; i < N; i += nth) m = fmaxf(m, __ldg(ref + i));
+        }
+    } else if (((reinterpret_cast<uintptr_t>(ref) | reinterpret_cast<uintptr_t>(ev)) & 15u) == 0) {
         const float4* r4 = reinterpret_cast<const float4*>(ref);
         const float4* e4 = reinterpret_cast<const float4*>(ev);
         const int n4 = N >> 2;
@@ -180,7 +201,11 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
     trace_waited(e.call, 1);
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
     const double dnorm = (double)dnormF;
-    const double thr = (double)e.cutoff * dnorm;      // decided in double (include/gamma_b200.h)
+    // The cutoff is decided in double (include/gamma_b200.h): D_r < cutoff * D_norm.  For a float D_r that is the same
+    // as D_r < thrUp with thrUp = the product rounded UP to float (if the product is a float, thrUp is the product;
+    // otherwise no float lies between it and thrUp) -- one fp32 compare per voxel, same decision bit for bit.  Likewise
+    // DD * D_r > 0 in double <=> D_r > 0 (DD > 0; the product of two floats cannot underflow in double).
+    const float thrUp = __double2float_ru((double)e.cutoff * dnorm);
     const float invGlobal = criterion_inv_dD(e, dnorm, 0.0f);
     const bool globalOk = invGlobal > 0.0f;
     if (blockIdx.x == 0 && threadIdx.x == 0) ctl->invGlobal = invGlobal;   // the later kernels read it from here
@@ -192,8 +217,7 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
         unsigned keepMask = 0;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const bool excluded = ((double)Dr[j] < thr) ||
-                                  (e.mode == 0 ? !globalOk : !((double)e.DD * (double)Dr[j] > 0.0));
+            const bool excluded = (Dr[j] < thrUp) || (e.mode == 0 ? !globalOk : !(Dr[j] > 0.0f));
             if (j < nval && !excluded) keepMask |= 1u << j;
         }
         if (keepMask == 0 && nval == 4 && vec) {
