@@ -35,14 +35,15 @@ SM_COUNT, FP32_LANES, SM_MAX_MHZ_NOMINAL = 148, 128, 1965.0
 F_CELL_3D, F_CELL_2D = 1911.0, 190.0       # canonical flops per visited cell, frozen in BASELINE.md
 L2_BYTES = 126e6
 # executed FP32 flops per unit (ncu smsp__sass_thread_inst_executed_op_{fadd,fmul,ffma}_pred_on, FFMA counted twice),
-# re-measured on the round-2 kernels (profiles/r2_mix_<case>.csv, profiles/r2_profile.md): k_star 65.55 Mflop / 160 256
-# voxels; k_table_search = 379 per owner-vertex visit + 1 211 per ring item (solved from the cfg2 and cfg3 launches,
-# reproduces cfg5 and cfg4_fine to 0.1 %)
-FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT, FLOP_PER_RING_ITEM = 409.0, 379.0, 1211.0
-# executed WARP instructions per unit (smsp__inst_executed.sum of the same capture): k_norm and k_classify per grid voxel,
-# k_star per evaluated voxel, k_table_search per owner-vertex visit / per ring item / fixed part per launch
-WINST = {"norm_per_voxel": 0.748, "classify_per_voxel": 1.74, "star_per_voxel": 36.76, "visit": 21.85, "ring_item": 44.4,
-         "search_fixed": 0.268e6}
+# measured on the final round-2 kernels (profiles/r2_mix_<case>.csv, profiles/r2_profile.md): k_star 451 per evaluated
+# voxel (450.6 / 451.5 / 450.6 / 451.0 on cfg2 / cfg3 / cfg5 / cfg4_fine); k_table_search = 380 per owner-vertex visit +
+# 1 212 per ring item (solved from the cfg2 and cfg3 launches, reproduces cfg5 and cfg4_fine to 0.1 %)
+FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT, FLOP_PER_RING_ITEM = 451.0, 380.0, 1212.0
+# executed WARP instructions (smsp__inst_executed.sum of the same captures) as unit costs plus a fixed part per launch:
+# k_norm and k_classify per grid voxel, k_star per evaluated voxel, k_table_search per owner-vertex visit and per ring
+# item (least squares over the four cases; reproduces each launch to a few per cent)
+WINST = {"norm_per_voxel": 0.0567, "norm_fixed": 0.474e6, "classify_per_voxel": 1.096, "classify_fixed": 0.674e6,
+         "star_per_voxel": 27.3, "star_fixed": 0.70e6, "visit": 19.84, "ring_item": 30.4, "search_fixed": 0.288e6}
 SCHEDULERS = 4 * SM_COUNT                   # one warp instruction per scheduler per cycle
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on cfg3 from the ncu --set full capture (profiles/r2_full_summary.csv)
 TRAFFIC_BYTES = {"k_star": 2.69e6, "k_table_search": 1.83e6}
@@ -402,7 +403,8 @@ def main():
     roof["frac_of_ffma_chain_probe"] = roof["achieved"] / probe_tflops if probe_tflops > 0 else None
     # the bound that actually limits this path: issue slots.  Warp instructions of one step (per-unit constants above x
     # the units the library counted) / (592 schedulers x 1 instruction per cycle x the SM clock)
-    winst = (N * (WINST["norm_per_voxel"] + WINST["classify_per_voxel"]) + M * WINST["star_per_voxel"]
+    winst = (N * (WINST["norm_per_voxel"] + WINST["classify_per_voxel"]) + WINST["norm_fixed"] + WINST["classify_fixed"]
+             + M * WINST["star_per_voxel"] + WINST["star_fixed"]
              + cnt["vertex_visits"] * WINST["visit"] + cnt["n_ring_search"] * WINST["ring_item"] + WINST["search_fixed"])
     clk_hz = (clk.get("sm_mhz") or SM_MAX_MHZ_NOMINAL) * 1e6
     issue_us = winst / SCHEDULERS / clk_hz * 1e6
@@ -454,6 +456,7 @@ def main():
         line["cpu_baseline"] = None
     print(json.dumps(line))
     rep.close()
+    binding.gamma_release()                 # a -DGAMMA_HOSTPROF build prints its host-side time profile here (stderr)
 
 
 if __name__ == "__main__":
