@@ -34,11 +34,11 @@ std::mutex g_mu;
 #include <chrono>
 namespace {
 struct HostProf {
-    double us[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long n[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    double us[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    long long n[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
 } g_hp;
-const char* const HP_NAMES[8] = {"gamma_eval_ex total", "back-pressure wait", "kernel launches", "events", "prepare/order/ctl",
-                                 "argument checks", "getenv", "enqueue_kernels"};
+const char* const HP_NAMES[10] = {"gamma_eval_ex total", "back-pressure wait", "kernel launches", "events", "prepare/order/ctl",
+                                  "argument checks", "getenv", "enqueue_kernels", "graph node update", "graph launch"};
 struct HpScope {
     int k;
     std::chrono::steady_clock::time_point t0;
@@ -108,7 +108,7 @@ cudaError_t launch_ex(void (*kernel)(KArgs...), int grid, int block, size_t smem
         kp.func = reinterpret_cast<void*>(kernel);
         kp.gridDim = dim3((unsigned)grid); kp.blockDim = dim3((unsigned)block);
         kp.sharedMemBytes = (unsigned)smem; kp.kernelParams = ptrs; kp.extra = nullptr;
-        HP(2);
+        HP(8);
         return cudaGraphExecKernelNodeSetParams(u.exec, u.nodes[u.idx++], &kp);
     }
     if (g_rec) {
@@ -1148,7 +1148,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             g_upd = nullptr;
             if (rc) return rc;
             if (u.ok && u.idx == u.count) {
-                HP(2);
+                HP(9);
                 CU_TRY(cudaGraphLaunch(hit->exec, st));
                 launchedByUpdate = true;
             } else {
@@ -1901,7 +1901,7 @@ void gamma_release(void)
     std::lock_guard<std::mutex> lock(g_mu);
     cudaDeviceSynchronize();
 #ifdef GAMMA_HOSTPROF
-    for (int k = 0; k < 8; ++k)
+    for (int k = 0; k < 10; ++k)
         if (g_hp.n[k])
             std::fprintf(stderr, "[gamma hostprof] %-22s %10lld x %8.3f us = %10.1f us\n", HP_NAMES[k], g_hp.n[k],
                          g_hp.us[k] / (double)g_hp.n[k], g_hp.us[k]);
