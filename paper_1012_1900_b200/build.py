@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgamma_b200.so")
 SOURCES = ["gamma_api.cu"]
 DEPENDS = ["common.cuh", "features_generated.cuh", "gamma_search.cuh", "ju_simplex.cuh", "offset_table.cuh", "radix_sort.cuh",
-           "stats.cuh", os.path.join("..", "..", "include", "gamma_b200.h")]
+           "stats.cuh", "tile_star.cuh", "general.cuh", "gen_features.py", os.path.join("..", "..", "include", "gamma_b200.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

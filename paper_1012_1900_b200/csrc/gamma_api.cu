@@ -309,7 +309,7 @@ unsigned g_callNo = 0;                 // gamma_eval* calls so far, all workspac
 #define g_ws (*g_cur)
 
 // Back-to-back calls.  A programmatic dependent that never waits is still not reported complete before its primary
-// (measured: profiles/r2_trace.md), so consecutive calls cannot run ahead of each other on ONE stream.  They are
+// (measured: profiles/r2_lanes.md), so consecutive calls cannot run ahead of each other on ONE stream.  They are
 // spread round-robin over LANES library-owned streams instead, each with its own workspace: the lane waits for what
 // was on the caller's stream when the sequence of back-to-back calls began (one event), the caller's stream waits for
 // every call (one event per call, so later work of the caller's sees all results), calls on one lane are in stream

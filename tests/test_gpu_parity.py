@@ -5,6 +5,8 @@ Bar (BASELINE.json north_star): |gamma_gpu - gamma_oracle| <= 1e-4 absolute per 
 (excluded) masks, and the gamma <= 1 pass count exact except for voxels within 1e-4 of 1.  Integer results
 (sort, histogram, counts, table entries) are bit-exact.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -688,6 +690,46 @@ def test_back_to_back_calls_overlap_safely(oracle_mod):
         torch.cuda.synchronize()
         assert torch.equal(got2, want2)
         assert torch.equal(e2, first)
+
+
+_LANE_STREAM_LAUNCH_SCRIPT = r"""
+import sys
+import numpy as np, torch
+sys.path.insert(0, %r)
+from paper_1012_1900_b200 import binding, phantoms
+from paper_1012_1900_b200.binding import GammaOpts
+nn = lambda t: torch.nan_to_num(t, nan=-1.0)
+b2b = GammaOpts(back_to_back=1)
+data = []
+for name in ("cfg2_small", "cfg4_coarse", "cfg2_small"):
+    c = phantoms.make_case(name)
+    r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+    e = torch.from_numpy(c.eval.ravel().copy()).cuda() * (1.0 + 0.01 * len(data))
+    args = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    want = binding.gamma_eval_ex(r, e, *args).clone()
+    torch.cuda.synchronize()
+    data.append((r, e, args, want))
+outs = [binding.gamma_eval_ex(*data[i %% 3][:2], *data[i %% 3][2], b2b) for i in range(48)]
+torch.cuda.synchronize()
+assert all(torch.equal(nn(o), nn(data[i %% 3][3])) for i, o in enumerate(outs))
+assert binding.gamma_get_counters()["pipelined"] == 1
+print("lanes-ok", binding.gamma_launch_count())
+"""
+
+
+@pytest.mark.parametrize("env", [{"GAMMA_UPDATE_GRAPHS": "0"}, {"GAMMA_UPDATE_GRAPHS": "0", "GAMMA_LANE_GRIDS": "4,8,9,6"},
+                                 {"GAMMA_LANE_GRIDS": "1,1,1,1"}])
+def test_lane_calls_by_stream_launches_and_other_grid_shares(env):
+    """The lanes' other launch path and other grid shares (both are process-wide environment switches, so a fresh
+    process): GAMMA_UPDATE_GRAPHS=0 launches the kernels of a lane call one by one, with k_norm started in the tail of
+    the lane's previous call instead of one graph launch per call; GAMMA_LANE_GRIDS changes how many blocks per SM the
+    lane kernels ask for (persistent kernels: any grid must give the same gamma).  Results must equal isolated calls."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = subprocess.run([sys.executable, "-c", _LANE_STREAM_LAUNCH_SCRIPT % root], env={**os.environ, **env},
+                         capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0 and "lanes-ok" in res.stdout, res.stdout[-2000:] + res.stderr[-4000:]
 
 
 def test_pipelined_calls_mixed_with_large_tables_and_other_entry_points():
