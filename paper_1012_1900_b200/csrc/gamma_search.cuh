@@ -199,16 +199,24 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
     if ((int)blockIdx.x < numChunks) nval = load_chunk(blockIdx.x, Dr);
     pdl_wait();                                       // k_norm's maxima from here on
     trace_waited(e.call, 1);
-    const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
-    const double dnorm = (double)dnormF;
     // The cutoff is decided in double (include/gamma_b200.h): D_r < cutoff * D_norm.  For a float D_r that is the same
     // as D_r < thrUp with thrUp = the product rounded UP to float (if the product is a float, thrUp is the product;
     // otherwise no float lies between it and thrUp) -- one fp32 compare per voxel, same decision bit for bit.  Likewise
     // DD * D_r > 0 in double <=> D_r > 0 (DD > 0; the product of two floats cannot underflow in double).
-    const float thrUp = __double2float_ru((double)e.cutoff * dnorm);
-    const float invGlobal = criterion_inv_dD(e, dnorm, 0.0f);
+    // The two constants take a double-precision division: one thread per block computes them (every thread doing so
+    // was 40 % of this kernel's instructions, a thread here has one chunk of four voxels).
+    __shared__ float sThrUp, sInvGlobal;
+    if (tid == 0) {
+        const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
+        const double dnorm = (double)dnormF;
+        sThrUp = __double2float_ru((double)e.cutoff * dnorm);
+        sInvGlobal = criterion_inv_dD(e, dnorm, 0.0f);
+        if (blockIdx.x == 0) ctl->invGlobal = sInvGlobal;   // the later kernels read it from here
+    }
+    __syncthreads();
+    const float thrUp = sThrUp;
+    const float invGlobal = sInvGlobal;
     const bool globalOk = invGlobal > 0.0f;
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctl->invGlobal = invGlobal;   // the later kernels read it from here
     const float qnan = __int_as_float(0x7fc00000);
 
     for (int chunk = blockIdx.x; chunk < numChunks; chunk += gridDim.x) {
