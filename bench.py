@@ -235,6 +235,7 @@ def main():
     # Rotating input sets larger than L2 (126 MB): every timed step reads buffers that the previous steps have
     # pushed out of L2.  Each set = ref + eval + out = 12 B/voxel.
     nsets = int(np.ceil(2.0 * L2_BYTES / (12.0 * N))) + 1
+    t_pinned = time.perf_counter()
     ref_h = torch.from_numpy(case.ref.ravel().copy()).pin_memory()
     ev_h = torch.from_numpy(case.eval.ravel().copy()).pin_memory()
     out_h = torch.empty(N, dtype=torch.float32).pin_memory()
@@ -281,8 +282,25 @@ def main():
     stages = {k: float(np.mean(v)) for k, v in stage_acc.items()}
 
     # ---- end to end through the host-buffer entry point ---------------------------------------------
-    for _ in range(3):
-        binding.gamma_eval_host(ref_h, ev_h, *args_c, opts, out_h, stream)
+    # warm-up: on this pool host<->device copies from pinned buffers run at a third of the link's rate for the first
+    # second or two after the buffers were pinned (plain cudaMemcpyAsync calls show the same; it settles by itself,
+    # busy or idle), so the untimed calls go on until that time has passed and two consecutive groups of calls agree
+    def settle(fn, t_pinned, min_s=2.5, max_s=8.0):
+        last = None
+        while True:
+            t0 = time.perf_counter()
+            fn()
+            dt = time.perf_counter() - t0
+            age = time.perf_counter() - t_pinned
+            if (age > min_s and last is not None and abs(dt - last) <= 0.03 * last) or age > max_s:
+                return
+            last = dt
+
+    def host_calls(n=20):
+        for _ in range(n):
+            binding.gamma_eval_host(ref_h, ev_h, *args_c, opts, out_h, stream)
+
+    settle(host_calls, t_pinned)
     barrier()
     ne2e = max(5, min(args.steps, 50))
     with clocks:
@@ -294,13 +312,14 @@ def main():
     e2e_s = max_over_ranks(e2e_s)
 
     # ---- end to end, a stream of cases: gamma_eval_host_batch overlaps the copies of consecutive cases with compute
-    nhb = 12
+    nhb = 32
     hb_refs = [ref_h] + [ref_h.clone().pin_memory() for _ in range(nhb - 1)]
     hb_evs = [ev_h] + [ev_h.clone().pin_memory() for _ in range(nhb - 1)]
     hb_outs = [torch.empty(N, dtype=torch.float32).pin_memory() for _ in range(nhb)]
     hb_dims, hb_sp = [case.dims] * nhb, [case.spacing_mm] * nhb
     hb_args = (case.dd, case.dta_mm, case.mode, case.cutoff)
-    binding.gamma_eval_host_batch(hb_refs, hb_evs, hb_dims, hb_sp, *hb_args, None, hb_outs, stream)
+    t_pinned_hb = time.perf_counter()
+    settle(lambda: binding.gamma_eval_host_batch(hb_refs, hb_evs, hb_dims, hb_sp, *hb_args, None, hb_outs, stream), t_pinned_hb)
     barrier()
     nrep_hb = 3
     with clocks:
@@ -323,6 +342,20 @@ def main():
     tc1.record(stream)
     torch.cuda.synchronize()
     h2d_gbs = 10 * 8 * N / (tc0.elapsed_time(tc1) * 1e-3) / 1e9
+    # ... and with the device-to-host copy of a result running at the same time on another stream, as in the pipeline
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s_out):
+        for _ in range(24):
+            out_h.copy_(outs[0], non_blocking=True)
+    with torch.cuda.stream(s_in):
+        tc0.record(s_in)
+        for _ in range(10):
+            dst[:N].copy_(ref_h, non_blocking=True)
+            dst[N:].copy_(ev_h, non_blocking=True)
+        tc1.record(s_in)
+    torch.cuda.synchronize()
+    h2d_gbs_duplex = 10 * 8 * N / (tc0.elapsed_time(tc1) * 1e-3) / 1e9
     del dst
 
     # ---- stats on the result (not timed: a6 is reported separately) ---------------------------------
@@ -437,6 +470,8 @@ def main():
                               "ms_per_case": e2e_pipe_s * 1e3, "cases_per_call": nhb, "same_result_as_single_call": e2e_pipe_ok,
                               "h2d_bytes_per_case": 8 * N, "d2h_bytes_per_case": 4 * N,
                               "h2d_gbs_of_this_box": h2d_gbs, "h2d_bound_ms_per_case": 8 * N / (h2d_gbs * 1e9) * 1e3,
+                              "h2d_gbs_while_d2h_runs": h2d_gbs_duplex,
+                              "h2d_bound_ms_per_case_while_d2h_runs": 8 * N / (h2d_gbs_duplex * 1e9) * 1e3,
                               "note": "gamma_eval_host_batch: pinned HOST buffers in and out, H2D of case i+1 and D2H of "
                                       "case i-1 overlapped with the kernels of case i; wall time of the synchronising call"}},
         "gpu_launches": int(launches), "host_submit_us_per_step": t_sub * 1e6,

@@ -732,6 +732,32 @@ def test_lane_calls_by_stream_launches_and_other_grid_shares(env):
     assert res.returncode == 0 and "lanes-ok" in res.stdout, res.stdout[-2000:] + res.stderr[-4000:]
 
 
+def test_option_variants_back_to_back_share_the_lanes(oracle_mod):
+    """Every option variant as a back-to-back call, interleaved without synchronisation: each kernel sequence gets its
+    own updatable graph per lane (four are kept, the oldest is rebuilt), sequences that cannot be updated in place (the
+    full radix sort launches a kernel several times) and options the lanes do not take (large tables) fall back to
+    stream launches or to the caller's stream -- the results must be those of the isolated calls, which are compared
+    with the oracle."""
+    c = phantoms.make_case("cfg2_small")
+    r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+    e = torch.from_numpy(c.eval.ravel().copy()).cuda()
+    args = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    o = cpu_gamma(oracle_mod, c.ref, c.eval, *args)
+    want = []
+    for v in VARIANTS:
+        want.append(binding.gamma_eval_ex(r, e, *args, v).clone())
+        torch.cuda.synchronize()
+        assert_parity(want[-1].cpu().numpy().astype(np.float64), o, str(v))
+    import dataclasses
+    outs = []
+    for rep in range(3):
+        for v in VARIANTS:
+            outs.append(binding.gamma_eval_ex(r, e, *args, dataclasses.replace(v, back_to_back=1)))
+    torch.cuda.synchronize()
+    for i, got in enumerate(outs):
+        assert torch.equal(_nn(got), _nn(want[i % len(VARIANTS)])), VARIANTS[i % len(VARIANTS)]
+
+
 def test_pipelined_calls_mixed_with_large_tables_and_other_entry_points():
     """a call with a side-stream table (table_radius 2, table_cap 4096) followed at once by default
     calls on another geometry must not have its table overwritten while its search is still walking it: the large
