@@ -9,16 +9,16 @@
 //   k_radix_hist    per-tile digit histogram            -> tileHist[digit][tile]
 //   k_radix_scan    exclusive scan along the tiles of every digit (one block per digit) + digit totals
 //   k_radix_scatter stable ranking inside the tile (warp match + per-warp counters) and scatter
-// Tile = 256 threads x 8 keys; a warp owns 256 consecutive keys and ranks them 32 at a time, which keeps
-// the sort stable.  Algorithmic traffic per pass: read keys twice + values once, write both: 20 B/pair.
+// Tile = 256 threads x 16 keys; a warp owns 512 consecutive keys and ranks them 32 at a time, which keeps
+// the sort stable; the scatter stages the tile in shared memory in digit order before it stores it.  Algorithmic traffic per pass: read keys twice + values once, write both: 20 B/pair.
 #pragma once
 #include "common.cuh"
 
 namespace gamma_b200 {
 
 constexpr int SORT_THREADS = 256;
-constexpr int SORT_ITEMS = 8;
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;  // 2048
+constexpr int SORT_ITEMS = 16;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;  // 4096
 constexpr int SORT_RADIX = 256;
 
 __device__ __forceinline__ unsigned sort_num_tiles(unsigned n) { return (n + SORT_TILE - 1) / SORT_TILE; }
@@ -34,10 +34,24 @@ k_radix_hist(const unsigned* __restrict__ keys, const unsigned* __restrict__ nPt
         hist[threadIdx.x] = 0;
         __syncthreads();
         const unsigned base = tile * SORT_TILE;
+        if (base + SORT_TILE <= n && (reinterpret_cast<uintptr_t>(keys) & 15u) == 0) {   // full tile: 16-byte loads
+            const uint4* k4 = reinterpret_cast<const uint4*>(keys + base);
+            uint4 v[SORT_ITEMS / 4];
 #pragma unroll
-        for (int j = 0; j < SORT_ITEMS; ++j) {
-            const unsigned i = base + j * SORT_THREADS + threadIdx.x;
-            if (i < n) atomicAdd(&hist[(keys[i] >> shift) & 0xffu], 1u);
+            for (int j = 0; j < SORT_ITEMS / 4; ++j) v[j] = k4[j * SORT_THREADS + threadIdx.x];
+#pragma unroll
+            for (int j = 0; j < SORT_ITEMS / 4; ++j) {
+                atomicAdd(&hist[(v[j].x >> shift) & 0xffu], 1u);
+                atomicAdd(&hist[(v[j].y >> shift) & 0xffu], 1u);
+                atomicAdd(&hist[(v[j].z >> shift) & 0xffu], 1u);
+                atomicAdd(&hist[(v[j].w >> shift) & 0xffu], 1u);
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < SORT_ITEMS; ++j) {
+                const unsigned i = base + j * SORT_THREADS + threadIdx.x;
+                if (i < n) atomicAdd(&hist[(keys[i] >> shift) & 0xffu], 1u);
+            }
         }
         __syncthreads();
         tileHist[(size_t)threadIdx.x * numTiles + tile] = hist[threadIdx.x];
@@ -81,7 +95,15 @@ k_radix_scan(unsigned* __restrict__ tileHist, const unsigned* __restrict__ nPtr,
     if (threadIdx.x == 0) digitTotal[blockIdx.x] = carry;
 }
 
-__global__ void __launch_bounds__(SORT_THREADS)
+// Scatter of one tile.  Ranking: a warp owns SORT_ITEMS x 32 consecutive keys and ranks them 32 at a time (warp match +
+// per-warp digit counters), which keeps the sort stable.  The pairs are then STAGED in shared memory in digit order and
+// written out from there: consecutive threads store consecutive positions of a digit's run, so a tile's 4 096 pairs leave
+// as 256 runs of 16 pairs on average (full 32-byte sectors) instead of 4 096 single 4-byte stores whose partial sectors
+// the memory system has to read back and merge (profiles/r2_sort.md).
+#ifndef GAMMA_SORT_SCATTER_BLOCKS
+#define GAMMA_SORT_SCATTER_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(SORT_THREADS, GAMMA_SORT_SCATTER_BLOCKS)
 k_radix_scatter(const unsigned* __restrict__ keysIn, const unsigned* __restrict__ valsIn,
                 unsigned* __restrict__ keysOut, unsigned* __restrict__ valsOut,
                 const unsigned* __restrict__ nPtr, int shift, const unsigned* __restrict__ tileHist,
@@ -90,38 +112,46 @@ k_radix_scatter(const unsigned* __restrict__ keysIn, const unsigned* __restrict_
     const unsigned n = *nPtr;
     const unsigned numTiles = sort_num_tiles(n);
     constexpr int WARPS = SORT_THREADS / 32;
-    __shared__ unsigned wc[WARPS][SORT_RADIX];
-    __shared__ unsigned digitBase[SORT_RADIX];
-    __shared__ unsigned baseWarp[WARPS];
+    __shared__ unsigned wc[WARPS][SORT_RADIX];      // per-warp digit counts, then the warp's first local slot of the digit
+    __shared__ unsigned digitBase[SORT_RADIX];      // global base of the digit (all tiles)
+    __shared__ int toGlobal[SORT_RADIX];            // global position = local slot + toGlobal[digit]
+    __shared__ unsigned scanWarp[WARPS];
+    __shared__ unsigned sKey[SORT_TILE], sVal[SORT_TILE];
     const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const unsigned ltMask = (1u << lane) - 1u;
-    {   // global base of digit d = exclusive scan of the 256 digit totals (thread d)
-        const unsigned v = digitTotal[threadIdx.x];
+    // exclusive scan over the 256 digits, one value per thread
+    auto scan256 = [&](unsigned v) -> unsigned {
         unsigned incl = v;
 #pragma unroll
         for (int s = 1; s < 32; s <<= 1) {
             const unsigned t = __shfl_up_sync(0xffffffffu, incl, s);
             if (lane >= (unsigned)s) incl += t;
         }
-        if (lane == 31) baseWarp[warp] = incl;
+        if (lane == 31) scanWarp[warp] = incl;
         __syncthreads();
         unsigned off = 0;
 #pragma unroll
-        for (int w = 0; w < WARPS; ++w) off += (unsigned)w < warp ? baseWarp[w] : 0u;
-        digitBase[threadIdx.x] = off + incl - v;
+        for (int w = 0; w < WARPS; ++w) off += (unsigned)w < warp ? scanWarp[w] : 0u;
         __syncthreads();
-    }
+        return off + incl - v;
+    };
+    digitBase[threadIdx.x] = scan256(digitTotal[threadIdx.x]);
     for (unsigned tile = blockIdx.x; tile < numTiles; tile += gridDim.x) {
 #pragma unroll
         for (int w = 0; w < WARPS; ++w) wc[w][threadIdx.x] = 0;
         __syncthreads();
         unsigned key[SORT_ITEMS], rank[SORT_ITEMS];
         const unsigned base = tile * SORT_TILE + warp * (32 * SORT_ITEMS);
+        const unsigned tileCount = min((unsigned)SORT_TILE, n - tile * SORT_TILE);
 #pragma unroll
         for (int r = 0; r < SORT_ITEMS; ++r) {
             const unsigned i = base + r * 32 + lane;
             const bool valid = i < n;
             key[r] = valid ? keysIn[i] : 0xffffffffu;
+        }
+#pragma unroll
+        for (int r = 0; r < SORT_ITEMS; ++r) {
+            const bool valid = base + r * 32 + lane < n;
             const unsigned digit = valid ? ((key[r] >> shift) & 0xffu) : 0x100u;
             const unsigned peers = __match_any_sync(0xffffffffu, digit);
             unsigned prev = 0;
@@ -132,23 +162,38 @@ k_radix_scatter(const unsigned* __restrict__ keysIn, const unsigned* __restrict_
             rank[r] = prev + __popc(peers & ltMask);
         }
         __syncthreads();
-        {   // thread d turns the per-warp counts of digit d into global base positions
-            unsigned run = digitBase[threadIdx.x] + tileHist[(size_t)threadIdx.x * numTiles + tile];
+        {   // thread d: the digit's count in the tile, its first local slot (scan over the digits), the warps' first slots
+            unsigned cnt = 0;
+#pragma unroll
+            for (int w = 0; w < WARPS; ++w) cnt += wc[w][threadIdx.x];
+            const unsigned start = scan256(cnt);
+            unsigned run = start;
 #pragma unroll
             for (int w = 0; w < WARPS; ++w) {
                 const unsigned t = wc[w][threadIdx.x];
                 wc[w][threadIdx.x] = run;
                 run += t;
             }
+            toGlobal[threadIdx.x] = (int)(digitBase[threadIdx.x] + tileHist[(size_t)threadIdx.x * numTiles + tile]) - (int)start;
         }
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < SORT_ITEMS; ++r) {
-            const unsigned i = base + r * 32 + lane;
-            if (i < n) {
-                const unsigned pos = wc[warp][(key[r] >> shift) & 0xffu] + rank[r];
-                keysOut[pos] = key[r];
-                valsOut[pos] = valsIn[i];
+            if (base + r * 32 + lane < n) {
+                const unsigned slot = wc[warp][(key[r] >> shift) & 0xffu] + rank[r];
+                sKey[slot] = key[r];
+                sVal[slot] = valsIn[base + r * 32 + lane];       // fetched here: 16 registers less while ranking
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < SORT_ITEMS; ++r) {
+            const unsigned slot = r * SORT_THREADS + threadIdx.x;
+            if (slot < tileCount) {
+                const unsigned k = sKey[slot];
+                const unsigned pos = (unsigned)((int)slot + toGlobal[(k >> shift) & 0xffu]);
+                keysOut[pos] = k;
+                valsOut[pos] = sVal[slot];
             }
         }
         __syncthreads();
