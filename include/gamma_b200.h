@@ -102,12 +102,14 @@ typedef struct gamma_opts {
                              continues by exhaustive enumeration, so results never depend on it            */
     int profile_stages;   /* 1: record CUDA events between the stages of this call on `stream`, to be read
                              with gamma_get_stage_times (adds a few event records, no synchronisation)     */
-    int graph;            /* 0: default (= 2); 1: a call whose arguments (pointers included) were seen before
-                             replays a cached CUDA graph of its kernels (96 graphs are kept; a call needs one per
-                             rotating control-block slot, so up to 32 argument sets replay without re-capture):
-                             less host time per call, but replays do not overlap with the previous call the
-                             way stream launches do; 2: launch the kernels one by one.  Ignored (= 2) while
-                             `stream` is being captured by the caller (the kernels then become nodes of the
+    int graph;            /* 0: default (= 2); 1: the call goes out as ONE CUDA-graph launch: the library keeps an
+                             instantiated graph of the call's kernels (captured once per kernel sequence, programmatic
+                             edges included) and rewrites grid sizes and arguments of its kernel nodes for every call
+                             (cudaGraphExecKernelNodeSetParams) -- a third of the host time of four stream launches; this
+                             is also how back_to_back calls are launched.  Kernel sequences that cannot be rewritten in
+                             place (side-stream table, full radix sort) replay a cached graph keyed by the exact
+                             arguments, pointers included (96 are kept).  2: launch the kernels one by one.  Ignored
+                             (= 2) while `stream` is being captured by the caller (the kernels then become nodes of the
                              caller's graph, with their own control block) and with profile_stages          */
     int table_radius;     /* 0: default (= 1); 1: the table is a data-independent PREFIX of the paper's table,
                              as far as table_cap allows, built beside a0 (nothing on the critical path);
