@@ -41,8 +41,9 @@ L2_BYTES = 126e6
 FLOP_PER_STAR_VOXEL, FLOP_PER_VISIT, FLOP_PER_RING_ITEM = 451.0, 380.0, 1212.0
 # executed WARP instructions (smsp__inst_executed.sum of the same captures) as unit costs plus a fixed part per launch:
 # k_norm and k_classify per grid voxel, k_star per evaluated voxel, k_table_search per owner-vertex visit and per ring
-# item (least squares over the four cases; reproduces each launch to a few per cent)
-WINST = {"norm_per_voxel": 0.0567, "norm_fixed": 0.474e6, "classify_per_voxel": 1.096, "classify_fixed": 0.674e6,
+# item (least squares over the four cases; reproduces each launch to a few per cent; k_classify's fixed part after its
+# constants moved to one thread per block: 1.634 M on cfg3 instead of the 1.823 M of that capture)
+WINST = {"norm_per_voxel": 0.0567, "norm_fixed": 0.474e6, "classify_per_voxel": 1.096, "classify_fixed": 0.47e6,
          "star_per_voxel": 27.3, "star_fixed": 0.70e6, "visit": 19.84, "ring_item": 30.4, "search_fixed": 0.288e6}
 SCHEDULERS = 4 * SM_COUNT                   # one warp instruction per scheduler per cycle
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on cfg3 from the ncu --set full capture (profiles/r2_full_summary.csv)
