@@ -245,11 +245,14 @@ struct Workspace {
     UpdGraph upd[UPD_CACHE];
     int numUpd = 0;
     unsigned long long graphGen = 0, useClock = 0;
-    void dropGraphs()
+    // keyed graphs hold workspace addresses and go when a buffer moves; the updatable ones get every argument anew with
+    // each call and only go with the workspace itself
+    void dropGraphs(bool updatableToo = false)
     {
         for (int i = 0; i < numGraphs; ++i)
             if (graph[i].exec) { cudaGraphExecDestroy(graph[i].exec); graph[i].exec = nullptr; }
         numGraphs = 0;
+        if (!updatableToo) return;
         for (int i = 0; i < numUpd; ++i) {
             if (upd[i].exec) { cudaGraphExecDestroy(upd[i].exec); upd[i].exec = nullptr; }
             if (upd[i].graph) { cudaGraphDestroy(upd[i].graph); upd[i].graph = nullptr; }
@@ -282,7 +285,7 @@ struct Workspace {
         if (done) { cudaEventDestroy(done); done = nullptr; }
         for (cudaEvent_t& ev : stage)
             if (ev) { cudaEventDestroy(ev); ev = nullptr; }
-        dropGraphs();
+        dropGraphs(true);
         if (aux) { cudaStreamDestroy(aux); aux = nullptr; }
         if (cap) { cudaStreamDestroy(cap); cap = nullptr; }
         if (evFork) { cudaEventDestroy(evFork); evFork = nullptr; }
@@ -1089,7 +1092,6 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     int launched = 0;
     bool launchedByUpdate = false;
     if (useUpd) {
-        if (g_ws.graphGen != g_allocGen) { g_ws.dropGraphs(); g_ws.graphGen = g_allocGen; }
         UpdKey uk;
         std::memset(&uk, 0, sizeof uk);
         uk.star = r.star; uk.lanes = r.lanes; uk.algoJu = r.algo == 2; uk.classes = g.all_active; uk.presort = r.presort;
