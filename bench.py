@@ -253,6 +253,12 @@ def main():
     clocks = ClockSampler(local_rank)
 
     # ---- device-resident timing --------------------------------------------------------------------
+    # one-time set-up of the library, not part of the W warm-up steps: the first call on each of the six lane streams
+    # allocates that lane's workspace (cudaMalloc synchronises) and builds its graph; two rounds over the lanes
+    INIT_CALLS = 12
+    for i in range(INIT_CALLS):
+        step(i)
+    torch.cuda.synchronize()
     for i in range(args.warmup):
         step(i)
     barrier()
@@ -463,7 +469,8 @@ def main():
         "config": {"workload": case_desc(case), "grid_voxels": N, "evaluated_voxels": M,
                    "l2_policy": f"{nsets} rotating input/output sets ({nsets * 12 * N / 1e6:.0f} MB) > 126 MB L2",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "options": {"presort": args.presort, "star_phase": args.star_phase, "lanes": args.lanes}},
+                   "options": {"presort": args.presort, "star_phase": args.star_phase, "lanes": args.lanes},
+                   "init_calls_before_warmup": INIT_CALLS},
         "grid_voxels_per_s": world * N / (ms_step * 1e-3), "ms_per_case": ms_step,
         "e2e": {"value": world * M / e2e_s, "unit": "evaluated reference voxels/s", "ms_per_case": e2e_s * 1e3,
                 "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N,
