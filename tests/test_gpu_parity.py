@@ -758,6 +758,39 @@ def test_option_variants_back_to_back_share_the_lanes(oracle_mod):
         assert torch.equal(_nn(got), _nn(want[i % len(VARIANTS)])), VARIANTS[i % len(VARIANTS)]
 
 
+def test_random_mix_of_back_to_back_calls():
+    """600 calls drawn at random from four geometries x three evaluation doses x five option variants, back to back with
+    an occasional plain call (which ends the sequence) and an occasional synchronisation: every result must be
+    bit-identical to the isolated call with the same arguments (isolated calls meet the oracle in the tests above)."""
+    import dataclasses
+    import random
+    rnd = random.Random(1)
+    cases = []
+    for name in ("cfg2_small", "cfg4_coarse", "cfg1", "cfg2"):
+        c = phantoms.make_case(name)
+        r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+        for k in range(3):
+            e = (torch.from_numpy(c.eval.ravel().copy()).cuda() * (1.0 + 0.01 * k)).contiguous()
+            cases.append((r, e, (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)))
+    variants = [GammaOpts(), GammaOpts(presort=1), GammaOpts(star_phase=2), GammaOpts(lanes_per_voxel=8), GammaOpts(presort=2)]
+    want = {}
+    for ci, (r, e, a) in enumerate(cases):
+        for vi, v in enumerate(variants):
+            want[(ci, vi)] = binding.gamma_eval_ex(r, e, *a, v).clone()
+    torch.cuda.synchronize()
+    outs = []
+    for _ in range(600):
+        ci, vi = rnd.randrange(len(cases)), rnd.randrange(len(variants))
+        r, e, a = cases[ci]
+        o = variants[vi] if rnd.random() < 0.05 else dataclasses.replace(variants[vi], back_to_back=1)
+        outs.append((ci, vi, binding.gamma_eval_ex(r, e, *a, o)))
+        if rnd.random() < 0.02:
+            torch.cuda.synchronize()
+    torch.cuda.synchronize()
+    bad = [(ci, vi) for ci, vi, got in outs if not torch.equal(_nn(got), _nn(want[(ci, vi)]))]
+    assert not bad, bad[:10]
+
+
 def test_pipelined_calls_mixed_with_large_tables_and_other_entry_points():
     """a call with a side-stream table (table_radius 2, table_cap 4096) followed at once by default
     calls on another geometry must not have its table overwritten while its search is still walking it: the large
