@@ -323,10 +323,12 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     const unsigned M = ctl->nEval;
     const unsigned warpsTotal = gridDim.x * (STAR_THREADS / 32);
     const unsigned numItems = (M + 31u) / 32u;
-    // Items are handed out in static rounds (item = warp + round * warps) while whole rounds are left; only the last,
-    // partial round goes through the ticket counter: 5 000 warps asking one address for a ticket at the same moment
+    // Items are handed out in static rounds (item = warp + round * warps) while whole rounds are left; only a last,
+    // partial round of less than half the warps goes through the ticket counter: 5 000 warps asking one address for a ticket at the same moment
     // queue up for microseconds (same-address atomics are served one at a time).
-    const unsigned staticRounds = numItems / warpsTotal;
+    unsigned staticRounds = numItems / warpsTotal;
+    const bool tickets = staticRounds && 2u * (numItems - staticRounds * warpsTotal) < warpsTotal;
+    if (!tickets) ++staticRounds;                          // a last round of half the warps or more is static too
     const unsigned one = ticket_one(ctl);
     unsigned round = 1;
     const float dnormF = e.norm_dose > 0.0f ? e.norm_dose : ordered_to_float(ctl->normOrd);
@@ -346,7 +348,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
     while (item < numItems) {
         unsigned nextItem = numItems;
         if (round < staticRounds) nextItem = item + warpsTotal;
-        else if (staticRounds && lane == 0) nextItem = ticket_next(&ctl->tileCounter, one) + staticRounds * warpsTotal;
+        else if (tickets && lane == 0) nextItem = ticket_next(&ctl->tileCounter, one) + staticRounds * warpsTotal;
         ++round;
         const unsigned j = item * 32u + lane;
         bool toSearch = false, starDone = false;
@@ -808,7 +810,11 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     const unsigned warpsTotal = gridDim.x * (SEARCH_THREADS / 32);
     unsigned unit = blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5);
     if (unit < numUnits) {
-        const unsigned staticRounds = numUnits / warpsTotal;      // whole rounds are static, the rest by tickets (k_star)
+        // whole rounds are static (k_star); a last partial round of less than half of the warps goes by tickets, a larger
+        // one is static too (thousands of tickets from one address cost more than the imbalance they would repair)
+        unsigned staticRounds = numUnits / warpsTotal;
+        const bool tickets = staticRounds && 2u * (numUnits - staticRounds * warpsTotal) < warpsTotal;
+        if (!tickets) ++staticRounds;
         const unsigned one = ticket_one(ctl);
         unsigned round = 1;
         c.ref = ref; c.ev = ev; c.out = out; c.table = table;
@@ -827,7 +833,7 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
             unsigned nextUnit = numUnits;
             const bool staticNext = round < staticRounds;
             if (staticNext) nextUnit = unit + warpsTotal;
-            else if (staticRounds && lane == 0) nextUnit = ticket_next(&ctl->workCounter, one) + staticRounds * warpsTotal;
+            else if (tickets && lane == 0) nextUnit = ticket_next(&ctl->workCounter, one) + staticRounds * warpsTotal;
             ++round;
             // the list entry of a statically known next unit is fetched now and used after this unit's search
             const bool havePre = pre;

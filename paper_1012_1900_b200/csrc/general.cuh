@@ -78,14 +78,16 @@ k_general_search(const float* __restrict__ ref, const float* __restrict__ ev, fl
     const unsigned numUnits = (M + 3u) / 4u;
     const unsigned warpsTotal = gridDim.x * (GENERAL_THREADS / 32);
     unsigned unit = blockIdx.x * (GENERAL_THREADS / 32) + (threadIdx.x >> 5);
-    const unsigned staticRounds = numUnits / warpsTotal;          // whole rounds are static, the rest by tickets (k_star)
+    unsigned staticRounds = numUnits / warpsTotal;                // whole rounds are static, a small rest by tickets (k_star)
+    const bool tickets = staticRounds && 2u * (numUnits - staticRounds * warpsTotal) < warpsTotal;
+    if (!tickets) ++staticRounds;
     const unsigned one = ticket_one(ctl);
     unsigned round = 1;
     const float qnan = __int_as_float(0x7fc00000);
     while (unit < numUnits) {
         unsigned nextUnit = numUnits;
         if (round < staticRounds) nextUnit = unit + warpsTotal;
-        else if (staticRounds && lane == 0) nextUnit = ticket_next(&ctl->workCounter, one) + staticRounds * warpsTotal;
+        else if (tickets && lane == 0) nextUnit = ticket_next(&ctl->workCounter, one) + staticRounds * warpsTotal;
         ++round;
         const unsigned item = unit * 4u + (unsigned)gid;
         const bool have = item < M;
