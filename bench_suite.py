@@ -367,6 +367,23 @@ def suite_trace(args, emit):
               "kernels_us_after_norm_start": {n: {"first": float(med[k, 0]), "waited": float(med[k, 1]),
                                                  "last": float(med[k, 2])} for k, n in enumerate(names)},
               "pipelined_calls": binding.gamma_get_counters()["calls_pipelined"]})
+    # the warps of one k_table_search launch (a call on its own, full-size grid): how long a work unit takes
+    torch.cuda.synchronize()
+    binding.gamma_eval_ex(refs[0], evs[0], *a, GammaOpts(), outs[0], stream)
+    torch.cuda.synchronize()
+    w = binding.gamma_trace_read_warps().astype(np.float64)
+    w = w[w[:, 3] > 0]
+    if len(w):
+        t0 = w[:, 0].min()
+        pct = lambda x: [round(float(v), 2) for v in np.percentile(x, [0, 10, 50, 90, 100])]
+        units = w[:, 4]
+        busy = (w[:, 3] - w[:, 1]) / 1e3
+        emit({"suite": "trace", "case": args.trace_case, "mode": "warps of one k_table_search (us after the first warp started; percentiles 0 / 10 / 50 / 90 / 100)",
+              "warps": int(len(w)), "warp_started": pct((w[:, 0] - t0) / 1e3), "wait_passed": pct((w[:, 1] - t0) / 1e3),
+              "first_unit_finished": pct((w[units > 0, 2] - t0) / 1e3), "warp_ended": pct((w[:, 3] - t0) / 1e3),
+              "first_unit_us": pct((w[units > 0, 2] - w[units > 0, 1]) / 1e3),
+              "warps_by_units_taken": {str(int(k)): int((units == k).sum()) for k in np.unique(units)},
+              "median_busy_us_by_units_taken": {str(int(k)): round(float(np.median(busy[units == k])), 2) for k in np.unique(units)}})
 
 
 def write_md(path, rows):

@@ -313,6 +313,11 @@ long long gamma_launch_count(void);
  */
 int gamma_trace_reset(void);
 int gamma_trace_read(unsigned long long* out_host, long long* next_call);
+/* The same build also keeps one record per warp of the LAST k_table_search launch: out_host HOST, max_warps (<= 8192)
+ * x 8 u64 = (warp started, dependency wait passed, first work unit finished, warp ended, work units taken, 0, 0, 0),
+ * warp w = block * 4 + warp in block; SYNCHRONISES.  Shows how long a work unit takes while every warp of the grid is
+ * busy and how long when few are left (profiles/r2_profile.md). */
+int gamma_trace_read_warps(unsigned long long* out_host, int max_warps);
 
 /* Device memory the library's workspaces hold right now, in bytes (host counter). */
 long long gamma_workspace_bytes(void);

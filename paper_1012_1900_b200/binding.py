@@ -17,7 +17,7 @@ from . import build as _build
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
     "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
-    "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_version",
+    "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_trace_reset", "gamma_trace_read", "gamma_trace_read_warps", "gamma_release", "gamma_version",
     "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
 
@@ -27,7 +27,7 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 exported_symbols = (
     "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats",
     "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
-    "gamma_trace_reset", "gamma_trace_read", "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
+    "gamma_trace_reset", "gamma_trace_read", "gamma_trace_read_warps", "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
 
 
@@ -151,6 +151,8 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_trace_reset.restype = ci
     lib.gamma_trace_read.argtypes = [vp, ctypes.POINTER(cll)]
     lib.gamma_trace_read.restype = ci
+    lib.gamma_trace_read_warps.argtypes = [vp, ci]
+    lib.gamma_trace_read_warps.restype = ci
     lib.gamma_workspace_bytes.argtypes = []
     lib.gamma_workspace_bytes.restype = cll
     for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats", "gamma_sort_pairs",
@@ -430,6 +432,15 @@ def gamma_trace_read():
     nxt = ctypes.c_longlong(0)
     _check(load_library().gamma_trace_read(buf.ctypes.data_as(ctypes.c_void_p), ctypes.byref(nxt)))
     return buf, int(nxt.value)
+
+
+def gamma_trace_read_warps(max_warps=8192):
+    """uint64 numpy [max_warps, 8] = warp x (started, wait passed, first unit finished, ended, units taken, 0, 0, 0) of
+    the last k_table_search launch, ns (library built with -DGAMMA_TRACE only)."""
+    import numpy as np
+    buf = np.zeros((int(max_warps), 8), dtype=np.uint64)
+    _check(load_library().gamma_trace_read_warps(buf.ctypes.data_as(ctypes.c_void_p), int(max_warps)))
+    return buf
 
 
 def gamma_workspace_bytes() -> int:

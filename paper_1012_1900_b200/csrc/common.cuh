@@ -94,7 +94,12 @@ struct TraceRec {
     unsigned long long first, waited, last;   // ns: earliest start, latest "dependency met", latest block end
     unsigned long long pad_;
 };
+// Per-warp records of the LAST k_table_search launch (same build): when the warp started, passed the dependency wait,
+// finished its first work unit and ended, and how many units it took.
+constexpr int TRACE_WARPS = 8192;
+struct TraceWarp { unsigned long long start, waited, firstUnit, end, units, pad_[3]; };
 #ifdef GAMMA_TRACE
+__device__ TraceWarp* g_trace_warps = nullptr;   // TRACE_WARPS records, set by the host
 __device__ TraceRec* g_trace_buf = nullptr;   // TRACE_CALLS x TRACE_KERNELS records, set by the host
 __device__ __forceinline__ unsigned long long trace_now()
 {

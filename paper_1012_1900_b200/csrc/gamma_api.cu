@@ -1822,7 +1822,7 @@ long long gamma_launch_count(void)
 
 // ---- device timeline (GAMMA_TRACE builds; common.cuh)
 #ifdef GAMMA_TRACE
-namespace { TraceRec* g_traceDev = nullptr; }
+namespace { TraceRec* g_traceDev = nullptr; TraceWarp* g_traceWarpsDev = nullptr; }
 #endif
 int gamma_trace_reset(void)
 {
@@ -1836,6 +1836,9 @@ int gamma_trace_reset(void)
     for (size_t i = 0; i < n; ++i) { init[i].first = ~0ull; init[i].waited = 0; init[i].last = 0; init[i].pad_ = 0; }
     CU_TRY(cudaMemcpy(g_traceDev, init, n * sizeof(TraceRec), cudaMemcpyHostToDevice));
     CU_TRY(cudaMemcpyToSymbol(g_trace_buf, &g_traceDev, sizeof g_traceDev));
+    if (!g_traceWarpsDev) CU_TRY(cudaMalloc(&g_traceWarpsDev, (size_t)TRACE_WARPS * sizeof(TraceWarp)));
+    CU_TRY(cudaMemset(g_traceWarpsDev, 0, (size_t)TRACE_WARPS * sizeof(TraceWarp)));
+    CU_TRY(cudaMemcpyToSymbol(g_trace_warps, &g_traceWarpsDev, sizeof g_traceWarpsDev));
     return GAMMA_OK;
 #else
     return fail(GAMMA_ERR_INVALID_ARGUMENT, "libgamma_b200 was built without -DGAMMA_TRACE");
@@ -1855,6 +1858,23 @@ int gamma_trace_read(unsigned long long* out_host, long long* next_call)
     return GAMMA_OK;
 #else
     (void)out_host; (void)next_call;
+    return fail(GAMMA_ERR_INVALID_ARGUMENT, "libgamma_b200 was built without -DGAMMA_TRACE");
+#endif
+}
+
+int gamma_trace_read_warps(unsigned long long* out_host, int max_warps)
+{
+    g_err.clear();
+#ifdef GAMMA_TRACE
+    if (!out_host || max_warps < 1) return fail(GAMMA_ERR_INVALID_ARGUMENT, "out_host is NULL or max_warps < 1");
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (!g_traceWarpsDev) return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_trace_reset has not been called");
+    CU_TRY(cudaDeviceSynchronize());
+    const int n = max_warps < TRACE_WARPS ? max_warps : TRACE_WARPS;
+    CU_TRY(cudaMemcpy(out_host, g_traceWarpsDev, (size_t)n * sizeof(TraceWarp), cudaMemcpyDeviceToHost));
+    return GAMMA_OK;
+#else
+    (void)out_host; (void)max_warps;
     return fail(GAMMA_ERR_INVALID_ARGUMENT, "libgamma_b200 was built without -DGAMMA_TRACE");
 #endif
 }

@@ -786,11 +786,18 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
     const int lane = threadIdx.x & 31;
     __shared__ FusedStats<SEARCH_THREADS> sStat;
     SearchCtx c;
+#ifdef GAMMA_TRACE
+    TraceWarp tw;
+    tw.start = trace_now(); tw.waited = 0; tw.firstUnit = 0; tw.end = 0; tw.units = 0;
+#endif
     fused_stats_init(sStat, st);
     trace_first(e.call, 3);
     pdl_wait();
     pdl_launch_dependents();                             // the next call's k_norm may use the SMs this kernel leaves
     trace_waited(e.call, 3);
+#ifdef GAMMA_TRACE
+    tw.waited = trace_now();
+#endif
     const unsigned nS = ctl->nSearch;
     unsigned nDeep = 0;
     if (MODE == 0 && classes) {
@@ -857,12 +864,22 @@ k_table_search(const float* __restrict__ ref, const float* __restrict__ ev, floa
                 visits += search_items<(MODE == 0 ? 8 : MODE), JU>(c, g, e, listKey, listIdx, nS, unit * VPW, lane);
             }
             unit = __shfl_sync(FULL, nextUnit, 0);
+#ifdef GAMMA_TRACE
+            if (tw.units++ == 0) tw.firstUnit = trace_now();
+#endif
         }
         // diagnostic counter: one atomic per warp
         for (int s = 16; s > 0; s >>= 1) visits += __shfl_xor_sync(FULL, visits, s);
         if (lane == 0 && visits) atomicAdd(&ctl->visits, (unsigned long long)visits);
     }
     fused_stats_flush(sStat, st);
+#ifdef GAMMA_TRACE
+    {
+        const unsigned wid = blockIdx.x * (SEARCH_THREADS / 32) + (threadIdx.x >> 5);
+        tw.end = trace_now();
+        if (lane == 0 && g_trace_warps && wid < TRACE_WARPS) g_trace_warps[wid] = tw;
+    }
+#endif
     trace_last(e.call, 3);
 }
 
