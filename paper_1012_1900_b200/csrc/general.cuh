@@ -32,8 +32,11 @@ constexpr int GENERAL_THREADS = 128;
 // The 26 faces owned by evaluation vertex c = c0 + o against the point c0 + f; returns min(best2, ...).
 __device__ __forceinline__ float general_owner_vertex(const float* __restrict__ ev, const GridP& g, const int (&c0)[3],
                                                       int lin0, const float (&f)[3], float Dr, float invdD, int ox, int oy,
-                                                      int oz, float best2, bool wantLoc, float (&loc)[4])
+                                                      int oz, float best2, bool wantLoc, float (&loc)[4],
+                                                      float cellL2 = 0.0f, float prune2 = INFINITY)
 {
+    // cellL2: exact squared minimum spatial distance of the vertex's cell to the point; prune2: the running gamma^2 --
+    // the vertex is skipped when nothing in its cell can be closer than that
     const int cx = c0[0] + ox, cy = c0[1] + oy, cz = c0[2] + oz;
     if ((unsigned)cx >= (unsigned)g.n[0] || (unsigned)cy >= (unsigned)g.n[1] || (unsigned)cz >= (unsigned)g.n[2])
         return best2;                                          // vertex outside the grid (reading 11)
@@ -44,6 +47,14 @@ __device__ __forceinline__ float general_owner_vertex(const float* __restrict__ 
 #pragma unroll
     for (int S = 0; S < 8; ++S)
         d[S] = (__ldg(p + (((S & 1) ? sx : 0) + ((S & 2) ? sy : 0) + ((S & 4) ? sz : 0))) - Dr) * invdD;
+    // exact prune: every face this vertex owns lies in its cell, whose points are at least cellL2 away
+    // in space and carry a dose between the smallest and the largest of the eight corners
+    {
+        const float dlo = fminf(fminf(fminf(d[0], d[1]), fminf(d[2], d[3])), fminf(fminf(d[4], d[5]), fminf(d[6], d[7])));
+        const float dhi = fmaxf(fmaxf(fmaxf(d[0], d[1]), fmaxf(d[2], d[3])), fmaxf(fmaxf(d[4], d[5]), fmaxf(d[6], d[7])));
+        const float dr = fmaxf(fmaxf(dlo, -dhi), 0.0f);
+        if (!(fmaf(dr, dr, cellL2) < prune2)) return best2;
+    }
     float lam[8], q[3], X[8];
     owned_face_terms(g, (float)ox - f[0], (float)oy - f[1], (float)oz - f[2], usable, lam, q, X);
     if (wantLoc) return gamma_owned_argmin(d, g.invA, lam, q, X, usable, best2, loc);
@@ -119,8 +130,8 @@ k_general_search(const float* __restrict__ ref, const float* __restrict__ ev, fl
         float mine2 = INFINITY;                          // best of the owner vertices THIS lane evaluated, and which one
         int mo[3] = {0, 0, 0};
         float loc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-        auto visit = [&](int ox, int oy, int oz) -> float {
-            const float own = general_owner_vertex(ev, g, c0, lin0, f, Dr, invdD, ox, oy, oz, INFINITY, false, loc);
+        auto visit = [&](int ox, int oy, int oz, float cellL2) -> float {
+            const float own = general_owner_vertex(ev, g, c0, lin0, f, Dr, invdD, ox, oy, oz, INFINITY, false, loc, cellL2, best2);
             if (own < mine2) { mine2 = own; mo[0] = ox; mo[1] = oy; mo[2] = oz; }
             return fminf(best2, own);
         };
@@ -140,7 +151,8 @@ k_general_search(const float* __restrict__ ref, const float* __restrict__ ev, fl
                 const int ox = (gl & 1) ? -t.y - 1 : t.y;
                 const int oy = (gl & 2) ? -t.z - 1 : t.z;
                 const int oz = (gl & 4) ? -t.w - 1 : t.w;
-                if (general_cell_L2(g, f, ox, oy, oz) < best2) cand = visit(ox, oy, oz);
+                const float cL2 = general_cell_L2(g, f, ox, oy, oz);
+                if (cL2 < best2) cand = visit(ox, oy, oz, cL2);
             }
             best2 = group_min<8>(cand);
         }
@@ -169,7 +181,8 @@ k_general_search(const float* __restrict__ ref, const float* __restrict__ ev, fl
                             const int ox = (gl & 1) ? -mx - 1 : mx;
                             const int oy = (gl & 2) ? -my - 1 : my;
                             const int oz = (gl & 4) ? -mz - 1 : mz;
-                            if (general_cell_L2(g, f, ox, oy, oz) < best2) cand = visit(ox, oy, oz);
+                            const float cL2 = general_cell_L2(g, f, ox, oy, oz);
+                if (cL2 < best2) cand = visit(ox, oy, oz, cL2);
                         }
                     }
                     best2 = group_min<8>(cand);
