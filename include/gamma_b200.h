@@ -80,7 +80,9 @@ int gamma_eval(const float* ref, const float* eval, const int dims[3], const flo
 /* Options of gamma_eval_ex / gamma_eval_host.  Zero-initialise, then set what differs. */
 struct gamma_summary;
 typedef struct gamma_opts {
-    float norm_dose;      /* D_norm; <= 0: max(ref), found on the device                                  */
+    float norm_dose;      /* D_norm; <= 0: max(ref), found on the device (k_norm).  > 0 (e.g. the prescription dose,
+                             PAPER.md:312): step a0 is not needed and, unless table_radius = 2, star_load >= 2 or
+                             stats_* ask for k_norm's other results, the call is three kernels instead of four  */
     int presort;          /* pre-sort of the search work list (A2 step 3).  0: default (= 4);
                              1: one-pass MSD radix sort on the 8-bit key digit (32 steps per octave of the key);
                              2: no sort (Table 2's "without sorting"); 3: full LSD radix sort of the

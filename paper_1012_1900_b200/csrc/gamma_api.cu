@@ -173,7 +173,7 @@ constexpr int GRAPH_CACHE = 96;    // argument sets x CTL_ROT rotating sets
 
 // One updatable graph per kernel sequence (GraphUpdate): the options that decide WHICH kernels a call launches.
 struct UpdKey {
-    int star, lanes, algoJu, classes, presort;
+    int star, lanes, algoJu, classes, presort, noNorm;
     bool operator==(const UpdKey& o) const { return std::memcmp(this, &o, sizeof *this) == 0; }
 };
 struct UpdGraph {
@@ -267,6 +267,7 @@ struct Workspace {
     int lastEarly = 0;                   // the last call started in the tail of its predecessor
     long long numEarly = 0;
     int lastClasses = 0;           // last call used depth classes: list A holds the ring items
+    float lastNormDose = 0.0f;     // opts.norm_dose of the last call (0: max(ref) from the control block)
     long long lastN = 0;
     bool haveLast = false;
     size_t bytes() const
@@ -815,7 +816,12 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     // a large prefix table needs nothing of this call: forked in front of it (a call with a large table is never
     // started early, so the previous call on the workspace has ended by the time the fork event fires)
     if (r.tableMode == 1 && !embed) { rc = fork_table(); if (rc) return rc; }
-    if (!cs.skipNorm) {                                                  // a0 + A1 step 1
+    // a0 is not needed at all when the caller gives D_norm and nothing else wants k_norm (its max |DD| sizes the paper's
+    // table, it zeroes the fused statistics, the tile kernels read its maxima): the call is then three kernels and
+    // k_classify, as its first kernel, takes over the wait and the zeroing of the next control block
+    const bool noNorm = !cs.skipNorm && r.normDose > 0.0f && r.tableMode == 1 && r.stats.hist == nullptr &&
+                        !(classes && r.starLoad >= 2);
+    if (!cs.skipNorm && !noNorm) {                                       // a0 + A1 step 1
         long long blocks = (N + 1023) / 1024;
         int grid = (int)(blocks < 1 ? 1 : (blocks > sm * normBlocks ? sm * normBlocks : blocks));
         CU_TRY(launch_ex(k_norm, grid, NORM_THREADS, 0, st, pdl, false, ref, ev, (int)N, mode, ctl, next, cs.waitFirst,
@@ -871,7 +877,8 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
     {                                                                    // a1: exclusion + compaction
         long long chunks = (N + PREP_CHUNK - 1) / PREP_CHUNK;
         int grid = (int)(chunks > sm * classifyBlocks ? sm * classifyBlocks : chunks);
-        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0, r.stats));
+        CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out, g, e, ctl, e0, r.stats,
+                         noNorm ? next : static_cast<Ctl*>(nullptr), noNorm ? 1 : 0));
         ++nk;
     }
     STAGE_MARK(1, st);
@@ -940,6 +947,7 @@ int enqueue_kernels(const float* ref, const float* ev, const GridP& g, float DD,
 #undef STAGE_MARK
     *launched = nk;
     g_ws.lastClasses = classes;
+    g_ws.lastNormDose = r.normDose;
     g_ws.lastCtl = ctl;
     return GAMMA_OK;
 }
@@ -1095,6 +1103,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         UpdKey uk;
         std::memset(&uk, 0, sizeof uk);
         uk.star = r.star; uk.lanes = r.lanes; uk.algoJu = r.algo == 2; uk.classes = g.all_active; uk.presort = r.presort;
+        uk.noNorm = r.normDose > 0.0f && r.stats.hist == nullptr;
         UpdGraph* hit = nullptr;
         for (int i = 0; i < g_ws.numUpd; ++i)
             if (g_ws.upd[i].key == uk) { hit = &g_ws.upd[i]; break; }
@@ -1487,7 +1496,7 @@ int gamma_eval_general(const float* ref, const int ref_dims[3], const float ref_
         long long chunks = (Nr + PREP_CHUNK - 1) / PREP_CHUNK;
         int grid = (int)(chunks > sm * 8 ? sm * 8 : chunks);
         CU_TRY(launch_ex(k_classify, grid, PREP_THREADS, 0, st, pdl, false, ref, out_gamma, gr, e, ctl,
-                         static_cast<unsigned*>(g_ws.evalIdx.p), noStats));
+                         static_cast<unsigned*>(g_ws.evalIdx.p), noStats, static_cast<Ctl*>(nullptr), 0));
     }
     // a3 on the evaluation grid: the same data-independent prefix table as gamma_eval (table_cap cells), here by the
     // stand-alone builder; beyond it the search enumerates
@@ -1785,7 +1794,7 @@ int gamma_get_counters(gamma_counters* out_host)
     union { unsigned u; float f; } cv;
     cv.u = c.maxKeyBits;
     out_host->max_key = cv.f;
-    out_host->norm_dose = ordered_to_float(c.normOrd);
+    out_host->norm_dose = w.lastNormDose > 0.0f ? w.lastNormDose : ordered_to_float(c.normOrd);
     out_host->table_truncated = (int)c.tableTrunc;
     out_host->n_ring_search = w.lastClasses ? (int)c.nSearch : 0;
     out_host->pipelined = (&w != &g_pool[0] && &w != &g_pool[WS_CAPTURE]) ? 1 : 0;

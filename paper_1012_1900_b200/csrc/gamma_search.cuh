@@ -166,8 +166,11 @@ __device__ __forceinline__ float criterion_inv_dD(const EvalP& e, double dnorm, 
 
 __global__ void __launch_bounds__(PREP_THREADS)
 k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, EvalP e, Ctl* __restrict__ ctl,
-           unsigned* __restrict__ evalIdx, StatsP st)
+           unsigned* __restrict__ evalIdx, StatsP st, Ctl* __restrict__ next, int first)
 {
+    // first != 0: the call has no k_norm (opts.norm_dose given, prefix table, no fused statistics: nothing of a0 is
+    // needed) and this is its first kernel -- it waits for the operation in front of it before it reads anything and
+    // zeroes the control block of the next call (`next`) in k_norm's place
     __shared__ unsigned sWarp[PREP_THREADS / 32];
     __shared__ unsigned sBase;
     __shared__ unsigned sNan;
@@ -191,8 +194,13 @@ k_classify(const float* __restrict__ ref, float* __restrict__ out, GridP g, Eval
         }
         return nval;
     };
+    if (first) pdl_wait();
     pdl_launch_dependents();
     trace_first(e.call, 1);
+    if (next != nullptr && blockIdx.x == gridDim.x - 1) {
+        unsigned* w = reinterpret_cast<unsigned*>(next);
+        for (int i = threadIdx.x; i < (int)(sizeof(Ctl) / 4); i += PREP_THREADS) w[i] = 0u;
+    }
     // ref is an input of the call, not a result of k_norm: the first chunk is fetched while k_norm drains
     float Dr[4] = {0.0f, 0.0f, 0.0f, 0.0f};
     int nval = 0;

@@ -437,6 +437,36 @@ def test_norm_dose_option_and_cutoff_decision(oracle_mod):
 # ----------------------------------------------------------------------------------------------------
 # host-buffer entry point, streams, determinism
 # ----------------------------------------------------------------------------------------------------
+def test_norm_dose_given_runs_without_k_norm(oracle_mod):
+    """With opts.norm_dose (and nothing else that needs a0) a call is three kernels: k_classify is its first kernel, waits
+    for the operation in front of it and zeroes the next control block.  Full maps against the oracle in global and local
+    mode, alternating with default calls on two geometries (the rotating control blocks are zeroed by k_norm in one call
+    and by k_classify in the next), back to back as well, and the kernel count is checked."""
+    cases = [phantoms.make_case(n) for n in ("cfg2_small", "cfg4_coarse")]
+    data = []
+    for c in cases:
+        r = torch.from_numpy(c.ref.ravel().copy()).cuda()
+        e = torch.from_numpy(c.eval.ravel().copy()).cuda()
+        for mode, nd in ((0, 1.7), (1, 2.3), (0, 0.0)):
+            args = (c.dims, c.spacing_mm, c.dd, c.dta_mm, mode, c.cutoff)
+            o = cpu_gamma(oracle_mod, c.ref, c.eval, *args, norm_dose=nd)
+            data.append((r, e, args, nd, o))
+    torch.cuda.synchronize()
+    l0 = binding.gamma_launch_count()
+    binding.gamma_eval_ex(data[0][0], data[0][1], *data[0][2], GammaOpts(norm_dose=1.7))
+    torch.cuda.synchronize()
+    assert binding.gamma_launch_count() - l0 == 3
+    assert abs(binding.gamma_get_counters()["norm_dose"] - 1.7) < 1e-6
+    for b2b in (0, 1):
+        outs = []
+        for i in range(36):                                      # no synchronisation in between
+            r, e, args, nd, _ = data[(i * 5) % len(data)]
+            outs.append(binding.gamma_eval_ex(r, e, *args, GammaOpts(norm_dose=nd, back_to_back=b2b)))
+        torch.cuda.synchronize()
+        for i, g in enumerate(outs):
+            assert_parity(g.cpu().numpy().astype(np.float64), data[(i * 5) % len(data)][4], f"b2b {b2b} call {i}")
+
+
 def test_gamma_eval_host_streams_and_determinism():
     c = phantoms.make_case("cfg2_small")
     base = gpu_gamma(c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
