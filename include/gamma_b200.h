@@ -258,6 +258,34 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
                      void* stream);
 
 /*
+ * gamma_sort_pairs_noalloc -- gamma_sort_pairs for callers that cannot allocate device memory: same kernels, same
+ * result bit for bit, but the second pair of buffers, the tile histograms and the element counter sit in an array that
+ * is part of the library image instead of coming from cudaMalloc.  The call (first one included) issues no cudaMalloc,
+ * cudaFree or other allocating routine; it enqueues kernels and, for an odd number of 8-bit passes, two device-to-device
+ * copies on `stream`.
+ *   Who needs it: code that runs while any thread of the process captures a stream in the global capture mode (the
+ *   runtime refuses cudaMalloc there and the refusal invalidates the capture); code in a loop with a latency budget
+ *   (cudaMalloc / cudaFree stall the whole device); and processes in which one pool owns the device memory (the PyTorch
+ *   caching allocator, a planning system's arena), where an allocation behind the pool's back fails or fragments it.
+ *   keys, vals, begin_bit, end_bit, stream   as gamma_sort_pairs; the device `stream` belongs to must be current
+ *   n          0 <= n <= GAMMA_SORT_NOALLOC_MAX_PAIRS; a larger n returns GAMMA_ERR_INVALID_ARGUMENT (nothing is
+ *              launched; the error string names the limit) -- such sorts need gamma_sort_pairs
+ * Cost: the array takes about 8.3 MB (8 B per pair of the limit + 260 KB) of EVERY GPU on which the library's code gets
+ * loaded, from then until the process exits, whether or not this function is ever called; gamma_release() does not
+ * return it and gamma_workspace_bytes() does not count it.
+ * First call on a device: looks up the array's address on that device (cudaGetSymbolAddress, once per device, may load
+ * the library's module).  Make that first call outside any stream capture.
+ * Sharing: all calls on a device use the same array, and it keeps what the last call left in it.  No part of it needs to
+ * be zero on entry (every word a pass reads was written earlier in the same call), so nothing is cleared.  Two calls
+ * whose kernels could overlap on the GPU -- different streams without an event between them, two host threads on two
+ * streams -- RACE on it and give garbage; calls on one stream are ordered and safe.  Unlike the other entry points this
+ * one is not ordered against the rest of the library by events: it touches none of the library's workspaces.
+ */
+#define GAMMA_SORT_NOALLOC_MAX_PAIRS (1 << 20)
+int gamma_sort_pairs_noalloc(unsigned int* keys, unsigned int* vals, long long n, int begin_bit, int end_bit,
+                             void* stream);
+
+/*
  * gamma_offset_table -- the sorted offset table {n, L_n} (Algorithm A1 steps 2-3; A2
  * steps 4-5) with the cell bound of reading 4.  (Inside gamma_eval the radius is the
  * paper's max|DD|/dD over the grid, A1 step 1.)  By the symmetry L(o) = L(-o-1) the

@@ -16,7 +16,7 @@ from . import build as _build
 
 __all__ = [
     "GammaError", "GammaOpts", "load_library", "exported_symbols", "gamma_eval", "gamma_eval_ex",
-    "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters",
+    "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats", "gamma_stats_async", "decode_summary", "gamma_sort_pairs", "gamma_sort_pairs_noalloc", "gamma_offset_table", "gamma_get_counters",
     "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe", "gamma_trace_reset", "gamma_trace_read", "gamma_trace_read_warps", "gamma_release", "gamma_version",
     "GAMMA_MODE_GLOBAL", "GAMMA_MODE_LOCAL",
 ]
@@ -26,7 +26,7 @@ GAMMA_MODE_GLOBAL, GAMMA_MODE_LOCAL = 0, 1
 # every symbol include/gamma_b200.h declares
 exported_symbols = (
     "gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats",
-    "gamma_sort_pairs", "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
+    "gamma_sort_pairs", "gamma_sort_pairs_noalloc", "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_launch_count", "gamma_workspace_bytes", "gamma_fp32_probe",
     "gamma_trace_reset", "gamma_trace_read", "gamma_trace_read_warps", "gamma_release", "gamma_abi_sizes", "gamma_last_error_string", "gamma_version",
 )
 
@@ -141,6 +141,7 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_eval_general.restype = ci
     lib.gamma_stats.argtypes = [vp, cll, ci, cf, vp, vp, vp]
     lib.gamma_sort_pairs.argtypes = [vp, vp, cll, ci, ci, vp]
+    lib.gamma_sort_pairs_noalloc.argtypes = [vp, vp, cll, ci, ci, vp]
     lib.gamma_offset_table.argtypes = [i3, f3, cf, cf, cll, vp, vp, vp]
     lib.gamma_get_counters.argtypes = [ctypes.POINTER(_CCounters)]
     lib.gamma_fp32_probe.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -156,7 +157,7 @@ def load_library(build_if_needed: bool = True):
     lib.gamma_workspace_bytes.argtypes = []
     lib.gamma_workspace_bytes.restype = cll
     for name in ("gamma_eval", "gamma_eval_ex", "gamma_eval_batch", "gamma_eval_general", "gamma_eval_host", "gamma_eval_host_batch", "gamma_stats", "gamma_sort_pairs",
-                 "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_fp32_probe"):
+                 "gamma_sort_pairs_noalloc", "gamma_offset_table", "gamma_get_counters", "gamma_get_stage_times", "gamma_fp32_probe"):
         getattr(lib, name).restype = ci
     lib.gamma_release.restype = None
     lib.gamma_abi_sizes.restype = None
@@ -386,6 +387,30 @@ def gamma_sort_pairs(keys, vals, begin_bit=0, end_bit=32, stream=None):
         raise GammaError("keys and vals differ in length")
     _check(lib.gamma_sort_pairs(keys.data_ptr(), vals.data_ptr(), keys.numel(), int(begin_bit), int(end_bit),
                                 _stream(stream)))
+    return keys, vals
+
+
+SORT_NOALLOC_MAX_PAIRS = 1 << 20      # GAMMA_SORT_NOALLOC_MAX_PAIRS of include/gamma_b200.h
+
+
+def gamma_sort_pairs_noalloc(keys, vals, begin_bit=0, end_bit=32, stream=None):
+    """``gamma_sort_pairs_noalloc``: ``gamma_sort_pairs`` without any device allocation by the library.
+
+    For code that must not call cudaMalloc -- it runs beside a global-mode stream capture, inside a latency-bound loop,
+    or in a process whose device memory belongs to one pool.  The sort's scratch is an array built into the library
+    (about 8.3 MB of every GPU that loads it), which limits it to ``SORT_NOALLOC_MAX_PAIRS`` pairs: a longer input raises
+    ``GammaError`` and nothing runs.  All calls on a device share that array, so calls that could overlap on the GPU
+    (different streams with no event between them) race; calls on one stream are safe.  Make the first call on a device
+    outside stream capture (it looks up the array's device address).  Same result as ``gamma_sort_pairs``, bit for bit.
+    """
+    lib = load_library()
+    for t in (keys, vals):
+        if not (t.is_cuda and t.is_contiguous() and t.element_size() == 4):
+            raise GammaError("keys / vals must be contiguous 4-byte CUDA tensors")
+    if keys.numel() != vals.numel():
+        raise GammaError("keys and vals differ in length")
+    _check(lib.gamma_sort_pairs_noalloc(keys.data_ptr(), vals.data_ptr(), keys.numel(), int(begin_bit), int(end_bit),
+                                        _stream(stream)))
     return keys, vals
 
 

@@ -1723,6 +1723,94 @@ int gamma_sort_pairs(unsigned int* keys, unsigned int* vals, long long n, int be
     return mark_done(st);
 }
 
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// gamma_sort_pairs_noalloc: the same radix sort for callers that must not allocate device memory.
+//
+// gamma_sort_pairs takes its ping-pong buffers, tile histograms and element counter from the library's grow-only
+// workspace, i.e. from cudaMalloc on first use and whenever n grows.  That is not an option for a caller that
+//   * runs while some thread of the process is capturing a stream in the global capture mode (cudaMalloc is refused
+//     there, and a refused call breaks the capture),
+//   * sits in a latency-critical loop (cudaMalloc / cudaFree synchronise the device and cost 0.1 - 1 ms), or
+//   * lives in a process whose device memory is handed out by one pool (the PyTorch caching allocator, a treatment
+//     planning system's arena) that has reserved all there is, so that a side allocation fails or fragments it.
+// For them the scratch lives in the library image itself: the file-scope array below, SORT_NOALLOC_WORDS * 4 bytes
+// (about 8.3 MB) of every GPU on which the library's module is loaded, held until the process exits.  The array is one
+// object per device.  Its name in HOST code is a stand-in, not an address a kernel could use; the address on the current
+// device comes from cudaGetSymbolAddress, asked once per device with that device current (noalloc_scratch()).
+//
+// Layout, in 32-bit words: [0, MAX) second key buffer | [MAX, 2 MAX) second value buffer | tile histograms
+// (256 x tiles, + 256 digit totals) | the element counter the kernels read n from.
+// Nothing in it has to start at zero: k_radix_hist writes every histogram word k_radix_scan and k_radix_scatter read,
+// k_radix_scan writes the digit totals, k_set_u32 the counter, and a pass overwrites the part of the ping-pong buffers the
+// next one reads.  What a call leaves behind is therefore harmless to the next call -- as long as the two do not overlap
+// on the device, see the header.
+constexpr long long SORT_NOALLOC_MAX = GAMMA_SORT_NOALLOC_MAX_PAIRS;
+constexpr size_t SORT_NOALLOC_TILES = (size_t)((SORT_NOALLOC_MAX + SORT_TILE - 1) / SORT_TILE);
+constexpr size_t SORT_NOALLOC_VALS = (size_t)SORT_NOALLOC_MAX;                  // word offsets, multiples of 64 (256 B)
+constexpr size_t SORT_NOALLOC_HIST = 2 * (size_t)SORT_NOALLOC_MAX;
+constexpr size_t SORT_NOALLOC_COUNT = SORT_NOALLOC_HIST + (SORT_NOALLOC_TILES + 1) * SORT_RADIX;
+constexpr size_t SORT_NOALLOC_WORDS = SORT_NOALLOC_COUNT + 64;
+static_assert(SORT_NOALLOC_MAX % 64 == 0, "keeps the parts of the scratch array 256-byte aligned");
+static __device__ __align__(256) unsigned g_sortNoallocScratch[SORT_NOALLOC_WORDS];
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+unsigned* g_sortNoallocPtr[NOALLOC_MAX_DEVICES] = {};   // device address of g_sortNoallocScratch, per device ordinal
+
+// Device address of the scratch array on the CURRENT device (looked up on the first call per device; g_mu held).
+int noalloc_scratch(unsigned** out)
+{
+    int dev = -1;
+    CU_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(GAMMA_ERR_INVALID_ARGUMENT, "device ordinal above 63");
+    if (!g_sortNoallocPtr[dev]) {
+        unsigned* p = nullptr;
+        CU_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_sortNoallocScratch));
+        if (!p) return fail(GAMMA_ERR_CUDA, "cudaGetSymbolAddress returned a null address for the sort scratch");
+        g_sortNoallocPtr[dev] = p;
+    }
+    *out = g_sortNoallocPtr[dev];
+    return GAMMA_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int gamma_sort_pairs_noalloc(unsigned int* keys, unsigned int* vals, long long n, int begin_bit, int end_bit,
+                             void* stream)
+{
+    g_err.clear();
+    if (n < 0) return fail(GAMMA_ERR_INVALID_ARGUMENT, "n must be >= 0");
+    if (n > SORT_NOALLOC_MAX)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT,
+                    "gamma_sort_pairs_noalloc: n = " + std::to_string(n) + " exceeds GAMMA_SORT_NOALLOC_MAX_PAIRS = " +
+                        std::to_string(SORT_NOALLOC_MAX) + " (the built-in scratch); use gamma_sort_pairs");
+    if (n > 0 && (!keys || !vals)) return fail(GAMMA_ERR_INVALID_ARGUMENT, "keys / vals is NULL");
+    if (begin_bit < 0 || end_bit > 32 || begin_bit >= end_bit || (begin_bit & 7) || (end_bit & 7))
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "need 0 <= begin_bit < end_bit <= 32, multiples of 8");
+    if (n == 0) return GAMMA_OK;
+    std::lock_guard<std::mutex> lock(g_mu);
+    end_b2b_sequence();                    // a host flag: a sort on `stream` ends a sequence of back-to-back gamma calls
+    unsigned* scratch = nullptr;
+    int rc = noalloc_scratch(&scratch);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    unsigned *k1 = scratch, *v1 = scratch + SORT_NOALLOC_VALS, *tileHist = scratch + SORT_NOALLOC_HIST;
+    unsigned* count = scratch + SORT_NOALLOC_COUNT;
+    k_set_u32<<<1, 1, 0, st>>>(count, (unsigned)n);
+    // tileHist is laid out for ceil(n / SORT_TILE) tiles by the kernels and by radix_sort_enqueue alike (<= SORT_NOALLOC_TILES)
+    int where = radix_sort_enqueue(keys, vals, k1, v1, count, n, begin_bit, end_bit, tileHist, st);
+    g_pool[0].launches += 1 + 3 * ((end_bit - begin_bit) / 8);
+    if (where) {    // an odd number of passes ends in the scratch: bring the result home (device-to-device, no staging)
+        CU_TRY(cudaMemcpyAsync(keys, k1, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+        CU_TRY(cudaMemcpyAsync(vals, v1, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    CU_TRY(cudaGetLastError());
+    return GAMMA_OK;
+}
+
 __global__ void k_table_export(const Ctl* __restrict__ ctl, const int4* __restrict__ table, long long maxEntries,
                                int* __restrict__ outEntries, int* __restrict__ outCount)
 {
