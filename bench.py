@@ -2,6 +2,7 @@
 """bench.py -- times the gamma-index hot path (one `gamma_eval` = one step) on the headline workload.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--case cfg3] [--no-cpu-baseline]
+                    [--no-configs] [--serial-calls]
 
 Workload (config.workload): BASELINE.json configs[2], the "3D 2%/2 mm case" that north_star and SURVEY.md
 section 8(d) name as the headline roofline case: 128x128x64 beam phantom at 2.5 mm, (2.0, 1.5, -1.0) mm shift,
@@ -13,6 +14,10 @@ roofline  dominant kernel, bound "alu": algorithmic FLOPs (DESIGN.md "Work model
           against the plain FP32 FMA peak 148 SM x 128 lanes x 2 x 1.965 GHz; the FFMA-chain rate measured on
           the box is reported beside it
 cpu_baseline / --impl reference: the CPU oracle (oracle/) as it stands, on the host cores
+parity    the map the last timed step wrote against the oracle's map of the cpu_baseline leg, element by element
+ms_per_step is the PIPELINED rate (opts.back_to_back = 1, about six calls in flight); ms_per_step_serial / serial_calls is
+the library default (one call after the other on the caller's stream, the plain gamma_eval signature), ms_per_call_isolated
+a single call; configs = the other BASELINE.json configs and cfg5 without the voxel pre-sort, same loop
 
 N > 1: replicas only: every rank runs the same case on its own GPU, no data-path
 collective; timing = max over ranks.
@@ -121,17 +126,38 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------------
 # the CPU oracle legs (the only places this file touches oracle/)
 # ------------------------------------------------------------------------------------------------------
+_last_oracle_gamma = None      # the map of the last oracle_time() call (the parity record of the bench line uses it)
+
+
 def oracle_time(case, voxels, reps):
+    global _last_oracle_gamma
     import oracle
     oracle.build()
     best = float("inf")
     sp = [f32(s) for s in case.spacing_mm]
     for _ in range(reps):
         t0 = time.perf_counter()
-        oracle.gamma(case.ref, case.eval, case.dims, sp, f32(case.dd), f32(case.dta_mm), case.mode, f32(case.cutoff),
-                     voxels=voxels)
+        _last_oracle_gamma = oracle.gamma(case.ref, case.eval, case.dims, sp, f32(case.dd), f32(case.dta_mm), case.mode,
+                                          f32(case.cutoff), voxels=voxels)
         best = min(best, time.perf_counter() - t0)
     return best, oracle.num_threads()
+
+
+def parity_record(case, keep, timed_map):
+    """The map the LAST TIMED step wrote (headline launch configuration) against the oracle, element by element, on the
+    voxels the cpu_baseline leg has just computed (all evaluated voxels).  Bar: |dgamma| <= 1e-4 (BASELINE.json north_star),
+    identical NaN masks, pass/fail equal outside 1e-4 of gamma = 1."""
+    og = _last_oracle_gamma
+    g = timed_map.astype(np.float64)
+    excluded = np.ones(g.size, dtype=bool)
+    excluded[keep] = False
+    d = np.abs(g[keep] - og)
+    near_one = np.abs(og - 1.0) <= 1e-4
+    return {"compared_voxels": int(keep.size), "max_abs_dgamma": float(np.nanmax(d)) if keep.size else 0.0,
+            "tolerance": 1e-4, "nan_mask_equal": bool(np.isnan(g[excluded]).all() and not np.isnan(g[keep]).any()
+                                                      and not np.isnan(og).any()),
+            "pass_equal": bool(np.array_equal((g[keep] <= 1.0)[~near_one], (og <= 1.0)[~near_one])),
+            "what": "gamma map written by the last timed step (opts.back_to_back as timed) vs oracle/ fp64, all evaluated voxels"}
 
 
 def evaluated_voxels(case):
@@ -143,7 +169,7 @@ def cpu_baseline(case):
     """The oracle on the whole workload (all evaluated voxels), best of 3: a few seconds of all host cores."""
     keep = evaluated_voxels(case)
     t, cores = oracle_time(case, keep, 3)
-    return {"value": keep.size / t, "unit": "evaluated reference voxels/s", "cores": cores, "kind": "oracle",
+    return keep, {"value": keep.size / t, "unit": "evaluated reference voxels/s", "cores": cores, "kind": "oracle",
             "sample": f"all {keep.size} evaluated voxels of {case.name}, shell-form double-precision search, "
                       f"best of 3 runs ({t:.2f} s each)", "seconds_per_case": t}
 
@@ -197,6 +223,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--case", default="cfg3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config records (cfg1 .. cfg5, cfg5 without pre-sort)")
     ap.add_argument("--presort", type=int, default=0)
     ap.add_argument("--star-phase", type=int, default=0)
     ap.add_argument("--lanes", type=int, default=0)
@@ -276,8 +303,46 @@ def main():
     ms_step = max_over_ranks(e0.elapsed_time(e1) / args.steps)
     cnt = binding.gamma_get_counters()
     M = cnt["n_evaluated"]
+    torch.cuda.synchronize()
+    timed_map = outs[(args.warmup + args.steps - 1) % nsets].cpu().numpy()      # what the last timed step wrote
 
-    # ---- per-stage CUDA events (library records them on the launching stream), same launch configuration
+    # ---- the same loop, one call after the other on the caller's stream (the library default, back_to_back = 0): with
+    # default options this is the plain north_star signature gamma_eval(...); then isolated calls (a synchronise between)
+    sopts = GammaOpts(**okw)
+    plain = not any(okw.values())
+
+    def serial_step(i):
+        k = i % nsets
+        if plain:
+            binding.gamma_eval(refs[k], evs[k], *args_c, outs[k], stream)
+        else:
+            binding.gamma_eval_ex(refs[k], evs[k], *args_c, sopts, outs[k], stream)
+
+    for i in range(max(args.warmup, 4)):
+        serial_step(i)
+    barrier()
+    ls0 = binding.gamma_launch_count()
+    ts0, ts1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with clocks:
+        ts0.record(stream)
+        for i in range(args.steps):
+            serial_step(args.warmup + i)
+        ts1.record(stream)
+        barrier()
+    serial_launches = binding.gamma_launch_count() - ls0
+    serial_ms_step = max_over_ranks(ts0.elapsed_time(ts1) / args.steps)
+    iso = []
+    for i in range(min(args.steps, 50)):
+        ti0, ti1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ti0.record(stream)
+        serial_step(i)
+        ti1.record(stream)
+        ti1.synchronize()
+        iso.append(ti0.elapsed_time(ti1))
+    isolated_ms = max_over_ranks(float(np.median(iso)))
+
+    # ---- per-stage CUDA events (library records them on the launching stream).  NOT the timed launch configuration:
+    # opts.profile_stages switches back_to_back off, so these are the kernels of a SERIAL call on full-size grids
     stage_acc = {}
     nprof = min(args.steps, 50)
     barrier()
@@ -424,6 +489,55 @@ def main():
     torch.cuda.synchronize()
     batch_ms_case = max_over_ranks(tb0.elapsed_time(tb1) / (nrep * nbatch))
 
+    # ---- the other BASELINE.json configs and Table 2's pair (cfg5 with / without the voxel pre-sort), so
+    # that the driver's run carries them: ms per case back to back (same loop as the headline), >= 50 timed steps each
+    def warp_inst(n_vox, c):
+        return (n_vox * (WINST["norm_per_voxel"] + WINST["classify_per_voxel"]) + WINST["norm_fixed"] + WINST["classify_fixed"]
+                + c["n_evaluated"] * WINST["star_per_voxel"] + WINST["star_fixed"]
+                + c["vertex_visits"] * WINST["visit"] + c["n_ring_search"] * WINST["ring_item"] + WINST["search_fixed"])
+
+    def time_config(name, extra, steps=60):
+        c = phantoms.make_case(name)
+        n = c.ref.size
+        ns = max(2, int(np.ceil(2.0 * L2_BYTES / (12.0 * n))) + 1)
+        r_h, e_h = torch.from_numpy(c.ref.ravel().copy()), torch.from_numpy(c.eval.ravel().copy())
+        rs, es = [r_h.to(dev) for _ in range(ns)], [e_h.to(dev) for _ in range(ns)]
+        os_ = [torch.empty(n, dtype=torch.float32, device=dev) for _ in range(ns)]
+        a = (c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+        res = {"case": name, "dims": list(c.dims), "criteria": f"{c.dd * 100:g}%/{c.dta_mm:g}mm", "grid_voxels": n,
+               "options": dict(extra), "steps": steps, "rotating_sets": ns}
+        for label, b2b in (("ms_per_case", 1), ("ms_per_case_serial", 0)):
+            o = GammaOpts(back_to_back=b2b, **extra)
+            for i in range(12):
+                binding.gamma_eval_ex(rs[i % ns], es[i % ns], *a, o, os_[i % ns], stream)
+            torch.cuda.synchronize()
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with clocks:
+                t0.record(stream)
+                for i in range(steps):
+                    binding.gamma_eval_ex(rs[i % ns], es[i % ns], *a, o, os_[i % ns], stream)
+                t1.record(stream)
+                torch.cuda.synchronize()
+            res[label] = max_over_ranks(t0.elapsed_time(t1) / steps)
+        cc = binding.gamma_get_counters()
+        _, sm = binding.gamma_stats(os_[0], 64, 4.0)
+        res.update({"evaluated_voxels": int(cc["n_evaluated"]), "n_table_search": int(cc["n_table_search"]),
+                    "vertex_visits": int(cc["vertex_visits"]),
+                    "value": world * cc["n_evaluated"] / (res["ms_per_case"] * 1e-3), "unit": "evaluated reference voxels/s",
+                    "pass_rate": sm["n_pass"] / max(1, sm["n_eval"]), "sum_gamma3": float(sm["sum_gamma3"]),
+                    "max_gamma": float(sm["max_gamma"])})
+        if sum(d > 1 for d in c.dims) == 3:
+            res["warp_inst"] = warp_inst(n, cc)
+        del rs, es, os_
+        torch.cuda.empty_cache()
+        return res
+
+    config_records = []
+    if not args.no_configs:
+        for name, extra in (("cfg1", {}), ("cfg2", {}), ("cfg4_coarse", {}), ("cfg4_fine", {}), ("cfg5", {}),
+                            ("cfg5", {"presort": 2})):
+            config_records.append(time_config(name, extra))
+
     probe_tflops = binding.gamma_fp32_probe(5)
     clk = clocks.report()
 
@@ -443,10 +557,20 @@ def main():
     units = {"k_star": M, "k_table_search": max(1, cnt["n_table_search"])}       # voxels the launch works on
     flop_per_unit = {"k_star": FLOP_PER_STAR_VOXEL if ndim == 3 else 0.0,
                      "k_table_search": search_flops / max(1, cnt["n_table_search"])}
-    dom = max(kernel_ms, key=kernel_ms.get)
     peak = SM_COUNT * FP32_LANES * 2 * SM_MAX_MHZ_NOMINAL * 1e6 / 1e12
+    per_kernel = {k: {"units_per_launch": units[k], "flop_per_unit": flop_per_unit[k],
+                      "algorithmic_flops_per_launch": units[k] * flop_per_unit[k], "kernel_ms": kernel_ms[k],
+                      "achieved": units[k] * flop_per_unit[k] / (kernel_ms[k] * 1e-3) / 1e12,
+                      "frac": units[k] * flop_per_unit[k] / (kernel_ms[k] * 1e-3) / 1e12 / peak,
+                      "traffic": TRAFFIC_BYTES.get(k)} for k in kernel_ms}
+    # the dominant kernel is the one that executes more FP32 work (a count, the same on every box), not the longer of two
+    # event times that differ by nanoseconds
+    dom = max(per_kernel, key=lambda k: per_kernel[k]["algorithmic_flops_per_launch"])
     alg = units[dom] * flop_per_unit[dom]
-    roof = {"bound": "alu", "kernel": dom, "peak": peak, "unit": "TFLOP/s", "traffic": TRAFFIC_BYTES.get(dom),
+    roof = {"bound": "alu", "kernel": dom, "kernels": per_kernel, "peak": peak, "unit": "TFLOP/s", "traffic": TRAFFIC_BYTES.get(dom),
+            "kernel_time_source": "serial call, opts.profile_stages (CUDA events between the stages of a call on the caller's "
+                                  "stream, full-size grids); the headline ms_per_step is the pipelined rate: whole_path.frac "
+                                  "is the fraction of the timed configuration",
             "peak_source": "148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and clocks.max.sm); "
                            "MEASURED_PEAKS.json has no FP32 figure",
             "ffma_chain_measured_tflops": probe_tflops, "stage_ms": stages,
@@ -457,11 +581,12 @@ def main():
     roof["frac_of_ffma_chain_probe"] = roof["achieved"] / probe_tflops if probe_tflops > 0 else None
     # the bound that actually limits this path: issue slots.  Warp instructions of one step (per-unit constants above x
     # the units the library counted) / (592 schedulers x 1 instruction per cycle x the SM clock)
-    winst = (N * (WINST["norm_per_voxel"] + WINST["classify_per_voxel"]) + WINST["norm_fixed"] + WINST["classify_fixed"]
-             + M * WINST["star_per_voxel"] + WINST["star_fixed"]
-             + cnt["vertex_visits"] * WINST["visit"] + cnt["n_ring_search"] * WINST["ring_item"] + WINST["search_fixed"])
+    winst = warp_inst(N, cnt)
     clk_hz = (clk.get("sm_mhz") or SM_MAX_MHZ_NOMINAL) * 1e6
     issue_us = winst / SCHEDULERS / clk_hz * 1e6
+    for r in config_records:
+        if "warp_inst" in r:
+            r["issue_frac"] = r["warp_inst"] / SCHEDULERS / clk_hz * 1e6 / (r["ms_per_case"] * 1e3)
     roof["issue"] = {"warp_inst": winst, "bound_us": issue_us, "frac": issue_us / (ms_step * 1e3),
                      "note": "executed warp instructions / (592 schedulers x 1 per cycle x SM clock) over the step time; "
                              "3D grids (per-unit constants measured on cfg2 / cfg3 / cfg5 / cfg4_fine)"}
@@ -483,8 +608,22 @@ def main():
         "config": {"workload": case_desc(case), "grid_voxels": N, "evaluated_voxels": M,
                    "l2_policy": f"{nsets} rotating input/output sets ({nsets * 12 * N / 1e6:.0f} MB) > 126 MB L2",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "options": {"presort": args.presort, "star_phase": args.star_phase, "lanes": args.lanes},
+                   "options": {"presort": args.presort, "star_phase": args.star_phase, "lanes": args.lanes,
+                               "star_load": args.star_load, "back_to_back": opts.back_to_back},
+                   "call_mode": ("pipelined: consecutive gamma_eval_ex calls with opts.back_to_back = 1 overlap on 6 library "
+                                 "streams, ms_per_step is a throughput with about six calls in flight"
+                                 if opts.back_to_back else "serial: one call after the other on the caller's stream"),
                    "init_calls_before_warmup": INIT_CALLS},
+        "headline_mode": "pipelined" if opts.back_to_back else "serial",
+        "ms_per_step_serial": serial_ms_step, "ms_per_call_isolated": isolated_ms,
+        "serial_calls": {"entry_point": "gamma_eval" if plain else "gamma_eval_ex", "back_to_back": 0,
+                         "ms_per_step": serial_ms_step, "value": world * M / (serial_ms_step * 1e-3),
+                         "unit": "evaluated reference voxels/s", "steps": args.steps, "gpu_launches": int(serial_launches),
+                         "ms_per_call_isolated": isolated_ms,
+                         "note": "the library default: calls one after the other on the caller's stream (round 1's headline "
+                                 "definition); isolated = median of calls with a synchronise between them"},
+        "configs": config_records,
+        "e2e_pipelined_ms_per_case": e2e_pipe_s * 1e3,
         "grid_voxels_per_s": world * N / (ms_step * 1e-3), "ms_per_case": ms_step,
         "e2e": {"value": world * M / e2e_s, "unit": "evaluated reference voxels/s", "ms_per_case": e2e_s * 1e3,
                 "h2d_bytes_per_step": 8 * N, "d2h_bytes_per_step": 4 * N,
@@ -510,7 +649,8 @@ def main():
                     "note": "gamma_eval_batch: independent cases spread over 6 library-owned streams"},
     }
     if not args.no_cpu_baseline and world == 1:
-        line["cpu_baseline"] = cpu_baseline(case)
+        keep, line["cpu_baseline"] = cpu_baseline(case)
+        line["parity"] = parity_record(case, keep, timed_map)
     elif world > 1:
         line["cpu_baseline"] = None
     print(json.dumps(line))

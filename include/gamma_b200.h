@@ -5,12 +5,15 @@
  * Citations are PAPER.md:<line> (+ section / equation / algorithm); "reading n" refers to the table of
  * readings in DESIGN.md.  Every entry point is plain C: raw pointers, sizes, a cudaStream_t passed as
  * void*.  Unless a parameter says HOST, pointers are DEVICE pointers owned by the caller (PyTorch in
- * the binding); the library never frees or modifies inputs.  The library owns one grow-only device
- * workspace per process (work lists, sort buffers, offset table), released by gamma_release().
+ * the binding); the library never frees or modifies inputs.  The library owns grow-only device workspaces
+ * (work lists, sort buffers, offset table): one for calls on the caller's stream, one per lane stream used by
+ * back-to-back / batched calls (6), one for calls captured into a caller's CUDA graph, plus the staging buffers of
+ * gamma_eval_host_batch; all released by gamma_release(), all counted by gamma_workspace_bytes().
  *
  * Conventions
  *   grids      dense fp32, x fastest: lin = ix + nx*(iy + ny*iz); reference and evaluation dose share
- *              one grid; an axis of size 1 is dropped (2D input; reading 12).
+ *              one grid in every entry point except gamma_eval_general, where the evaluation
+ *              dose has a grid of its own; an axis of size 1 is dropped (2D input; reading 12).
  *              N = nx*ny*nz must be < 2^31.
  *   result     gamma[N] fp32; voxels excluded by the low-dose cutoff (or with dD_v <= 0) hold NaN.
  *   async      all work is enqueued on `stream`; calls return without synchronising unless stated.
@@ -165,6 +168,9 @@ typedef struct gamma_opts {
  *   ref, eval, out_gamma   HOST arrays of n_cases DEVICE pointers (fp32, layout as in gamma_eval); the outputs must
  *                          not alias each other or any input (cases whose buffers overlap are run one after the other)
  *   dims, spacing_mm       HOST, n_cases x 3 (case-major); the criteria and options are shared by all cases
+ *   opts                   as gamma_eval_ex, except: profile_stages and back_to_back are ignored (the cases always run on
+ *                          the lanes), and stats_* cannot be honoured (one pair of buffers, n cases) -- passing stats_hist
+ *                          or stats_summary returns GAMMA_ERR_INVALID_ARGUMENT; run gamma_stats on each map instead
  *   stream                 the batch starts after the work already on `stream` and `stream` continues after the last
  *                          case; asynchronous.  Cannot be captured into a CUDA graph (INVALID_ARGUMENT).
  * Errors: as gamma_eval; every case is checked before anything is enqueued.  n_cases = 0 is a no-op. */
@@ -190,7 +196,10 @@ int gamma_eval_ex(const float* ref, const float* eval, const int dims[3], const 
  *   eval           DEVICE, product of eval_dims fp32; every eval_dims >= 2 (three active axes)
  *   *_dims, *_spacing_mm (> 0), *_origin_mm (finite)   HOST, 3 values each (x, y, z)
  *   DD, DTA_mm, mode, low_dose_cutoff   as gamma_eval (D_norm = max(ref) unless opts->norm_dose > 0)
- *   opts           NULL or gamma_opts of which norm_dose and table_cap are used
+ *   opts           NULL or gamma_opts of which norm_dose and table_cap are used.  presort, star_phase, lanes_per_voxel,
+ *                  sort_key_bits, profile_stages, graph, table_radius, interpolation, back_to_back and star_load are
+ *                  IGNORED (this path has one kernel sequence); stats_hist / stats_summary return
+ *                  GAMMA_ERR_INVALID_ARGUMENT (run gamma_stats on out_gamma)
  *   out_gamma      DEVICE, Nr fp32, written entirely (NaN = excluded)
  *   out_closest    DEVICE, Nr x 4 fp32 or NULL: (x, y, z in mm, evaluation dose) of one point of the surface at distance
  *                  gamma[v] (the minimiser need not be unique); NaN for excluded voxels.  The gamma angle follows as
@@ -222,6 +231,9 @@ int gamma_eval_host(const float* ref_host, const float* eval_host, const int dim
  * stream per direction, the kernels on a third).  Arguments as gamma_eval_batch with HOST pointers (pinned memory makes
  * the copies asynchronous; pageable memory works, more slowly).  Starts after what is on `stream`, SYNCHRONISES before
  * returning; cannot be captured.  Results are those of gamma_eval_host case by case, bit for bit.
+ * opts: as gamma_eval_batch (profile_stages, graph, back_to_back ignored; stats_* -> GAMMA_ERR_INVALID_ARGUMENT).  On a CUDA
+ * error in the middle of the batch the call still waits for every copy it has enqueued before it returns the error, so the
+ * caller's host buffers are no longer in use when it returns.
  */
 int gamma_eval_host_batch(int n_cases, const float* const* ref_host, const float* const* eval_host, const int* dims,
                           const float* spacing_mm, float DD, float DTA_mm, int mode, float low_dose_cutoff,
@@ -349,7 +361,8 @@ int gamma_trace_read(unsigned long long* out_host, long long* next_call);
  * busy and how long when few are left (profiles/r2_profile.md). */
 int gamma_trace_read_warps(unsigned long long* out_host, int max_warps);
 
-/* Device memory the library's workspaces hold right now, in bytes (host counter). */
+/* Device memory the library's workspaces hold right now, in bytes (host counter): all workspaces and the staging buffers
+ * of gamma_eval_host_batch; not the built-in scratch array of gamma_sort_pairs_noalloc (part of the library image). */
 long long gamma_workspace_bytes(void);
 
 /*

@@ -20,17 +20,18 @@ import numpy as np
 
 
 def stats(gamma, nbins: int, hist_max: float):
-    """Definition of gamma_stats: NaN = excluded; bin b counts finite gamma with floor(gamma/hist_max*nbins) == b,
-    the last bin also takes everything >= hist_max.  The bin index is decided in float32, as the header states
-    the inputs are fp32 (gamma * (nbins/hist_max) rounded to fp32)."""
+    """Definition of gamma_stats: NaN = excluded; bin b counts finite gamma with floor(gamma / hist_max * nbins) == b,
+    the last bin also takes everything >= hist_max.  The inputs are fp32 values (gamma, hist_max as the boundary receives
+    it); the bin is the plain real-number definition evaluated in float64 -- no device rounding in it (DESIGN.md reading
+    20: a kernel that decides the bin from an fp32 product may put a value that sits within an fp32 ulp of a bin edge
+    into the neighbouring bin; the GPU tests allow exactly that and nothing else)."""
     g = np.asarray(gamma, dtype=np.float32).ravel()
     fin = ~np.isnan(g)
     gf = g[fin]
-    scale = np.float32(nbins) / np.float32(hist_max)
-    fb = (gf * scale).astype(np.float32)
-    b = np.where(fb >= np.float32(nbins - 1), nbins - 1, np.floor(np.maximum(fb, 0)).astype(np.int64))
-    hist = np.bincount(b.astype(np.int64), minlength=nbins).astype(np.int64)
     g64 = gf.astype(np.float64)
+    t = g64 * float(nbins) / float(np.float32(hist_max))
+    b = np.minimum(np.floor(np.maximum(t, 0.0)), nbins - 1).astype(np.int64)
+    hist = np.bincount(b, minlength=nbins).astype(np.int64)
     return hist, {
         "n_eval": int(fin.sum()),
         "n_pass": int((gf <= np.float32(1.0)).sum()),

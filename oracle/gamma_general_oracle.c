@@ -19,6 +19,10 @@
  * Stock et al. 2005: the "gamma angle", i.e. which of dose difference and distance dominates) need the point where
  * the minimum is attained: closest[4] = (x, y, z in mm, interpolated evaluation dose) of one minimiser.
  *
+ * VALIDITY LIMIT (reading 21), as for gamma_oracle.c: under the local criterion with a reference dose far
+ * below the evaluation doses around it the Gram matrix is too ill conditioned for double precision and the result is an
+ * over-estimate; trusted where D_r >= 1e-4 D_norm (tests/test_exact_pins.py).
+ *
  * Point-to-simplex distance: PAPER.md:204-207 literally -- {w} = (V^T V)^-1 V^T P, w_{k+1} = 1 - sum w -- on EVERY
  * non-empty vertex subset of the simplex, feasible candidates (all weights >= 0) kept; the weights of
  * the winning candidate give the closest point.

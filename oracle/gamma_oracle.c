@@ -43,8 +43,21 @@
  * permutation invariance; brute-force barycentric sampling on tiny grids; 1D
  * polyline by hand; plain == shell; all-subsets == Ju recursion;
  * gamma_interp <= gamma_vertex_only.
+ * Since round 3 also against EXACT rational arithmetic, voxel by voxel
+ * (tests/test_exact_pins.py, tests/exact_gamma.py): equal to 1e-11.
  * Parity UNPINNED by the paper (conventions only, readings 6, 8-10):
  * orientation of the Kuhn diagonal; cutoff / local-mode / NaN policy.
+ *
+ * VALIDITY LIMIT (reading 21).  The normal equations square the
+ * condition number of V.  Under the local criterion a reference dose D_r that
+ * is tiny against the evaluation doses around it (dD_v = DD * D_r) stretches the
+ * dose axis by s ~ |D_e - D_r| / dD_v; the Gram matrix then has a condition
+ * number ~ s^2 and at s ~ 1e8 and beyond double precision has no digits left:
+ * this oracle then returns the distance to a point of the surface that is not
+ * the closest one (an OVER-estimate; measured 0.5 above the exact value at
+ * D_r = 1e-10).  It is trusted, and compared with the CUDA path, where
+ * D_r >= 1e-4 D_norm; below that the tests use exact arithmetic instead.
+ * Nothing in the arithmetic of this file was changed for it.
  *
  * Layout: dense, x fastest: lin = ix + nx*(iy + ny*iz).  An axis of size 1 is
  * dropped (reading 12).

@@ -184,6 +184,7 @@ struct UpdGraph {
     void* funcs[UPD_MAX_NODES];
     int count = 0;
     bool unusable = false;         // this sequence cannot be updated in place (a kernel twice, too many kernels)
+    unsigned long long lastUse = 0;
 };
 constexpr int UPD_CACHE = 4;
 
@@ -1108,7 +1109,11 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
         for (int i = 0; i < g_ws.numUpd; ++i)
             if (g_ws.upd[i].key == uk) { hit = &g_ws.upd[i]; break; }
         if (!hit) {                                        // build: capture this call once, keep graph, exec and nodes
-            int victim = g_ws.numUpd < UPD_CACHE ? g_ws.numUpd++ : 0;
+            int victim = 0;                                // a free entry, else the least recently used one
+            if (g_ws.numUpd < UPD_CACHE) victim = g_ws.numUpd++;
+            else
+                for (int i = 1; i < UPD_CACHE; ++i)
+                    if (g_ws.upd[i].lastUse < g_ws.upd[victim].lastUse) victim = i;
             UpdGraph& ug = g_ws.upd[victim];
             if (ug.exec) { cudaGraphExecDestroy(ug.exec); ug.exec = nullptr; }
             if (ug.graph) { cudaGraphDestroy(ug.graph); ug.graph = nullptr; }
@@ -1152,6 +1157,7 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
             }
             hit = &ug;
         }
+        hit->lastUse = ++g_ws.useClock;
         if (!hit->unusable) {
             GraphUpdate u = {hit->exec, hit->nodes, hit->funcs, hit->count, 0, true};
             g_upd = &u;
@@ -1226,8 +1232,10 @@ int enqueue_pipeline(const float* ref, const float* ev, const GridP& g, float DD
     ++g_callNo;
     g_ws.ctlClean = true;
     g_ws.lastStream = st; g_ws.lastN = g.N; g_ws.haveLast = true;
-    g_ws.lastEarly = early ? 1 : 0;
-    g_ws.numEarly += early ? 1 : 0;
+    // (a call without k_norm starts with a k_classify that waits for its predecessor at its top: not an early start)
+    const bool startedEarly = early && !(r.normDose > 0.0f && r.tableMode == 1 && r.stats.hist == nullptr && r.starLoad <= 1);
+    g_ws.lastEarly = startedEarly ? 1 : 0;
+    g_ws.numEarly += startedEarly ? 1 : 0;
     g_lastWs = g_cur;
     return GAMMA_OK;
 }
@@ -1387,6 +1395,8 @@ int gamma_eval_batch(int n_cases, const float* const* ref, const float* const* e
     rc = resolve_opts(opts, r);
     if (rc) return rc;
     r.profile = 0;
+    if (r.stats.hist || r.stats.summary)               // one pair of buffers cannot serve n cases
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_batch cannot honour opts.stats_*: use gamma_eval_ex per case or gamma_stats");
     // every case is checked before anything is enqueued: nothing is launched on an argument error
     for (int i = 0; i < n_cases; ++i) {
         if (!ref[i] || !eval[i] || !out_gamma[i]) return fail(GAMMA_ERR_INVALID_ARGUMENT, "ref[i] / eval[i] / out_gamma[i] is NULL");
@@ -1400,7 +1410,6 @@ int gamma_eval_batch(int n_cases, const float* const* ref, const float* const* e
     CU_TRY(cudaStreamIsCapturing(st, &capStatus));
     if (capStatus != cudaStreamCaptureStatusNone)
         return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_batch cannot be captured into a CUDA graph; capture gamma_eval calls");
-    r.stats.hist = nullptr; r.stats.summary = nullptr;                // one pair of buffers cannot serve n cases
     // The cases run like back-to-back calls: round-robin over the library's lane streams, the first one after what is
     // already on `stream`, `stream` continues after the last; hazards between the cases' buffers are checked.
     for (int i = 0; i < n_cases; ++i) {
@@ -1431,6 +1440,8 @@ int gamma_eval_general(const float* ref, const int ref_dims[3], const float ref_
     Resolved r;
     rc = resolve_opts(opts, r);
     if (rc) return rc;
+    if (r.stats.hist || r.stats.summary)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_general cannot honour opts.stats_*: run gamma_stats on out_gamma");
     GeneralP gp;
     std::memset(&gp, 0, sizeof gp);
     long long Nr = 1;
@@ -1593,7 +1604,8 @@ int gamma_eval_host_batch(int n_cases, const float* const* ref_host, const float
     rc = resolve_opts(opts, r);
     if (rc) return rc;
     r.profile = 0; r.graph = 0;
-    r.stats.hist = nullptr; r.stats.summary = nullptr;
+    if (r.stats.hist || r.stats.summary)
+        return fail(GAMMA_ERR_INVALID_ARGUMENT, "gamma_eval_host_batch cannot honour opts.stats_*: use gamma_eval_host per case or gamma_stats");
     long long maxN = 0;
     for (int i = 0; i < n_cases; ++i) {                  // every case is checked before anything is enqueued
         if (!ref_host[i] || !eval_host[i] || !out_gamma_host[i])
@@ -1632,29 +1644,38 @@ int gamma_eval_host_batch(int n_cases, const float* const* ref_host, const float
     CU_TRY(cudaEventRecord(H.start, user));              // everything starts after what is already on `stream`
     CU_TRY(cudaStreamWaitEvent(H.h2d, H.start, 0));
     g_lanes.laneDirty[0] = true;
+    // A failure inside the loop must not return while copies that were already enqueued may still read or write the
+    // caller's host buffers: note it, stop enqueuing, synchronise the three streams below, then report it.
+    cudaError_t ce = cudaSuccess;
+    const char* ceWhere = "";
+#define HB_TRY(call) { ce = (call); if (ce != cudaSuccess) { ceWhere = #call; break; } }
     for (int i = 0; i < n_cases; ++i) {
         const int k = i % HB_DEPTH;
         GridP g;
         make_grid(dims + 3 * i, spacing_mm + 3 * i, DTA_mm, g);
         const size_t bytes = (size_t)g.N * 4;
-        if (i >= HB_DEPTH) CU_TRY(cudaStreamWaitEvent(H.h2d, H.freed[k], 0));          // set k has been read back
-        CU_TRY(cudaMemcpyAsync(H.ref[k].p, ref_host[i], bytes, cudaMemcpyHostToDevice, H.h2d));      // A2 step 1
-        CU_TRY(cudaMemcpyAsync(H.ev[k].p, eval_host[i], bytes, cudaMemcpyHostToDevice, H.h2d));
-        CU_TRY(cudaEventRecord(H.copied[k], H.h2d));
-        CU_TRY(cudaStreamWaitEvent(comp, H.copied[k], 0));
+        if (i >= HB_DEPTH) HB_TRY(cudaStreamWaitEvent(H.h2d, H.freed[k], 0));          // set k has been read back
+        HB_TRY(cudaMemcpyAsync(H.ref[k].p, ref_host[i], bytes, cudaMemcpyHostToDevice, H.h2d));      // A2 step 1
+        HB_TRY(cudaMemcpyAsync(H.ev[k].p, eval_host[i], bytes, cudaMemcpyHostToDevice, H.h2d));
+        HB_TRY(cudaEventRecord(H.copied[k], H.h2d));
+        HB_TRY(cudaStreamWaitEvent(comp, H.copied[k], 0));
         Workspace* keep = g_cur;
         g_cur = &g_pool[1];
         rc = enqueue_pipeline(static_cast<const float*>(H.ref[k].p), static_cast<const float*>(H.ev[k].p), g, DD, mode,
                               low_dose_cutoff, r, static_cast<float*>(H.out[k].p), comp, false);
         g_cur = keep;
         if (rc) break;
-        CU_TRY(cudaEventRecord(H.computed[k], comp));
-        CU_TRY(cudaStreamWaitEvent(H.d2h, H.computed[k], 0));
-        CU_TRY(cudaMemcpyAsync(out_gamma_host[i], H.out[k].p, bytes, cudaMemcpyDeviceToHost, H.d2h));  // A2 step 8
-        CU_TRY(cudaEventRecord(H.freed[k], H.d2h));
+        HB_TRY(cudaEventRecord(H.computed[k], comp));
+        HB_TRY(cudaStreamWaitEvent(H.d2h, H.computed[k], 0));
+        HB_TRY(cudaMemcpyAsync(out_gamma_host[i], H.out[k].p, bytes, cudaMemcpyDeviceToHost, H.d2h));  // A2 step 8
+        HB_TRY(cudaEventRecord(H.freed[k], H.d2h));
     }
+#undef HB_TRY
     cudaError_t e1 = cudaStreamSynchronize(H.d2h), e2 = cudaStreamSynchronize(comp), e3 = cudaStreamSynchronize(H.h2d);
     if (rc) return rc;
+    if (ce != cudaSuccess)
+        return fail(ce == cudaErrorMemoryAllocation ? GAMMA_ERR_OUT_OF_MEMORY : GAMMA_ERR_CUDA,
+                    std::string(ceWhere) + ": " + cudaGetErrorString(ce));
     CU_TRY(e1); CU_TRY(e2); CU_TRY(e3);
     return GAMMA_OK;
 }
@@ -1981,6 +2002,7 @@ long long gamma_workspace_bytes(void)
     std::lock_guard<std::mutex> lock(g_mu);
     size_t n = 0;
     for (const Workspace& w : g_pool) n += w.bytes();
+    for (int k = 0; k < HB_DEPTH; ++k) n += g_hb.ref[k].cap + g_hb.ev[k].cap + g_hb.out[k].cap;   // gamma_eval_host_batch
     return (long long)n;
 }
 

@@ -5,13 +5,12 @@
 //                    list exists; zeroes the caller's fused-statistics buffers and the control block of the NEXT call.
 //   k_classify       a1: cutoff decision, NaN for excluded voxels, compaction of the evaluated voxels.
 // Consecutive kernels of a call are chained by programmatic dependent launch (pdl_wait / pdl_launch_dependents).
-//   k_prep_star      a1 + first part of a4: per voxel DD, cutoff, key (Algorithm A2 step 2 / CUDA Kernel 1,
-//                    PAPER.md:231-233); evaluated voxels are compacted into a block-local queue so that the
-//                    arithmetic always runs on full warps, then interior voxels try the 75 faces of the
-//                    evaluation surface that touch the voxel ("star").  A voxel whose gamma_star is not larger
+//   k_star           a1 + first part of a4: per evaluated voxel (from k_classify's compacted list) DD and key
+//                    (Algorithm A2 step 2 / CUDA Kernel 1), then interior voxels try the 75 faces of
+//                    the evaluation surface that touch the voxel ("star").  A voxel whose gamma_star is not larger
 //                    than the distance to the rest of the surface is final; the others are appended to the
-//                    search work list with key gamma_star (a much tighter key than |DD|/dD)
-//                    and counted into the digit histogram of the presort.
+//                    search work list with key gamma_star (a much tighter key than |DD|/dD),
+//                    split into depth classes (presort 4) or counted into the digit histogram of the presort.
 //   k_bucket_scatter a2: one-pass MSD radix presort of the work list on the 8-bit key digit.
 //   k_table_search   a4 + a5: Algorithm A1 step 4-b over the sorted offset table, G lanes
 //                    cooperating on one reference voxel, running best shared by shuffles, exit when the
@@ -468,7 +467,7 @@ k_star(const float* __restrict__ ref, const float* __restrict__ ev, float* __res
 
 // ------------------------------------------------------------------------------------------------
 // a2: one-pass MSD radix presort of the search work list on the 8-bit key digit.  The digit histogram
-// was accumulated by k_prep_star; every block scans it (256 values) and scatters its share of the list.
+// was accumulated by k_star; every block scans it (256 values) and scatters its share of the list.
 // Order inside a digit is arbitrary (the search result does not depend on the order of the list).
 // ------------------------------------------------------------------------------------------------
 constexpr int SCATTER_THREADS = 256;

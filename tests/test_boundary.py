@@ -102,3 +102,21 @@ def test_product_never_imports_the_oracle():
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".c")):
             assert "paper_1012_1900_b200" not in re.sub(r'""".*?"""|/\*.*?\*/', "", open(os.path.join(ROOT, "oracle", f)).read(), flags=re.S), f
+
+
+def test_stats_options_are_refused_where_they_cannot_be_honoured(lib):
+    """gamma_eval_batch / gamma_eval_host_batch / gamma_eval_general cannot write opts.stats_* (one pair of buffers for n
+    cases; no fused statistics in the general kernels): INVALID_ARGUMENT, not silently unwritten buffers."""
+    from paper_1012_1900_b200.binding import _COpts
+    o = _COpts()
+    o.stats_nbins, o.stats_hist, o.stats_summary, o.stats_hist_max = 16, 0x7000, 0x8000, 4.0
+    one = (ctypes.c_void_p * 1)(0x1000)
+    dims, sp = (ctypes.c_int * 3)(8, 8, 8), (ctypes.c_float * 3)(1.0, 1.0, 1.0)
+    org = (ctypes.c_float * 3)(0.0, 0.0, 0.0)
+    assert lib.gamma_eval_batch(1, one, one, dims, sp, 0.03, 3.0, 0, 0.1, ctypes.byref(o), one, None) == 1
+    assert b"stats" in lib.gamma_last_error_string()
+    assert lib.gamma_eval_host_batch(1, one, one, dims, sp, 0.03, 3.0, 0, 0.1, ctypes.byref(o), one, None) == 1
+    assert b"stats" in lib.gamma_last_error_string()
+    assert lib.gamma_eval_general(0x1000, dims, sp, org, 0x2000, dims, sp, org, 0.03, 3.0, 0, 0.1, ctypes.byref(o), 0x3000, None,
+                                  None) == 1
+    assert b"stats" in lib.gamma_last_error_string()

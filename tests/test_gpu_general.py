@@ -8,7 +8,7 @@ import torch
 
 from paper_1012_1900_b200 import binding, phantoms
 from paper_1012_1900_b200.binding import GammaOpts
-from test_gpu_parity import assert_parity, f32
+from test_gpu_parity import assert_parity, assert_parity_local_tiny_doses, f32
 from test_oracle_pins import _kuhn_interp, to_xyz_order
 
 pytestmark = pytest.mark.gpu
@@ -145,3 +145,39 @@ def test_general_argument_errors():
         binding.gamma_eval_general(one, (2, 2, 2), (1, 0, 1), (0, 0, 0), one, (2, 2, 2), (1, 1, 1), (0, 0, 0), 0.03, 3.0)
     with pytest.raises(binding.GammaError):
         binding.gamma_eval_general(one, (2, 2, 2), (1, 1, 1), (0, float("nan"), 0), one, (2, 2, 2), (1, 1, 1), (0, 0, 0), 0.03, 3.0)
+
+
+@pytest.mark.parametrize("geometry", ["identical", "general_small"])
+def test_general_path_local_mode_zero_and_negative_reference_dose(oracle_mod, geometry):
+    """SURVEY.md 8(b) / reading 9 on gamma_eval_general: reference doses of zero and below under the local criterion with
+    cutoff 0 are NaN (gamma and closest point), everything else meets the oracle."""
+    if geometry == "identical":
+        c = phantoms.make_case("cfg2_small")
+        ref, rd, rs, ro, ev, ed, es, eo, dd, dta = c.ref.copy(), c.dims, c.spacing_mm, (0.0, 0.0, 0.0), c.eval, c.dims, \
+            c.spacing_mm, (0.0, 0.0, 0.0), c.dd, c.dta_mm
+    else:
+        q = phantoms.make_general_case("general_small")
+        ref, rd, rs, ro, ev, ed, es, eo, dd, dta = q.ref.copy(), q.ref_dims, q.ref_spacing_mm, q.ref_origin_mm, q.eval, \
+            q.eval_dims, q.eval_spacing_mm, q.eval_origin_mm, q.dd, q.dta_mm
+    rng = np.random.default_rng(4)
+    inside = np.flatnonzero(ref.ravel() > 0.5)
+    ref.ravel()[rng.choice(inside, size=9, replace=False)] = np.float32(-0.02)
+    assert (ref == 0).sum() > 500
+    wg, wc = cpu_general(oracle_mod, ref, rd, rs, ro, ev, ed, es, eo, dd, dta, 1, 0.0)
+    assert np.array_equal(np.isnan(wg), ref.ravel() <= 0)
+    g, clo = gpu_general(ref, rd, rs, ro, ev, ed, es, eo, dd, dta, 1, 0.0)
+    what = f"general path ({geometry}), local mode, zero / negative reference dose"
+    assert np.array_equal(np.isnan(clo[:, 0]), np.isnan(wg))
+    if geometry == "identical":
+        # same grid: the exact-arithmetic helper applies to the voxels whose tiny D_r defeats the float64 oracle (reading 21)
+        err, err_exact, n_ill, n_off = assert_parity_local_tiny_doses(g, wg, ref, ev, rd, rs, dd, dta, what, "general-identical")
+        print(f"{what}: max|dgamma| {err:.2e}; {n_ill} voxels with tiny D_r ({n_off} where the oracle is off), vs exact {err_exact:.2e}")
+    else:
+        # own evaluation grid: the oracle where float64 can decide (D_r >= 1e-4 D_norm), the masks and the one-sided bound
+        # (the oracle can only over-estimate) everywhere
+        assert np.array_equal(np.isnan(g), np.isnan(wg))
+        r = ref.ravel().astype(np.float64)
+        well = ~np.isnan(wg) & (r >= 1e-4 * r.max())
+        assert_parity(np.where(well, g, np.nan), np.where(well, wg, np.nan), what)
+        ill = ~np.isnan(wg) & ~well
+        assert np.all(g[ill] <= wg[ill] + 1e-4)

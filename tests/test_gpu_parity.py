@@ -55,6 +55,25 @@ def assert_parity(g_gpu, g_cpu, what=""):
     return float(np.abs(g_gpu[m] - g_cpu[m]).max()) if m.any() else 0.0
 
 
+def assert_hist(hist_gpu, gamma, nbins, hmax, eh, what=""):
+    """The device histogram against the float64 definition (aux_oracle.stats).  Exact, except that a value within an fp32
+    ulp of a bin edge may sit in either neighbouring bin (the kernel decides the bin from an fp32 product, DESIGN.md
+    reading 20): for every edge k the number of values counted below it may differ from the definition's by at most the
+    number of values that close to that edge.  Returns how many values ended up in the neighbouring bin."""
+    hist_gpu = np.asarray(hist_gpu, dtype=np.int64)
+    assert hist_gpu.sum() == eh.sum(), what
+    if np.array_equal(hist_gpu, eh):
+        return 0
+    g = np.asarray(gamma, dtype=np.float32).ravel()
+    t = g[~np.isnan(g)].astype(np.float64) * float(nbins) / float(np.float32(hmax))
+    k = np.rint(t)
+    near = (np.abs(t - k) <= 2.0 ** -22 * np.maximum(1.0, t)) & (k >= 1) & (k <= nbins - 1)
+    slack = np.bincount(k[near].astype(np.int64), minlength=nbins + 1)[: nbins + 1]      # values near edge k
+    below_gpu, below_def = np.cumsum(hist_gpu)[:-1], np.cumsum(eh)[:-1]                  # counted below edge 1 .. nbins-1
+    assert np.all(np.abs(below_gpu - below_def) <= slack[1:nbins]), (what, np.flatnonzero(below_gpu != below_def)[:8])
+    return int(np.abs(below_gpu - below_def).sum())                # values that sit in the neighbouring bin
+
+
 # ----------------------------------------------------------------------------------------------------
 # the BASELINE.json configs, full grids, default options = the configuration bench.py times
 # ----------------------------------------------------------------------------------------------------
@@ -97,6 +116,102 @@ def test_local_criterion_full_size_full_map_parity(oracle_mod, name, cutoff):
     print(f"{name} local: max|dgamma| {err:.2e} over all {int((~np.isnan(o)).sum())} evaluated voxels")
 
 
+def _with_zero_and_negative_reference(c):
+    """cfg2_small's reference is exactly 0 outside the body ellipse; a dozen voxels are also set below zero."""
+    ref = c.ref.copy()
+    rng = np.random.default_rng(3)
+    inside = np.flatnonzero(ref.ravel() > 0.5)
+    ref.ravel()[rng.choice(inside, size=12, replace=False)] = np.float32(-0.01)
+    assert (ref == 0).sum() > 1000 and (ref < 0).sum() == 12
+    return ref
+
+
+_exact_cache = {}
+
+
+def assert_parity_local_tiny_doses(g, o, ref, ev, dims, sp, dd, dta, what, tag):
+    """Parity under the LOCAL criterion when the reference holds doses that are tiny against the evaluation doses around
+    them (the tail of the analytic phantom: D_r ~ 1e-10, dD_v = DD * D_r ~ 1e-12).  DESIGN.md reading 21: the dose axis is
+    then stretched by 1e10, the Gram matrix of the normal equations has a condition number ~1e20 and the
+    float64 oracle loses its digits (it over-estimates: oracle/gamma_oracle.c header; tests/test_exact_pins.py).  So:
+      * NaN masks: identical on the whole map;
+      * voxels with D_r >= 1e-4 D_norm (condition number small enough for float64): the usual bar against the oracle;
+      * the others: never above the oracle by more than the tolerance (the oracle can only over-estimate there), and on a
+        sample -- the voxels where device and oracle differ most, plus seeded random ones -- against EXACT rational
+        arithmetic (tests/exact_gamma.py) at the same 1e-4."""
+    from exact_gamma import exact_gamma
+    r = np.asarray(ref, dtype=np.float32).ravel().astype(np.float64)
+    assert np.array_equal(np.isnan(g), np.isnan(o)), f"{what}: excluded masks differ"
+    fin = ~np.isnan(o)
+    well = fin & (r >= 1e-4 * r.max())
+    gw, ow = np.where(well, g, np.nan), np.where(well, o, np.nan)
+    err = assert_parity(gw, ow, what + " (D_r >= 1e-4 D_norm)")
+    ill = np.flatnonzero(fin & ~well)
+    assert ill.size > 100, "the case is meant to contain tiny reference doses"
+    assert np.all(g[ill] <= o[ill] + TOL), f"{what}: device gamma above the (over-estimating) oracle at tiny D_r"
+    rng = np.random.default_rng(11)
+    pick = np.unique(np.concatenate([ill[np.argsort(-(o[ill] - g[ill]))[:10]], rng.choice(ill, size=10, replace=False)]))
+    worst = 0.0
+    for v in pick:
+        key = (tag, int(v))
+        if key not in _exact_cache:
+            _exact_cache[key] = exact_gamma(ref, ev, dims, [f32(x) for x in sp], f32(dd), f32(dta), 1, int(v),
+                                            gamma_ub=1.5 * o[v] + 0.1)
+        worst = max(worst, abs(g[v] - _exact_cache[key]))
+        assert abs(g[v] - _exact_cache[key]) <= TOL, (f"{what}: voxel {v} (D_r = {r[v]:.3e}): device {g[v]:.7f}, exact "
+                                                      f"{_exact_cache[key]:.7f}, float64 oracle {o[v]:.7f}")
+    return err, worst, int(ill.size), int((np.abs(g[ill] - o[ill]) > TOL).sum())
+
+
+@pytest.mark.parametrize("variant", [dict(), dict(back_to_back=1), dict(star_load=2), dict(star_load=3), dict(star_phase=2),
+                                     dict(presort=3), dict(norm_dose=2.0)])
+def test_local_mode_zero_and_negative_reference_dose(oracle_mod, variant):
+    """"Local mode with dD_v = 0 (D_r[v] = 0, only possible when cutoff = 0): gamma[v] = NaN" (reading 9),
+    on the device: zeros and negative reference doses under the local criterion with no cutoff, in every kernel that
+    classifies voxels (list, tiles, no star phase), full map.  The zeros and negatives are NaN and still serve as
+    evaluation points; the voxels next to them carry doses down to 1e-10 and keep a finite gamma, which is compared with
+    the oracle where float64 can decide and with exact arithmetic where it cannot (assert_parity_local_tiny_doses)."""
+    c = phantoms.make_case("cfg2_small")
+    ref = _with_zero_and_negative_reference(c)
+    o = cpu_gamma(oracle_mod, ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 1, 0.0, norm_dose=variant.get("norm_dose", 0.0))
+    assert np.array_equal(np.isnan(o), ref.ravel() <= 0)                      # what the definition says (oracle pin :463)
+    g = gpu_gamma(ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 1, 0.0, GammaOpts(**variant))
+    err, err_exact, n_ill, n_off = assert_parity_local_tiny_doses(g, o, ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm,
+                                                                  f"local, zero / negative reference, {variant}", "same-grid")
+    if variant.get("back_to_back"):                                           # a second call on the next lane, same answer
+        g2 = gpu_gamma(ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, 1, 0.0, GammaOpts(**variant))
+        assert np.array_equal(np.isnan(g2), np.isnan(g)) and np.array_equal(g2[~np.isnan(g2)], g[~np.isnan(g)])
+    print(f"local mode, {int(np.isnan(o).sum())} zero / negative voxels, {variant}: max|dgamma| {err:.2e} vs oracle; {n_ill} "
+          f"voxels with tiny D_r ({n_off} where the float64 oracle is off by > 1e-4), vs exact arithmetic {err_exact:.2e}")
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg5"])
+def test_timed_configuration_back_to_back_full_size_against_the_oracle(oracle_mod, name):
+    """The configuration bench.py times -- consecutive gamma_eval_ex calls with opts.back_to_back = 1, no synchronisation
+    between them, rotating buffers -- directly against the oracle at full size: 24 calls (four rounds over the six lane
+    streams, half-size grids, one rewritten graph launch each), every one of the 24 maps compared element by element."""
+    c = phantoms.make_case(name)
+    o = cpu_gamma(oracle_mod, c.ref, c.eval, c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff)
+    nsets = 6
+    refs = [torch.from_numpy(c.ref.ravel().copy()).cuda() for _ in range(nsets)]
+    evs = [torch.from_numpy(c.eval.ravel().copy()).cuda() for _ in range(nsets)]
+    outs = [torch.full((c.ref.size,), -7.0, dtype=torch.float32, device="cuda") for _ in range(24)]
+    opts = GammaOpts(back_to_back=1)
+    stream = torch.cuda.current_stream()
+    torch.cuda.synchronize()
+    n0 = binding.gamma_get_counters()["calls_pipelined"]
+    for i in range(24):
+        binding.gamma_eval_ex(refs[i % nsets], evs[i % nsets], c.dims, c.spacing_mm, c.dd, c.dta_mm, c.mode, c.cutoff, opts,
+                              outs[i], stream)
+    torch.cuda.synchronize()
+    cnt = binding.gamma_get_counters()
+    assert cnt["pipelined"] == 1 and cnt["calls_pipelined"] - n0 == 24        # the lanes were really used
+    worst = 0.0
+    for i in range(24):
+        worst = max(worst, assert_parity(outs[i].cpu().numpy().astype(np.float64), o, f"{name} back-to-back call {i}"))
+    print(f"{name}: 24 back-to-back calls, max|dgamma| {worst:.2e} over {int((~np.isnan(o)).sum())} evaluated voxels each")
+
+
 def test_criteria_sweep_table3(oracle_mod):
     """The 9 DD x DTA combinations of Table 3 on the cfg3 phantom: every device map against the
     whole oracle map; on the DEVICE maps the exact law gamma(k dD, k dd) = gamma(dD, dd) / k and the monotonicity in dD
@@ -134,7 +249,7 @@ def test_criteria_sweep_table3(oracle_mod):
 
 @pytest.mark.parametrize("name", ["cfg4_fine", "cfg5", "cfg2_small"])
 def test_star_load_paths_agree_bit_for_bit(name):
-    """opts.star_load: compacted list + __ldg (1), TMA-staged tiles (2, default) and tiles filled by cooperative loads (3)
+    """opts.star_load: compacted list + __ldg (1, default), TMA-staged tiles (2) and tiles filled by cooperative loads (3)
     evaluate the same faces with the same arithmetic: identical maps, identical counters."""
     c = phantoms.make_case(name)
     r = torch.from_numpy(c.ref.ravel().copy()).cuda()
@@ -888,7 +1003,7 @@ def test_fused_stats_equal_the_definition(name, nbins, hmax):
         torch.cuda.synchronize()
         s = binding.decode_summary(summ)
         eh, es = aux_oracle.stats(g.cpu().numpy(), nbins, hmax)
-        assert np.array_equal(hist.cpu().numpy(), eh), kw
+        assert_hist(hist.cpu().numpy(), g.cpu().numpy(), nbins, hmax, eh, f"{name} {kw}")
         for k in ("n_eval", "n_pass", "n_nan"):
             assert s[k] == es[k], (k, kw)
         assert s["max_gamma"] == es["max_gamma"]
@@ -930,7 +1045,7 @@ def test_gamma_stats_against_definition(n, nbins, hmax):
     t = torch.from_numpy(g).cuda() if n else torch.empty(0, dtype=torch.float32, device="cuda")
     hist, s = binding.gamma_stats(t, nbins, hmax)
     eh, es = aux_oracle.stats(g, nbins, hmax)
-    assert np.array_equal(hist.cpu().numpy(), eh)                                 # integer work: exact
+    assert_hist(hist.cpu().numpy(), g, nbins, hmax, eh, f"n={n}")                  # integer work: exact up to bin-edge ties
     for k in ("n_eval", "n_pass", "n_nan"):
         assert s[k] == es[k], k
     assert s["max_gamma"] == es["max_gamma"]
