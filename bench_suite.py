@@ -41,7 +41,7 @@ def f32(x):
     return float(np.float32(x))
 
 
-def measure(case, opts_kw, reps, dd=None, dta=None, keep_map=False):
+def measure(case, opts_kw, reps, dd=None, dta=None, keep_map=False, mode=None):
     import torch
     from paper_1012_1900_b200 import binding
     from paper_1012_1900_b200.binding import GammaOpts
@@ -57,7 +57,7 @@ def measure(case, opts_kw, reps, dd=None, dta=None, keep_map=False):
     evs = [ev_h.to(dev) for _ in range(nsets)]
     outs = [torch.empty(N, dtype=torch.float32, device=dev) for _ in range(nsets)]
     stream = torch.cuda.current_stream()
-    a = (case.dims, case.spacing_mm, dd, dta, case.mode, case.cutoff)
+    a = (case.dims, case.spacing_mm, dd, dta, case.mode if mode is None else mode, case.cutoff)
     opts = GammaOpts(**opts_kw)
     popts = GammaOpts(profile_stages=1, **opts_kw)
     for i in range(4):
@@ -162,9 +162,11 @@ def suite_configs(args, emit):
         orc = oracle_sample(case, args.oracle_seconds)
         if name in ("cfg1", "cfg2") and orc is not None:     # per-core figure; the paper's CPU threading is unstated
             orc["one_core"] = oracle_sample(case, args.oracle_seconds, nthreads=1)
+        if name in ("cfg3", "cfg5"):     # the local criterion (dD_v = DD * D_r[v], reading 9): a reciprocal per voxel in double
+            variants.append(("local criterion (mode 1)", {}))
         for label, kw in variants:
             reps = args.reps if "thread per voxel" not in label else max(3, args.reps // 6)
-            r = measure(case, kw, reps)
+            r = measure(case, kw, reps, mode=1 if label.startswith("local criterion") else None)
             r.update({"suite": "configs", "case": name, "variant": label, "cpu_oracle": orc if label == "default" else None})
             emit(r)
             rows.append(r)
